@@ -1,0 +1,116 @@
+"""Workload descriptions (plain data, no arithmetic of the method).
+
+The five data configs and the metadata-only config are BASELINE.json `configs`
+(model shapes like the paper's GPT-3-style workloads, §IV-A;
+reconfigurations like Table II's).  Fields BASELINE.json leaves
+open follow DESIGN.md readings A11 (tied embeddings unless "untied" is said),
+A13 (max_pos) and the 5b head/ffn/vocab choice.
+
+A workload is a dict:
+  {"name", "model": {...}, "old": {"tp","pp","dp","dist_opt"}, "new": {...}, "data": bool}
+"""
+from __future__ import annotations
+import copy
+import itertools
+
+KIND_PARAM, KIND_MASTER, KIND_ADAM_M, KIND_ADAM_V = 0, 1, 2, 3
+KIND_NAMES = ("param", "master", "adam_m", "adam_v")
+STYLE_GPT, STYLE_LLAMA = 0, 1
+
+_ALL4 = 0b1111
+_PMV = 0b1101  # PARAM | ADAM_M | ADAM_V (config 1: fp32 params plus Adam m and v, no separate master)
+
+
+def _model(style, n_layers, hidden, n_q, n_kv, head_dim, ffn, vocab, max_pos, tied, param_bytes, kinds):
+    return dict(style=style, n_layers=n_layers, hidden=hidden, n_q_heads=n_q, n_kv_heads=n_kv,
+                head_dim=head_dim, ffn_hidden=ffn, vocab=vocab, max_pos=max_pos, tied=tied,
+                param_bytes=param_bytes, kinds=kinds)
+
+
+def _cfg(tp, pp, dp, dist_opt=0):
+    return dict(tp=tp, pp=pp, dp=dp, dist_opt=dist_opt)
+
+
+WORKLOADS = {
+    # BASELINE.json configs[0]
+    "c1": dict(name="c1", data=True, seed=0xE7C00001,
+               model=_model(STYLE_GPT, 2, 256, 4, 4, 64, 1024, 1024, 128, 0, 4, _PMV),
+               old=_cfg(2, 2, 1), new=_cfg(1, 2, 2)),
+    # BASELINE.json configs[1]
+    "c2": dict(name="c2", data=True, seed=0xE7C00002,
+               model=_model(STYLE_GPT, 24, 1024, 16, 16, 64, 4096, 50304, 2048, 1, 2, _ALL4),
+               old=_cfg(2, 2, 2), new=_cfg(4, 2, 1)),
+    # BASELINE.json configs[2]
+    "c3": dict(name="c3", data=True, seed=0xE7C00003,
+               model=_model(STYLE_GPT, 24, 2048, 32, 32, 64, 8192, 50304, 2048, 1, 2, _ALL4),
+               old=_cfg(4, 4, 1), new=_cfg(4, 3, 1)),
+    # BASELINE.json configs[3]
+    "c4": dict(name="c4", data=True, seed=0xE7C00004,
+               model=_model(STYLE_GPT, 32, 2560, 32, 32, 80, 10240, 50304, 2048, 1, 2, _ALL4),
+               old=_cfg(2, 4, 2, 1), new=_cfg(4, 2, 4, 1)),
+    # BASELINE.json configs[4], data part
+    "c5": dict(name="c5", data=True, seed=0xE7C00005,
+               model=_model(STYLE_LLAMA, 8, 4096, 32, 8, 128, 14336, 128256, 0, 0, 2, _ALL4),
+               old=_cfg(8, 1, 1), new=_cfg(4, 2, 1)),
+    # BASELINE.json configs[4], metadata-only part (cost matrix + sketch only)
+    "c5b": dict(name="c5b", data=False, seed=0xE7C00006,
+                model=_model(STYLE_LLAMA, 80, 8192, 64, 8, 128, 28672, 128256, 0, 0, 2, _ALL4),
+                old=_cfg(8, 16, 4), new=_cfg(8, 16, 3)),
+}
+
+# Scaled-down twins: same parallel reconfiguration, same style/kinds/tied-ness, dims shrunk so the
+# element-wise oracle finishes in seconds while slices still span several copy tiles and ragged tails.
+_SCALED = {
+    "s2": ("c2", dict(n_layers=4, hidden=192, n_q_heads=12, n_kv_heads=12, head_dim=16, ffn_hidden=768,
+                      vocab=3000, max_pos=96)),
+    "s3": ("c3", dict(n_layers=12, hidden=256, n_q_heads=8, n_kv_heads=8, head_dim=32, ffn_hidden=1024,
+                      vocab=2052, max_pos=64)),
+    "s4": ("c4", dict(n_layers=8, hidden=320, n_q_heads=4, n_kv_heads=4, head_dim=80, ffn_hidden=1280,
+                      vocab=3004, max_pos=80)),
+    "s5": ("c5", dict(n_layers=4, hidden=512, n_q_heads=16, n_kv_heads=8, head_dim=32, ffn_hidden=1792,
+                      vocab=4008, max_pos=0)),
+    # odd sizes: rows that are not multiples of 16 bytes (exercises the scalar/unaligned copy path)
+    "s4odd": ("c4", dict(n_layers=8, hidden=20, n_q_heads=4, n_kv_heads=4, head_dim=5, ffn_hidden=36,
+                         vocab=52, max_pos=7)),
+    "s5b": ("c5b", dict(n_layers=16, hidden=64, n_q_heads=16, n_kv_heads=8, head_dim=4, ffn_hidden=128,
+                        vocab=256, max_pos=0)),
+}
+
+
+def workload(name: str) -> dict:
+    """Return a deep copy of the named workload ("c1".."c5", "c5b", "s2".."s5", "s4odd", "s5b")."""
+    if name in WORKLOADS:
+        return copy.deepcopy(WORKLOADS[name])
+    base, over = _SCALED[name]
+    w = copy.deepcopy(WORKLOADS[base])
+    w["name"] = name
+    w["model"].update(over)
+    w["data"] = True
+    w["seed"] = WORKLOADS[base]["seed"] ^ 0x5CA1ED
+    return w
+
+
+def scaled_workloads():
+    return [workload(k) for k in _SCALED]
+
+
+def tiny_models():
+    """Micro models for exhaustive sweeps (P12): both styles, tied and untied, a non-power-of-two hidden."""
+    out = []
+    out.append(("gpt_t", _model(STYLE_GPT, 4, 8, 4, 4, 2, 16, 8, 4, 1, 2, _ALL4)))
+    out.append(("gpt_u", _model(STYLE_GPT, 2, 24, 4, 4, 6, 20, 12, 3, 0, 4, _PMV)))
+    out.append(("gpt_np", _model(STYLE_GPT, 4, 12, 2, 2, 6, 28, 20, 0, 1, 2, _ALL4)))
+    out.append(("llama_u", _model(STYLE_LLAMA, 4, 16, 4, 2, 4, 12, 8, 0, 0, 2, _ALL4)))
+    out.append(("llama_t", _model(STYLE_LLAMA, 2, 24, 4, 4, 6, 20, 16, 0, 1, 2, _ALL4)))
+    return out
+
+
+def tiny_parallel_cfgs(max_devices=8, sizes=(1, 2, 4)):
+    """All (tp,pp,dp,dist_opt) with sizes in `sizes` and tp*pp*dp <= max_devices."""
+    out = []
+    for tp, pp, dp in itertools.product(sizes, sizes, sizes):
+        if tp * pp * dp <= max_devices:
+            out.append(_cfg(tp, pp, dp, 0))
+            if dp > 1:
+                out.append(_cfg(tp, pp, dp, 1))
+    return out

@@ -1,0 +1,248 @@
+"""ctypes wrapper around oracle/etc_oracle.c — TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference` legs may import this.
+It never imports paper_2607_04749_b200 (the CUDA path) and shares no code with it.
+
+`build()` compiles etc_oracle.c with gcc (OpenMP) into oracle/liboracle.so.
+"""
+from __future__ import annotations
+import ctypes as C
+import os
+import subprocess
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "etc_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+
+class Model(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("style", "n_layers", "hidden", "n_q_heads", "n_kv_heads", "head_dim",
+                                          "ffn_hidden", "vocab", "max_pos", "tied", "param_bytes", "kinds")]
+
+
+class Cfg(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("tp", "pp", "dp", "dist_opt")]
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", _LIB, _SRC])
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(_LIB)
+        vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+        P = C.POINTER
+        L.orc_num_logical.restype = i32
+        L.orc_logical_info.restype = i32
+        L.orc_kind_bytes.restype = i32
+        L.orc_layout_new.restype = i32
+        L.orc_layout_new.argtypes = [P(Model), P(Cfg), P(vp)]
+        L.orc_layout_free.argtypes = [vp]
+        L.orc_layout_free.restype = None
+        L.orc_num_devices.restype = i32
+        L.orc_num_devices.argtypes = [vp]
+        L.orc_buffer_elems.restype = i64
+        L.orc_buffer_elems.argtypes = [vp, i32, i32]
+        L.orc_global_of_range.restype = i32
+        L.orc_global_of_range.argtypes = [vp, i32, i32, i64, i64, vp, vp, vp, vp]
+        L.orc_holders_of.restype = i32
+        L.orc_holders_of.argtypes = [vp, i32, i32, i64, i64, i32, vp, vp]
+        L.orc_overlap_elementwise.restype = i32
+        L.orc_overlap_elementwise.argtypes = [vp, vp, i32, vp, vp, vp]
+        L.orc_overlap_ranges.restype = i32
+        L.orc_overlap_ranges.argtypes = [vp, vp, vp, vp, vp]
+        L.orc_sketch_bruteforce.restype = i64
+        L.orc_sketch_bruteforce.argtypes = [vp, i32, i32, vp, vp, P(i64)]
+        L.orc_sketch_hungarian.restype = i32
+        L.orc_sketch_hungarian.argtypes = [vp, i32, i32, vp, vp, P(i64)]
+        L.orc_source_of.restype = i32
+        L.orc_source_of.argtypes = [vp, vp, vp, i32, i32, vp, i64, vp, vp]
+        L.orc_migrate_range.restype = i32
+        L.orc_migrate_range.argtypes = [vp, vp, vp, i32, i32, i64, i64, vp, vp, vp, vp, vp]
+        L.orc_migrate.restype = i32
+        L.orc_migrate.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+        L.orc_max_threads.restype = i32
+        _lib = L
+    return _lib
+
+
+class OracleError(RuntimeError):
+    def __init__(self, code):
+        super().__init__(f"oracle error {code}")
+        self.code = code
+
+
+def _model(m: dict) -> Model:
+    return Model(**{k: int(m[k]) for k, _ in Model._fields_})
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def max_threads() -> int:
+    return int(lib().orc_max_threads())
+
+
+def logical_tensors(model: dict):
+    """[(rows, cols, split, where, layer)] for every logical tensor, in id order."""
+    m = _model(model)
+    n = lib().orc_num_logical(C.byref(m))
+    rows = np.zeros(n, np.int64); cols = np.zeros(n, np.int64)
+    split = np.zeros(n, np.int32); where = np.zeros(n, np.int32); layer = np.zeros(n, np.int32)
+    lib().orc_logical_info(C.byref(m), _ptr(rows), _ptr(cols), _ptr(split), _ptr(where), _ptr(layer))
+    return [(int(rows[i]), int(cols[i]), int(split[i]), int(where[i]), int(layer[i])) for i in range(n)]
+
+
+def kind_bytes(model: dict, kind: int) -> int:
+    m = _model(model)
+    return int(lib().orc_kind_bytes(C.byref(m), kind))
+
+
+class Layout:
+    """Oracle-side layout of one (model, parallel config)."""
+
+    def __init__(self, model: dict, cfg: dict):
+        self.model, self.cfg = dict(model), dict(cfg)
+        m = _model(model)
+        c = Cfg(**{k: int(cfg.get(k, 0)) for k, _ in Cfg._fields_})
+        h = C.c_void_p()
+        rc = lib().orc_layout_new(C.byref(m), C.byref(c), C.byref(h))
+        if rc:
+            raise OracleError(rc)
+        self.h = h
+        self.n_dev = int(lib().orc_num_devices(h))
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            lib().orc_layout_free(self.h)
+            self.h = None
+
+    def kinds(self):
+        return [k for k in range(4) if (self.model["kinds"] >> k) & 1]
+
+    def elem_bytes(self, kind):
+        return kind_bytes(self.model, kind)
+
+    def buffer_elems(self, dev, kind) -> int:
+        return int(lib().orc_buffer_elems(self.h, dev, kind))
+
+    def global_of(self, dev, kind, l0=0, count=None):
+        """(lt, post_copy, row, col) arrays for local indices [l0, l0+count)."""
+        if count is None:
+            count = self.buffer_elems(dev, kind) - l0
+        lt = np.zeros(count, np.int32); pc = np.zeros(count, np.int32)
+        row = np.zeros(count, np.int64); col = np.zeros(count, np.int64)
+        rc = lib().orc_global_of_range(self.h, dev, kind, l0, count, _ptr(lt), _ptr(pc), _ptr(row), _ptr(col))
+        if rc:
+            raise OracleError(rc)
+        return lt, pc, row, col
+
+    def holders_of(self, kind, lt, row, col):
+        cap = 2 * self.n_dev + 2
+        dev = np.zeros(cap, np.int32); l = np.zeros(cap, np.int64)
+        n = lib().orc_holders_of(self.h, kind, lt, row, col, cap, _ptr(dev), _ptr(l))
+        return [(int(dev[i]), int(l[i])) for i in range(n)]
+
+    # ---- data helpers built on global_of + plain numpy indexing
+    def shard_from_logical(self, dev, kind, logical: list) -> np.ndarray:
+        """Buffer (dev, kind) cut out of the logical tensors (list of 2-D arrays indexed by tensor id)."""
+        lt, _, row, col = self.global_of(dev, kind)
+        dt = np.uint16 if self.elem_bytes(kind) == 2 else np.uint32
+        out = np.zeros(lt.shape[0], dt)
+        for t in np.unique(lt):
+            sel = lt == t
+            out[sel] = logical[t][row[sel], col[sel]]
+        return out
+
+
+def P_of(old: Layout, new: Layout) -> int:
+    return max(old.n_dev, new.n_dev)
+
+
+def overlap(old: Layout, new: Layout, only_layers: bool = False, method: str = "elementwise"):
+    """(overlap[n_new][P], need[n_new], hold[P]) in bytes."""
+    P = P_of(old, new)
+    ov = np.zeros((new.n_dev, P), np.int64); need = np.zeros(new.n_dev, np.int64); hold = np.zeros(P, np.int64)
+    if method == "elementwise":
+        rc = lib().orc_overlap_elementwise(old.h, new.h, int(only_layers), _ptr(ov), _ptr(need), _ptr(hold))
+    else:
+        assert not only_layers
+        rc = lib().orc_overlap_ranges(old.h, new.h, _ptr(ov), _ptr(need), _ptr(hold))
+    if rc:
+        raise OracleError(rc)
+    return ov, need, hold
+
+
+def sketch_bruteforce(ov: np.ndarray, avail=None):
+    ov = np.ascontiguousarray(ov, np.int64)
+    n, P = ov.shape
+    m = np.zeros(n, np.int32); val = C.c_int64()
+    av = None if avail is None else np.ascontiguousarray(avail, np.uint8)
+    cnt = lib().orc_sketch_bruteforce(_ptr(ov), n, P, _ptr(av), _ptr(m), C.byref(val))
+    return m, int(val.value), int(cnt)
+
+
+def sketch_hungarian(ov: np.ndarray, avail=None):
+    ov = np.ascontiguousarray(ov, np.int64)
+    n, P = ov.shape
+    m = np.zeros(n, np.int32); val = C.c_int64()
+    av = None if avail is None else np.ascontiguousarray(avail, np.uint8)
+    rc = lib().orc_sketch_hungarian(_ptr(ov), n, P, _ptr(av), _ptr(m), C.byref(val))
+    if rc:
+        raise OracleError(rc)
+    return m, int(val.value)
+
+
+def source_of(old: Layout, new: Layout, device_map, n, kind, l_list):
+    dm = np.ascontiguousarray(device_map, np.int32)
+    ll = np.ascontiguousarray(l_list, np.int64)
+    sd = np.zeros(ll.shape[0], np.int32); sl = np.zeros(ll.shape[0], np.int64)
+    rc = lib().orc_source_of(old.h, new.h, _ptr(dm), n, kind, _ptr(ll), ll.shape[0], _ptr(sd), _ptr(sl))
+    if rc:
+        raise OracleError(rc)
+    return sd, sl
+
+
+def _ptr_table(bufs, n_dev):
+    tab = (C.c_void_p * (n_dev * 4))()
+    for (dev, kind), a in bufs.items():
+        tab[dev * 4 + kind] = a.ctypes.data
+    return tab
+
+
+def migrate(old: Layout, new: Layout, device_map, src_bufs: dict | None, want_overrides=False):
+    """Element-wise migration.  src_bufs: {(old_dev, kind): 1-D uint16/uint32 array} or None (traffic only).
+    Returns (dst_bufs {(n, kind): array} or None, T[P][P], overrides)."""
+    P = P_of(old, new)
+    dm = np.ascontiguousarray(device_map, np.int32)
+    T = np.zeros((P, P), np.int64); ovr = C.c_int64(0)
+    dst = None; st = None; dt = None
+    if src_bufs is not None:
+        st = _ptr_table(src_bufs, old.n_dev)
+        dst = {}
+        for n in range(new.n_dev):
+            for k in new.kinds():
+                cnt = new.buffer_elems(n, k)
+                dst[(n, k)] = np.zeros(cnt, np.uint16 if new.elem_bytes(k) == 2 else np.uint32)
+        dt = _ptr_table(dst, new.n_dev)
+    rc = lib().orc_migrate(old.h, new.h, _ptr(dm), st, dt, _ptr(T), C.byref(ovr) if want_overrides else None)
+    if rc:
+        raise OracleError(rc)
+    return dst, T, int(ovr.value)
+
+
+def migrate_range(old: Layout, new: Layout, device_map, n, kind, l0, l1, src_bufs: dict | None, dst=None,
+                  T=None, written=None):
+    dm = np.ascontiguousarray(device_map, np.int32)
+    st = _ptr_table(src_bufs, old.n_dev) if src_bufs is not None else None
+    rc = lib().orc_migrate_range(old.h, new.h, _ptr(dm), n, kind, l0, l1, st, _ptr(dst), _ptr(T), None, _ptr(written))
+    if rc:
+        raise OracleError(rc)

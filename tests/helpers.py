@@ -1,0 +1,78 @@
+"""Test helpers that use ONLY the oracle and the seeded input generators (never the CUDA path)."""
+from __future__ import annotations
+import os
+import numpy as np
+from etc_inputs import logical_values, index_stamp, position_stamp
+from oracle import oracle as O
+
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def read_golden(name):
+    rows = []
+    with open(os.path.join(GOLDEN, name)) as f:
+        for line in f:
+            line = line.split("#")[0].strip()
+            if line:
+                rows.append(line.split())
+    return rows
+
+
+def make_logical(model: dict, seed: int, payload: str = "values"):
+    """{kind: [2-D array per logical tensor]} in logical space (uint16 / uint32 bit patterns)."""
+    lts = O.logical_tensors(model)
+    out = {}
+    for k in range(4):
+        if not (model["kinds"] >> k) & 1:
+            continue
+        es = O.kind_bytes(model, k)
+        arrs = []
+        for t, (rows, cols, *_r) in enumerate(lts):
+            n = rows * cols
+            v = logical_values(seed, k, t, n, es) if payload == "values" else index_stamp(k, t, n, es)
+            arrs.append(v.reshape(rows, cols))
+        out[k] = arrs
+    return out
+
+
+def shard_all(layout: O.Layout, logical: dict):
+    """{(dev, kind): 1-D array} — the oracle cuts every buffer out of the logical tensors."""
+    return {(d, k): layout.shard_from_logical(d, k, logical[k]) for d in range(layout.n_dev) for k in layout.kinds()}
+
+
+def stamp_all(layout: O.Layout):
+    """{(dev, kind): position-stamped 1-D array} (pin P9: values name the buffer and position they came from)."""
+    return {(d, k): position_stamp(d, k, layout.buffer_elems(d, k), layout.elem_bytes(k))
+            for d in range(layout.n_dev) for k in layout.kinds()}
+
+
+def reassemble(layout: O.Layout, bufs: dict, logical_like: dict):
+    """Rebuild every logical tensor from shard buffers.  Returns (rebuilt {kind: [arrays]}, cover {kind: [counts]},
+    consistent: bool) — cover counts how many buffers held each element; consistent is False if replicas differ."""
+    rebuilt = {k: [np.zeros_like(a) for a in v] for k, v in logical_like.items()}
+    cover = {k: [np.zeros(a.shape, np.int32) for a in v] for k, v in logical_like.items()}
+    consistent = True
+    for (d, k), buf in bufs.items():
+        if buf.shape[0] == 0:
+            continue
+        lt, _, row, col = layout.global_of(d, k)
+        for t in np.unique(lt):
+            sel = lt == t
+            r, c = row[sel], col[sel]
+            seen = cover[k][t][r, c] > 0
+            if seen.any() and not np.array_equal(rebuilt[k][t][r[seen], c[seen]], buf[sel][seen]):
+                consistent = False
+            rebuilt[k][t][r, c] = buf[sel]
+            np.add.at(cover[k][t], (r, c), 1)
+    return rebuilt, cover, consistent
+
+
+def replication_factor(layout: O.Layout, kind: int, split: int, t: int) -> int:
+    """R(t) of pin P3: how many buffers hold each element of tensor t of this kind."""
+    c, m = layout.cfg, layout.model
+    f = c["tp"] if split == 0 else 1
+    dp_sharded = c.get("dist_opt", 0) and c["dp"] > 1 and kind >= 1
+    f *= 1 if dp_sharded else c["dp"]
+    if m["tied"] and c["pp"] > 1 and t == 0:
+        f *= 2
+    return f
