@@ -1,0 +1,162 @@
+/*
+ * etc.h — C ABI of libetc.so: the data-parallel hot path of ETC's checkpoint-free model-state migration
+ * (arxiv/paper_2607_04749, "ETC"; citations below are PAPER.md line numbers and DESIGN.md readings A1-A24).
+ *
+ * The paper's primitive takes the previous parallel configuration, the current one and the model state, and
+ * returns the migrated state.  Here that is four steps, each a call:
+ *
+ *   etc_layout_create   (a1)  (model_desc, parallel_cfg) -> index rectangles of every state tensor on every device
+ *                             (PAPER.md:106 workload abstraction, :110 "each device can derive its workload following
+ *                             these rules", :199 TP slices)
+ *   etc_cost_matrix     (a2)  old x new index-range intersection -> overlap / need / hold, the paper's cost matrix is
+ *                             c[n][o] = need[n] - overlap[n][o]  (worked example :108)
+ *   etc_sketch          (a3)  device-side assignment search -> device_map (Eq. 1-4, Algorithm 1)
+ *   etc_plan_create     (a4)  Send/Recv/Refer instruction lists as a slice table, coalesced per (src,dst) pair
+ *
+ *   etc_migrate      (a5,a6)  pack -> staging -> unpack, plus direct copies of what stays on its device
+ *                             ("packed to the instructions when Send and then unpacked")
+ *
+ * All virtual devices' shard buffers live in ONE GPU's memory; the interconnect hop between pack and unpack is the
+ * identity (unpack reads the staging buffer pack wrote).  Every step runs in CUDA kernels for sm_100a; there is no CPU
+ * fallback: without a CUDA device every compute entry point returns ETC_ERR_CUDA.
+ *
+ * Conventions
+ *  - Plain C types only.  "device pointer" = CUDA device memory of the current device; "host pointer" = ordinary memory.
+ *  - `stream` is a cudaStream_t passed as void* (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream.
+ *  - Ownership: the caller owns every data buffer, the staging buffer and the output matrices.  The library owns only
+ *    etc_layout / etc_plan objects (and their device-side tables), released by the matching destroy call.
+ *  - Errors: a negative etc_status; nothing is written to the outputs on error.  etc_last_error_detail() returns a
+ *    static/thread-local string with the CUDA error text after ETC_ERR_CUDA.
+ *  - Old logical rank j sits on physical device j; new logical rank n is placed on physical device
+ *    device_map[n]; P = max(n_old, n_new) physical devices exist.
+ *  - Device id = r + tp*(d + dp*s) for TP rank r, DP rank d, PP stage s (reading A9).
+ */
+#ifndef ETC_H_
+#define ETC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef int32_t etc_status;
+enum {
+  ETC_OK = 0,
+  ETC_ERR_INVALID_ARG = -1,  /* null pointer, non-positive size, unknown enum, misaligned buffer */
+  ETC_ERR_INDIVISIBLE = -2,  /* n_layers % pp, n_kv_heads % tp, ffn_hidden % tp or vocab % tp != 0 */
+  ETC_ERR_MISMATCH = -3,     /* old and new layouts describe different models / kinds */
+  ETC_ERR_BAD_MAP = -4,      /* device_map not injective or out of [0,P) */
+  ETC_ERR_WORKSPACE = -5,    /* problem larger than the kernel's on-chip workspace (sketch: P > ETC_SKETCH_MAX_P) */
+  ETC_ERR_UNSUPPORTED = -6,  /* tp > n_kv_heads (KV-head replication, reading A10) */
+  ETC_ERR_CUDA = -7          /* a CUDA call failed, or no CUDA device */
+};
+
+enum { ETC_GPT = 0, ETC_LLAMA = 1 };                 /* etc_model_desc.style */
+enum { ETC_BF16 = 2, ETC_FP32 = 4 };                 /* etc_model_desc.param_dtype = element size in bytes */
+enum { ETC_K_PARAM = 1, ETC_K_MASTER = 2, ETC_K_ADAM_M = 4, ETC_K_ADAM_V = 8 };   /* kinds bitmask; kind index 0..3 */
+#define ETC_NUM_KINDS 4
+#define ETC_SKETCH_MAX_P 2048
+
+/* Logical model: the tensors a TP=PP=DP=1 run would hold (table of tensors and split types).
+ * ETC_GPT: LayerNorm weight+bias, linear biases, learned position embeddings; ETC_LLAMA: RMSNorm, no bias, SwiGLU. */
+typedef struct {
+  int32_t style;
+  int32_t n_layers, hidden, n_q_heads, n_kv_heads, head_dim, ffn_hidden, vocab, max_pos;
+  int32_t tied_embeddings;   /* 1: the output layer shares word_embeddings (replica on the last PP stage if pp > 1) */
+  int32_t param_dtype;       /* ETC_BF16 | ETC_FP32: element size of kind PARAM; MASTER / ADAM_M / ADAM_V are fp32 */
+  int32_t kinds;             /* bitmask of state kinds present */
+} etc_model_desc;
+
+/* Megatron-style parallel configuration.  dist_opt = 1: MASTER/ADAM_M/ADAM_V are sharded over DP as
+ * contiguous flat ranges of each (stage, tp-rank) local parameter space (reading A14); PARAM stays replicated. */
+typedef struct { int32_t tp, pp, dp, dist_opt; } etc_parallel_cfg;
+
+typedef struct etc_layout etc_layout;   /* opaque, immutable after create */
+typedef struct etc_plan etc_plan;       /* opaque, immutable after create */
+
+/* Select the CUDA device the library works on (default 0).  Call once per process before anything else. */
+etc_status etc_init(int32_t cuda_device);
+
+/* (a1) Build the layout descriptor on the host and upload its piece tables.  *out is written only on success. */
+etc_status etc_layout_create(const etc_model_desc* model, const etc_parallel_cfg* cfg, etc_layout** out);
+void etc_layout_destroy(etc_layout* layout);
+int32_t etc_layout_num_devices(const etc_layout* layout);                         /* tp*pp*dp */
+int64_t etc_layout_num_pieces(const etc_layout* layout);                          /* index rectangles in the table */
+/* bytes of the buffer of state kind `kind` (0..3) on device `dev`; 0 if the kind is absent; <0 on bad arguments */
+int64_t etc_layout_buffer_bytes(const etc_layout* layout, int32_t dev, int32_t kind);
+
+/* (a2) Cost matrix.  Device outputs, all int64:
+ *   d_overlap [n_new][P] row-major: bytes held both by new rank n and by old device o (0 for o >= n_old)
+ *   d_need    [n_new]: bytes new rank n needs;  d_hold [P]: bytes old device o holds (0 for o >= n_old)
+ * Rows = curr ranks, columns = prev ranks, as in the paper (reading A1).  Enqueues on `stream`. */
+etc_status etc_cost_matrix(const etc_layout* old_l, const etc_layout* new_l,
+                           int64_t* d_overlap, int64_t* d_need, int64_t* d_hold, void* stream);
+
+/* (a3) Migration sketch: device_map = argmax over injective maps pi:[0,n_new)->[0,P) of sum_n overlap[n][pi(n)]
+ * (= Eq. 2's minimisation under Eq. 3/4, reading A4).  d_avail: optional device mask [P] (0 = device may not be
+ * used, e.g. pre-empted; NULL = all usable).  method: ETC_SKETCH_AUTO picks exhaustive search for P <= 8, else the
+ * shortest-augmenting-path Hungarian.  Outputs (device memory): d_device_map [n_new] int32, d_local_bytes [1] int64 =
+ * the achieved objective.  If no feasible map exists both are filled with -1.  Enqueues on `stream`. */
+enum { ETC_SKETCH_AUTO = 0, ETC_SKETCH_EXHAUSTIVE = 1, ETC_SKETCH_HUNGARIAN = 2 };
+etc_status etc_sketch(const int64_t* d_overlap, int32_t n_new, int32_t P, const uint8_t* d_avail, int32_t method,
+                      int32_t* d_device_map, int64_t* d_local_bytes, void* stream);
+
+/* (a4) Plan.  device_map: [n_new] int32, host OR device pointer.  flags: ETC_LOCAL_DIRECT (slices whose source device
+ * is the destination device are copied old buffer -> new buffer, never staged: the paper's Refer, reading A19) or
+ * ETC_ALL_STAGED (every slice goes through pack/unpack: a measurement mode).  Synchronises `stream` once (sizes must
+ * come back to the host).  Fails with ETC_ERR_BAD_MAP if the map is not injective into [0,P). */
+enum { ETC_LOCAL_DIRECT = 0, ETC_ALL_STAGED = 1 };
+etc_status etc_plan_create(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
+                           int32_t flags, etc_plan** out, void* stream);
+void etc_plan_destroy(etc_plan* plan);
+
+typedef struct {
+  int64_t staging_bytes;   /* size the caller must allocate for `staging` (payload + alignment padding) */
+  int64_t local_bytes;     /* payload bytes whose source device is their destination device */
+  int64_t remote_bytes;    /* payload bytes that change device (sum of off-diagonal traffic) */
+  int64_t staged_bytes;    /* payload bytes that go through pack/unpack (= remote_bytes, or all bytes if ALL_STAGED) */
+  int64_t n_slices_local, n_slices_staged;   /* 2-D strided copy descriptors */
+  int64_t n_chunks_local, n_chunks_staged;   /* copy work items (<= ETC_CHUNK_BYTES each) */
+  int32_t n_old, n_new, P, flags;
+} etc_plan_stats;
+etc_status etc_plan_get_stats(const etc_plan* plan, etc_plan_stats* out);
+/* traffic matrix T [P][P] row-major, int64, copied to HOST memory: T[o][p] = payload bytes whose source is old device
+ * o and whose destination is physical device p (diagonal = local bytes).  Synchronous. */
+etc_status etc_plan_get_traffic(const etc_plan* plan, int64_t* h_traffic);
+
+/* One slice = one 2-D strided copy (rows x row_bytes).  For tests / inspection; copied to HOST memory.
+ * which = 0: staged slices, 1: local slices.  h_out must hold n_slices_* entries. */
+typedef struct {
+  int64_t src_off, dst_off, stg_off;          /* byte offsets inside src buffer, dst buffer, staging buffer (-1: none) */
+  int64_t row_bytes;                          /* contiguous bytes per row */
+  int32_t src_stride, dst_stride;             /* row pitch in bytes on each side (in staging the pitch is row_bytes) */
+  int32_t nrows;
+  int32_t src_dev, dst_rank, dst_phys, kind;  /* src buffer = src_bufs[src_dev*4+kind], dst = dst_bufs[dst_rank*4+kind] */
+  int32_t pad;
+} etc_slice;
+etc_status etc_plan_get_slices(const etc_plan* plan, int32_t which, etc_slice* h_out);
+
+/* (a5,a6) Migrate.  src_bufs[old_dev*4 + kind], dst_bufs[new_rank*4 + kind]: HOST arrays of DEVICE pointers (NULL
+ * where the buffer has 0 bytes), each 16-byte aligned and at least etc_layout_buffer_bytes() long.  staging: device
+ * pointer, >= staging_bytes (may be NULL if staging_bytes == 0).  Enqueues on `stream`:
+ *   ETC_PHASE_PACK   : pack staged slices old buffers -> staging, and copy local slices old -> new directly
+ *   ETC_PHASE_UNPACK : unpack staged slices staging -> new buffers
+ * etc_migrate runs both phases.  No allocation, no host synchronisation.  Every destination byte is written exactly
+ * once. */
+enum { ETC_PHASE_PACK = 1, ETC_PHASE_UNPACK = 2, ETC_PHASE_ALL = 3 };
+etc_status etc_migrate(const etc_plan* plan, const void* const* src_bufs, void* const* dst_bufs,
+                       void* staging, void* stream);
+etc_status etc_migrate_phase(const etc_plan* plan, const void* const* src_bufs, void* const* dst_bufs,
+                             void* staging, int32_t phases, void* stream);
+
+#define ETC_CHUNK_BYTES 65536
+
+const char* etc_status_string(etc_status s);   /* static strings */
+const char* etc_last_error_detail(void);       /* thread-local; CUDA error text after ETC_ERR_CUDA, else "" */
+int64_t etc_kernel_launches(void);             /* number of kernels this library has launched in this process */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ETC_H_ */

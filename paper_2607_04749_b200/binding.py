@@ -1,0 +1,296 @@
+"""ctypes binding of libetc.so (include/etc.h).  Same names as the C ABI; argument marshalling only.
+
+torch is used for device memory and streams, nothing else: every step of the path runs in the library's kernels.
+"""
+from __future__ import annotations
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libetc.so")
+_lib = None
+_inited = False
+
+ETC_LOCAL_DIRECT, ETC_ALL_STAGED = 0, 1
+ETC_SKETCH_AUTO, ETC_SKETCH_EXHAUSTIVE, ETC_SKETCH_HUNGARIAN = 0, 1, 2
+ETC_PHASE_PACK, ETC_PHASE_UNPACK, ETC_PHASE_ALL = 1, 2, 3
+
+EXPORTED_SYMBOLS = (
+    "etc_init", "etc_layout_create", "etc_layout_destroy", "etc_layout_num_devices", "etc_layout_num_pieces",
+    "etc_layout_buffer_bytes", "etc_cost_matrix", "etc_sketch", "etc_plan_create", "etc_plan_destroy",
+    "etc_plan_get_stats", "etc_plan_get_traffic", "etc_plan_get_slices", "etc_migrate", "etc_migrate_phase",
+    "etc_status_string", "etc_last_error_detail", "etc_kernel_launches",
+)
+
+
+class EtcError(RuntimeError):
+    def __init__(self, code, detail=""):
+        name = lib().etc_status_string(code).decode() if _lib is not None else str(code)
+        super().__init__(f"{name} ({code}){': ' + detail if detail else ''}")
+        self.code = code
+
+
+class _ModelDesc(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("style", "n_layers", "hidden", "n_q_heads", "n_kv_heads", "head_dim",
+                                          "ffn_hidden", "vocab", "max_pos", "tied_embeddings", "param_dtype", "kinds")]
+
+
+class _ParallelCfg(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("tp", "pp", "dp", "dist_opt")]
+
+
+class _PlanStats(C.Structure):
+    _fields_ = [(n, C.c_int64) for n in ("staging_bytes", "local_bytes", "remote_bytes", "staged_bytes",
+                                          "n_slices_local", "n_slices_staged", "n_chunks_local", "n_chunks_staged")] + \
+               [(n, C.c_int32) for n in ("n_old", "n_new", "P", "flags")]
+
+
+class _Slice(C.Structure):
+    _fields_ = [("src_off", C.c_int64), ("dst_off", C.c_int64), ("stg_off", C.c_int64), ("row_bytes", C.c_int64),
+                ("src_stride", C.c_int32), ("dst_stride", C.c_int32), ("nrows", C.c_int32),
+                ("src_dev", C.c_int32), ("dst_rank", C.c_int32), ("dst_phys", C.c_int32), ("kind", C.c_int32),
+                ("pad", C.c_int32)]
+
+
+def lib():
+    """Load libetc.so; fail loudly if it is missing (there is no fallback path)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise RuntimeError(f"{_LIB_PATH} not found: build it with `python -m paper_2607_04749_b200._build` "
+                               "(or __graft_entry__.build()); there is no CPU fallback")
+        L = C.CDLL(_LIB_PATH)
+        vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+        L.etc_init.restype = i32; L.etc_init.argtypes = [i32]
+        L.etc_layout_create.restype = i32
+        L.etc_layout_create.argtypes = [C.POINTER(_ModelDesc), C.POINTER(_ParallelCfg), C.POINTER(vp)]
+        L.etc_layout_destroy.restype = None; L.etc_layout_destroy.argtypes = [vp]
+        L.etc_layout_num_devices.restype = i32; L.etc_layout_num_devices.argtypes = [vp]
+        L.etc_layout_num_pieces.restype = i64; L.etc_layout_num_pieces.argtypes = [vp]
+        L.etc_layout_buffer_bytes.restype = i64; L.etc_layout_buffer_bytes.argtypes = [vp, i32, i32]
+        L.etc_cost_matrix.restype = i32; L.etc_cost_matrix.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.etc_sketch.restype = i32; L.etc_sketch.argtypes = [vp, i32, i32, vp, i32, vp, vp, vp]
+        L.etc_plan_create.restype = i32; L.etc_plan_create.argtypes = [vp, vp, vp, i32, C.POINTER(vp), vp]
+        L.etc_plan_destroy.restype = None; L.etc_plan_destroy.argtypes = [vp]
+        L.etc_plan_get_stats.restype = i32; L.etc_plan_get_stats.argtypes = [vp, C.POINTER(_PlanStats)]
+        L.etc_plan_get_traffic.restype = i32; L.etc_plan_get_traffic.argtypes = [vp, vp]
+        L.etc_plan_get_slices.restype = i32; L.etc_plan_get_slices.argtypes = [vp, i32, vp]
+        L.etc_migrate.restype = i32; L.etc_migrate.argtypes = [vp, vp, vp, vp, vp]
+        L.etc_migrate_phase.restype = i32; L.etc_migrate_phase.argtypes = [vp, vp, vp, vp, i32, vp]
+        L.etc_status_string.restype = C.c_char_p; L.etc_status_string.argtypes = [i32]
+        L.etc_last_error_detail.restype = C.c_char_p
+        L.etc_kernel_launches.restype = i64
+        _lib = L
+    return _lib
+
+
+def _check(code):
+    if code != 0:
+        raise EtcError(code, lib().etc_last_error_detail().decode())
+
+
+def init(device: int | None = None):
+    """Bind the library to a CUDA device (default: torch's current device).  Raises without a GPU."""
+    global _inited
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2607_04749_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
+    if device is None:
+        device = torch.cuda.current_device()
+    torch.cuda.init()
+    _check(lib().etc_init(int(device)))
+    _inited = True
+
+
+def _ensure_init():
+    if not _inited:
+        init()
+
+
+def _stream(stream=None) -> int:
+    import torch
+    return (stream or torch.cuda.current_stream()).cuda_stream
+
+
+def kernel_launches() -> int:
+    return int(lib().etc_kernel_launches())
+
+
+class Layout:
+    """Handle of an etc_layout (immutable)."""
+
+    def __init__(self, handle, model, cfg):
+        self.h, self.model, self.cfg = handle, dict(model), dict(cfg)
+        self.n_dev = int(lib().etc_layout_num_devices(handle))
+        self.n_pieces = int(lib().etc_layout_num_pieces(handle))
+
+    def buffer_bytes(self, dev: int, kind: int) -> int:
+        return int(lib().etc_layout_buffer_bytes(self.h, dev, kind))
+
+    def kinds(self):
+        return [k for k in range(4) if (self.model["kinds"] >> k) & 1]
+
+    def total_bytes(self) -> int:
+        return sum(self.buffer_bytes(d, k) for d in range(self.n_dev) for k in range(4))
+
+    def __del__(self):
+        if getattr(self, "h", None) and _lib is not None:
+            _lib.etc_layout_destroy(self.h)
+            self.h = None
+
+
+def etc_layout_create(model: dict, cfg: dict) -> Layout:
+    """(a1) include/etc.h etc_layout_create.  model: etc_inputs workload["model"] dict; cfg: {"tp","pp","dp","dist_opt"}."""
+    _ensure_init()
+    m = _ModelDesc(style=model["style"], n_layers=model["n_layers"], hidden=model["hidden"],
+                   n_q_heads=model["n_q_heads"], n_kv_heads=model["n_kv_heads"], head_dim=model["head_dim"],
+                   ffn_hidden=model["ffn_hidden"], vocab=model["vocab"], max_pos=model["max_pos"],
+                   tied_embeddings=model["tied"], param_dtype=model["param_bytes"], kinds=model["kinds"])
+    c = _ParallelCfg(tp=cfg["tp"], pp=cfg["pp"], dp=cfg["dp"], dist_opt=cfg.get("dist_opt", 0))
+    h = C.c_void_p()
+    _check(lib().etc_layout_create(C.byref(m), C.byref(c), C.byref(h)))
+    return Layout(h, model, cfg)
+
+
+def etc_cost_matrix(old: Layout, new: Layout, stream=None, out=None):
+    """(a2) -> (overlap [n_new][P], need [n_new], hold [P]) int64 CUDA tensors.  Asynchronous."""
+    import torch
+    P = max(old.n_dev, new.n_dev)
+    if out is None:
+        dev = torch.device("cuda", torch.cuda.current_device())
+        out = (torch.empty((new.n_dev, P), dtype=torch.int64, device=dev),
+               torch.empty(new.n_dev, dtype=torch.int64, device=dev), torch.empty(P, dtype=torch.int64, device=dev))
+    ov, need, hold = out
+    _check(lib().etc_cost_matrix(old.h, new.h, ov.data_ptr(), need.data_ptr(), hold.data_ptr(), _stream(stream)))
+    return ov, need, hold
+
+
+def etc_sketch(overlap, avail=None, method: int = ETC_SKETCH_AUTO, stream=None, out=None):
+    """(a3) -> (device_map [n_new] int32, local_bytes [1] int64) CUDA tensors.  Asynchronous."""
+    import torch
+    _ensure_init()
+    n_new, P = overlap.shape
+    assert overlap.is_cuda and overlap.dtype == torch.int64 and overlap.is_contiguous()
+    if out is None:
+        out = (torch.empty(n_new, dtype=torch.int32, device=overlap.device),
+               torch.empty(1, dtype=torch.int64, device=overlap.device))
+    dm, lb = out
+    av = 0
+    if avail is not None:
+        assert avail.is_cuda and avail.dtype == torch.uint8 and avail.numel() == P
+        av = avail.data_ptr()
+    _check(lib().etc_sketch(overlap.data_ptr(), n_new, P, av, method, dm.data_ptr(), lb.data_ptr(), _stream(stream)))
+    return dm, lb
+
+
+@dataclass
+class PlanStats:
+    staging_bytes: int
+    local_bytes: int
+    remote_bytes: int
+    staged_bytes: int
+    n_slices_local: int
+    n_slices_staged: int
+    n_chunks_local: int
+    n_chunks_staged: int
+    n_old: int
+    n_new: int
+    P: int
+    flags: int
+
+    @property
+    def hbm_bytes(self) -> int:
+        """Algorithmic HBM traffic of one etc_migrate: 1R+1W per local byte, 2R+2W per staged byte."""
+        direct = self.local_bytes + self.remote_bytes - self.staged_bytes
+        return 2 * direct + 4 * self.staged_bytes
+
+
+class Plan:
+    def __init__(self, handle):
+        self.h = handle
+        s = _PlanStats()
+        _check(lib().etc_plan_get_stats(handle, C.byref(s)))
+        self.stats = PlanStats(**{n: int(getattr(s, n)) for n, _ in _PlanStats._fields_})
+
+    def traffic(self):
+        import numpy as np
+        P = self.stats.P
+        T = np.zeros((P, P), np.int64)
+        _check(lib().etc_plan_get_traffic(self.h, T.ctypes.data))
+        return T
+
+    def slices(self, which: int):
+        """which = 0 staged, 1 local -> numpy structured array of etc_slice records."""
+        import numpy as np
+        n = self.stats.n_slices_staged if which == 0 else self.stats.n_slices_local
+        dt = np.dtype([(f, np.int64 if t is C.c_int64 else np.int32) for f, t in _Slice._fields_], align=True)
+        assert dt.itemsize == C.sizeof(_Slice)
+        arr = np.zeros(max(n, 1), dt)
+        _check(lib().etc_plan_get_slices(self.h, which, arr.ctypes.data))
+        return arr[:n]
+
+    def __del__(self):
+        if getattr(self, "h", None) and _lib is not None:
+            _lib.etc_plan_destroy(self.h)
+            self.h = None
+
+
+def etc_plan_create(old: Layout, new: Layout, device_map, flags: int = ETC_LOCAL_DIRECT, stream=None) -> Plan:
+    """(a4) device_map: CUDA int32 tensor (e.g. from etc_sketch) or a host sequence.  Synchronises the stream once."""
+    import numpy as np
+    import torch
+    if isinstance(device_map, torch.Tensor):
+        assert device_map.dtype == torch.int32 and device_map.numel() == new.n_dev and device_map.is_contiguous()
+        keep = device_map
+        ptr = device_map.data_ptr()
+    else:
+        keep = np.ascontiguousarray(device_map, np.int32)
+        assert keep.shape == (new.n_dev,)
+        ptr = keep.ctypes.data
+    h = C.c_void_p()
+    _check(lib().etc_plan_create(old.h, new.h, ptr, flags, C.byref(h), _stream(stream)))
+    del keep
+    return Plan(h)
+
+
+def _ptr_table(bufs, n_dev):
+    tab = (C.c_void_p * (n_dev * 4))()
+    for (dev, kind), t in bufs.items():
+        if t is not None and t.numel() > 0:
+            tab[dev * 4 + kind] = t.data_ptr()
+    return tab
+
+
+def etc_migrate(plan: Plan, src_bufs: dict, dst_bufs: dict, staging, phases: int = ETC_PHASE_ALL, stream=None):
+    """(a5,a6) src_bufs {(old_dev, kind): CUDA tensor}, dst_bufs {(new_rank, kind): CUDA tensor}, staging: CUDA tensor
+    of at least plan.stats.staging_bytes bytes (or None).  Asynchronous; no allocation."""
+    st = plan.stats
+    if isinstance(src_bufs, dict):
+        src_bufs = _ptr_table(src_bufs, st.n_old)
+    if isinstance(dst_bufs, dict):
+        dst_bufs = _ptr_table(dst_bufs, st.n_new)
+    sp = 0
+    if staging is not None and staging.numel() > 0:
+        assert staging.numel() * staging.element_size() >= st.staging_bytes
+        sp = staging.data_ptr()
+    _check(lib().etc_migrate_phase(plan.h, src_bufs, dst_bufs, sp, phases, _stream(stream)))
+
+
+def pointer_tables(plan: Plan, src_bufs: dict, dst_bufs: dict):
+    """Pre-marshalled pointer tables (avoids rebuilding them on every etc_migrate call)."""
+    return _ptr_table(src_bufs, plan.stats.n_old), _ptr_table(dst_bufs, plan.stats.n_new)
+
+
+def alloc_buffers(layout: Layout, device=None, fill=None):
+    """{(dev, kind): uint8 CUDA tensor of etc_layout_buffer_bytes} for every non-empty buffer."""
+    import torch
+    device = device or torch.device("cuda", torch.cuda.current_device())
+    out = {}
+    for d in range(layout.n_dev):
+        for k in range(4):
+            n = layout.buffer_bytes(d, k)
+            if n > 0:
+                out[(d, k)] = torch.empty(n, dtype=torch.uint8, device=device) if fill is None else \
+                    torch.full((n,), fill, dtype=torch.uint8, device=device)
+    return out

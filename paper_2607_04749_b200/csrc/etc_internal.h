@@ -1,0 +1,73 @@
+// etc_internal.h — structures shared by the host layout builder and the CUDA kernels of libetc.so.
+// Nothing here is shared with oracle/ (the CPU oracle is written separately from the paper).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+#include "../../include/etc.h"
+
+namespace etc {
+
+// Split type of a logical tensor (PAPER.md:199 replaced by an explicit type, reading A8).
+enum Split : int32_t { REPL = 0, COL = 1, ROW = 2, COL2 = 3 };
+
+// Piece flags
+enum : uint16_t {
+  PF_POST_COPY = 1,   // tied word_embeddings replica held by the last PP stage (reading A11)
+  PF_SOLE_INST = 2,   // the tensor is held by exactly one PP stage in this layout
+  PF_TP_SHARDED = 4,  // split != REPL: exactly one TP rank holds each element
+  PF_DP_SHARDED = 8,  // kind is sharded over DP (distributed optimizer, reading A14)
+};
+
+// One index rectangle [r0,r0+nr) x [c0,c0+nc) of a logical tensor held in the buffer of (dev, kind).
+// Local (shard) coordinates: element (r0,c0) is element (lrow0, lcol0) of the TP shard, whose row length is W.
+// [f0,f1) is the flat range of the SHARD (shard-relative, in elements) that this buffer holds; all pieces of one
+// (dev, group) carry the same [f0,f1).
+struct Piece {
+  int32_t dev;        // logical device / rank in this layout
+  int32_t grp;        // kind * n_tensors + logical tensor id
+  int32_t r0, nr, c0, nc;
+  int32_t lrow0, lcol0;
+  int32_t W;          // row pitch in elements inside the buffer
+  int16_t s, r, d;    // PP stage, TP rank, DP rank of dev
+  uint16_t flags;
+  int64_t boff;       // byte offset of element (r0,c0) inside the buffer of (dev, kind)
+  int64_t f0, f1;
+};
+static_assert(sizeof(Piece) == 72, "Piece layout");
+
+struct DeviceTables {            // device memory
+  const Piece* pieces;           // sorted by (dev, grp, local order)
+  const int32_t* dev_start;      // [n_dev + 1]
+  const int32_t* first;          // [n_dev][n_grp]: index of the first piece of (dev, grp) or -1
+  const uint32_t* ltmask;        // [n_dev][mask_words]: bit t set if dev holds any piece of logical tensor t
+  int32_t n_dev, n_grp, n_tensors, mask_words;
+  int32_t n_pieces;
+  int32_t tp, pp, dp;
+  int32_t elem_bytes[ETC_NUM_KINDS];
+};
+
+}  // namespace etc
+
+struct etc_layout {
+  etc_model_desc model;
+  etc_parallel_cfg cfg;
+  etc::DeviceTables t;                    // device pointers + sizes
+  int64_t* h_buffer_bytes = nullptr;      // [n_dev][4] host
+  void* d_blob = nullptr;                 // one allocation holding all device tables
+};
+
+// ---- error plumbing
+namespace etc {
+void set_error_detail(const char* what, cudaError_t e);
+void clear_error_detail();
+void count_launch(int n = 1);
+int current_device();
+}
+#define ETC_CUDA_TRY(expr)                                          \
+  do {                                                              \
+    cudaError_t _e = (expr);                                        \
+    if (_e != cudaSuccess) {                                        \
+      etc::set_error_detail(#expr, _e);                             \
+      return ETC_ERR_CUDA;                                          \
+    }                                                               \
+  } while (0)

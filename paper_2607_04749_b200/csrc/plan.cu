@@ -1,0 +1,444 @@
+// plan.cu — (a4) plan: turn (old layout, new layout, device_map) into the instruction lists of PAPER.md:193-201 as a
+// table of 2-D strided copies ("slices"):
+//   Refer  (workload in both prev and curr process)  -> local slice, old buffer -> new buffer on the same device
+//   Send / Recv (workload moves)                      -> staged slice, packed into the contiguous segment of its
+//                                                        (source, destination) pair — message coalescing
+// Source of every needed element (reading A6): local first, else the designated holder.
+//
+// One warp owns one (source device od, new rank n) unit, i.e. one cell of the traffic matrix and one pair segment.
+// Pass 1 counts slices / chunks / bytes per unit; a single-CTA scan turns the counts into slice indices, chunk indices
+// and segment offsets (warp-shuffle prefix sums); pass 2 recomputes the slices and writes them at their final
+// positions.  Order inside a segment is canonical (piece order), so the staging layout is deterministic.
+#include <cstring>
+#include <vector>
+#include "etc_internal.h"
+#include "plan_types.h"
+
+bool etc_same_model(const etc_layout* a, const etc_layout* b);
+
+namespace etc {
+
+struct Rect { int32_t r0, nr, c0, nc; };
+
+__device__ __forceinline__ bool rect_isect(const Piece& a, const Piece& b, Rect& out) {
+  const int r0 = max(a.r0, b.r0), r1 = min(a.r0 + a.nr, b.r0 + b.nr);
+  const int c0 = max(a.c0, b.c0), c1 = min(a.c0 + a.nc, b.c0 + b.nc);
+  out = Rect{r0, r1 - r0, c0, c1 - c0};
+  return r1 > r0 && c1 > c0;
+}
+
+// Is old piece o the designated holder for new piece q (reading A6 (ii))?
+__device__ __forceinline__ bool designated(const Piece& o, const Piece& q, int tp_old, int dp_old) {
+  const bool stage_ok = (o.flags & PF_SOLE_INST) || ((o.flags & PF_POST_COPY) == (q.flags & PF_POST_COPY));
+  const bool r_ok = (o.flags & PF_TP_SHARDED) || o.r == q.r % tp_old;
+  const bool d_ok = (o.flags & PF_DP_SHARDED) || o.d == q.d % dp_old;
+  return stage_ok && r_ok && d_ok;
+}
+
+// I minus the flat interval [b0,b1) of the shard (row pitch W) that I lives in.  I's first element is local
+// (i0, j0).  Writes up to 4 rectangles (logical coordinates) and returns how many.
+__device__ __forceinline__ int subtract_interval(const Rect& I, int64_t i0, int64_t j0, int64_t W, int64_t b0, int64_t b1,
+                                                 Rect out[4]) {
+  if (b1 <= b0) { out[0] = I; return 1; }
+  const int64_t i1 = i0 + I.nr, j1 = j0 + I.nc;
+  const int64_t ib = b0 / W, jb = b0 - ib * W, ie = b1 / W, je = b1 - ie * W;
+  int n = 0;
+  // A: rows strictly above the interval's first row
+  { const int64_t e = min(i1, ib); if (e > i0) out[n++] = Rect{I.r0, (int32_t)(e - i0), I.c0, I.nc}; }
+  // B: the interval's first row, columns before it starts
+  if (ib >= i0 && ib < i1) { const int64_t e = min(j1, jb); if (e > j0) out[n++] = Rect{(int32_t)(I.r0 + (ib - i0)), 1, I.c0, (int32_t)(e - j0)}; }
+  // C: the interval's last (partial) row, columns after it ends
+  if (ie >= i0 && ie < i1) { const int64_t s = max(j0, je); if (j1 > s) out[n++] = Rect{(int32_t)(I.r0 + (ie - i0)), 1, (int32_t)(I.c0 + (s - j0)), (int32_t)(j1 - s)}; }
+  // D: rows strictly below the interval's last row
+  { const int64_t s = max(i0, ie + 1); if (i1 > s) out[n++] = Rect{(int32_t)(I.r0 + (s - i0)), (int32_t)(i1 - s), I.c0, I.nc}; }
+  return n;
+}
+
+struct SliceGeom {           // one 2-D strided copy
+  int64_t src_off, dst_off, row_bytes;
+  int32_t src_stride, dst_stride, nrows, kind;
+};
+
+__device__ __forceinline__ SliceGeom make_slice(const Rect& R, const Piece& o, const Piece& q, int es, int kind) {
+  SliceGeom s;
+  s.src_off = o.boff + ((int64_t)(R.r0 - o.r0) * o.W + (R.c0 - o.c0)) * es;
+  s.dst_off = q.boff + ((int64_t)(R.r0 - q.r0) * q.W + (R.c0 - q.c0)) * es;
+  s.src_stride = o.W * es; s.dst_stride = q.W * es;
+  s.nrows = R.nr; s.row_bytes = (int64_t)R.nc * es; s.kind = kind;
+  if (s.nrows > 1 && s.row_bytes == s.src_stride && s.row_bytes == s.dst_stride) {   // contiguous on both sides
+    s.row_bytes *= s.nrows; s.nrows = 1;
+  }
+  return s;
+}
+
+__device__ __forceinline__ int64_t slice_chunks(const SliceGeom& s) {
+  if (s.nrows == 1) return (s.row_bytes + ETC_CHUNK_BYTES - 1) / ETC_CHUNK_BYTES;
+  if (s.row_bytes >= ETC_CHUNK_BYTES) return (int64_t)s.nrows * ((s.row_bytes + ETC_CHUNK_BYTES - 1) / ETC_CHUNK_BYTES);
+  const int rpc = (int)(ETC_CHUNK_BYTES / s.row_bytes);
+  return (s.nrows + rpc - 1) / rpc;
+}
+__device__ __forceinline__ int64_t slice_padded(const SliceGeom& s) { return (s.nrows * s.row_bytes + 15) & ~(int64_t)15; }
+
+// Enumerate, in canonical order, the slices that new piece q receives from source device od.
+template <typename F>
+__device__ __forceinline__ void for_each_slice(const DeviceTables& oldT, const Piece& q, int od, int p, bool local_unit,
+                                               int es, int kind, F&& f) {
+  int j = oldT.first[(size_t)od * oldT.n_grp + q.grp];
+  if (j < 0) return;
+  const int oe = oldT.dev_start[od + 1];
+  for (; j < oe; ++j) {
+    const Piece o = oldT.pieces[j];
+    if (o.grp != q.grp) break;
+    Rect I;
+    if (!rect_isect(q, o, I)) continue;
+    if (local_unit) { f(make_slice(I, o, q, es, kind)); continue; }              // (i) local first
+    if (!designated(o, q, oldT.tp, oldT.dp)) continue;                           // (ii) designated holder only
+    Rect parts[4]; int np = 1; parts[0] = I;
+    if (p >= 0 && p < oldT.n_dev) {                                              // minus what the destination device holds
+      const int pj = oldT.first[(size_t)p * oldT.n_grp + q.grp];
+      if (pj >= 0) {
+        const Piece& h = oldT.pieces[pj];
+        if (!(o.flags & PF_TP_SHARDED) || h.r == o.r)                            // same TP shard: subtract its held range
+          np = subtract_interval(I, (int64_t)o.lrow0 + (I.r0 - o.r0), (int64_t)o.lcol0 + (I.c0 - o.c0), o.W, h.f0, h.f1, parts);
+      }
+    }
+    for (int k = 0; k < np; ++k) f(make_slice(parts[k], o, q, es, kind));
+  }
+}
+
+__device__ __forceinline__ int64_t warp_sum64(int64_t v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ int64_t warp_excl_scan64(int64_t v, int lane, int64_t& total) {
+  int64_t x = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int64_t y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+  total = __shfl_sync(0xffffffffu, x, 31);
+  return x - v;
+}
+
+constexpr int PLAN_WARPS = 8;
+
+// pass 1: per-unit counts.  unit u = od * n_new + n.
+__global__ void __launch_bounds__(PLAN_WARPS * 32)
+plan_count_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict__ device_map, int flags,
+                  UnitCount* __restrict__ units) {
+  const int lane = threadIdx.x & 31;
+  const long long u = (long long)blockIdx.x * PLAN_WARPS + (threadIdx.x >> 5);
+  const long long U = (long long)oldT.n_dev * newT.n_dev;
+  if (u >= U) return;
+  const int od = (int)(u / newT.n_dev), n = (int)(u % newT.n_dev);
+  const int p = device_map[n];
+  const bool local_unit = (od == p);
+  int64_t n_sl = 0, n_ch = 0, bytes = 0, padded = 0;
+  bool common = false;
+  for (int w = lane; w < newT.mask_words; w += 32)
+    common |= (newT.ltmask[(size_t)n * newT.mask_words + w] & oldT.ltmask[(size_t)od * oldT.mask_words + w]) != 0;
+  if (__any_sync(0xffffffffu, common)) {
+    const int qb = newT.dev_start[n], qe = newT.dev_start[n + 1];
+    for (int i = qb + lane; i < qe; i += 32) {
+      const Piece q = newT.pieces[i];
+      const int kind = q.grp / newT.n_tensors, es = newT.elem_bytes[kind];
+      for_each_slice(oldT, q, od, p, local_unit, es, kind, [&](const SliceGeom& s) {
+        n_sl += 1; n_ch += slice_chunks(s); bytes += s.nrows * s.row_bytes; padded += slice_padded(s);
+      });
+    }
+  }
+  n_sl = warp_sum64(n_sl); n_ch = warp_sum64(n_ch); bytes = warp_sum64(bytes); padded = warp_sum64(padded);
+  if (lane == 0) {
+    UnitCount c;
+    c.slices = n_sl; c.chunks = n_ch; c.bytes = bytes;
+    c.padded = (padded + 511) & ~(int64_t)511;                 // pair segments start 512-byte aligned
+    c.staged = (!local_unit || (flags & ETC_ALL_STAGED)) ? 1 : 0;
+    units[u] = c;
+  }
+}
+
+// single-CTA exclusive scan over units (+ map validation, traffic matrix, totals)
+constexpr int SCAN_THREADS = 1024;
+__global__ void __launch_bounds__(SCAN_THREADS)
+plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int n_old, int n_new, int P,
+                 const int32_t* __restrict__ device_map, UnitBase* __restrict__ bases, int64_t* __restrict__ traffic,
+                 PlanTotals* __restrict__ totals) {
+  __shared__ int64_t s_w[5][32];
+  __shared__ int64_t s_carry[5];
+  __shared__ int64_t s_loc[32], s_rem[32];
+  __shared__ uint32_t s_seen[1024];          // P <= 32767 bits
+  __shared__ int s_bad;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  if (tid < 5) s_carry[tid] = 0;
+  if (tid == 0) s_bad = 0;
+  for (int i = tid; i < 1024; i += SCAN_THREADS) s_seen[i] = 0;
+  __syncthreads();
+  for (int n = tid; n < n_new; n += SCAN_THREADS) {            // injective into [0,P)?
+    const int p = device_map[n];
+    if (p < 0 || p >= P) s_bad = 1;
+    else if (atomicOr(&s_seen[p >> 5], 1u << (p & 31)) & (1u << (p & 31))) s_bad = 1;
+  }
+  for (long long i = tid; i < (long long)P * P; i += SCAN_THREADS) traffic[i] = 0;
+  __syncthreads();
+  const bool bad = s_bad != 0;
+  int64_t loc = 0, rem = 0;
+  for (long long base = 0; base < U; base += SCAN_THREADS) {
+    const long long u = base + tid;
+    UnitCount c{0, 0, 0, 0, 0};
+    if (u < U) c = units[u];
+    int64_t v[5];
+    v[0] = c.staged ? c.slices : 0; v[1] = c.staged ? c.chunks : 0; v[2] = c.staged ? c.padded : 0;
+    v[3] = c.staged ? 0 : c.slices; v[4] = c.staged ? 0 : c.chunks;
+    int64_t ex[5];
+#pragma unroll
+    for (int k = 0; k < 5; ++k) { int64_t tot; ex[k] = warp_excl_scan64(v[k], lane, tot); if (lane == 31) s_w[k][wid] = tot; }
+    __syncthreads();
+    if (wid == 0) {
+#pragma unroll
+      for (int k = 0; k < 5; ++k) { int64_t tot; s_w[k][lane] = warp_excl_scan64(s_w[k][lane], lane, tot); }
+    }
+    __syncthreads();
+    if (u < U) {
+      UnitBase b;
+      b.slice0 = s_carry[c.staged ? 0 : 3] + s_w[c.staged ? 0 : 3][wid] + ex[c.staged ? 0 : 3];
+      b.chunk0 = s_carry[c.staged ? 1 : 4] + s_w[c.staged ? 1 : 4][wid] + ex[c.staged ? 1 : 4];
+      b.stg0 = c.staged ? s_carry[2] + s_w[2][wid] + ex[2] : -1;
+      bases[u] = b;
+      if (!bad && c.bytes) {
+        const int od = (int)(u / n_new), n = (int)(u % n_new), p = device_map[n];
+        traffic[(size_t)od * P + p] = c.bytes;
+        if (od == p) loc += c.bytes; else rem += c.bytes;
+      }
+    }
+    __syncthreads();
+    if (tid == SCAN_THREADS - 1) {
+#pragma unroll
+      for (int k = 0; k < 5; ++k) s_carry[k] += s_w[k][wid] + ex[k] + v[k];
+    }
+    __syncthreads();
+  }
+  loc = warp_sum64(loc); rem = warp_sum64(rem);
+  if (lane == 0) { s_loc[wid] = loc; s_rem[wid] = rem; }
+  __syncthreads();
+  if (wid == 0) {
+    loc = warp_sum64(s_loc[lane]); rem = warp_sum64(s_rem[lane]);
+    if (lane == 0) {
+      PlanTotals t;
+      t.n_slices_staged = s_carry[0]; t.n_chunks_staged = s_carry[1]; t.staging_bytes = s_carry[2];
+      t.n_slices_local = s_carry[3]; t.n_chunks_local = s_carry[4];
+      t.local_bytes = loc; t.remote_bytes = rem; t.bad_map = bad ? 1 : 0;
+      *totals = t;
+    }
+  }
+}
+
+__device__ __forceinline__ int vec_of(int64_t a) {
+  const int64_t low = a & -a;
+  return a == 0 ? 16 : (low >= 16 ? 16 : (int)low);
+}
+
+// pass 2: recompute the slices of each unit and write slice records (+ first chunk index) at their final positions
+__global__ void __launch_bounds__(PLAN_WARPS * 32)
+plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict__ device_map, int flags,
+                 const UnitCount* __restrict__ units, const UnitBase* __restrict__ bases,
+                 etc_slice* __restrict__ sl_staged, etc_slice* __restrict__ sl_local,
+                 int64_t* __restrict__ c0_staged, int64_t* __restrict__ c0_local) {
+  const int lane = threadIdx.x & 31;
+  const long long u = (long long)blockIdx.x * PLAN_WARPS + (threadIdx.x >> 5);
+  const long long U = (long long)oldT.n_dev * newT.n_dev;
+  if (u >= U) return;
+  const UnitCount cnt = units[u];
+  if (cnt.slices == 0) return;
+  const UnitBase ub = bases[u];
+  const int od = (int)(u / newT.n_dev), n = (int)(u % newT.n_dev);
+  const int p = device_map[n];
+  const bool local_unit = (od == p), staged = cnt.staged != 0;
+  etc_slice* sl_out = staged ? sl_staged : sl_local;
+  int64_t* c0_out = staged ? c0_staged : c0_local;
+  int64_t run_sl = ub.slice0, run_ch = ub.chunk0, run_stg = staged ? ub.stg0 : 0;
+  const int qb = newT.dev_start[n], qe = newT.dev_start[n + 1];
+  for (int ib = qb; ib < qe; ib += 32) {                       // all lanes iterate together (warp scans inside)
+    const int i = ib + lane;
+    Piece q; int kind = 0, es = 0;
+    int64_t my_sl = 0, my_ch = 0, my_pad = 0;
+    if (i < qe) {
+      q = newT.pieces[i]; kind = q.grp / newT.n_tensors; es = newT.elem_bytes[kind];
+      for_each_slice(oldT, q, od, p, local_unit, es, kind, [&](const SliceGeom& s) {
+        my_sl += 1; my_ch += slice_chunks(s); my_pad += slice_padded(s);
+      });
+    }
+    int64_t tot_sl, tot_ch, tot_pad;
+    int64_t o_sl = run_sl + warp_excl_scan64(my_sl, lane, tot_sl);       // warp-level prefix sums for slice offsets
+    int64_t o_ch = run_ch + warp_excl_scan64(my_ch, lane, tot_ch);
+    int64_t o_stg = run_stg + warp_excl_scan64(my_pad, lane, tot_pad);
+    run_sl += tot_sl; run_ch += tot_ch; run_stg += tot_pad;
+    if (i < qe && my_sl) {
+      for_each_slice(oldT, q, od, p, local_unit, es, kind, [&](const SliceGeom& s) {
+        etc_slice r;
+        r.src_off = s.src_off; r.dst_off = s.dst_off; r.stg_off = staged ? o_stg : -1; r.row_bytes = s.row_bytes;
+        r.src_stride = s.src_stride; r.dst_stride = s.dst_stride; r.nrows = s.nrows;
+        r.src_dev = od; r.dst_rank = n; r.dst_phys = p; r.kind = kind; r.pad = 0;
+        sl_out[o_sl] = r; c0_out[o_sl] = o_ch;
+        o_sl += 1; o_ch += slice_chunks(s); o_stg += slice_padded(s);
+      });
+    }
+  }
+}
+
+// pass 3: one thread per chunk: find its slice by binary search over the slices' first-chunk indices, cut the chunk out
+__global__ void __launch_bounds__(256)
+plan_chunks_kernel(const etc_slice* __restrict__ slices, const int64_t* __restrict__ chunk0, long long n_slices,
+                   long long n_chunks, Chunk* __restrict__ out) {
+  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= n_chunks) return;
+  long long lo = 0, hi = n_slices - 1;                          // last slice with chunk0 <= c
+  while (lo < hi) { const long long mid = (lo + hi + 1) >> 1; if (chunk0[mid] <= c) lo = mid; else hi = mid - 1; }
+  const etc_slice s = slices[lo];
+  const long long k = c - chunk0[lo];
+  Chunk ch;
+  ch.src_buf = (uint16_t)(s.src_dev * ETC_NUM_KINDS + s.kind); ch.dst_buf = (uint16_t)(s.dst_rank * ETC_NUM_KINDS + s.kind);
+  ch.src_stride = s.src_stride; ch.dst_stride = s.dst_stride; ch.pad = 0;
+  const int64_t stg = s.stg_off >= 0 ? s.stg_off : 0;
+  int64_t al = s.src_off | s.dst_off | stg | s.row_bytes;
+  if (s.nrows > 1) al |= (int64_t)s.src_stride | (int64_t)s.dst_stride;
+  ch.vec = (int16_t)vec_of(al);
+  if (s.nrows == 1 || s.row_bytes >= ETC_CHUNK_BYTES) {
+    const long long cpr = (s.row_bytes + ETC_CHUNK_BYTES - 1) / ETC_CHUNK_BYTES;
+    const long long row = k / cpr; const int64_t b = (k % cpr) * ETC_CHUNK_BYTES;
+    ch.src_off = s.src_off + row * s.src_stride + b;
+    ch.dst_off = s.dst_off + row * s.dst_stride + b;
+    ch.stg_off = stg + row * s.row_bytes + b;
+    ch.nrows = 1; ch.row_bytes = (int32_t)min((int64_t)ETC_CHUNK_BYTES, s.row_bytes - b);
+  } else {
+    const int rpc = (int)(ETC_CHUNK_BYTES / s.row_bytes);
+    const long long row = k * rpc;
+    ch.src_off = s.src_off + row * s.src_stride;
+    ch.dst_off = s.dst_off + row * s.dst_stride;
+    ch.stg_off = stg + row * s.row_bytes;
+    ch.nrows = (int32_t)min((long long)rpc, s.nrows - row); ch.row_bytes = (int32_t)s.row_bytes;
+  }
+  out[c] = ch;
+}
+
+}  // namespace etc
+
+using namespace etc;
+
+extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
+                                      int32_t flags, etc_plan** out, void* stream) {
+  clear_error_detail();
+  if (!old_l || !new_l || !device_map || !out) return ETC_ERR_INVALID_ARG;
+  if (flags != ETC_LOCAL_DIRECT && flags != ETC_ALL_STAGED) return ETC_ERR_INVALID_ARG;
+  if (!etc_same_model(old_l, new_l)) return ETC_ERR_MISMATCH;
+  const int n_old = old_l->t.n_dev, n_new = new_l->t.n_dev, P = n_old > n_new ? n_old : n_new;
+  if ((long long)P * ETC_NUM_KINDS > 65535) return ETC_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)stream;
+  const long long U = (long long)n_old * n_new;
+
+  etc_plan* pl = new etc_plan();
+  pl->n_old = n_old; pl->n_new = n_new; pl->P = P; pl->flags = flags; pl->stream_created_on = st;
+  pl->old_bytes.assign(old_l->h_buffer_bytes, old_l->h_buffer_bytes + (size_t)n_old * ETC_NUM_KINDS);
+  pl->new_bytes.assign(new_l->h_buffer_bytes, new_l->h_buffer_bytes + (size_t)n_new * ETC_NUM_KINDS);
+  auto fail = [&](etc_status s) { etc_plan_destroy(pl); return s; };
+#define PLAN_TRY(expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) { set_error_detail(#expr, _e); return fail(ETC_ERR_CUDA); } } while (0)
+
+  // device_map may live on the host or on the device
+  cudaPointerAttributes attr{};
+  cudaError_t pe = cudaPointerGetAttributes(&attr, device_map);
+  if (pe != cudaSuccess) { (void)cudaGetLastError(); attr.type = cudaMemoryTypeUnregistered; }
+  const bool on_device = attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged;
+  if (!on_device) {
+    std::vector<char> seen((size_t)P, 0);
+    for (int n = 0; n < n_new; ++n) {
+      const int p = device_map[n];
+      if (p < 0 || p >= P || seen[p]) return fail(ETC_ERR_BAD_MAP);
+      seen[p] = 1;
+    }
+  }
+  PLAN_TRY(cudaMallocAsync(&pl->d_map, sizeof(int32_t) * (size_t)n_new, st));
+  PLAN_TRY(cudaMemcpyAsync(pl->d_map, device_map, sizeof(int32_t) * (size_t)n_new,
+                           on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+  PLAN_TRY(cudaMallocAsync(&pl->d_units, sizeof(UnitCount) * (size_t)U, st));
+  PLAN_TRY(cudaMallocAsync(&pl->d_bases, sizeof(UnitBase) * (size_t)U, st));
+  PLAN_TRY(cudaMallocAsync(&pl->d_traffic, sizeof(int64_t) * (size_t)P * P, st));
+  PLAN_TRY(cudaMallocAsync(&pl->d_totals, sizeof(PlanTotals), st));
+
+  const unsigned grid = (unsigned)((U + PLAN_WARPS - 1) / PLAN_WARPS);
+  plan_count_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, flags, pl->d_units);
+  PLAN_TRY(cudaGetLastError());
+  plan_scan_kernel<<<1, SCAN_THREADS, 0, st>>>(pl->d_units, U, n_old, n_new, P, pl->d_map, pl->d_bases, pl->d_traffic,
+                                               pl->d_totals);
+  PLAN_TRY(cudaGetLastError());
+  count_launch(2);
+  PLAN_TRY(cudaMemcpyAsync(&pl->totals, pl->d_totals, sizeof(PlanTotals), cudaMemcpyDeviceToHost, st));
+  PLAN_TRY(cudaStreamSynchronize(st));                          // the one host sync: sizes must come back
+  if (pl->totals.bad_map) return fail(ETC_ERR_BAD_MAP);
+
+  const PlanTotals& t = pl->totals;
+  if (t.n_slices_staged) PLAN_TRY(cudaMallocAsync(&pl->d_sl_staged, sizeof(etc_slice) * (size_t)t.n_slices_staged, st));
+  if (t.n_slices_local) PLAN_TRY(cudaMallocAsync(&pl->d_sl_local, sizeof(etc_slice) * (size_t)t.n_slices_local, st));
+  if (t.n_chunks_staged) PLAN_TRY(cudaMallocAsync(&pl->d_ch_staged, sizeof(Chunk) * (size_t)t.n_chunks_staged, st));
+  if (t.n_chunks_local) PLAN_TRY(cudaMallocAsync(&pl->d_ch_local, sizeof(Chunk) * (size_t)t.n_chunks_local, st));
+  if (t.n_slices_staged) PLAN_TRY(cudaMallocAsync(&pl->d_c0_staged, sizeof(int64_t) * (size_t)t.n_slices_staged, st));
+  if (t.n_slices_local) PLAN_TRY(cudaMallocAsync(&pl->d_c0_local, sizeof(int64_t) * (size_t)t.n_slices_local, st));
+  if (t.n_slices_staged + t.n_slices_local) {
+    plan_fill_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, flags, pl->d_units, pl->d_bases,
+                                                       pl->d_sl_staged, pl->d_sl_local, pl->d_c0_staged, pl->d_c0_local);
+    PLAN_TRY(cudaGetLastError());
+    count_launch();
+  }
+  if (t.n_chunks_staged) {
+    plan_chunks_kernel<<<(unsigned)((t.n_chunks_staged + 255) / 256), 256, 0, st>>>(
+        pl->d_sl_staged, pl->d_c0_staged, t.n_slices_staged, t.n_chunks_staged, pl->d_ch_staged);
+    PLAN_TRY(cudaGetLastError());
+    count_launch();
+  }
+  if (t.n_chunks_local) {
+    plan_chunks_kernel<<<(unsigned)((t.n_chunks_local + 255) / 256), 256, 0, st>>>(
+        pl->d_sl_local, pl->d_c0_local, t.n_slices_local, t.n_chunks_local, pl->d_ch_local);
+    PLAN_TRY(cudaGetLastError());
+    count_launch();
+  }
+  // pointer tables for migrate (filled per call)
+  PLAN_TRY(cudaMallocAsync(&pl->d_ptrs, sizeof(void*) * (size_t)(n_old + n_new) * ETC_NUM_KINDS, st));
+#undef PLAN_TRY
+  *out = pl;
+  return ETC_OK;
+}
+
+extern "C" void etc_plan_destroy(etc_plan* pl) {
+  if (!pl) return;
+  cudaStream_t st = pl->stream_created_on;
+  void* ptrs[] = {pl->d_map, pl->d_units, pl->d_bases, pl->d_traffic, pl->d_totals, pl->d_sl_staged, pl->d_sl_local,
+                  pl->d_ch_staged, pl->d_ch_local, pl->d_c0_staged, pl->d_c0_local, pl->d_ptrs};
+  for (void* p : ptrs) if (p) cudaFreeAsync(p, st);
+  delete pl;
+}
+
+extern "C" etc_status etc_plan_get_stats(const etc_plan* pl, etc_plan_stats* out) {
+  if (!pl || !out) return ETC_ERR_INVALID_ARG;
+  const PlanTotals& t = pl->totals;
+  out->staging_bytes = t.staging_bytes; out->local_bytes = t.local_bytes; out->remote_bytes = t.remote_bytes;
+  out->staged_bytes = (pl->flags & ETC_ALL_STAGED) ? t.local_bytes + t.remote_bytes : t.remote_bytes;
+  out->n_slices_local = t.n_slices_local; out->n_slices_staged = t.n_slices_staged;
+  out->n_chunks_local = t.n_chunks_local; out->n_chunks_staged = t.n_chunks_staged;
+  out->n_old = pl->n_old; out->n_new = pl->n_new; out->P = pl->P; out->flags = pl->flags;
+  return ETC_OK;
+}
+
+extern "C" etc_status etc_plan_get_traffic(const etc_plan* pl, int64_t* h_traffic) {
+  clear_error_detail();
+  if (!pl || !h_traffic) return ETC_ERR_INVALID_ARG;
+  ETC_CUDA_TRY(cudaStreamSynchronize(pl->stream_created_on));
+  ETC_CUDA_TRY(cudaMemcpy(h_traffic, pl->d_traffic, sizeof(int64_t) * (size_t)pl->P * pl->P, cudaMemcpyDeviceToHost));
+  return ETC_OK;
+}
+
+extern "C" etc_status etc_plan_get_slices(const etc_plan* pl, int32_t which, etc_slice* h_out) {
+  clear_error_detail();
+  if (!pl || !h_out || (which != 0 && which != 1)) return ETC_ERR_INVALID_ARG;
+  const int64_t n = which == 0 ? pl->totals.n_slices_staged : pl->totals.n_slices_local;
+  const etc_slice* src = which == 0 ? pl->d_sl_staged : pl->d_sl_local;
+  ETC_CUDA_TRY(cudaStreamSynchronize(pl->stream_created_on));
+  if (n) ETC_CUDA_TRY(cudaMemcpy(h_out, src, sizeof(etc_slice) * (size_t)n, cudaMemcpyDeviceToHost));
+  return ETC_OK;
+}

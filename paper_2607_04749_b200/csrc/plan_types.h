@@ -1,0 +1,42 @@
+// plan_types.h — plan-side tables shared by plan.cu (which writes them) and migrate.cu (which reads them).
+#pragma once
+#include <vector>
+#include "etc_internal.h"
+
+namespace etc {
+
+struct UnitCount { int64_t slices, chunks, bytes, padded; int64_t staged; };   // per (source device, new rank) unit
+struct UnitBase { int64_t slice0, chunk0, stg0; };
+struct PlanTotals {
+  int64_t n_slices_staged, n_chunks_staged, staging_bytes, n_slices_local, n_chunks_local;
+  int64_t local_bytes, remote_bytes, bad_map;
+};
+
+// One copy work item: nrows x row_bytes, at most ETC_CHUNK_BYTES in total (or one row segment of that size).
+struct Chunk {
+  int64_t src_off, dst_off, stg_off;   // byte offsets inside the source buffer, destination buffer, staging buffer
+  int32_t src_stride, dst_stride;      // row pitch in bytes (staging pitch = row_bytes)
+  int32_t row_bytes, nrows;
+  uint16_t src_buf, dst_buf;           // pointer-table indices: device*4 + kind
+  int16_t vec;                         // widest power-of-two access (<= 16 B) every address of the chunk is aligned to
+  int16_t pad;
+};
+static_assert(sizeof(Chunk) == 48, "Chunk layout");
+
+}  // namespace etc
+
+struct etc_plan {
+  int32_t n_old = 0, n_new = 0, P = 0, flags = 0;
+  cudaStream_t stream_created_on = nullptr;
+  etc::PlanTotals totals{};
+  int32_t* d_map = nullptr;
+  etc::UnitCount* d_units = nullptr;
+  etc::UnitBase* d_bases = nullptr;
+  int64_t* d_traffic = nullptr;
+  etc::PlanTotals* d_totals = nullptr;
+  etc_slice* d_sl_staged = nullptr; etc_slice* d_sl_local = nullptr;
+  etc::Chunk* d_ch_staged = nullptr; etc::Chunk* d_ch_local = nullptr;
+  int64_t* d_c0_staged = nullptr; int64_t* d_c0_local = nullptr;
+  std::vector<int64_t> old_bytes, new_bytes;   // buffer sizes [dev*4+kind], for argument checks in migrate
+  void** d_ptrs = nullptr;             // [n_old*4] source pointers then [n_new*4] destination pointers
+};

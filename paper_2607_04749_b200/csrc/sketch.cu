@@ -1,0 +1,223 @@
+// sketch.cu — (a3) migration sketch: pair current ranks with previous devices so that the most bytes stay in place
+// (PAPER.md:110-132 assignment problem, Eq. 1-4; :134-163 Algorithm 1).  Objective (reading A4):
+//   device_map = argmax over injective pi:[0,n_new)->[0,P) of sum_n overlap[n][pi(n)].
+// Two device-side searches, both single-CTA (the problem is a few hundred rows: latency-bound integer work):
+//   * exhaustive: every injective map enumerated by its mixed-radix index (P <= 8: at most 40 320 maps);
+//   * Hungarian:  shortest augmenting paths with dual potentials on the rectangular matrix (rows <= columns, so no
+//     zero padding is needed: padded rows of Algorithm 1 line 3 would cost 0 on every column and are dropped again by
+//     lines 6-8).  One thread per column, block-wide arg-min per Dijkstra step.
+#include "etc_internal.h"
+
+namespace etc {
+
+constexpr int SK_THREADS = 1024;
+constexpr int64_t SK_INF = (int64_t)1 << 62;
+
+// ---------------------------------------------------------------------------------------------- exhaustive
+__global__ void __launch_bounds__(SK_THREADS)
+sketch_exhaustive_kernel(const int64_t* __restrict__ overlap, int N, int P, const uint8_t* __restrict__ avail,
+                         int32_t* __restrict__ device_map, int64_t* __restrict__ local_bytes) {
+  __shared__ int64_t ov[64];
+  __shared__ int64_t s_val[32];
+  __shared__ int s_idx[32];
+  __shared__ uint32_t s_avail;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  if (tid < N * P) ov[tid] = overlap[tid];
+  if (tid == 0) {
+    uint32_t m = 0;
+    for (int j = 0; j < P; ++j) if (!avail || avail[j]) m |= 1u << j;
+    s_avail = m;
+  }
+  __syncthreads();
+  int total = 1;
+  for (int n = 0; n < N; ++n) total *= (P - n);
+  const uint32_t all = (1u << P) - 1u, av = s_avail;
+
+  int64_t best = -1; int best_idx = 0x7fffffff;
+  for (int idx = tid; idx < total; idx += SK_THREADS) {
+    int rem = idx; uint32_t used = 0; int64_t sum = 0;
+    for (int n = 0; n < N; ++n) {
+      const int radix = P - n, digit = rem % radix; rem /= radix;
+      const int c = __fns(~used & all, 0, digit + 1);      // the digit-th still unused column
+      used |= 1u << c; sum += ov[n * P + c];
+    }
+    if ((used & ~av) == 0 && sum > best) { best = sum; best_idx = idx; }   // idx ascending: ties keep the smallest
+  }
+  // block arg-max, ties -> smallest index (deterministic)
+  auto better = [](int64_t v, int i, int64_t bv, int bi) { return v > bv || (v == bv && i < bi); };
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const int64_t v = __shfl_xor_sync(0xffffffffu, best, o); const int i = __shfl_xor_sync(0xffffffffu, best_idx, o);
+    if (better(v, i, best, best_idx)) { best = v; best_idx = i; }
+  }
+  if (lane == 0) { s_val[wid] = best; s_idx[wid] = best_idx; }
+  __syncthreads();
+  if (wid == 0) {
+    best = s_val[lane]; best_idx = s_idx[lane];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const int64_t v = __shfl_xor_sync(0xffffffffu, best, o); const int i = __shfl_xor_sync(0xffffffffu, best_idx, o);
+      if (better(v, i, best, best_idx)) { best = v; best_idx = i; }
+    }
+    if (lane == 0) {
+      if (best < 0) {                                           // no feasible map
+        for (int n = 0; n < N; ++n) device_map[n] = -1;
+        *local_bytes = -1;
+      } else {
+        int rem = best_idx; uint32_t used = 0;
+        for (int n = 0; n < N; ++n) {
+          const int radix = P - n, digit = rem % radix; rem /= radix;
+          const int c = __fns(~used & all, 0, digit + 1);
+          used |= 1u << c; device_map[n] = c;
+        }
+        *local_bytes = best;
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- Hungarian
+// Shortest augmenting path with potentials (the O(k^3) method Algorithm 1 calls through SciPy, ref [39]).
+// cost(i,j) = -overlap[i][j]; columns masked by `avail` are never entered.  Per-column state lives in registers
+// (CPT columns per thread), row potentials / matching / back-pointers in shared memory.
+constexpr int SK_CPT = ETC_SKETCH_MAX_P / SK_THREADS;   // columns per thread
+
+struct ArgMin { int64_t v; int j; int matched; };
+__device__ __forceinline__ bool argmin_less(const ArgMin& a, const ArgMin& b) {
+  if (a.v != b.v) return a.v < b.v;
+  if (a.matched != b.matched) return a.matched < b.matched;     // prefer a free column: the path ends at once
+  return a.j < b.j;
+}
+__device__ __forceinline__ ArgMin argmin_shfl(const ArgMin& a, int o) {
+  ArgMin b;
+  b.v = __shfl_xor_sync(0xffffffffu, a.v, o); b.j = __shfl_xor_sync(0xffffffffu, a.j, o);
+  b.matched = __shfl_xor_sync(0xffffffffu, a.matched, o);
+  return b;
+}
+
+__global__ void __launch_bounds__(SK_THREADS)
+sketch_hungarian_kernel(const int64_t* __restrict__ overlap, int N, int P, const uint8_t* __restrict__ avail,
+                        int32_t* __restrict__ device_map, int64_t* __restrict__ local_bytes) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  int64_t* u = reinterpret_cast<int64_t*>(smem_raw);            // [N] row potentials
+  int32_t* rowof = reinterpret_cast<int32_t*>(u + N);           // [P] column -> matched row or -1
+  int32_t* way = rowof + P;                                     // [P] previous column on the alternating path
+  __shared__ int64_t s_v[32]; __shared__ int s_j[32]; __shared__ int s_m[32];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+
+  int64_t v[SK_CPT], minv[SK_CPT]; bool used[SK_CPT], usable[SK_CPT];
+#pragma unroll
+  for (int c = 0; c < SK_CPT; ++c) {
+    const int j = tid + c * SK_THREADS;
+    v[c] = 0; usable[c] = j < P && (!avail || avail[j]);
+    if (j < P) { rowof[j] = -1; way[j] = -1; }
+  }
+  for (int i = tid; i < N; i += SK_THREADS) u[i] = 0;
+  __syncthreads();
+
+  bool fail = false;                                            // uniform across the block
+  for (int i = 0; i < N; ++i) {
+#pragma unroll
+    for (int c = 0; c < SK_CPT; ++c) { minv[c] = SK_INF; used[c] = !usable[c]; }
+    int i0 = i, j0 = -1;
+    while (true) {
+      // relax the edges of row i0, then block-wide arg-min of minv over the columns not yet on the tree
+      const int64_t ui0 = u[i0];
+      ArgMin best{SK_INF, 0x7fffffff, 1};
+#pragma unroll
+      for (int c = 0; c < SK_CPT; ++c) {
+        const int j = tid + c * SK_THREADS;
+        if (!used[c]) {
+          const int64_t cur = -overlap[(size_t)i0 * P + j] - ui0 - v[c];
+          if (cur < minv[c]) { minv[c] = cur; way[j] = j0; }
+          ArgMin a{minv[c], j, rowof[j] >= 0 ? 1 : 0};
+          if (argmin_less(a, best)) best = a;
+        }
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) { ArgMin b = argmin_shfl(best, o); if (argmin_less(b, best)) best = b; }
+      if (lane == 0) { s_v[wid] = best.v; s_j[wid] = best.j; s_m[wid] = best.matched; }
+      __syncthreads();
+      best = ArgMin{s_v[lane], s_j[lane], s_m[lane]};
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) { ArgMin b = argmin_shfl(best, o); if (argmin_less(b, best)) best = b; }
+      if (best.v >= SK_INF) { fail = true; break; }                       // no column left: infeasible
+      const int64_t delta = best.v; const int j1 = best.j;
+      // dual update: tree rows gain delta, tree columns lose delta, the rest get closer by delta
+      if (tid == 0) u[i] += delta;
+#pragma unroll
+      for (int c = 0; c < SK_CPT; ++c) {
+        const int j = tid + c * SK_THREADS;
+        if (j < P && usable[c]) {
+          if (used[c]) { u[rowof[j]] += delta; v[c] -= delta; }
+          else minv[c] -= delta;
+          if (j == j1) used[c] = true;
+        }
+      }
+      j0 = j1; i0 = rowof[j1];
+      __syncthreads();
+      if (i0 < 0) break;
+    }
+    if (fail) break;
+    if (tid == 0) {                                                       // augment along the alternating path
+      int j = j0;
+      while (j >= 0) { const int jp = way[j]; rowof[j] = jp >= 0 ? rowof[jp] : i; j = jp; }
+    }
+    __syncthreads();
+  }
+
+  __syncthreads();
+  if (fail) {
+    for (int n = tid; n < N; n += SK_THREADS) device_map[n] = -1;
+    if (tid == 0) *local_bytes = -1;
+    return;
+  }
+  int64_t acc = 0;
+#pragma unroll
+  for (int c = 0; c < SK_CPT; ++c) {
+    const int j = tid + c * SK_THREADS;
+    if (j < P && rowof[j] >= 0) { device_map[rowof[j]] = j; acc += overlap[(size_t)rowof[j] * P + j]; }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  __syncthreads();
+  if (lane == 0) s_v[wid] = acc;
+  __syncthreads();
+  if (wid == 0) {
+    acc = s_v[lane];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) *local_bytes = acc;
+  }
+}
+
+}  // namespace etc
+
+using namespace etc;
+
+extern "C" etc_status etc_sketch(const int64_t* d_overlap, int32_t n_new, int32_t P, const uint8_t* d_avail,
+                                 int32_t method, int32_t* d_device_map, int64_t* d_local_bytes, void* stream) {
+  clear_error_detail();
+  if (!d_overlap || !d_device_map || !d_local_bytes || n_new < 1 || P < n_new) return ETC_ERR_INVALID_ARG;
+  if (method == ETC_SKETCH_AUTO) method = P <= 8 ? ETC_SKETCH_EXHAUSTIVE : ETC_SKETCH_HUNGARIAN;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (method == ETC_SKETCH_EXHAUSTIVE) {
+    if (P > 8) return ETC_ERR_WORKSPACE;
+    sketch_exhaustive_kernel<<<1, SK_THREADS, 0, st>>>(d_overlap, n_new, P, d_avail, d_device_map, d_local_bytes);
+  } else if (method == ETC_SKETCH_HUNGARIAN) {
+    if (P > ETC_SKETCH_MAX_P) return ETC_ERR_WORKSPACE;
+    const size_t smem = (size_t)n_new * 8 + (size_t)P * 8;
+    static bool attr_set = false;
+    if (!attr_set) {
+      ETC_CUDA_TRY(cudaFuncSetAttribute(sketch_hungarian_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        ETC_SKETCH_MAX_P * 16));
+      attr_set = true;
+    }
+    sketch_hungarian_kernel<<<1, SK_THREADS, smem, st>>>(d_overlap, n_new, P, d_avail, d_device_map, d_local_bytes);
+  } else {
+    return ETC_ERR_INVALID_ARG;
+  }
+  ETC_CUDA_TRY(cudaGetLastError());
+  count_launch();
+  return ETC_OK;
+}

@@ -1,0 +1,71 @@
+"""CPU-side checks of the C-ABI boundary: libetc.so loads and exports every symbol include/etc.h declares; argument
+validation that needs no GPU.  (No compute calls here.)"""
+from __future__ import annotations
+import ctypes as C
+import os
+import re
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2607_04749_b200 import _build, binding
+    _build.build()
+    return binding.lib()
+
+
+def _declared_functions():
+    src = open(os.path.join(ROOT, "include", "etc.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(etc_[a-z_]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol(lib):
+    names = _declared_functions()
+    assert len(names) >= 18
+    for n in names:
+        assert hasattr(lib, n), f"libetc.so does not export {n}"
+    from paper_2607_04749_b200 import EXPORTED_SYMBOLS
+    assert sorted(EXPORTED_SYMBOLS) == names
+
+
+def test_status_strings(lib):
+    assert lib.etc_status_string(0) == b"ETC_OK"
+    for code, name in [(-1, b"ETC_ERR_INVALID_ARG"), (-2, b"ETC_ERR_INDIVISIBLE"), (-3, b"ETC_ERR_MISMATCH"),
+                       (-4, b"ETC_ERR_BAD_MAP"), (-5, b"ETC_ERR_WORKSPACE"), (-6, b"ETC_ERR_UNSUPPORTED"),
+                       (-7, b"ETC_ERR_CUDA")]:
+        assert lib.etc_status_string(code) == name
+
+
+def test_layout_validation_without_gpu(lib):
+    """Validation errors are reported before any CUDA call (PAPER.md:277 divisibility; reading A10)."""
+    from paper_2607_04749_b200.binding import _ModelDesc, _ParallelCfg
+    m = _ModelDesc(style=0, n_layers=4, hidden=12, n_q_heads=2, n_kv_heads=2, head_dim=6, ffn_hidden=28, vocab=20,
+                   max_pos=0, tied_embeddings=1, param_dtype=2, kinds=15)
+    h = C.c_void_p()
+    assert lib.etc_layout_create(C.byref(m), C.byref(_ParallelCfg(1, 3, 1, 0)), C.byref(h)) == -2   # layers % pp
+    assert lib.etc_layout_create(C.byref(m), C.byref(_ParallelCfg(4, 1, 1, 0)), C.byref(h)) == -6   # tp > kv heads
+    assert lib.etc_layout_create(C.byref(m), C.byref(_ParallelCfg(0, 1, 1, 0)), C.byref(h)) == -1
+    assert lib.etc_layout_create(None, C.byref(_ParallelCfg(1, 1, 1, 0)), C.byref(h)) == -1
+    m.param_dtype = 3
+    assert lib.etc_layout_create(C.byref(m), C.byref(_ParallelCfg(1, 1, 1, 0)), C.byref(h)) == -1
+    assert h.value is None
+
+
+def test_product_path_has_no_oracle_or_cpu_fallback():
+    """The package must not import the oracle, and must fail loudly without a CUDA device."""
+    import torch
+    import paper_2607_04749_b200 as E
+    pkg = os.path.join(ROOT, "paper_2607_04749_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".h", ".cpp")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in txt and "from oracle" not in txt and "liboracle" not in txt, f
+    if not torch.cuda.is_available():
+        with pytest.raises(RuntimeError):
+            E.etc_layout_create(dict(style=0, n_layers=2, hidden=8, n_q_heads=2, n_kv_heads=2, head_dim=4,
+                                     ffn_hidden=16, vocab=8, max_pos=0, tied=0, param_bytes=2, kinds=15),
+                                dict(tp=1, pp=1, dp=1, dist_opt=0))
