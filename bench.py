@@ -278,6 +278,7 @@ def run_cuda(args, w):
             "breakdown_ms": bd, "cost_sketch_ms": bd["cost_matrix_ms"] + bd["sketch_ms"],
             "roofline": roofline, "clocks": clocks, "gpu_launches": launches}
 
+    del staging
     if rank == 0 and not args.no_extras:
         line["extras"] = extras(E, torch, w, dev, src, dst, lay_old, lay_new, peak)
 
@@ -285,6 +286,7 @@ def run_cuda(args, w):
     #      are inside the timed region
     if not args.no_e2e:
         try:
+            staging = torch.empty(max(st0.staging_bytes, 16), dtype=torch.uint8, device=dev)
             line["e2e"] = e2e(E, torch, args, w, dev, src, dst, staging, step, hbm_bytes, world, barrier)
         except Exception as ex:       # e.g. not enough pinned host memory on the box
             line["e2e"] = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
@@ -292,7 +294,7 @@ def run_cuda(args, w):
     if rank == 0:
         if world == 1 and not args.no_cpu:
             from oracle import oracle as O
-            o = oracle_sample(w, budget_elems=args.ref_elems)
+            o = oracle_sample(w, budget_elems=args.cpu_elems)
             line["cpu_baseline"] = {
                 "value": 2 * o["payload_bytes"] / o["migrate_s"] / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
                 "sample": f"element-wise oracle migration of the first {o['elems_per_buffer']} elements of each of "
@@ -396,7 +398,8 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--ref-elems", type=int, default=6_000_000, help="oracle sample size (elements) per step")
+    ap.add_argument("--ref-elems", type=int, default=6_000_000, help="--impl reference: oracle sample (elements) per step")
+    ap.add_argument("--cpu-elems", type=int, default=300_000_000, help="cpu_baseline leg: oracle sample (elements), ~10 s")
     args = ap.parse_args()
     from etc_inputs import workload
     w = workload(args.config)

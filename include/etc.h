@@ -95,8 +95,9 @@ etc_status etc_cost_matrix(const etc_layout* old_l, const etc_layout* new_l,
 
 /* (a3) Migration sketch: device_map = argmax over injective maps pi:[0,n_new)->[0,P) of sum_n overlap[n][pi(n)]
  * (= Eq. 2's minimisation under Eq. 3/4, reading A4).  d_avail: optional device mask [P] (0 = device may not be
- * used, e.g. pre-empted; NULL = all usable).  method: ETC_SKETCH_AUTO picks exhaustive search for P <= 8, else the
- * shortest-augmenting-path Hungarian.  Outputs (device memory): d_device_map [n_new] int32, d_local_bytes [1] int64 =
+ * used, e.g. pre-empted; NULL = all usable).  method: ETC_SKETCH_HUNGARIAN = shortest augmenting paths (any P up to
+ * ETC_SKETCH_MAX_P), ETC_SKETCH_EXHAUSTIVE = every injective map enumerated (P <= 8, the cross-check), ETC_SKETCH_AUTO
+ * = the faster one (Hungarian).  Outputs (device memory): d_device_map [n_new] int32, d_local_bytes [1] int64 =
  * the achieved objective.  If no feasible map exists both are filled with -1.  Enqueues on `stream`. */
 enum { ETC_SKETCH_AUTO = 0, ETC_SKETCH_EXHAUSTIVE = 1, ETC_SKETCH_HUNGARIAN = 2 };
 etc_status etc_sketch(const int64_t* d_overlap, int32_t n_new, int32_t P, const uint8_t* d_avail, int32_t method,

@@ -4,6 +4,8 @@
 #include <algorithm>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
+#include <ctime>
 #include <string>
 #include <vector>
 #include "etc_internal.h"
@@ -98,6 +100,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   if (!out) return ETC_ERR_INVALID_ARG;
   etc_status st = validate(model, cfg);
   if (st != ETC_OK) return st;
+  if (getenv("ETC_TIME_LAYOUT")) { timespec ts; clock_gettime(CLOCK_MONOTONIC, &ts); fprintf(stderr, "layout start at %ld.%09ld\n", ts.tv_sec, ts.tv_nsec); }
   const etc_model_desc& m = *model;
   const int tp = cfg->tp, pp = cfg->pp, dp = cfg->dp;
   const int n_dev = tp * pp * dp;
@@ -215,6 +218,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   memcpy(host.data() + o_first, first.data(), first.size() * 4);
   memcpy(host.data() + o_mask, ltmask.data(), ltmask.size() * 4);
 
+  if (getenv("ETC_TIME_LAYOUT")) { timespec ts; clock_gettime(CLOCK_MONOTONIC, &ts); fprintf(stderr, "layout host build done at %ld.%09ld pieces=%zu total=%zu\n", ts.tv_sec, ts.tv_nsec, pieces.size(), total); }
   etc_layout* L = new etc_layout();
   L->model = m; L->cfg = *cfg;
   cudaError_t e = cudaSetDevice(current_device());
