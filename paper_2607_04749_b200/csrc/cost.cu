@@ -1,7 +1,7 @@
 // cost.cu — (a2) cost matrix by integer index-range intersection (PAPER.md:106 c_ij = len(curr_i) - len(curr_i ∩ prev_j);
 // :167-169 TP units and PP/TP merge are subsumed by intersecting index rectangles directly).
 //
-// One warp owns one matrix cell (new rank n, old device o): lanes walk n's pieces, look the matching (kind, tensor)
+// One warp (or one CTA, when there are few cells) owns one matrix cell (new rank n, old device o): lanes walk n's pieces, look the matching (kind, tensor)
 // group of o up in o's dense first-piece table, intersect rectangles and warp-reduce.  No atomics, so every cell is
 // written exactly once and the result is order-independent.  Extra warps past the matrix compute need[] and hold[].
 #include "etc_internal.h"
@@ -22,15 +22,24 @@ __device__ __forceinline__ int64_t warp_sum(int64_t v) {
 
 constexpr int COST_WARPS = 8;
 
+// WPC = warps per job.  WPC = 1: eight jobs per CTA (many cells: 512 x 384 layouts).  WPC = 8: the whole CTA shares one
+// job and reduces through shared memory (few cells: the piece lists are long compared with the cell count, so one
+// warp per cell would leave most of the machine idle and serialise ~20 dependent loads per lane).
+template <int WPC>
 __global__ void __launch_bounds__(COST_WARPS * 32)
 cost_matrix_kernel(DeviceTables oldT, DeviceTables newT, int P,
                    int64_t* __restrict__ overlap, int64_t* __restrict__ need, int64_t* __restrict__ hold) {
-  const int lane = threadIdx.x & 31;
-  const long long warp = (long long)blockIdx.x * COST_WARPS + (threadIdx.x >> 5);
+  __shared__ int64_t s_part[COST_WARPS];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int sub = wid % WPC;                                  // this warp's share of the job
+  const long long job = ((long long)blockIdx.x * COST_WARPS + wid) / WPC;
   const long long cells = (long long)newT.n_dev * P;
-  if (warp < cells) {
-    const int n = (int)(warp / P), o = (int)(warp % P);
-    int64_t acc = 0;
+  const int stride = 32 * WPC;
+  int64_t acc = 0;
+  int64_t* out = nullptr;
+  if (job < cells) {
+    const int n = (int)(job / P), o = (int)(job % P);
+    out = overlap + job;
     if (o < oldT.n_dev) {
       // early out: no logical tensor in common (different pipeline stages)
       bool common = false;
@@ -39,7 +48,7 @@ cost_matrix_kernel(DeviceTables oldT, DeviceTables newT, int P,
       if (__any_sync(0xffffffffu, common)) {
         const int qb = newT.dev_start[n], qe = newT.dev_start[n + 1], oe = oldT.dev_start[o + 1];
         const int nT = newT.n_tensors;
-        for (int i = qb + lane; i < qe; i += 32) {
+        for (int i = qb + sub * 32 + lane; i < qe; i += stride) {
           const Piece q = newT.pieces[i];
           int j = oldT.first[(size_t)o * oldT.n_grp + q.grp];
           if (j < 0) continue;
@@ -53,24 +62,32 @@ cost_matrix_kernel(DeviceTables oldT, DeviceTables newT, int P,
         }
       }
     }
-    acc = warp_sum(acc);
-    if (lane == 0) overlap[warp] = acc;
-    return;
-  }
-  // need[n] / hold[o]: bytes of all pieces of one device
-  const long long job = warp - cells;
-  if (job < newT.n_dev + P) {
-    const bool is_need = job < newT.n_dev;
-    const DeviceTables& T = is_need ? newT : oldT;
-    const int dev = is_need ? (int)job : (int)(job - newT.n_dev);
-    int64_t acc = 0;
-    if (dev < T.n_dev)
-      for (int i = T.dev_start[dev] + lane; i < T.dev_start[dev + 1]; i += 32) {
-        const Piece& q = T.pieces[i];
-        acc += (int64_t)q.nr * q.nc * T.elem_bytes[q.grp / T.n_tensors];
+  } else if (job < cells + newT.n_dev + P) {                  // need[n] / hold[o]: bytes of all pieces of one device
+    const long long k = job - cells;
+    const bool is_need = k < newT.n_dev;
+    const int dev = is_need ? (int)k : (int)(k - newT.n_dev);
+    const Piece* pieces = is_need ? newT.pieces : oldT.pieces;
+    const int32_t* dev_start = is_need ? newT.dev_start : oldT.dev_start;
+    const int n_dev = is_need ? newT.n_dev : oldT.n_dev, nT = newT.n_tensors;
+    out = (is_need ? need : hold) + dev;
+    if (dev < n_dev)
+      for (int i = dev_start[dev] + sub * 32 + lane; i < dev_start[dev + 1]; i += stride) {
+        const Piece& q = pieces[i];
+        acc += (int64_t)q.nr * q.nc * newT.elem_bytes[q.grp / nT];
       }
-    acc = warp_sum(acc);
-    if (lane == 0) (is_need ? need : hold)[dev] = acc;
+  }
+  acc = warp_sum(acc);
+  if (WPC == 1) {
+    if (lane == 0 && out) *out = acc;
+  } else {
+    if (lane == 0) s_part[wid] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0 && out) {
+      int64_t t = 0;
+#pragma unroll
+      for (int k = 0; k < COST_WARPS; ++k) t += s_part[k];
+      *out = t;
+    }
   }
 }
 
@@ -93,11 +110,15 @@ extern "C" etc_status etc_cost_matrix(const etc_layout* old_l, const etc_layout*
   if (!old_l || !new_l || !d_overlap || !d_need || !d_hold) return ETC_ERR_INVALID_ARG;
   if (!same_model(old_l, new_l)) return ETC_ERR_MISMATCH;
   const int P = old_l->t.n_dev > new_l->t.n_dev ? old_l->t.n_dev : new_l->t.n_dev;
-  const long long warps = (long long)new_l->t.n_dev * P + new_l->t.n_dev + P;
-  const unsigned grid = (unsigned)((warps + COST_WARPS - 1) / COST_WARPS);
-  cost_matrix_kernel<<<grid, COST_WARPS * 32, 0, (cudaStream_t)stream>>>(old_l->t, new_l->t, P, d_overlap, d_need,
-                                                                          d_hold);
+  const long long jobs = (long long)new_l->t.n_dev * P + new_l->t.n_dev + P;
+  if (jobs <= 8192)
+    cost_matrix_kernel<COST_WARPS><<<(unsigned)jobs, COST_WARPS * 32, 0, (cudaStream_t)stream>>>(
+        old_l->t, new_l->t, P, d_overlap, d_need, d_hold);
+  else
+    cost_matrix_kernel<1><<<(unsigned)((jobs + COST_WARPS - 1) / COST_WARPS), COST_WARPS * 32, 0, (cudaStream_t)stream>>>(
+        old_l->t, new_l->t, P, d_overlap, d_need, d_hold);
   ETC_CUDA_TRY(cudaGetLastError());
   count_launch();
+  old_l->last_stream = new_l->last_stream = (cudaStream_t)stream;
   return ETC_OK;
 }

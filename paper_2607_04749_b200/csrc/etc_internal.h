@@ -53,7 +53,9 @@ struct etc_layout {
   etc_parallel_cfg cfg;
   etc::DeviceTables t;                    // device pointers + sizes
   int64_t* h_buffer_bytes = nullptr;      // [n_dev][4] host
+  int32_t max_dev_pieces = 0;             // largest piece count of one device
   void* d_blob = nullptr;                 // one allocation holding all device tables
+  mutable cudaStream_t last_stream = nullptr;   // last stream a kernel reading the tables was enqueued on
 };
 
 // ---- error plumbing

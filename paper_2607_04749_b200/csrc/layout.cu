@@ -4,8 +4,7 @@
 #include <algorithm>
 #include <cstdio>
 #include <cstring>
-#include <cstdlib>
-#include <ctime>
+#include <mutex>
 #include <string>
 #include <vector>
 #include "etc_internal.h"
@@ -74,8 +73,6 @@ static etc_status validate(const etc_model_desc* m, const etc_parallel_cfg* c) {
   return ETC_OK;
 }
 
-struct Inst { int32_t lt; bool post_copy; };
-
 }  // namespace etc
 
 using namespace etc;
@@ -95,12 +92,31 @@ extern "C" etc_status etc_init(int32_t cuda_device) {
   return ETC_OK;
 }
 
+// grow-only pinned staging buffer + private upload stream (layout tables are built straight into pinned memory and
+// uploaded with one async copy; the only wait is on that private stream)
+namespace etc {
+static std::mutex g_up_mu;
+static void* g_pinned = nullptr; static size_t g_pinned_cap = 0;
+static cudaStream_t g_up_stream = nullptr;
+static cudaError_t upload_prepare(size_t bytes) {
+  if (!g_up_stream) { cudaError_t e = cudaStreamCreateWithFlags(&g_up_stream, cudaStreamNonBlocking); if (e) return e; }
+  if (bytes > g_pinned_cap) {
+    if (g_pinned) cudaFreeHost(g_pinned);
+    g_pinned = nullptr; g_pinned_cap = 0;
+    const size_t cap = std::max<size_t>(bytes + bytes / 2, 1 << 20);
+    cudaError_t e = cudaMallocHost(&g_pinned, cap); if (e) return e;
+    g_pinned_cap = cap;
+  }
+  return cudaSuccess;
+}
+struct Sh { int64_t start, n, rb[2], nrb, c0, W; int nblk; int32_t lt; uint16_t flags; };
+}  // namespace etc
+
 extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_parallel_cfg* cfg, etc_layout** out) {
   clear_error_detail();
   if (!out) return ETC_ERR_INVALID_ARG;
   etc_status st = validate(model, cfg);
   if (st != ETC_OK) return st;
-  if (getenv("ETC_TIME_LAYOUT")) { timespec ts; clock_gettime(CLOCK_MONOTONIC, &ts); fprintf(stderr, "layout start at %ld.%09ld\n", ts.tv_sec, ts.tv_nsec); }
   const etc_model_desc& m = *model;
   const int tp = cfg->tp, pp = cfg->pp, dp = cfg->dp;
   const int n_dev = tp * pp * dp;
@@ -108,18 +124,34 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   const int nT = (int)lts.size(), nG = nT * ETC_NUM_KINDS;
   const int per_stage = m.n_layers / pp;
   const bool two_inst = m.tied_embeddings && pp > 1;     // word_embeddings held by first AND last stage
-
-  std::vector<Piece> pieces;
-  std::vector<int64_t> bufbytes((size_t)n_dev * ETC_NUM_KINDS, 0);
-  std::vector<int32_t> dev_start(n_dev + 1, 0);
   const int mask_words = (nT + 31) / 32;
-  std::vector<uint32_t> ltmask((size_t)n_dev * mask_words, 0u);
+  int n_kinds = 0; for (int k = 0; k < ETC_NUM_KINDS; ++k) n_kinds += (m.kinds >> k) & 1;
 
-  for (int dev = 0; dev < n_dev; ++dev) {
-    const int r = dev % tp, d = (dev / tp) % dp, s = dev / (tp * dp);
-    dev_start[dev] = (int32_t)pieces.size();
-    // the stage's tensor instances in local order: pre, layers ascending, post, tied replica
-    std::vector<Inst> inst;
+  // blob: dev_start | first | ltmask | pieces (pieces last: their count is known only after the build)
+  auto al = [](size_t x) { return (x + 255) & ~size_t(255); };
+  const size_t max_inst = (size_t)per_stage * (m.style == ETC_GPT ? 12 : 6) + 6;
+  const size_t o_start = 0, o_first = al((size_t)(n_dev + 1) * 4), o_mask = o_first + al((size_t)n_dev * nG * 4),
+               o_pieces = o_mask + al((size_t)n_dev * mask_words * 4);
+  const size_t max_total = o_pieces + (size_t)n_dev * n_kinds * max_inst * 4 * sizeof(Piece);
+
+  std::lock_guard<std::mutex> lock(g_up_mu);
+  cudaError_t e = cudaSetDevice(current_device());
+  if (e == cudaSuccess) e = upload_prepare(max_total);
+  if (e != cudaSuccess) { set_error_detail("etc_layout_create staging", e); return ETC_ERR_CUDA; }
+  char* host = static_cast<char*>(g_pinned);
+  int32_t* dev_start = reinterpret_cast<int32_t*>(host + o_start);
+  int32_t* first = reinterpret_cast<int32_t*>(host + o_first);
+  uint32_t* ltmask = reinterpret_cast<uint32_t*>(host + o_mask);
+  Piece* pieces = reinterpret_cast<Piece*>(host + o_pieces);
+  memset(first, 0xFF, (size_t)n_dev * nG * 4);
+  memset(ltmask, 0, (size_t)n_dev * mask_words * 4);
+  int64_t* bufbytes = new int64_t[(size_t)n_dev * ETC_NUM_KINDS]();
+  size_t np = 0;
+
+  std::vector<std::vector<Sh>> shr(tp);     // shards of (stage, tp-rank r), in GROUP order: tied replica first
+  for (int s = 0; s < pp; ++s) {
+    // the stage's tensor instances in LOCAL order: pre, layers ascending, post, tied replica (reading A11)
+    std::vector<std::pair<int32_t, bool>> inst;
     for (int pass = 0; pass < 3; ++pass)
       for (int t = 0; t < nT; ++t) {
         const LTensor& T = lts[t];
@@ -129,105 +161,99 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
         if (pass == 2 && s != pp - 1) continue;
         inst.push_back({t, false});
       }
-    if (two_inst && s == pp - 1) inst.push_back({0, true});
-    // shard geometry + start offsets in the (s,r) local flat space
-    struct Sh { int64_t start, n, rb[2], nrb, c0, W; int nblk; };
-    std::vector<Sh> sh(inst.size());
-    int64_t Lloc = 0;
-    for (size_t i = 0; i < inst.size(); ++i) {
-      const LTensor& T = lts[inst[i].lt];
-      Sh& q = sh[i];
-      q.nblk = 1; q.rb[0] = q.rb[1] = 0; q.nrb = T.rows; q.c0 = 0; q.W = T.cols;
-      switch (T.split) {
-        case COL: q.nrb = T.rows / tp; q.rb[0] = r * q.nrb; break;
-        case ROW: q.W = T.cols / tp; q.c0 = r * q.W; break;
-        case COL2: { const int64_t F = T.rows / 2; q.nblk = 2; q.nrb = F / tp; q.rb[0] = r * q.nrb; q.rb[1] = F + r * q.nrb; break; }
-        default: break;
-      }
-      q.n = (int64_t)q.nblk * q.nrb * q.W; q.start = Lloc; Lloc += q.n;
-    }
-    const size_t dev_first_piece = pieces.size();
-    for (int kind = 0; kind < ETC_NUM_KINDS; ++kind) {
-      if (!((m.kinds >> kind) & 1)) continue;
-      const int64_t es = kind == 0 ? m.param_dtype : 4;
-      const bool dp_sharded = cfg->dist_opt && dp > 1 && kind >= 1;
-      int64_t lo = 0, hi = Lloc;
-      if (dp_sharded) {                                      // reading A14: contiguous flat range, chunk = ceil(Lloc/dp)
-        const int64_t chunk = (Lloc + dp - 1) / dp;
-        lo = std::min<int64_t>(Lloc, (int64_t)d * chunk); hi = std::min<int64_t>(Lloc, (int64_t)(d + 1) * chunk);
-      }
-      bufbytes[(size_t)dev * ETC_NUM_KINDS + kind] = (hi - lo) * es;
+    const bool has_replica = two_inst && s == pp - 1;
+    if (has_replica) inst.push_back({0, true});
+    for (int r = 0; r < tp; ++r) {           // shard geometry depends on (s, r) only
+      std::vector<Sh>& sh = shr[r];
+      sh.resize(inst.size());
+      int64_t pos = 0;
       for (size_t i = 0; i < inst.size(); ++i) {
-        const Sh& q = sh[i];
-        const LTensor& T = lts[inst[i].lt];
-        const int64_t a = std::max(lo, q.start) - q.start, b = std::min(hi, q.start + q.n) - q.start;
-        if (b <= a) continue;
-        uint16_t flags = 0;
-        if (inst[i].post_copy) flags |= PF_POST_COPY;
-        if (!(two_inst && inst[i].lt == 0)) flags |= PF_SOLE_INST;
-        if (T.split != REPL) flags |= PF_TP_SHARDED;
-        if (dp_sharded) flags |= PF_DP_SHARDED;
-        // decompose the held flat range [a,b) of the shard into rectangles of local rows x local cols
-        struct LR { int64_t i0, i1, j0, j1; };
-        LR rects[4]; int nr = 0;
-        const int64_t ia = a / q.W, ja = a % q.W, ib = b / q.W, jb = b % q.W;
-        if (ia == ib) rects[nr++] = {ia, ia + 1, ja, jb};
-        else {
-          int64_t body0 = ia;
-          if (ja > 0) { rects[nr++] = {ia, ia + 1, ja, q.W}; body0 = ia + 1; }
-          if (ib > body0) {
-            if (q.nblk == 2 && body0 < q.nrb && ib > q.nrb) {          // body spans the gate/up block boundary
-              rects[nr++] = {body0, q.nrb, 0, q.W}; rects[nr++] = {q.nrb, ib, 0, q.W};
-            } else rects[nr++] = {body0, ib, 0, q.W};
-          }
-          if (jb > 0) rects[nr++] = {ib, ib + 1, 0, jb};
+        const LTensor& T = lts[inst[i].first];
+        // start offsets follow LOCAL order; the slot order is GROUP order (the replica, tensor 0, goes first)
+        Sh& q = sh[inst[i].second ? 0 : i + (has_replica ? 1 : 0)];
+        q.nblk = 1; q.rb[0] = q.rb[1] = 0; q.nrb = T.rows; q.c0 = 0; q.W = T.cols; q.lt = inst[i].first;
+        switch (T.split) {
+          case COL: q.nrb = T.rows / tp; q.rb[0] = r * q.nrb; break;
+          case ROW: q.W = T.cols / tp; q.c0 = r * q.W; break;
+          case COL2: { const int64_t F = T.rows / 2; q.nblk = 2; q.nrb = F / tp; q.rb[0] = r * q.nrb; q.rb[1] = F + r * q.nrb; break; }
+          default: break;
         }
-        for (int k = 0; k < nr; ++k) {
-          const LR& R = rects[k];
-          const int blk = (int)(R.i0 / q.nrb);
-          Piece p;
-          p.dev = dev; p.grp = kind * nT + inst[i].lt;
-          p.r0 = (int32_t)(q.rb[blk] + R.i0 % q.nrb); p.nr = (int32_t)(R.i1 - R.i0);
-          p.c0 = (int32_t)(q.c0 + R.j0); p.nc = (int32_t)(R.j1 - R.j0);
-          p.lrow0 = (int32_t)R.i0; p.lcol0 = (int32_t)R.j0; p.W = (int32_t)q.W;
-          p.s = (int16_t)s; p.r = (int16_t)r; p.d = (int16_t)d; p.flags = flags;
-          p.boff = (q.start + R.i0 * q.W + R.j0 - lo) * es;
-          p.f0 = a; p.f1 = b;
-          pieces.push_back(p);
-        }
-        ltmask[(size_t)dev * mask_words + inst[i].lt / 32] |= 1u << (inst[i].lt % 32);
+        q.n = (int64_t)q.nblk * q.nrb * q.W; q.start = pos; pos += q.n;
+        q.flags = (inst[i].second ? PF_POST_COPY : 0) | ((two_inst && inst[i].first == 0) ? 0 : PF_SOLE_INST) |
+                  (T.split != REPL ? PF_TP_SHARDED : 0);
       }
     }
-    std::stable_sort(pieces.begin() + dev_first_piece, pieces.end(),
-                     [](const Piece& x, const Piece& y) { return x.grp < y.grp; });
+    for (int d = 0; d < dp; ++d)
+      for (int r = 0; r < tp; ++r) {
+        const int dev = r + tp * (d + dp * s);
+        const std::vector<Sh>& sh = shr[r];
+        int64_t Lloc = 0; for (const Sh& q : sh) Lloc += q.n;
+        dev_start[dev] = (int32_t)np;
+        for (const Sh& q : sh) ltmask[(size_t)dev * mask_words + q.lt / 32] |= 1u << (q.lt % 32);
+        for (int kind = 0; kind < ETC_NUM_KINDS; ++kind) {
+          if (!((m.kinds >> kind) & 1)) continue;
+          const int64_t es = kind == 0 ? m.param_dtype : 4;
+          const bool dp_sharded = cfg->dist_opt && dp > 1 && kind >= 1;
+          int64_t lo = 0, hi = Lloc;
+          if (dp_sharded) {                                  // reading A14: contiguous flat range, chunk = ceil(Lloc/dp)
+            const int64_t chunk = (Lloc + dp - 1) / dp;
+            lo = std::min<int64_t>(Lloc, (int64_t)d * chunk); hi = std::min<int64_t>(Lloc, (int64_t)(d + 1) * chunk);
+          }
+          bufbytes[(size_t)dev * ETC_NUM_KINDS + kind] = (hi - lo) * es;
+          for (const Sh& q : sh) {
+            const int64_t a = std::max(lo, q.start) - q.start, b = std::min(hi, q.start + q.n) - q.start;
+            if (b <= a) continue;
+            const uint16_t flags = q.flags | (dp_sharded ? PF_DP_SHARDED : 0);
+            const int32_t grp = kind * nT + q.lt;
+            first[(size_t)dev * nG + grp] = (int32_t)np;
+            // decompose the held flat range [a,b) of the shard into rectangles of local rows x local cols
+            int64_t rect[4][4]; int nr = 0;
+            auto add = [&](int64_t i0, int64_t i1, int64_t j0, int64_t j1) { rect[nr][0] = i0; rect[nr][1] = i1; rect[nr][2] = j0; rect[nr][3] = j1; ++nr; };
+            if (a == 0 && b == q.n) {                        // whole shard (the common case)
+              if (q.nblk == 2) { add(0, q.nrb, 0, q.W); add(q.nrb, 2 * q.nrb, 0, q.W); } else add(0, q.nrb, 0, q.W);
+            } else {
+              const int64_t ia = a / q.W, ja = a % q.W, ib = b / q.W, jb = b % q.W;
+              if (ia == ib) add(ia, ia + 1, ja, jb);
+              else {
+                int64_t body0 = ia;
+                if (ja > 0) { add(ia, ia + 1, ja, q.W); body0 = ia + 1; }
+                if (ib > body0) {
+                  if (q.nblk == 2 && body0 < q.nrb && ib > q.nrb) { add(body0, q.nrb, 0, q.W); add(q.nrb, ib, 0, q.W); }
+                  else add(body0, ib, 0, q.W);
+                }
+                if (jb > 0) add(ib, ib + 1, 0, jb);
+              }
+            }
+            for (int k = 0; k < nr; ++k) {
+              const int64_t i0 = rect[k][0], i1 = rect[k][1], j0 = rect[k][2], j1 = rect[k][3];
+              const int blk = (int)(i0 / q.nrb);
+              Piece& p = pieces[np++];
+              p.dev = dev; p.grp = grp;
+              p.r0 = (int32_t)(q.rb[blk] + i0 % q.nrb); p.nr = (int32_t)(i1 - i0);
+              p.c0 = (int32_t)(q.c0 + j0); p.nc = (int32_t)(j1 - j0);
+              p.lrow0 = (int32_t)i0; p.lcol0 = (int32_t)j0; p.W = (int32_t)q.W;
+              p.s = (int16_t)s; p.r = (int16_t)r; p.d = (int16_t)d; p.flags = flags;
+              p.boff = (q.start + i0 * q.W + j0 - lo) * es;
+              p.f0 = a; p.f1 = b;
+            }
+          }
+        }
+      }
   }
-  dev_start[n_dev] = (int32_t)pieces.size();
-  if (pieces.size() > (size_t)INT32_MAX) return ETC_ERR_INVALID_ARG;
+  dev_start[n_dev] = (int32_t)np;
+  int32_t max_dev_pieces = 0;
+  for (int i = 0; i < n_dev; ++i) max_dev_pieces = std::max(max_dev_pieces, dev_start[i + 1] - dev_start[i]);
+  const size_t total = o_pieces + al(np * sizeof(Piece));
 
-  std::vector<int32_t> first((size_t)n_dev * nG, -1);
-  for (int32_t i = (int32_t)pieces.size() - 1; i >= 0; --i) first[(size_t)pieces[i].dev * nG + pieces[i].grp] = i;
-
-  // one device blob: pieces | dev_start | first | ltmask
-  auto al = [](size_t x) { return (x + 255) & ~size_t(255); };
-  const size_t o_pieces = 0, o_start = al(pieces.size() * sizeof(Piece)),
-               o_first = o_start + al(dev_start.size() * 4), o_mask = o_first + al(first.size() * 4),
-               total = o_mask + al(ltmask.size() * 4);
-  std::vector<char> host(total, 0);
-  if (!pieces.empty()) memcpy(host.data() + o_pieces, pieces.data(), pieces.size() * sizeof(Piece));
-  memcpy(host.data() + o_start, dev_start.data(), dev_start.size() * 4);
-  memcpy(host.data() + o_first, first.data(), first.size() * 4);
-  memcpy(host.data() + o_mask, ltmask.data(), ltmask.size() * 4);
-
-  if (getenv("ETC_TIME_LAYOUT")) { timespec ts; clock_gettime(CLOCK_MONOTONIC, &ts); fprintf(stderr, "layout host build done at %ld.%09ld pieces=%zu total=%zu\n", ts.tv_sec, ts.tv_nsec, pieces.size(), total); }
   etc_layout* L = new etc_layout();
-  L->model = m; L->cfg = *cfg;
-  cudaError_t e = cudaSetDevice(current_device());
-  if (e == cudaSuccess) e = cudaMalloc(&L->d_blob, total);
-  if (e == cudaSuccess) e = cudaMemcpy(L->d_blob, host.data(), total, cudaMemcpyHostToDevice);
+  L->model = m; L->cfg = *cfg; L->h_buffer_bytes = bufbytes; L->max_dev_pieces = max_dev_pieces;
+  e = cudaMallocAsync(&L->d_blob, total, g_up_stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(L->d_blob, host, total, cudaMemcpyHostToDevice, g_up_stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(g_up_stream);
   if (e != cudaSuccess) {
     set_error_detail("etc_layout_create upload", e);
-    if (L->d_blob) cudaFree(L->d_blob);
-    delete L;
+    if (L->d_blob) cudaFreeAsync(L->d_blob, g_up_stream);
+    delete[] bufbytes; delete L;
     return ETC_ERR_CUDA;
   }
   char* base = (char*)L->d_blob;
@@ -236,18 +262,17 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   L->t.first = (const int32_t*)(base + o_first);
   L->t.ltmask = (const uint32_t*)(base + o_mask);
   L->t.n_dev = n_dev; L->t.n_grp = nG; L->t.n_tensors = nT; L->t.mask_words = mask_words;
-  L->t.n_pieces = (int32_t)pieces.size();
+  L->t.n_pieces = (int32_t)np;
   L->t.tp = tp; L->t.pp = pp; L->t.dp = dp;
   for (int k = 0; k < ETC_NUM_KINDS; ++k) L->t.elem_bytes[k] = k == 0 ? m.param_dtype : 4;
-  L->h_buffer_bytes = new int64_t[bufbytes.size()];
-  memcpy(L->h_buffer_bytes, bufbytes.data(), bufbytes.size() * sizeof(int64_t));
   *out = L;
   return ETC_OK;
 }
 
 extern "C" void etc_layout_destroy(etc_layout* L) {
   if (!L) return;
-  if (L->d_blob) cudaFree(L->d_blob);
+  // stream-ordered free on the last stream that used the tables: kernels already enqueued there finish first
+  if (L->d_blob) cudaFreeAsync(L->d_blob, L->last_stream ? L->last_stream : g_up_stream);
   delete[] L->h_buffer_bytes;
   delete L;
 }

@@ -113,6 +113,7 @@ extern "C" etc_status etc_migrate_phase(const etc_plan* pl, const void* const* s
     if (reinterpret_cast<uintptr_t>(dst_bufs[i]) & 15) return ETC_ERR_INVALID_ARG;
   }
   cudaStream_t st = (cudaStream_t)stream;
+  pl->last_stream = st;
   // pointer tables: source pointers then destination pointers
   ETC_CUDA_TRY(cudaMemcpyAsync(pl->d_ptrs, src_bufs, sizeof(void*) * ns, cudaMemcpyHostToDevice, st));
   ETC_CUDA_TRY(cudaMemcpyAsync(pl->d_ptrs + ns, dst_bufs, sizeof(void*) * nd, cudaMemcpyHostToDevice, st));

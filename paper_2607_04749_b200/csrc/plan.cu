@@ -9,6 +9,7 @@
 // Pass 1 counts slices / chunks / bytes per unit; a single-CTA scan turns the counts into slice indices, chunk indices
 // and segment offsets (warp-shuffle prefix sums); pass 2 recomputes the slices and writes them at their final
 // positions.  Order inside a segment is canonical (piece order), so the staging layout is deterministic.
+#include <algorithm>
 #include <cstring>
 #include <vector>
 #include "etc_internal.h"
@@ -121,24 +122,33 @@ __device__ __forceinline__ int64_t warp_excl_scan64(int64_t v, int lane, int64_t
 
 constexpr int PLAN_WARPS = 8;
 
-// pass 1: per-unit counts.  unit u = od * n_new + n.
+// A unit u = od * n_new + n is cut into B sub-blocks of `span` consecutive pieces of rank n (span a multiple of 32), one
+// warp each, so that small device counts still fill the machine.  [i0,i1) = the piece range of sub-block b.
+__device__ __forceinline__ void sub_range(const DeviceTables& newT, int n, int B, int b, int& i0, int& i1) {
+  const int qb = newT.dev_start[n], qe = newT.dev_start[n + 1];
+  const int span = (((qe - qb) + B - 1) / B + 31) & ~31;
+  i0 = min(qe, qb + b * span); i1 = min(qe, i0 + span);
+}
+
+// pass 1: per-(unit, sub-block) counts; unit totals accumulated with integer atomics (order-independent sums).
 __global__ void __launch_bounds__(PLAN_WARPS * 32)
-plan_count_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict__ device_map, int flags,
-                  UnitCount* __restrict__ units) {
+plan_count_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict__ device_map, int B,
+                  UnitCount* __restrict__ units, BlockCount* __restrict__ blocks) {
   const int lane = threadIdx.x & 31;
-  const long long u = (long long)blockIdx.x * PLAN_WARPS + (threadIdx.x >> 5);
+  const long long w = (long long)blockIdx.x * PLAN_WARPS + (threadIdx.x >> 5);
   const long long U = (long long)oldT.n_dev * newT.n_dev;
-  if (u >= U) return;
+  if (w >= U * B) return;
+  const long long u = w / B; const int b = (int)(w % B);
   const int od = (int)(u / newT.n_dev), n = (int)(u % newT.n_dev);
   const int p = device_map[n];
   const bool local_unit = (od == p);
   int64_t n_sl = 0, n_ch = 0, bytes = 0, padded = 0;
   bool common = false;
-  for (int w = lane; w < newT.mask_words; w += 32)
-    common |= (newT.ltmask[(size_t)n * newT.mask_words + w] & oldT.ltmask[(size_t)od * oldT.mask_words + w]) != 0;
+  for (int k = lane; k < newT.mask_words; k += 32)
+    common |= (newT.ltmask[(size_t)n * newT.mask_words + k] & oldT.ltmask[(size_t)od * oldT.mask_words + k]) != 0;
   if (__any_sync(0xffffffffu, common)) {
-    const int qb = newT.dev_start[n], qe = newT.dev_start[n + 1];
-    for (int i = qb + lane; i < qe; i += 32) {
+    int i0, i1; sub_range(newT, n, B, b, i0, i1);
+    for (int i = i0 + lane; i < i1; i += 32) {
       const Piece q = newT.pieces[i];
       const int kind = q.grp / newT.n_tensors, es = newT.elem_bytes[kind];
       for_each_slice(oldT, q, od, p, local_unit, es, kind, [&](const SliceGeom& s) {
@@ -148,18 +158,20 @@ plan_count_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restric
   }
   n_sl = warp_sum64(n_sl); n_ch = warp_sum64(n_ch); bytes = warp_sum64(bytes); padded = warp_sum64(padded);
   if (lane == 0) {
-    UnitCount c;
-    c.slices = n_sl; c.chunks = n_ch; c.bytes = bytes;
-    c.padded = (padded + 511) & ~(int64_t)511;                 // pair segments start 512-byte aligned
-    c.staged = (!local_unit || (flags & ETC_ALL_STAGED)) ? 1 : 0;
-    units[u] = c;
+    blocks[w] = BlockCount{n_sl, n_ch, padded};
+    if (n_sl) {
+      atomicAdd(reinterpret_cast<unsigned long long*>(&units[u].slices), (unsigned long long)n_sl);
+      atomicAdd(reinterpret_cast<unsigned long long*>(&units[u].chunks), (unsigned long long)n_ch);
+      atomicAdd(reinterpret_cast<unsigned long long*>(&units[u].bytes), (unsigned long long)bytes);
+      atomicAdd(reinterpret_cast<unsigned long long*>(&units[u].padded), (unsigned long long)padded);
+    }
   }
 }
 
 // single-CTA exclusive scan over units (+ map validation, traffic matrix, totals)
 constexpr int SCAN_THREADS = 1024;
 __global__ void __launch_bounds__(SCAN_THREADS)
-plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int n_old, int n_new, int P,
+plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int n_old, int n_new, int P, int flags,
                  const int32_t* __restrict__ device_map, UnitBase* __restrict__ bases, int64_t* __restrict__ traffic,
                  PlanTotals* __restrict__ totals) {
   __shared__ int64_t s_w[5][32];
@@ -183,11 +195,17 @@ plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int n_old, in
   int64_t loc = 0, rem = 0;
   for (long long base = 0; base < U; base += SCAN_THREADS) {
     const long long u = base + tid;
-    UnitCount c{0, 0, 0, 0, 0};
-    if (u < U) c = units[u];
+    UnitCount c{0, 0, 0, 0};
+    bool staged = false; int od = 0, p = 0;
+    if (u < U) {
+      c = units[u];
+      od = (int)(u / n_new); p = device_map[(int)(u % n_new)];
+      staged = (od != p) || (flags & ETC_ALL_STAGED);
+      c.padded = (c.padded + 511) & ~(int64_t)511;             // pair segments start 512-byte aligned
+    }
     int64_t v[5];
-    v[0] = c.staged ? c.slices : 0; v[1] = c.staged ? c.chunks : 0; v[2] = c.staged ? c.padded : 0;
-    v[3] = c.staged ? 0 : c.slices; v[4] = c.staged ? 0 : c.chunks;
+    v[0] = staged ? c.slices : 0; v[1] = staged ? c.chunks : 0; v[2] = staged ? c.padded : 0;
+    v[3] = staged ? 0 : c.slices; v[4] = staged ? 0 : c.chunks;
     int64_t ex[5];
 #pragma unroll
     for (int k = 0; k < 5; ++k) { int64_t tot; ex[k] = warp_excl_scan64(v[k], lane, tot); if (lane == 31) s_w[k][wid] = tot; }
@@ -198,13 +216,12 @@ plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int n_old, in
     }
     __syncthreads();
     if (u < U) {
-      UnitBase b;
-      b.slice0 = s_carry[c.staged ? 0 : 3] + s_w[c.staged ? 0 : 3][wid] + ex[c.staged ? 0 : 3];
-      b.chunk0 = s_carry[c.staged ? 1 : 4] + s_w[c.staged ? 1 : 4][wid] + ex[c.staged ? 1 : 4];
-      b.stg0 = c.staged ? s_carry[2] + s_w[2][wid] + ex[2] : -1;
-      bases[u] = b;
+      UnitBase ub;
+      ub.slice0 = s_carry[staged ? 0 : 3] + s_w[staged ? 0 : 3][wid] + ex[staged ? 0 : 3];
+      ub.chunk0 = s_carry[staged ? 1 : 4] + s_w[staged ? 1 : 4][wid] + ex[staged ? 1 : 4];
+      ub.stg0 = staged ? s_carry[2] + s_w[2][wid] + ex[2] : -1;
+      bases[u] = ub;
       if (!bad && c.bytes) {
-        const int od = (int)(u / n_new), n = (int)(u % n_new), p = device_map[n];
         traffic[(size_t)od * P + p] = c.bytes;
         if (od == p) loc += c.bytes; else rem += c.bytes;
       }
@@ -236,31 +253,35 @@ __device__ __forceinline__ int vec_of(int64_t a) {
   return a == 0 ? 16 : (low >= 16 ? 16 : (int)low);
 }
 
-// pass 2: recompute the slices of each unit and write slice records (+ first chunk index) at their final positions
+// pass 2: recompute the slices of each (unit, sub-block) and write slice records (+ first chunk index) at their final
+// positions: unit base (scan) + earlier sub-blocks of the unit + warp-level prefix inside the sub-block.
 __global__ void __launch_bounds__(PLAN_WARPS * 32)
-plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict__ device_map, int flags,
-                 const UnitCount* __restrict__ units, const UnitBase* __restrict__ bases,
+plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict__ device_map, int flags, int B,
+                 const BlockCount* __restrict__ blocks, const UnitBase* __restrict__ bases,
                  etc_slice* __restrict__ sl_staged, etc_slice* __restrict__ sl_local,
                  int64_t* __restrict__ c0_staged, int64_t* __restrict__ c0_local) {
   const int lane = threadIdx.x & 31;
-  const long long u = (long long)blockIdx.x * PLAN_WARPS + (threadIdx.x >> 5);
+  const long long w = (long long)blockIdx.x * PLAN_WARPS + (threadIdx.x >> 5);
   const long long U = (long long)oldT.n_dev * newT.n_dev;
-  if (u >= U) return;
-  const UnitCount cnt = units[u];
-  if (cnt.slices == 0) return;
+  if (w >= U * B) return;
+  const long long u = w / B; const int b = (int)(w % B);
+  if (blocks[w].slices == 0) return;
   const UnitBase ub = bases[u];
   const int od = (int)(u / newT.n_dev), n = (int)(u % newT.n_dev);
   const int p = device_map[n];
-  const bool local_unit = (od == p), staged = cnt.staged != 0;
+  const bool local_unit = (od == p), staged = !local_unit || (flags & ETC_ALL_STAGED);
   etc_slice* sl_out = staged ? sl_staged : sl_local;
   int64_t* c0_out = staged ? c0_staged : c0_local;
-  int64_t run_sl = ub.slice0, run_ch = ub.chunk0, run_stg = staged ? ub.stg0 : 0;
-  const int qb = newT.dev_start[n], qe = newT.dev_start[n + 1];
-  for (int ib = qb; ib < qe; ib += 32) {                       // all lanes iterate together (warp scans inside)
+  int64_t pre_sl = 0, pre_ch = 0, pre_pad = 0;                 // totals of the unit's earlier sub-blocks
+  for (int k = lane; k < b; k += 32) { const BlockCount c = blocks[u * B + k]; pre_sl += c.slices; pre_ch += c.chunks; pre_pad += c.padded; }
+  int64_t run_sl = ub.slice0 + warp_sum64(pre_sl), run_ch = ub.chunk0 + warp_sum64(pre_ch);
+  int64_t run_stg = (staged ? ub.stg0 : 0) + warp_sum64(pre_pad);
+  int i0, i1; sub_range(newT, n, B, b, i0, i1);
+  for (int ib = i0; ib < i1; ib += 32) {                       // all lanes iterate together (warp scans inside)
     const int i = ib + lane;
     Piece q; int kind = 0, es = 0;
     int64_t my_sl = 0, my_ch = 0, my_pad = 0;
-    if (i < qe) {
+    if (i < i1) {
       q = newT.pieces[i]; kind = q.grp / newT.n_tensors; es = newT.elem_bytes[kind];
       for_each_slice(oldT, q, od, p, local_unit, es, kind, [&](const SliceGeom& s) {
         my_sl += 1; my_ch += slice_chunks(s); my_pad += slice_padded(s);
@@ -271,7 +292,7 @@ plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict
     int64_t o_ch = run_ch + warp_excl_scan64(my_ch, lane, tot_ch);
     int64_t o_stg = run_stg + warp_excl_scan64(my_pad, lane, tot_pad);
     run_sl += tot_sl; run_ch += tot_ch; run_stg += tot_pad;
-    if (i < qe && my_sl) {
+    if (i < i1 && my_sl) {
       for_each_slice(oldT, q, od, p, local_unit, es, kind, [&](const SliceGeom& s) {
         etc_slice r;
         r.src_off = s.src_off; r.dst_off = s.dst_off; r.stg_off = staged ? o_stg : -1; r.row_bytes = s.row_bytes;
@@ -323,6 +344,11 @@ plan_chunks_kernel(const etc_slice* __restrict__ slices, const int64_t* __restri
 
 using namespace etc;
 
+// pinned slots for the totals read-back (a pageable destination would make the copy synchronous and slower)
+static PlanTotals* g_pinned_totals = nullptr;
+static unsigned g_pinned_next = 0;
+constexpr unsigned N_PINNED_TOTALS = 64;
+
 extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
                                       int32_t flags, etc_plan** out, void* stream) {
   clear_error_detail();
@@ -332,7 +358,11 @@ extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout*
   const int n_old = old_l->t.n_dev, n_new = new_l->t.n_dev, P = n_old > n_new ? n_old : n_new;
   if ((long long)P * ETC_NUM_KINDS > 65535) return ETC_ERR_WORKSPACE;
   cudaStream_t st = (cudaStream_t)stream;
+  old_l->last_stream = new_l->last_stream = st;
   const long long U = (long long)n_old * n_new;
+  // sub-blocks per unit: enough warps to fill the machine when there are few units, 1 when there are many
+  const int want = (new_l->max_dev_pieces + 31) / 32;
+  const int B = (int)std::max<long long>(1, std::min<long long>(want, 65536 / U));
 
   etc_plan* pl = new etc_plan();
   pl->n_old = n_old; pl->n_new = n_new; pl->P = P; pl->flags = flags; pl->stream_created_on = st;
@@ -340,6 +370,9 @@ extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout*
   pl->new_bytes.assign(new_l->h_buffer_bytes, new_l->h_buffer_bytes + (size_t)n_new * ETC_NUM_KINDS);
   auto fail = [&](etc_status s) { etc_plan_destroy(pl); return s; };
 #define PLAN_TRY(expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) { set_error_detail(#expr, _e); return fail(ETC_ERR_CUDA); } } while (0)
+
+  if (!g_pinned_totals) PLAN_TRY(cudaMallocHost(&g_pinned_totals, sizeof(PlanTotals) * N_PINNED_TOTALS));
+  PlanTotals* h_tot = &g_pinned_totals[__atomic_fetch_add(&g_pinned_next, 1u, __ATOMIC_RELAXED) % N_PINNED_TOTALS];
 
   // device_map may live on the host or on the device
   cudaPointerAttributes attr{};
@@ -354,34 +387,52 @@ extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout*
       seen[p] = 1;
     }
   }
-  PLAN_TRY(cudaMallocAsync(&pl->d_map, sizeof(int32_t) * (size_t)n_new, st));
+  // workspace blob 1: units | bases | blocks | traffic | totals | map | pointer tables
+  auto al = [](size_t x) { return (x + 255) & ~size_t(255); };
+  const size_t o_units = 0, o_bases = o_units + al(sizeof(UnitCount) * (size_t)U),
+               o_blocks = o_bases + al(sizeof(UnitBase) * (size_t)U),
+               o_traffic = o_blocks + al(sizeof(BlockCount) * (size_t)U * B),
+               o_totals = o_traffic + al(sizeof(int64_t) * (size_t)P * P), o_map = o_totals + al(sizeof(PlanTotals)),
+               o_ptrs = o_map + al(sizeof(int32_t) * (size_t)n_new),
+               ws_bytes = o_ptrs + al(sizeof(void*) * (size_t)(n_old + n_new) * ETC_NUM_KINDS);
+  PLAN_TRY(cudaMallocAsync(&pl->d_ws, ws_bytes, st));
+  char* ws = static_cast<char*>(pl->d_ws);
+  pl->d_units = reinterpret_cast<UnitCount*>(ws + o_units); pl->d_bases = reinterpret_cast<UnitBase*>(ws + o_bases);
+  pl->d_blocks = reinterpret_cast<BlockCount*>(ws + o_blocks); pl->d_traffic = reinterpret_cast<int64_t*>(ws + o_traffic);
+  pl->d_totals = reinterpret_cast<PlanTotals*>(ws + o_totals); pl->d_map = reinterpret_cast<int32_t*>(ws + o_map);
+  pl->d_ptrs = reinterpret_cast<void**>(ws + o_ptrs);
   PLAN_TRY(cudaMemcpyAsync(pl->d_map, device_map, sizeof(int32_t) * (size_t)n_new,
                            on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
-  PLAN_TRY(cudaMallocAsync(&pl->d_units, sizeof(UnitCount) * (size_t)U, st));
-  PLAN_TRY(cudaMallocAsync(&pl->d_bases, sizeof(UnitBase) * (size_t)U, st));
-  PLAN_TRY(cudaMallocAsync(&pl->d_traffic, sizeof(int64_t) * (size_t)P * P, st));
-  PLAN_TRY(cudaMallocAsync(&pl->d_totals, sizeof(PlanTotals), st));
+  PLAN_TRY(cudaMemsetAsync(pl->d_units, 0, sizeof(UnitCount) * (size_t)U, st));
 
-  const unsigned grid = (unsigned)((U + PLAN_WARPS - 1) / PLAN_WARPS);
-  plan_count_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, flags, pl->d_units);
+  const unsigned grid = (unsigned)((U * B + PLAN_WARPS - 1) / PLAN_WARPS);
+  plan_count_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, B, pl->d_units, pl->d_blocks);
   PLAN_TRY(cudaGetLastError());
-  plan_scan_kernel<<<1, SCAN_THREADS, 0, st>>>(pl->d_units, U, n_old, n_new, P, pl->d_map, pl->d_bases, pl->d_traffic,
-                                               pl->d_totals);
+  plan_scan_kernel<<<1, SCAN_THREADS, 0, st>>>(pl->d_units, U, n_old, n_new, P, flags, pl->d_map, pl->d_bases,
+                                               pl->d_traffic, pl->d_totals);
   PLAN_TRY(cudaGetLastError());
   count_launch(2);
-  PLAN_TRY(cudaMemcpyAsync(&pl->totals, pl->d_totals, sizeof(PlanTotals), cudaMemcpyDeviceToHost, st));
+  PLAN_TRY(cudaMemcpyAsync(h_tot, pl->d_totals, sizeof(PlanTotals), cudaMemcpyDeviceToHost, st));
   PLAN_TRY(cudaStreamSynchronize(st));                          // the one host sync: sizes must come back
+  pl->totals = *h_tot;
   if (pl->totals.bad_map) return fail(ETC_ERR_BAD_MAP);
 
+  // blob 2: slice records | first-chunk indices | chunk descriptors
   const PlanTotals& t = pl->totals;
-  if (t.n_slices_staged) PLAN_TRY(cudaMallocAsync(&pl->d_sl_staged, sizeof(etc_slice) * (size_t)t.n_slices_staged, st));
-  if (t.n_slices_local) PLAN_TRY(cudaMallocAsync(&pl->d_sl_local, sizeof(etc_slice) * (size_t)t.n_slices_local, st));
-  if (t.n_chunks_staged) PLAN_TRY(cudaMallocAsync(&pl->d_ch_staged, sizeof(Chunk) * (size_t)t.n_chunks_staged, st));
-  if (t.n_chunks_local) PLAN_TRY(cudaMallocAsync(&pl->d_ch_local, sizeof(Chunk) * (size_t)t.n_chunks_local, st));
-  if (t.n_slices_staged) PLAN_TRY(cudaMallocAsync(&pl->d_c0_staged, sizeof(int64_t) * (size_t)t.n_slices_staged, st));
-  if (t.n_slices_local) PLAN_TRY(cudaMallocAsync(&pl->d_c0_local, sizeof(int64_t) * (size_t)t.n_slices_local, st));
+  const size_t o_sls = 0, o_sll = o_sls + al(sizeof(etc_slice) * (size_t)t.n_slices_staged),
+               o_c0s = o_sll + al(sizeof(etc_slice) * (size_t)t.n_slices_local),
+               o_c0l = o_c0s + al(8 * (size_t)t.n_slices_staged), o_chs = o_c0l + al(8 * (size_t)t.n_slices_local),
+               o_chl = o_chs + al(sizeof(Chunk) * (size_t)t.n_chunks_staged),
+               tb_bytes = o_chl + al(sizeof(Chunk) * (size_t)t.n_chunks_local);
+  if (tb_bytes) {
+    PLAN_TRY(cudaMallocAsync(&pl->d_tb, tb_bytes, st));
+    char* tb = static_cast<char*>(pl->d_tb);
+    pl->d_sl_staged = reinterpret_cast<etc_slice*>(tb + o_sls); pl->d_sl_local = reinterpret_cast<etc_slice*>(tb + o_sll);
+    pl->d_c0_staged = reinterpret_cast<int64_t*>(tb + o_c0s); pl->d_c0_local = reinterpret_cast<int64_t*>(tb + o_c0l);
+    pl->d_ch_staged = reinterpret_cast<Chunk*>(tb + o_chs); pl->d_ch_local = reinterpret_cast<Chunk*>(tb + o_chl);
+  }
   if (t.n_slices_staged + t.n_slices_local) {
-    plan_fill_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, flags, pl->d_units, pl->d_bases,
+    plan_fill_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, flags, B, pl->d_blocks, pl->d_bases,
                                                        pl->d_sl_staged, pl->d_sl_local, pl->d_c0_staged, pl->d_c0_local);
     PLAN_TRY(cudaGetLastError());
     count_launch();
@@ -398,8 +449,6 @@ extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout*
     PLAN_TRY(cudaGetLastError());
     count_launch();
   }
-  // pointer tables for migrate (filled per call)
-  PLAN_TRY(cudaMallocAsync(&pl->d_ptrs, sizeof(void*) * (size_t)(n_old + n_new) * ETC_NUM_KINDS, st));
 #undef PLAN_TRY
   *out = pl;
   return ETC_OK;
@@ -407,10 +456,9 @@ extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout*
 
 extern "C" void etc_plan_destroy(etc_plan* pl) {
   if (!pl) return;
-  cudaStream_t st = pl->stream_created_on;
-  void* ptrs[] = {pl->d_map, pl->d_units, pl->d_bases, pl->d_traffic, pl->d_totals, pl->d_sl_staged, pl->d_sl_local,
-                  pl->d_ch_staged, pl->d_ch_local, pl->d_c0_staged, pl->d_c0_local, pl->d_ptrs};
-  for (void* p : ptrs) if (p) cudaFreeAsync(p, st);
+  cudaStream_t st = pl->last_stream ? pl->last_stream : pl->stream_created_on;
+  if (pl->d_ws) cudaFreeAsync(pl->d_ws, st);
+  if (pl->d_tb) cudaFreeAsync(pl->d_tb, st);
   delete pl;
 }
 

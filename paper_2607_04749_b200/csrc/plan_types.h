@@ -5,7 +5,8 @@
 
 namespace etc {
 
-struct UnitCount { int64_t slices, chunks, bytes, padded; int64_t staged; };   // per (source device, new rank) unit
+struct UnitCount { int64_t slices, chunks, bytes, padded; };   // per (source device, new rank) unit
+struct BlockCount { int64_t slices, chunks, padded; };          // per (unit, sub-block of pieces)
 struct UnitBase { int64_t slice0, chunk0, stg0; };
 struct PlanTotals {
   int64_t n_slices_staged, n_chunks_staged, staging_bytes, n_slices_local, n_chunks_local;
@@ -28,15 +29,19 @@ static_assert(sizeof(Chunk) == 48, "Chunk layout");
 struct etc_plan {
   int32_t n_old = 0, n_new = 0, P = 0, flags = 0;
   cudaStream_t stream_created_on = nullptr;
+  mutable cudaStream_t last_stream = nullptr;      // last stream a migrate was enqueued on (frees are ordered after it)
   etc::PlanTotals totals{};
+  void* d_ws = nullptr;                            // blob 1: the tables below up to d_ptrs
+  void* d_tb = nullptr;                            // blob 2: slices, first-chunk indices, chunks
   int32_t* d_map = nullptr;
   etc::UnitCount* d_units = nullptr;
   etc::UnitBase* d_bases = nullptr;
+  etc::BlockCount* d_blocks = nullptr;
   int64_t* d_traffic = nullptr;
   etc::PlanTotals* d_totals = nullptr;
   etc_slice* d_sl_staged = nullptr; etc_slice* d_sl_local = nullptr;
   etc::Chunk* d_ch_staged = nullptr; etc::Chunk* d_ch_local = nullptr;
   int64_t* d_c0_staged = nullptr; int64_t* d_c0_local = nullptr;
-  std::vector<int64_t> old_bytes, new_bytes;   // buffer sizes [dev*4+kind], for argument checks in migrate
-  void** d_ptrs = nullptr;             // [n_old*4] source pointers then [n_new*4] destination pointers
+  std::vector<int64_t> old_bytes, new_bytes;       // buffer sizes [dev*4+kind], for argument checks in migrate
+  void** d_ptrs = nullptr;                         // [n_old*4] source pointers then [n_new*4] destination pointers
 };

@@ -191,6 +191,69 @@ sketch_hungarian_kernel(const int64_t* __restrict__ overlap, int N, int P, const
   }
 }
 
+// Same algorithm for P <= 32: one warp, lane j owns column j, the matrix sits in shared memory, and every step is a
+// handful of shuffles — no block barrier, no global-memory latency inside the Dijkstra loop.
+__global__ void __launch_bounds__(32)
+sketch_hungarian_warp_kernel(const int64_t* __restrict__ overlap, int N, int P, const uint8_t* __restrict__ avail,
+                             int32_t* __restrict__ device_map, int64_t* __restrict__ local_bytes) {
+  __shared__ int64_t ov[32 * 32];
+  __shared__ int32_t way[32];
+  __shared__ int64_t u[32];                   // row potentials
+  const int lane = threadIdx.x;
+  for (int i = lane; i < N * P; i += 32) ov[i] = overlap[i];
+  u[lane] = 0;
+  __syncwarp();
+  const bool usable = lane < P && (!avail || avail[lane]);
+  int64_t v = 0;                              // potential of column `lane`
+  int rowof = -1;                             // row matched to column `lane`
+  bool fail = false;
+  for (int i = 0; i < N && !fail; ++i) {
+    int64_t minv = SK_INF; bool used = !usable;
+    int i0 = i, j0 = -1;
+    while (true) {
+      const int64_t ui0 = u[i0];
+      ArgMin best{SK_INF, 0x7fffffff, 1};
+      if (!used) {
+        const int64_t cur = -ov[i0 * P + lane] - ui0 - v;
+        if (cur < minv) { minv = cur; way[lane] = j0; }
+        best = ArgMin{minv, lane, rowof >= 0 ? 1 : 0};
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) { ArgMin b = argmin_shfl(best, o); if (argmin_less(b, best)) best = b; }
+      if (best.v >= SK_INF) { fail = true; break; }
+      const int64_t delta = best.v; const int j1 = best.j;
+      // dual update: tree rows (the root i and the rows matched to tree columns) gain delta, tree columns lose it
+      __syncwarp();
+      if (lane == 0) u[i] += delta;
+      if (usable) { if (used) { u[rowof] += delta; v -= delta; } else minv -= delta; if (lane == j1) used = true; }
+      __syncwarp();
+      j0 = j1; i0 = __shfl_sync(0xffffffffu, rowof, j1);
+      if (i0 < 0) break;
+    }
+    if (fail) break;
+    __syncwarp();
+    // augment along the alternating path (every lane walks it; lane j updates its own column)
+    int j = j0;
+    while (j >= 0) {
+      const int jp = way[j];
+      const int r = jp >= 0 ? __shfl_sync(0xffffffffu, rowof, jp) : i;
+      if (lane == j) rowof = r;
+      j = jp;
+    }
+    __syncwarp();
+  }
+  if (fail) {
+    if (lane < N) device_map[lane] = -1;
+    if (lane == 0) *local_bytes = -1;
+    return;
+  }
+  int64_t acc = 0;
+  if (lane < P && rowof >= 0) { device_map[rowof] = lane; acc = ov[rowof * P + lane]; }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if (lane == 0) *local_bytes = acc;
+}
+
 }  // namespace etc
 
 using namespace etc;
@@ -206,6 +269,12 @@ extern "C" etc_status etc_sketch(const int64_t* d_overlap, int32_t n_new, int32_
     sketch_exhaustive_kernel<<<1, SK_THREADS, 0, st>>>(d_overlap, n_new, P, d_avail, d_device_map, d_local_bytes);
   } else if (method == ETC_SKETCH_HUNGARIAN) {
     if (P > ETC_SKETCH_MAX_P) return ETC_ERR_WORKSPACE;
+    if (P <= 32) {
+      sketch_hungarian_warp_kernel<<<1, 32, 0, st>>>(d_overlap, n_new, P, d_avail, d_device_map, d_local_bytes);
+      ETC_CUDA_TRY(cudaGetLastError());
+      count_launch();
+      return ETC_OK;
+    }
     const size_t smem = (size_t)n_new * 8 + (size_t)P * 8;
     static bool attr_set = false;
     if (!attr_set) {
