@@ -8,5 +8,5 @@ index map, no cost/overlap/sketch/plan logic.  Neither `oracle/` nor
 from .workloads import (KIND_PARAM, KIND_MASTER, KIND_ADAM_M, KIND_ADAM_V, KIND_NAMES,
                         STYLE_GPT, STYLE_LLAMA, WORKLOADS, workload, scaled_workloads,
                         tiny_models, tiny_parallel_cfgs)
-from .values import (logical_values, index_stamp, position_stamp, position_stamp_torch,
+from .values import (logical_values, index_stamp, position_stamp, position_stamp_at, position_stamp_torch,
                      fp32_to_bf16_bits, bench_fill_torch)

@@ -96,6 +96,14 @@ def position_stamp(dev: int, kind: int, n: int, elem_bytes: int, start: int = 0)
     return ((w >> np.uint64(5)) & np.uint64(0xFFFFFFFF)).astype(np.uint32)
 
 
+def position_stamp_at(dev: int, kind: int, idx, elem_bytes: int) -> np.ndarray:
+    """`position_stamp` evaluated at arbitrary positions idx (int array)."""
+    w = _pos_words(dev, kind, np.asarray(idx).astype(np.uint64))
+    if elem_bytes == 2:
+        return ((w >> np.uint64(7)) & np.uint64(0xFFFF)).astype(np.uint16)
+    return ((w >> np.uint64(5)) & np.uint64(0xFFFFFFFF)).astype(np.uint32)
+
+
 def position_stamp_torch(dev: int, kind: int, n: int, elem_bytes: int, device):
     """Same values as `position_stamp`, produced directly in device memory (int16 / int32 bit patterns)."""
     import torch
