@@ -26,9 +26,18 @@ sys.path.insert(0, ROOT)
 METRIC = "migrate GB/s (read+write)"
 UNIT = "GB/s"
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
-# capture (profiles/), keyed by workload.  None until a capture exists.
-NCU_TRAFFIC = {}
+def ncu_traffic(workload_name: str, mode: str, kernel_prefix: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
+    captures (profiles/ncu_traffic.csv names the capture each row was read from).  None where no capture exists."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    try:
+        import csv
+        for row in csv.DictReader(open(p)):
+            if row["workload"] == workload_name and row["mode"] == mode and kernel_prefix.startswith(row["kernel"]):
+                return int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
+    except Exception:
+        pass
+    return None
 
 
 def measured_peak():
@@ -94,6 +103,23 @@ class ClockSampler:
 
 def dist_env():
     return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def max_over_ranks(ms: float, world: int, device=None) -> float:
+    """Timing of a multi-rank run = the slowest rank's device time (the only data `torch.distributed` carries here:
+    "replicas only").  Works on any backend (nccl on the GPU box, gloo in the CPU tests)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(world: int, hbm_bytes_per_replica: int, ms_per_step: float) -> float:
+    """Whole-job GB/s: every rank migrates one replica of the workload (weak scaling), time = max over ranks."""
+    return world * hbm_bytes_per_replica / (ms_per_step * 1e-3) / 1e9
 
 
 # ------------------------------------------------------------------------------------------------ reference arm (oracle)
@@ -241,16 +267,13 @@ def run_cuda(args, w):
     launches = E.kernel_launches() - launches0
     clocks = sampler.stop()
     total_ms = t_begin.elapsed_time(t_end)
-    if world > 1:
-        t = torch.tensor([total_ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, world, dev)
     ms_per_step = total_ms / args.steps
     stats = plan.stats
     phase = lambda a, b: statistics.mean(r[a].elapsed_time(r[b]) for r in recs)
     bd = {"layout_ms": phase(0, 1), "cost_matrix_ms": phase(1, 2), "sketch_ms": phase(2, 3), "plan_ms": phase(3, 4),
           "pack_local_ms": phase(4, 5), "unpack_ms": phase(5, 6)}
-    value = world * hbm_bytes / (ms_per_step * 1e-3) / 1e9
+    value = job_value(world, hbm_bytes, ms_per_step)
 
     # ---- roofline of the dominant kernel, timed live with CUDA events over the timed region
     peak, peak_src = measured_peak()
@@ -264,7 +287,7 @@ def run_cuda(args, w):
     achieved = kbytes / (kms * 1e-3) / 1e9 if kms > 0 else 0.0
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "peak_source": peak_src, "algorithmic_bytes_per_launch": kbytes,
-                "avg_launch_ms": kms, "traffic": NCU_TRAFFIC.get(w["name"] + ("_staged" if args.all_staged else "")),
+                "avg_launch_ms": kms, "traffic": ncu_traffic(w["name"], "ALL_STAGED" if args.all_staged else "LOCAL_DIRECT", kname),
                 "frac_of_8TBs_nominal": achieved / 8000.0}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -378,10 +401,8 @@ def e2e(E, torch, args, w, dev, src, dst, staging, step, hbm_bytes, world, barri
     b.record(stream)
     barrier()
     ms = a.elapsed_time(b) / n
-    if world > 1:
-        import torch.distributed as dist
-        t = torch.tensor([ms], device=dev); dist.all_reduce(t, op=dist.ReduceOp.MAX); ms = float(t.item())
-    return {"value": world * hbm_bytes / (ms * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ms, "steps": n,
+    ms = max_over_ranks(ms, world, dev)
+    return {"value": job_value(world, hbm_bytes, ms), "unit": UNIT, "ms_per_step": ms, "steps": n,
             "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo,
             "note": "host-pinned old shards -> H2D -> whole path -> D2H of new shards, all inside the timed region"}
 
