@@ -103,6 +103,24 @@ enum { ETC_SKETCH_AUTO = 0, ETC_SKETCH_EXHAUSTIVE = 1, ETC_SKETCH_HUNGARIAN = 2 
 etc_status etc_sketch(const int64_t* d_overlap, int32_t n_new, int32_t P, const uint8_t* d_avail, int32_t method,
                       int32_t* d_device_map, int64_t* d_local_bytes, void* stream);
 
+/* (f1) Virtual rank allocator: Algorithm 2 "Placement-Aware Remapping" (the garbled listing is read
+ * from the prose PAPER.md:220-222, reading A23) composed with the sketch into one final device map
+ * (communication coalescing): pass d_out_map to etc_plan_create and every element moves in ONE hop.
+ *   d_device_map [cw] int32 (device memory): the sketch, curr rank -> physical device, injective into [0,P),
+ *                 P = max(pw, cw); pw / cw = world size of the prev / curr state; devices_per_node = n of Algorithm 2.
+ *   mode: ETC_DEFRAG_OCCUPANCY (lines 1-9: idle devices in ascending order are paired with occupied devices in descending
+ *         order until they meet, so the occupied devices become exactly [0,cw) and whole nodes are freed),
+ *         ETC_DEFRAG_EFFICIENCY (lines 10-20: every device of a fragmented node takes its target rank, rank k on device k,
+ *         so each TP group sits inside a node), ETC_DEFRAG_BOTH (occupancy, then efficiency on its result).
+ * Outputs (device memory): d_out_map [cw] int32 (must not alias d_device_map); d_n_ops [2] int32 = number of migration
+ * operators of the occupancy and of the efficiency stage; d_ops: optional (NULL to skip) [2][cw][2] int32, operators
+ * <a,b> in the paper's order: occupancy <idle device, occupied device> at d_ops[0..], efficiency <target rank, current
+ * load or -1> at d_ops[2*cw..].  If the input is not an injective map, d_out_map is filled with -1 and d_n_ops with -1.
+ * Enqueues on `stream`; no host synchronisation. */
+enum { ETC_DEFRAG_OCCUPANCY = 1, ETC_DEFRAG_EFFICIENCY = 2, ETC_DEFRAG_BOTH = 3 };
+etc_status etc_defrag(const int32_t* d_device_map, int32_t pw, int32_t cw, int32_t devices_per_node, int32_t mode,
+                      int32_t* d_out_map, int32_t* d_ops, int32_t* d_n_ops, void* stream);
+
 /* (a4) Plan.  device_map: [n_new] int32, host OR device pointer.  flags: ETC_LOCAL_DIRECT (slices whose source device
  * is the destination device are copied old buffer -> new buffer, never staged: the paper's Refer, reading A19) or
  * ETC_ALL_STAGED (every slice goes through pack/unpack: a measurement mode).  Synchronises `stream` once (sizes must

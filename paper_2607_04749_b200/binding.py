@@ -15,12 +15,13 @@ _inited = False
 ETC_LOCAL_DIRECT, ETC_ALL_STAGED = 0, 1
 ETC_SKETCH_AUTO, ETC_SKETCH_EXHAUSTIVE, ETC_SKETCH_HUNGARIAN = 0, 1, 2
 ETC_PHASE_PACK, ETC_PHASE_UNPACK, ETC_PHASE_ALL = 1, 2, 3
+ETC_DEFRAG_OCCUPANCY, ETC_DEFRAG_EFFICIENCY, ETC_DEFRAG_BOTH = 1, 2, 3
 
 EXPORTED_SYMBOLS = (
     "etc_init", "etc_layout_create", "etc_layout_destroy", "etc_layout_num_devices", "etc_layout_num_pieces",
     "etc_layout_buffer_bytes", "etc_cost_matrix", "etc_sketch", "etc_plan_create", "etc_plan_destroy",
     "etc_plan_get_stats", "etc_plan_get_traffic", "etc_plan_get_slices", "etc_migrate", "etc_migrate_phase",
-    "etc_status_string", "etc_last_error_detail", "etc_kernel_launches",
+    "etc_status_string", "etc_last_error_detail", "etc_kernel_launches", "etc_defrag",
 )
 
 
@@ -71,6 +72,7 @@ def lib():
         L.etc_layout_buffer_bytes.restype = i64; L.etc_layout_buffer_bytes.argtypes = [vp, i32, i32]
         L.etc_cost_matrix.restype = i32; L.etc_cost_matrix.argtypes = [vp, vp, vp, vp, vp, vp]
         L.etc_sketch.restype = i32; L.etc_sketch.argtypes = [vp, i32, i32, vp, i32, vp, vp, vp]
+        L.etc_defrag.restype = i32; L.etc_defrag.argtypes = [vp, i32, i32, i32, i32, vp, vp, vp, vp]
         L.etc_plan_create.restype = i32; L.etc_plan_create.argtypes = [vp, vp, vp, i32, C.POINTER(vp), vp]
         L.etc_plan_destroy.restype = None; L.etc_plan_destroy.argtypes = [vp]
         L.etc_plan_get_stats.restype = i32; L.etc_plan_get_stats.argtypes = [vp, C.POINTER(_PlanStats)]
@@ -182,6 +184,22 @@ def etc_sketch(overlap, avail=None, method: int = ETC_SKETCH_AUTO, stream=None, 
         av = avail.data_ptr()
     _check(lib().etc_sketch(overlap.data_ptr(), n_new, P, av, method, dm.data_ptr(), lb.data_ptr(), _stream(stream)))
     return dm, lb
+
+
+def etc_defrag(device_map, pw: int, cw: int, devices_per_node: int, mode: int = ETC_DEFRAG_BOTH, want_ops: bool = True,
+               stream=None):
+    """(f1) include/etc.h etc_defrag.  device_map: CUDA int32 tensor [cw].  -> (out_map [cw] int32, n_ops [2] int32,
+    ops [2][cw][2] int32 or None), all CUDA tensors.  Asynchronous."""
+    import torch
+    _ensure_init()
+    assert device_map.is_cuda and device_map.dtype == torch.int32 and device_map.numel() == cw
+    assert device_map.is_contiguous()
+    out = torch.empty(cw, dtype=torch.int32, device=device_map.device)
+    n_ops = torch.empty(2, dtype=torch.int32, device=device_map.device)
+    ops = torch.full((2, cw, 2), -9, dtype=torch.int32, device=device_map.device) if want_ops else None
+    _check(lib().etc_defrag(device_map.data_ptr(), pw, cw, devices_per_node, mode, out.data_ptr(),
+                            ops.data_ptr() if want_ops else 0, n_ops.data_ptr(), _stream(stream)))
+    return out, n_ops, ops
 
 
 @dataclass
