@@ -123,9 +123,11 @@ etc_status etc_defrag(const int32_t* d_device_map, int32_t pw, int32_t cw, int32
 
 /* (a4) Plan.  device_map: [n_new] int32, host OR device pointer.  flags: ETC_LOCAL_DIRECT (slices whose source device
  * is the destination device are copied old buffer -> new buffer, never staged: the paper's Refer, reading A19) or
- * ETC_ALL_STAGED (every slice goes through pack/unpack: a measurement mode).  Synchronises `stream` once (sizes must
- * come back to the host).  Fails with ETC_ERR_BAD_MAP if the map is not injective into [0,P). */
-enum { ETC_LOCAL_DIRECT = 0, ETC_ALL_STAGED = 1 };
+ * ETC_ALL_STAGED (every slice goes through pack/unpack: a measurement mode); OR-ed with ETC_KIND_MAJOR to order
+ * slices, chunks and staging segments by state kind first (one segment per (kind, source, destination) instead of one
+ * per (source, destination)): required for state chunking, etc_plan_set_rounds below.  Synchronises `stream` once
+ * (sizes must come back to the host).  Fails with ETC_ERR_BAD_MAP if the map is not injective into [0,P). */
+enum { ETC_LOCAL_DIRECT = 0, ETC_ALL_STAGED = 1, ETC_KIND_MAJOR = 2 };
 etc_status etc_plan_create(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
                            int32_t flags, etc_plan** out, void* stream);
 void etc_plan_destroy(etc_plan* plan);
@@ -170,6 +172,28 @@ etc_status etc_migrate_phase(const etc_plan* plan, const void* const* src_bufs, 
                              void* staging, int32_t phases, void* stream);
 
 #define ETC_CHUNK_BYTES 65536
+
+/* (f2) State chunking with bounded staging and eager release ("state chunking to migrate states in
+ * sequential chunks with on-demand buffer allocation, and eager release of source-side state ... after each round";
+ * :378 "reduces the peak to one optimizer component at a time").  For a plan created with ETC_KIND_MAJOR,
+ * etc_plan_set_rounds cuts the migration into rounds, kind by kind (PARAM, MASTER, ADAM_M, ADAM_V), each kind into as
+ * many rounds as it takes for every round to use at most max_staging_bytes (>= 2*ETC_CHUNK_BYTES) of staging.
+ * Synchronises `stream` once (round sizes come back to the host).  May be called again with another bound.
+ * etc_migrate_round enqueues round `round` (pack + local, unpack; `phases` as in etc_migrate_phase).  It reads only the
+ * source buffers and writes only the destination buffers of the round's kind: pointers of other kinds are not looked
+ * at (they may be NULL: already released, or not yet allocated).  `staging` needs only etc_round_info.staging_bytes
+ * bytes and may be reused by the next round on the same stream.  After all rounds every destination byte has been
+ * written exactly once, bit-identical to etc_migrate. */
+typedef struct {
+  int32_t kind, sub, n_sub, pad;     /* state kind; round `sub` of `n_sub` of that kind */
+  int64_t staging_bytes;             /* staging bytes this round uses (<= max_staging_bytes) */
+  int64_t staged_bytes, local_bytes; /* payload bytes through pack/unpack, and copied directly */
+  int64_t n_chunks_staged, n_chunks_local;
+} etc_round_info;
+etc_status etc_plan_set_rounds(etc_plan* plan, int64_t max_staging_bytes, int32_t* n_rounds, void* stream);
+etc_status etc_plan_get_round(const etc_plan* plan, int32_t round, etc_round_info* out);
+etc_status etc_migrate_round(const etc_plan* plan, int32_t round, const void* const* src_bufs, void* const* dst_bufs,
+                             void* staging, int32_t phases, void* stream);
 
 const char* etc_status_string(etc_status s);   /* static strings */
 const char* etc_last_error_detail(void);       /* thread-local; CUDA error text after ETC_ERR_CUDA, else "" */

@@ -12,7 +12,7 @@ _LIB_PATH = os.path.join(_HERE, "libetc.so")
 _lib = None
 _inited = False
 
-ETC_LOCAL_DIRECT, ETC_ALL_STAGED = 0, 1
+ETC_LOCAL_DIRECT, ETC_ALL_STAGED, ETC_KIND_MAJOR = 0, 1, 2
 ETC_SKETCH_AUTO, ETC_SKETCH_EXHAUSTIVE, ETC_SKETCH_HUNGARIAN = 0, 1, 2
 ETC_PHASE_PACK, ETC_PHASE_UNPACK, ETC_PHASE_ALL = 1, 2, 3
 ETC_DEFRAG_OCCUPANCY, ETC_DEFRAG_EFFICIENCY, ETC_DEFRAG_BOTH = 1, 2, 3
@@ -22,6 +22,7 @@ EXPORTED_SYMBOLS = (
     "etc_layout_buffer_bytes", "etc_cost_matrix", "etc_sketch", "etc_plan_create", "etc_plan_destroy",
     "etc_plan_get_stats", "etc_plan_get_traffic", "etc_plan_get_slices", "etc_migrate", "etc_migrate_phase",
     "etc_status_string", "etc_last_error_detail", "etc_kernel_launches", "etc_defrag",
+    "etc_plan_set_rounds", "etc_plan_get_round", "etc_migrate_round",
 )
 
 
@@ -45,6 +46,12 @@ class _PlanStats(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("staging_bytes", "local_bytes", "remote_bytes", "staged_bytes",
                                           "n_slices_local", "n_slices_staged", "n_chunks_local", "n_chunks_staged")] + \
                [(n, C.c_int32) for n in ("n_old", "n_new", "P", "flags")]
+
+
+class _RoundInfo(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("kind", "sub", "n_sub", "pad")] + \
+               [(n, C.c_int64) for n in ("staging_bytes", "staged_bytes", "local_bytes", "n_chunks_staged",
+                                          "n_chunks_local")]
 
 
 class _Slice(C.Structure):
@@ -80,6 +87,9 @@ def lib():
         L.etc_plan_get_slices.restype = i32; L.etc_plan_get_slices.argtypes = [vp, i32, vp]
         L.etc_migrate.restype = i32; L.etc_migrate.argtypes = [vp, vp, vp, vp, vp]
         L.etc_migrate_phase.restype = i32; L.etc_migrate_phase.argtypes = [vp, vp, vp, vp, i32, vp]
+        L.etc_plan_set_rounds.restype = i32; L.etc_plan_set_rounds.argtypes = [vp, i64, C.POINTER(i32), vp]
+        L.etc_plan_get_round.restype = i32; L.etc_plan_get_round.argtypes = [vp, i32, C.POINTER(_RoundInfo)]
+        L.etc_migrate_round.restype = i32; L.etc_migrate_round.argtypes = [vp, i32, vp, vp, vp, i32, vp]
         L.etc_status_string.restype = C.c_char_p; L.etc_status_string.argtypes = [i32]
         L.etc_last_error_detail.restype = C.c_char_p
         L.etc_kernel_launches.restype = i64
@@ -293,6 +303,49 @@ def etc_migrate(plan: Plan, src_bufs: dict, dst_bufs: dict, staging, phases: int
         assert staging.numel() * staging.element_size() >= st.staging_bytes
         sp = staging.data_ptr()
     _check(lib().etc_migrate_phase(plan.h, src_bufs, dst_bufs, sp, phases, _stream(stream)))
+
+
+@dataclass
+class RoundInfo:
+    kind: int
+    sub: int
+    n_sub: int
+    staging_bytes: int
+    staged_bytes: int
+    local_bytes: int
+    n_chunks_staged: int
+    n_chunks_local: int
+
+    @property
+    def hbm_bytes(self) -> int:
+        return 2 * self.local_bytes + 4 * self.staged_bytes
+
+
+def etc_plan_set_rounds(plan: Plan, max_staging_bytes: int, stream=None):
+    """(f2) include/etc.h etc_plan_set_rounds -> [RoundInfo].  The plan must have been created with ETC_KIND_MAJOR."""
+    n = C.c_int32()
+    _check(lib().etc_plan_set_rounds(plan.h, int(max_staging_bytes), C.byref(n), _stream(stream)))
+    out = []
+    for r in range(n.value):
+        info = _RoundInfo()
+        _check(lib().etc_plan_get_round(plan.h, r, C.byref(info)))
+        out.append(RoundInfo(**{f: int(getattr(info, f)) for f, _ in _RoundInfo._fields_ if f != "pad"}))
+    plan.rounds = out
+    return out
+
+
+def etc_migrate_round(plan: Plan, rnd: int, src_bufs, dst_bufs, staging, phases: int = ETC_PHASE_ALL, stream=None):
+    """(f2) one round; only the buffers of the round's kind need to exist in src_bufs / dst_bufs."""
+    st = plan.stats
+    if isinstance(src_bufs, dict):
+        src_bufs = _ptr_table(src_bufs, st.n_old)
+    if isinstance(dst_bufs, dict):
+        dst_bufs = _ptr_table(dst_bufs, st.n_new)
+    sp = 0
+    if staging is not None and staging.numel() > 0:
+        assert staging.numel() * staging.element_size() >= plan.rounds[rnd].staging_bytes
+        sp = staging.data_ptr()
+    _check(lib().etc_migrate_round(plan.h, rnd, src_bufs, dst_bufs, sp, phases, _stream(stream)))
 
 
 def pointer_tables(plan: Plan, src_bufs: dict, dst_bufs: dict):

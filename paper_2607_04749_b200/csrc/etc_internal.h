@@ -40,6 +40,7 @@ struct DeviceTables {            // device memory
   const int32_t* dev_start;      // [n_dev + 1]
   const int32_t* first;          // [n_dev][n_grp]: index of the first piece of (dev, grp) or -1
   const uint32_t* ltmask;        // [n_dev][mask_words]: bit t set if dev holds any piece of logical tensor t
+  const int32_t* kind_start;     // [n_dev][ETC_NUM_KINDS + 1]: piece range of each state kind on dev (pieces are kind-major)
   int32_t n_dev, n_grp, n_tensors, mask_words;
   int32_t n_pieces;
   int32_t tp, pp, dp;

@@ -127,11 +127,12 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   const int mask_words = (nT + 31) / 32;
   int n_kinds = 0; for (int k = 0; k < ETC_NUM_KINDS; ++k) n_kinds += (m.kinds >> k) & 1;
 
-  // blob: dev_start | first | ltmask | pieces (pieces last: their count is known only after the build)
+  // blob: dev_start | first | ltmask | kind_start | pieces (pieces last: their count is known only after the build)
   auto al = [](size_t x) { return (x + 255) & ~size_t(255); };
   const size_t max_inst = (size_t)per_stage * (m.style == ETC_GPT ? 12 : 6) + 6;
   const size_t o_start = 0, o_first = al((size_t)(n_dev + 1) * 4), o_mask = o_first + al((size_t)n_dev * nG * 4),
-               o_pieces = o_mask + al((size_t)n_dev * mask_words * 4);
+               o_kstart = o_mask + al((size_t)n_dev * mask_words * 4),
+               o_pieces = o_kstart + al((size_t)n_dev * (ETC_NUM_KINDS + 1) * 4);
   const size_t max_total = o_pieces + (size_t)n_dev * n_kinds * max_inst * 4 * sizeof(Piece);
 
   std::lock_guard<std::mutex> lock(g_up_mu);
@@ -142,6 +143,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   int32_t* dev_start = reinterpret_cast<int32_t*>(host + o_start);
   int32_t* first = reinterpret_cast<int32_t*>(host + o_first);
   uint32_t* ltmask = reinterpret_cast<uint32_t*>(host + o_mask);
+  int32_t* kind_start = reinterpret_cast<int32_t*>(host + o_kstart);
   Piece* pieces = reinterpret_cast<Piece*>(host + o_pieces);
   memset(first, 0xFF, (size_t)n_dev * nG * 4);
   memset(ltmask, 0, (size_t)n_dev * mask_words * 4);
@@ -191,6 +193,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
         dev_start[dev] = (int32_t)np;
         for (const Sh& q : sh) ltmask[(size_t)dev * mask_words + q.lt / 32] |= 1u << (q.lt % 32);
         for (int kind = 0; kind < ETC_NUM_KINDS; ++kind) {
+          kind_start[(size_t)dev * (ETC_NUM_KINDS + 1) + kind] = (int32_t)np;
           if (!((m.kinds >> kind) & 1)) continue;
           const int64_t es = kind == 0 ? m.param_dtype : 4;
           const bool dp_sharded = cfg->dist_opt && dp > 1 && kind >= 1;
@@ -238,6 +241,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
             }
           }
         }
+        kind_start[(size_t)dev * (ETC_NUM_KINDS + 1) + ETC_NUM_KINDS] = (int32_t)np;
       }
   }
   dev_start[n_dev] = (int32_t)np;
@@ -261,6 +265,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   L->t.dev_start = (const int32_t*)(base + o_start);
   L->t.first = (const int32_t*)(base + o_first);
   L->t.ltmask = (const uint32_t*)(base + o_mask);
+  L->t.kind_start = (const int32_t*)(base + o_kstart);
   L->t.n_dev = n_dev; L->t.n_grp = nG; L->t.n_tensors = nT; L->t.mask_words = mask_words;
   L->t.n_pieces = (int32_t)np;
   L->t.tp = tp; L->t.pp = pp; L->t.dp = dp;

@@ -96,45 +96,68 @@ migrate_copy_kernel(const Chunk* __restrict__ chA, long long nA, const Chunk* __
 
 using namespace etc;
 
-extern "C" etc_status etc_migrate_phase(const etc_plan* pl, const void* const* src_bufs, void* const* dst_bufs,
-                                        void* staging, int32_t phases, void* stream) {
-  clear_error_detail();
+// Validate the caller's pointer tables (only the buffers of `only_kind` if >= 0: the other kinds may already be
+// released or not yet allocated), upload them into `d_ptrs`, and launch the copy kernels over the given
+// chunk ranges.  `staging` is addressed relative to stg_base.
+static etc_status launch_migrate(const etc_plan* pl, const void* const* src_bufs, void* const* dst_bufs, void* staging,
+                                 int32_t phases, cudaStream_t st, void** d_ptrs, int only_kind, long long ca, long long nA,
+                                 long long la, long long nB, int64_t stg_base, int64_t stg_need) {
   if (!pl || !src_bufs || !dst_bufs || phases < 1 || phases > ETC_PHASE_ALL) return ETC_ERR_INVALID_ARG;
-  const PlanTotals& t = pl->totals;
-  if (t.staging_bytes > 0 && !staging) return ETC_ERR_INVALID_ARG;
+  if (stg_need > 0 && !staging) return ETC_ERR_INVALID_ARG;
   if (reinterpret_cast<uintptr_t>(staging) & 15) return ETC_ERR_INVALID_ARG;
   const size_t ns = (size_t)pl->n_old * ETC_NUM_KINDS, nd = (size_t)pl->n_new * ETC_NUM_KINDS;
   for (size_t i = 0; i < ns; ++i) {
+    if (only_kind >= 0 && (int)(i % ETC_NUM_KINDS) != only_kind) continue;
     if (pl->old_bytes[i] > 0 && !src_bufs[i]) return ETC_ERR_INVALID_ARG;
     if (reinterpret_cast<uintptr_t>(src_bufs[i]) & 15) return ETC_ERR_INVALID_ARG;
   }
   for (size_t i = 0; i < nd; ++i) {
+    if (only_kind >= 0 && (int)(i % ETC_NUM_KINDS) != only_kind) continue;
     if (pl->new_bytes[i] > 0 && !dst_bufs[i]) return ETC_ERR_INVALID_ARG;
     if (reinterpret_cast<uintptr_t>(dst_bufs[i]) & 15) return ETC_ERR_INVALID_ARG;
   }
-  cudaStream_t st = (cudaStream_t)stream;
   pl->last_stream = st;
   // pointer tables: source pointers then destination pointers
-  ETC_CUDA_TRY(cudaMemcpyAsync(pl->d_ptrs, src_bufs, sizeof(void*) * ns, cudaMemcpyHostToDevice, st));
-  ETC_CUDA_TRY(cudaMemcpyAsync(pl->d_ptrs + ns, dst_bufs, sizeof(void*) * nd, cudaMemcpyHostToDevice, st));
-  const void* const* d_src = pl->d_ptrs; void* const* d_dst = pl->d_ptrs + ns;
-  const long long nA = t.n_chunks_staged, nB = t.n_chunks_local;
+  ETC_CUDA_TRY(cudaMemcpyAsync(d_ptrs, src_bufs, sizeof(void*) * ns, cudaMemcpyHostToDevice, st));
+  ETC_CUDA_TRY(cudaMemcpyAsync(d_ptrs + ns, dst_bufs, sizeof(void*) * nd, cudaMemcpyHostToDevice, st));
+  const void* const* d_src = d_ptrs; void* const* d_dst = d_ptrs + ns;
+  char* stg = static_cast<char*>(staging) - stg_base;          // chunk records carry offsets of the full staging layout
   if ((phases & ETC_PHASE_PACK) && nA + nB > 0) {
-    migrate_copy_kernel<false><<<(unsigned)(nA + nB), CP_THREADS, 0, st>>>(pl->d_ch_staged, nA, pl->d_ch_local, d_src,
-                                                                           d_dst, static_cast<char*>(staging));
+    migrate_copy_kernel<false><<<(unsigned)(nA + nB), CP_THREADS, 0, st>>>(pl->d_ch_staged + ca, nA, pl->d_ch_local + la,
+                                                                           d_src, d_dst, stg);
     ETC_CUDA_TRY(cudaGetLastError());
     count_launch();
   }
   if ((phases & ETC_PHASE_UNPACK) && nA > 0) {
-    migrate_copy_kernel<true><<<(unsigned)nA, CP_THREADS, 0, st>>>(pl->d_ch_staged, nA, nullptr, d_src, d_dst,
-                                                                   static_cast<char*>(staging));
+    migrate_copy_kernel<true><<<(unsigned)nA, CP_THREADS, 0, st>>>(pl->d_ch_staged + ca, nA, nullptr, d_src, d_dst, stg);
     ETC_CUDA_TRY(cudaGetLastError());
     count_launch();
   }
   return ETC_OK;
 }
 
+extern "C" etc_status etc_migrate_phase(const etc_plan* pl, const void* const* src_bufs, void* const* dst_bufs,
+                                        void* staging, int32_t phases, void* stream) {
+  clear_error_detail();
+  if (!pl) return ETC_ERR_INVALID_ARG;
+  const PlanTotals& t = pl->totals;
+  return launch_migrate(pl, src_bufs, dst_bufs, staging, phases, (cudaStream_t)stream, pl->d_ptrs, -1, 0,
+                        t.n_chunks_staged, 0, t.n_chunks_local, 0, t.staging_bytes);
+}
+
 extern "C" etc_status etc_migrate(const etc_plan* pl, const void* const* src_bufs, void* const* dst_bufs, void* staging,
                                   void* stream) {
   return etc_migrate_phase(pl, src_bufs, dst_bufs, staging, ETC_PHASE_ALL, stream);
+}
+
+// (f2) one round of state chunking: see rounds.cu
+extern "C" etc_status etc_migrate_round(const etc_plan* pl, int32_t round, const void* const* src_bufs,
+                                        void* const* dst_bufs, void* staging, int32_t phases, void* stream) {
+  clear_error_detail();
+  if (!pl || round < 0 || (size_t)round >= pl->rounds.size()) return ETC_ERR_INVALID_ARG;
+  const RoundRec& r = pl->rounds[round];
+  const size_t n_ptrs = ((size_t)(pl->n_old + pl->n_new) * ETC_NUM_KINDS * sizeof(void*) + 255) / 256 * 256 / sizeof(void*);
+  return launch_migrate(pl, src_bufs, dst_bufs, staging, phases, (cudaStream_t)stream,
+                        pl->d_round_ptrs + n_ptrs * (size_t)round, r.kind, r.ca, r.cb - r.ca, r.la, r.lb - r.la,
+                        r.stg_base, r.stg_span);
 }

@@ -122,24 +122,26 @@ __device__ __forceinline__ int64_t warp_excl_scan64(int64_t v, int lane, int64_t
 
 constexpr int PLAN_WARPS = 8;
 
-// A unit u = od * n_new + n is cut into B sub-blocks of `span` consecutive pieces of rank n (span a multiple of 32), one
-// warp each, so that small device counts still fill the machine.  [i0,i1) = the piece range of sub-block b.
-__device__ __forceinline__ void sub_range(const DeviceTables& newT, int n, int B, int b, int& i0, int& i1) {
-  const int qb = newT.dev_start[n], qe = newT.dev_start[n + 1];
+// A unit u = (kq * n_old + od) * n_new + n (kq = 0 unless the plan is kind-major: then kq = state kind) is cut into B
+// sub-blocks of `span` consecutive pieces of rank n (span a multiple of 32), one warp each, so that small device counts
+// still fill the machine.  [i0,i1) = the piece range of sub-block b.
+__device__ __forceinline__ void sub_range(const DeviceTables& newT, int n, int kq, int K, int B, int b, int& i0, int& i1) {
+  const int qb = K == 1 ? newT.dev_start[n] : newT.kind_start[n * (ETC_NUM_KINDS + 1) + kq];
+  const int qe = K == 1 ? newT.dev_start[n + 1] : newT.kind_start[n * (ETC_NUM_KINDS + 1) + kq + 1];
   const int span = (((qe - qb) + B - 1) / B + 31) & ~31;
   i0 = min(qe, qb + b * span); i1 = min(qe, i0 + span);
 }
 
 // pass 1: per-(unit, sub-block) counts; unit totals accumulated with integer atomics (order-independent sums).
 __global__ void __launch_bounds__(PLAN_WARPS * 32)
-plan_count_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict__ device_map, int B,
+plan_count_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict__ device_map, int K, int B,
                   UnitCount* __restrict__ units, BlockCount* __restrict__ blocks) {
   const int lane = threadIdx.x & 31;
   const long long w = (long long)blockIdx.x * PLAN_WARPS + (threadIdx.x >> 5);
-  const long long U = (long long)oldT.n_dev * newT.n_dev;
+  const long long U = (long long)K * oldT.n_dev * newT.n_dev;
   if (w >= U * B) return;
   const long long u = w / B; const int b = (int)(w % B);
-  const int od = (int)(u / newT.n_dev), n = (int)(u % newT.n_dev);
+  const int n = (int)(u % newT.n_dev), od = (int)((u / newT.n_dev) % oldT.n_dev), kq = (int)(u / newT.n_dev / oldT.n_dev);
   const int p = device_map[n];
   const bool local_unit = (od == p);
   int64_t n_sl = 0, n_ch = 0, bytes = 0, padded = 0;
@@ -147,7 +149,7 @@ plan_count_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restric
   for (int k = lane; k < newT.mask_words; k += 32)
     common |= (newT.ltmask[(size_t)n * newT.mask_words + k] & oldT.ltmask[(size_t)od * oldT.mask_words + k]) != 0;
   if (__any_sync(0xffffffffu, common)) {
-    int i0, i1; sub_range(newT, n, B, b, i0, i1);
+    int i0, i1; sub_range(newT, n, kq, K, B, b, i0, i1);
     for (int i = i0 + lane; i < i1; i += 32) {
       const Piece q = newT.pieces[i];
       const int kind = q.grp / newT.n_tensors, es = newT.elem_bytes[kind];
@@ -171,7 +173,7 @@ plan_count_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restric
 // single-CTA exclusive scan over units (+ map validation, traffic matrix, totals)
 constexpr int SCAN_THREADS = 1024;
 __global__ void __launch_bounds__(SCAN_THREADS)
-plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int n_old, int n_new, int P, int flags,
+plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int K, int n_old, int n_new, int P, int flags,
                  const int32_t* __restrict__ device_map, UnitBase* __restrict__ bases, int64_t* __restrict__ traffic,
                  PlanTotals* __restrict__ totals) {
   __shared__ int64_t s_w[5][32];
@@ -179,7 +181,10 @@ plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int n_old, in
   __shared__ int64_t s_loc[32], s_rem[32];
   __shared__ uint32_t s_seen[1024];          // P <= 32767 bits
   __shared__ int s_bad;
+  __shared__ int64_t s_kind[ETC_NUM_KINDS][3];
+  const long long U1 = U / K;                                  // units per kind (kind-major) or all units
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  if (tid < ETC_NUM_KINDS * 3) s_kind[tid / 3][tid % 3] = 0;
   if (tid < 5) s_carry[tid] = 0;
   if (tid == 0) s_bad = 0;
   for (int i = tid; i < 1024; i += SCAN_THREADS) s_seen[i] = 0;
@@ -199,7 +204,7 @@ plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int n_old, in
     bool staged = false; int od = 0, p = 0;
     if (u < U) {
       c = units[u];
-      od = (int)(u / n_new); p = device_map[(int)(u % n_new)];
+      od = (int)((u / n_new) % n_old); p = device_map[(int)(u % n_new)];
       staged = (od != p) || (flags & ETC_ALL_STAGED);
       c.padded = (c.padded + 511) & ~(int64_t)511;             // pair segments start 512-byte aligned
     }
@@ -221,8 +226,14 @@ plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int n_old, in
       ub.chunk0 = s_carry[staged ? 1 : 4] + s_w[staged ? 1 : 4][wid] + ex[staged ? 1 : 4];
       ub.stg0 = staged ? s_carry[2] + s_w[2][wid] + ex[2] : -1;
       bases[u] = ub;
+      if (K > 1 && u % U1 == 0) {                              // first unit of a kind: where the kind's tables start
+        const int kq = (int)(u / U1);
+        s_kind[kq][0] = s_carry[1] + s_w[1][wid] + ex[1];
+        s_kind[kq][1] = s_carry[2] + s_w[2][wid] + ex[2];
+        s_kind[kq][2] = s_carry[4] + s_w[4][wid] + ex[4];
+      }
       if (!bad && c.bytes) {
-        traffic[(size_t)od * P + p] = c.bytes;
+        atomicAdd(reinterpret_cast<unsigned long long*>(&traffic[(size_t)od * P + p]), (unsigned long long)c.bytes);
         if (od == p) loc += c.bytes; else rem += c.bytes;
       }
     }
@@ -243,6 +254,9 @@ plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int n_old, in
       t.n_slices_staged = s_carry[0]; t.n_chunks_staged = s_carry[1]; t.staging_bytes = s_carry[2];
       t.n_slices_local = s_carry[3]; t.n_chunks_local = s_carry[4];
       t.local_bytes = loc; t.remote_bytes = rem; t.bad_map = bad ? 1 : 0;
+      for (int k = 0; k < ETC_NUM_KINDS; ++k) for (int j = 0; j < 3; ++j) t.kind_base[k][j] = s_kind[k][j];
+      t.kind_base[ETC_NUM_KINDS][0] = s_carry[1]; t.kind_base[ETC_NUM_KINDS][1] = s_carry[2];
+      t.kind_base[ETC_NUM_KINDS][2] = s_carry[4];
       *totals = t;
     }
   }
@@ -256,18 +270,18 @@ __device__ __forceinline__ int vec_of(int64_t a) {
 // pass 2: recompute the slices of each (unit, sub-block) and write slice records (+ first chunk index) at their final
 // positions: unit base (scan) + earlier sub-blocks of the unit + warp-level prefix inside the sub-block.
 __global__ void __launch_bounds__(PLAN_WARPS * 32)
-plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict__ device_map, int flags, int B,
+plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict__ device_map, int flags, int K, int B,
                  const BlockCount* __restrict__ blocks, const UnitBase* __restrict__ bases,
                  etc_slice* __restrict__ sl_staged, etc_slice* __restrict__ sl_local,
                  int64_t* __restrict__ c0_staged, int64_t* __restrict__ c0_local) {
   const int lane = threadIdx.x & 31;
   const long long w = (long long)blockIdx.x * PLAN_WARPS + (threadIdx.x >> 5);
-  const long long U = (long long)oldT.n_dev * newT.n_dev;
+  const long long U = (long long)K * oldT.n_dev * newT.n_dev;
   if (w >= U * B) return;
   const long long u = w / B; const int b = (int)(w % B);
   if (blocks[w].slices == 0) return;
   const UnitBase ub = bases[u];
-  const int od = (int)(u / newT.n_dev), n = (int)(u % newT.n_dev);
+  const int n = (int)(u % newT.n_dev), od = (int)((u / newT.n_dev) % oldT.n_dev), kq = (int)(u / newT.n_dev / oldT.n_dev);
   const int p = device_map[n];
   const bool local_unit = (od == p), staged = !local_unit || (flags & ETC_ALL_STAGED);
   etc_slice* sl_out = staged ? sl_staged : sl_local;
@@ -276,7 +290,7 @@ plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict
   for (int k = lane; k < b; k += 32) { const BlockCount c = blocks[u * B + k]; pre_sl += c.slices; pre_ch += c.chunks; pre_pad += c.padded; }
   int64_t run_sl = ub.slice0 + warp_sum64(pre_sl), run_ch = ub.chunk0 + warp_sum64(pre_ch);
   int64_t run_stg = (staged ? ub.stg0 : 0) + warp_sum64(pre_pad);
-  int i0, i1; sub_range(newT, n, B, b, i0, i1);
+  int i0, i1; sub_range(newT, n, kq, K, B, b, i0, i1);
   for (int ib = i0; ib < i1; ib += 32) {                       // all lanes iterate together (warp scans inside)
     const int i = ib + lane;
     Piece q; int kind = 0, es = 0;
@@ -353,15 +367,16 @@ extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout*
                                       int32_t flags, etc_plan** out, void* stream) {
   clear_error_detail();
   if (!old_l || !new_l || !device_map || !out) return ETC_ERR_INVALID_ARG;
-  if (flags != ETC_LOCAL_DIRECT && flags != ETC_ALL_STAGED) return ETC_ERR_INVALID_ARG;
+  if (flags < 0 || flags > (ETC_ALL_STAGED | ETC_KIND_MAJOR)) return ETC_ERR_INVALID_ARG;
   if (!etc_same_model(old_l, new_l)) return ETC_ERR_MISMATCH;
   const int n_old = old_l->t.n_dev, n_new = new_l->t.n_dev, P = n_old > n_new ? n_old : n_new;
   if ((long long)P * ETC_NUM_KINDS > 65535) return ETC_ERR_WORKSPACE;
   cudaStream_t st = (cudaStream_t)stream;
   old_l->last_stream = new_l->last_stream = st;
-  const long long U = (long long)n_old * n_new;
+  const int K = (flags & ETC_KIND_MAJOR) ? ETC_NUM_KINDS : 1;
+  const long long U = (long long)K * n_old * n_new;
   // sub-blocks per unit: enough warps to fill the machine when there are few units, 1 when there are many
-  const int want = (new_l->max_dev_pieces + 31) / 32;
+  const int want = (new_l->max_dev_pieces / K + 31) / 32;
   const int B = (int)std::max<long long>(1, std::min<long long>(want, 65536 / U));
 
   etc_plan* pl = new etc_plan();
@@ -406,9 +421,9 @@ extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout*
   PLAN_TRY(cudaMemsetAsync(pl->d_units, 0, sizeof(UnitCount) * (size_t)U, st));
 
   const unsigned grid = (unsigned)((U * B + PLAN_WARPS - 1) / PLAN_WARPS);
-  plan_count_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, B, pl->d_units, pl->d_blocks);
+  plan_count_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, K, B, pl->d_units, pl->d_blocks);
   PLAN_TRY(cudaGetLastError());
-  plan_scan_kernel<<<1, SCAN_THREADS, 0, st>>>(pl->d_units, U, n_old, n_new, P, flags, pl->d_map, pl->d_bases,
+  plan_scan_kernel<<<1, SCAN_THREADS, 0, st>>>(pl->d_units, U, K, n_old, n_new, P, flags, pl->d_map, pl->d_bases,
                                                pl->d_traffic, pl->d_totals);
   PLAN_TRY(cudaGetLastError());
   count_launch(2);
@@ -432,7 +447,7 @@ extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout*
     pl->d_ch_staged = reinterpret_cast<Chunk*>(tb + o_chs); pl->d_ch_local = reinterpret_cast<Chunk*>(tb + o_chl);
   }
   if (t.n_slices_staged + t.n_slices_local) {
-    plan_fill_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, flags, B, pl->d_blocks, pl->d_bases,
+    plan_fill_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, flags, K, B, pl->d_blocks, pl->d_bases,
                                                        pl->d_sl_staged, pl->d_sl_local, pl->d_c0_staged, pl->d_c0_local);
     PLAN_TRY(cudaGetLastError());
     count_launch();
@@ -459,6 +474,7 @@ extern "C" void etc_plan_destroy(etc_plan* pl) {
   cudaStream_t st = pl->last_stream ? pl->last_stream : pl->stream_created_on;
   if (pl->d_ws) cudaFreeAsync(pl->d_ws, st);
   if (pl->d_tb) cudaFreeAsync(pl->d_tb, st);
+  if (pl->d_rounds_ws) cudaFreeAsync(pl->d_rounds_ws, st);
   delete pl;
 }
 

@@ -11,6 +11,9 @@ struct UnitBase { int64_t slice0, chunk0, stg0; };
 struct PlanTotals {
   int64_t n_slices_staged, n_chunks_staged, staging_bytes, n_slices_local, n_chunks_local;
   int64_t local_bytes, remote_bytes, bad_map;
+  // kind-major plans: [kind][0] first staged chunk, [1] first staging byte, [2] first local chunk of the kind;
+  // entry [ETC_NUM_KINDS] = the totals
+  int64_t kind_base[ETC_NUM_KINDS + 1][3];
 };
 
 // One copy work item: nrows x row_bytes, at most ETC_CHUNK_BYTES in total (or one row segment of that size).
@@ -23,6 +26,16 @@ struct Chunk {
   int16_t pad;
 };
 static_assert(sizeof(Chunk) == 48, "Chunk layout");
+
+// One round of state chunking: a contiguous range of staged chunks whose staging footprint fits the
+// caller's bound, plus a share of the same kind's local chunks.
+struct RoundRec {
+  int64_t ca, cb;                      // staged chunk range [ca,cb)
+  int64_t la, lb;                      // local chunk range [la,lb)
+  int64_t stg_base, stg_span;          // the round uses staging bytes [stg_base, stg_base + stg_span) of the full layout
+  int64_t staged_bytes, local_bytes;   // payload
+  int32_t kind, sub, n_sub, pad;
+};
 
 }  // namespace etc
 
@@ -44,4 +57,9 @@ struct etc_plan {
   int64_t* d_c0_staged = nullptr; int64_t* d_c0_local = nullptr;
   std::vector<int64_t> old_bytes, new_bytes;       // buffer sizes [dev*4+kind], for argument checks in migrate
   void** d_ptrs = nullptr;                         // [n_old*4] source pointers then [n_new*4] destination pointers
+  // state chunking (f2): rounds of bounded staging, set by etc_plan_set_rounds
+  std::vector<etc::RoundRec> rounds;
+  int64_t round_staging_cap = 0;
+  void* d_rounds_ws = nullptr;                     // round records + one pointer table per round
+  void** d_round_ptrs = nullptr;
 };
