@@ -111,8 +111,7 @@ def test_rounds_errors(E):
     rounds = E.etc_plan_set_rounds(km, 1 << 20)
     src, dst = E.alloc_buffers(old), E.alloc_buffers(new)
     stg = torch.empty(1 << 20, dtype=torch.uint8, device="cuda")
-    with pytest.raises(E.EtcError):
-        E.lib().etc_migrate_round(km.h, len(rounds), None, None, None, 3, None)
+    assert E.lib().etc_migrate_round(km.h, len(rounds), None, None, None, 3, None) == -1   # no such round
     k0 = rounds[0].kind
     src_missing = {key: v for key, v in src.items() if key[1] != k0}
     with pytest.raises(E.EtcError):                                # the round's own kind must be present
