@@ -230,21 +230,33 @@ def run_cuda(args, w):
     stream = torch.cuda.current_stream()
     ev = lambda: torch.cuda.Event(enable_timing=True)
 
+    plan_stream = torch.cuda.Stream(dev)
+    planned = [torch.cuda.Event() for _ in range(4)]
+    step_no = [0]
+
     def step(record=None):
-        """One pass of the whole hot path.  record: dict of event lists to append to."""
-        e = [ev() for _ in range(7)] if record is not None else None
-        if e: e[0].record(stream)
-        lo, ln = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])     # (a1)
-        if e: e[1].record(stream)
-        ov, need, hold = E.etc_cost_matrix(lo, ln, out=out_cost)                                 # (a2)
-        if e: e[2].record(stream)
-        dm, lb = E.etc_sketch(ov, out=out_sk)                                                    # (a3)
-        if e: e[3].record(stream)
-        plan = E.etc_plan_create(lo, ln, dm, flags)                                              # (a4)
-        if e: e[4].record(stream)
-        E.etc_migrate(plan, src_tab, dst_tab, staging, E.ETC_PHASE_PACK)                         # (a5) + local
+        """One pass of the whole hot path.  Planning (a1-a4, metadata only, one host sync for table sizes) is enqueued
+        on its own stream so that its host sync does not wait for the previous step's copy kernels; the copy stream waits
+        for the plan by event.  record: list to which this step's timing events are appended."""
+        e = [ev() for _ in range(8)] if record is not None else None
+        with torch.cuda.stream(plan_stream):
+            if e: e[0].record(plan_stream)
+            lo, ln = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])     # (a1)
+            if e: e[1].record(plan_stream)
+            ov, need, hold = E.etc_cost_matrix(lo, ln, out=out_cost, stream=plan_stream)             # (a2)
+            if e: e[2].record(plan_stream)
+            dm, lb = E.etc_sketch(ov, out=out_sk, stream=plan_stream)                                # (a3)
+            if e: e[3].record(plan_stream)
+            plan = E.etc_plan_create(lo, ln, dm, flags, stream=plan_stream)                          # (a4)
+            if e: e[4].record(plan_stream)
+            done = planned[step_no[0] % len(planned)]
+            done.record(plan_stream)
+        step_no[0] += 1
+        stream.wait_event(done)
+        if e: e[7].record(stream)
+        E.etc_migrate(plan, src_tab, dst_tab, staging, E.ETC_PHASE_PACK, stream=stream)          # (a5) + local
         if e: e[5].record(stream)
-        E.etc_migrate(plan, src_tab, dst_tab, staging, E.ETC_PHASE_UNPACK)                       # (a6)
+        E.etc_migrate(plan, src_tab, dst_tab, staging, E.ETC_PHASE_UNPACK, stream=stream)        # (a6)
         if e: e[6].record(stream)
         if record is not None:
             record.append(e)
@@ -272,7 +284,7 @@ def run_cuda(args, w):
     stats = plan.stats
     phase = lambda a, b: statistics.mean(r[a].elapsed_time(r[b]) for r in recs)
     bd = {"layout_ms": phase(0, 1), "cost_matrix_ms": phase(1, 2), "sketch_ms": phase(2, 3), "plan_ms": phase(3, 4),
-          "pack_local_ms": phase(4, 5), "unpack_ms": phase(5, 6)}
+          "pack_local_ms": phase(7, 5), "unpack_ms": phase(5, 6)}
     value = job_value(world, hbm_bytes, ms_per_step)
 
     # ---- roofline of the dominant kernel, timed live with CUDA events over the timed region
@@ -295,6 +307,7 @@ def run_cuda(args, w):
             "vs_baseline": None, "dtype": "u8", "data": "synthetic",
             "config": {"workload": w["name"], "old": w["old"], "new": w["new"],
                        "mode": "ALL_STAGED" if args.all_staged else "LOCAL_DIRECT", "l2": "inputs_larger_than_L2",
+                       "pipelining": "planning (a1-a4) of step i+1 on its own stream overlaps the copy kernels of step i",
                        "parallelism": "replicas only" if world > 1 else "1 GPU, all virtual devices in one HBM"},
             "hbm_bytes_per_step": hbm_bytes, "payload": {"local": stats.local_bytes, "remote": stats.remote_bytes,
                                                          "staged": stats.staged_bytes},
@@ -302,6 +315,7 @@ def run_cuda(args, w):
             "roofline": roofline, "clocks": clocks, "gpu_launches": launches}
 
     del staging
+    torch.cuda.empty_cache()
     if rank == 0 and not args.no_extras:
         line["extras"] = extras(E, torch, w, dev, src, dst, lay_old, lay_new, peak)
 
@@ -309,10 +323,16 @@ def run_cuda(args, w):
     #      are inside the timed region
     if not args.no_e2e:
         try:
-            staging = torch.empty(max(st0.staging_bytes, 16), dtype=torch.uint8, device=dev)
-            line["e2e"] = e2e(E, torch, args, w, dev, src, dst, staging, step, hbm_bytes, world, barrier)
+            line["e2e"] = e2e(E, torch, args, w, dev, src, dst, hbm_bytes, world, barrier)
         except Exception as ex:       # e.g. not enough pinned host memory on the box
             line["e2e"] = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
+    if rank == 0 and not args.no_extras:
+        try:                          # destroys src: last GPU leg
+            del dst
+            torch.cuda.empty_cache()
+            line["extras"]["chunked_eager_release"] = chunked(E, torch, w, dev, src, lay_old, lay_new, args.e2e_staging)
+        except Exception as ex:
+            line["extras"]["chunked_eager_release"] = {"error": repr(ex)[:200]}
 
     if rank == 0:
         if world == 1 and not args.no_cpu:
@@ -376,35 +396,60 @@ def extras(E, torch, w, dev, src, dst, lay_old, lay_new, peak):
     return out
 
 
-def e2e(E, torch, args, w, dev, src, dst, staging, step, hbm_bytes, world, barrier):
-    stream = torch.cuda.current_stream()
+def e2e(E, torch, args, w, dev, src, dst, hbm_bytes, world, barrier):
+    """The same metric through the public API with HOST buffers: old shards in pinned host memory -> H2D -> whole path
+    (a1-a6, as kind-by-kind rounds of a kind-major plan) -> D2H -> new shards in pinned host memory, every copy inside
+    the timed region.  Uploads, rounds and downloads of different kinds overlap on three streams (host_pipeline.py)."""
+    from paper_2607_04749_b200.host_pipeline import HostMigration
     h_src = {k: torch.empty(t.shape, dtype=t.dtype, pin_memory=True) for k, t in src.items()}
     h_dst = {k: torch.empty(t.shape, dtype=t.dtype, pin_memory=True) for k, t in dst.items()}
     for k, t in src.items():
         h_src[k].copy_(t)
     torch.cuda.synchronize()
-    bi = sum(t.numel() for t in h_src.values()); bo = sum(t.numel() for t in h_dst.values())
-
-    def one():
-        for k, t in src.items():
-            t.copy_(h_src[k], non_blocking=True)
-        step()
-        for k, t in dst.items():
-            h_dst[k].copy_(t, non_blocking=True)
-
     n = max(1, min(args.steps, args.e2e_steps))
-    one(); barrier()
-    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    a.record(stream)
-    for _ in range(n):
-        one()
-    b.record(stream)
+    flags = E.ETC_ALL_STAGED if args.all_staged else E.ETC_LOCAL_DIRECT
+    warm = HostMigration(w["model"], w["old"], w["new"], h_src, h_dst, dev, args.e2e_staging, flags, d_src=src, d_dst=dst)
+    warm.run(); barrier()
+    hm = HostMigration(w["model"], w["old"], w["new"], h_src, h_dst, dev, args.e2e_staging, flags, d_src=src, d_dst=dst)
+    del warm
     barrier()
-    ms = a.elapsed_time(b) / n
+    for _ in range(n):
+        plan = hm.run()
+    barrier()
+    ms = hm.begin.elapsed_time(hm.done) / n
     ms = max_over_ranks(ms, world, dev)
     return {"value": job_value(world, hbm_bytes, ms), "unit": UNIT, "ms_per_step": ms, "steps": n,
-            "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo,
-            "note": "host-pinned old shards -> H2D -> whole path -> D2H of new shards, all inside the timed region"}
+            "h2d_bytes_per_step": hm.h2d_bytes, "d2h_bytes_per_step": hm.d2h_bytes,
+            "pcie_GBs_each_way": [hm.h2d_bytes / ms / 1e6, hm.d2h_bytes / ms / 1e6],
+            "rounds": len(plan.rounds), "staging_bytes": args.e2e_staging,
+            "note": "host-pinned old shards -> H2D -> whole path (kind-major rounds) -> D2H of new shards, all inside "
+                    "the timed region; upload, rounds and download of different kinds overlap on three streams"}
+
+
+def chunked(E, torch, w, dev, src, lay_old, lay_new, cap):
+    """(f2) device-resident state chunking with eager release: DESTROYS `src` (run last).  Reports the peak of live
+    bytes relative to the old state, the quantity of the paper's Fig. 12 (1.25x there)."""
+    from paper_2607_04749_b200.host_pipeline import migrate_chunked
+    stream = torch.cuda.current_stream()
+    ov, _, _ = E.etc_cost_matrix(lay_old, lay_new)
+    dm, _ = E.etc_sketch(ov)
+    plan = E.etc_plan_create(lay_old, lay_new, dm, E.ETC_KIND_MAJOR)
+    torch.cuda.synchronize()
+    torch.cuda.reset_peak_memory_stats(dev)
+    base = torch.cuda.memory_allocated(dev)
+    old_bytes = sum(t.numel() for t in src.values())
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    dst, info = migrate_chunked(plan, lay_new, src, cap, dev)
+    b.record(stream)
+    torch.cuda.synchronize()
+    ms = a.elapsed_time(b)
+    peak_alloc = torch.cuda.max_memory_allocated(dev) - (base - old_bytes)
+    return {"staging_cap_bytes": cap, "rounds": info["rounds"], "ms": ms, "GBs": plan.stats.hbm_bytes / ms / 1e6,
+            "peak_live_over_old": info["peak_live_bytes"] / info["old_bytes"],
+            "torch_peak_allocated_over_old": peak_alloc / old_bytes,
+            "all_at_once_over_old": (info["old_bytes"] + info["new_bytes"] + plan.stats.staging_bytes) / info["old_bytes"],
+            "note": "includes on-demand allocation of the new buffers (torch caching allocator) inside the timed region"}
 
 
 def main():
@@ -419,6 +464,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-staging", type=int, default=1 << 30, help="staging bound (bytes) of the e2e / chunked legs")
     ap.add_argument("--ref-elems", type=int, default=6_000_000, help="--impl reference: oracle sample (elements) per step")
     ap.add_argument("--cpu-elems", type=int, default=300_000_000, help="cpu_baseline leg: oracle sample (elements), ~10 s")
     args = ap.parse_args()
