@@ -230,7 +230,7 @@ def run_cuda(args, w):
     stream = torch.cuda.current_stream()
     ev = lambda: torch.cuda.Event(enable_timing=True)
 
-    plan_stream = torch.cuda.Stream(dev)
+    plan_stream = torch.cuda.Stream(dev, priority=-1)     # high priority: its small kernels cut in front of copy CTAs
     planned = [torch.cuda.Event() for _ in range(4)]
     step_no = [0]
 

@@ -33,7 +33,7 @@
 #define ORC_MAX_KINDS 4
 enum { ORC_REPL = 0, ORC_COL = 1, ORC_ROW = 2, ORC_COL2 = 3 };
 enum { ORC_PRE = 0, ORC_LAYER = 1, ORC_POST = 2 };
-enum { ORC_OK = 0, ORC_ERR_ARG = -1, ORC_ERR_INDIVISIBLE = -2, ORC_ERR_UNSUPPORTED = -6 };
+enum { ORC_OK = 0, ORC_ERR_ARG = -1, ORC_ERR_INDIVISIBLE = -2, ORC_ERR_UNSUPPORTED = -6, ORC_ERR_UNRECOVERABLE = -8 };
 
 typedef struct {
   int32_t style;       /* 0 = GPT (LayerNorm+bias, linear bias, learned pos-emb); 1 = LLaMA (RMSNorm, SwiGLU) */
@@ -63,6 +63,7 @@ typedef struct {
   int32_t* n_sh; orc_shard** sh; int64_t* Lloc;      /* indexed by s*tp + r */
   int32_t* idx;        /* [pp][n_lt]: position of tensor lt in stage s's shard list (same for every r), or -1 */
   int32_t* tied_idx;   /* [pp]: position of the tied word_embeddings replica in stage s's list, or -1 */
+  uint8_t* failed;     /* optional [n_dev]: 1 = the device failed and its state is lost (reading A26), NULL = none */
 } orc_layout;
 
 /* ---------------------------------------------------------------- logical model */
@@ -157,8 +158,20 @@ static void orc_make_shard(const orc_lt* t, int lt, int post_copy, int tp, int r
 void orc_layout_free(orc_layout* L) {
   if (!L) return;
   if (L->sh) for (int i = 0; i < L->c.pp * L->c.tp; i++) free(L->sh[i]);
-  free(L->sh); free(L->n_sh); free(L->Lloc); free(L->lt); free(L->idx); free(L->tied_idx); free(L);
+  free(L->sh); free(L->n_sh); free(L->Lloc); free(L->lt); free(L->idx); free(L->tied_idx); free(L->failed); free(L);
 }
+
+/* Failure mask of an OLD layout ("Fault-tolerance through DP"; reading A26): failed[o] != 0 means
+ * device o is lost with everything it held.  NULL clears the mask. */
+void orc_layout_set_failed(orc_layout* L, const uint8_t* failed) {
+  free(L->failed); L->failed = NULL;
+  if (failed) {
+    int n = L->c.tp * L->c.pp * L->c.dp;
+    L->failed = (uint8_t*)malloc((size_t)n);
+    for (int i = 0; i < n; i++) L->failed[i] = failed[i] ? 1 : 0;
+  }
+}
+static int orc_is_failed(const orc_layout* L, int dev) { return L->failed && dev >= 0 && L->failed[dev]; }
 
 int32_t orc_layout_new(const orc_model* m, const orc_cfg* c, orc_layout** out) {
   int rc = orc_validate(m, c);
@@ -304,6 +317,15 @@ static int orc_same_model(const orc_layout* A, const orc_layout* B) {
  * overlap[n][o] = bytes of elements held by both (row-major [n_new][P], P = max(n_old, n_new)).
  * Element by element: each element of new rank n is looked up among the holders in the old layout.
  * only_layers != 0 restricts all three to transformer-layer tensors (for the paper's layer-only example P1). */
+/* A26: a failed old device holds nothing: its column of the overlap matrix and its hold entry are zero. */
+static void orc_drop_failed(const orc_layout* Lo, int nn, int P, int64_t* overlap, int64_t* hold) {
+  int no = Lo->c.tp * Lo->c.pp * Lo->c.dp;
+  for (int o = 0; o < no; o++) if (orc_is_failed(Lo, o)) {
+    hold[o] = 0;
+    for (int n = 0; n < nn; n++) overlap[(size_t)n * P + o] = 0;
+  }
+}
+
 int32_t orc_overlap_elementwise(const orc_layout* Lo, const orc_layout* Ln, int32_t only_layers,
                                 int64_t* overlap, int64_t* need, int64_t* hold) {
   if (!orc_same_model(Lo, Ln)) return ORC_ERR_ARG;
@@ -338,6 +360,7 @@ int32_t orc_overlap_elementwise(const orc_layout* Lo, const orc_layout* Ln, int3
     }
     free(h);
   }
+  orc_drop_failed(Lo, nn, P, overlap, hold);
   return ORC_OK;
 }
 
@@ -407,6 +430,7 @@ int32_t orc_overlap_ranges(const orc_layout* Lo, const orc_layout* Ln, int64_t* 
       overlap[(size_t)n * P + o] = acc;
     }
   }
+  orc_drop_failed(Lo, nn, P, overlap, hold);
   return ORC_OK;
 }
 
@@ -485,7 +509,7 @@ static int orc_pick_source(const orc_layout* Lo, const orc_layout* Ln, int n, in
                            int lt, int post_copy, int64_t row, int64_t col, orc_holder* h, orc_holder* src) {
   int nh = orc_holders(Lo, kind, lt, row, col, h);
   if (nh == 0) return -1;
-  for (int i = 0; i < nh; i++) if (h[i].dev == p) { *src = h[i]; return 0; }          /* (i) */
+  for (int i = 0; i < nh; i++) if (h[i].dev == p && !orc_is_failed(Lo, p)) { *src = h[i]; return 0; }   /* (i) */
   int dn, sn, rn; orc_coords(Ln, n, &dn, &sn, &rn);
   int smin = h[0].s, smax = h[0].s;
   for (int i = 1; i < nh; i++) { if (h[i].s < smin) smin = h[i].s; if (h[i].s > smax) smax = h[i].s; }
@@ -496,7 +520,17 @@ static int orc_pick_source(const orc_layout* Lo, const orc_layout* Ln, int n, in
   if (orc_dp_sharded(Lo, kind)) {
     for (int i = 0; i < nh; i++) if (h[i].s == s_des && h[i].r == r_des) d_first = h[i].d;
     d_des = d_first;
-  } else d_des = dn % Lo->c.dp;
+    if (orc_is_failed(Lo, orc_dev(Lo, d_des, s_des, r_des))) return -2;    /* A26: the only holder is lost */
+  } else {
+    /* A26: the designated DP rank, else the next surviving replica in cyclic DP order with the
+     * same PP/TP ranks ("obtained from other DP groups via the PP/TP ranks") */
+    d_des = -1;
+    for (int j = 0; j < Lo->c.dp; j++) {
+      int d = (dn % Lo->c.dp + j) % Lo->c.dp;
+      if (!orc_is_failed(Lo, orc_dev(Lo, d, s_des, r_des))) { d_des = d; break; }
+    }
+    if (d_des < 0) return -2;                                              /* every replica is lost */
+  }
   for (int i = 0; i < nh; i++) if (h[i].s == s_des && h[i].r == r_des && h[i].d == d_des) { *src = h[i]; return 1; }
   return -1;
 }
@@ -509,7 +543,8 @@ int32_t orc_source_of(const orc_layout* Lo, const orc_layout* Ln, const int32_t*
   for (int64_t i = 0; i < count; i++) {
     int32_t lt, pc; int64_t row, col; orc_holder s;
     if (orc_global_of(Ln, n, kind, l_list[i], &lt, &pc, &row, &col)) { rc = ORC_ERR_ARG; break; }
-    if (orc_pick_source(Lo, Ln, n, device_map[n], kind, lt, pc, row, col, h, &s) < 0) { rc = ORC_ERR_ARG; break; }
+    int how = orc_pick_source(Lo, Ln, n, device_map[n], kind, lt, pc, row, col, h, &s);
+    if (how < 0) { rc = how == -2 ? ORC_ERR_UNRECOVERABLE : ORC_ERR_ARG; break; }
     src_dev[i] = s.dev; src_l[i] = s.l;
   }
   free(h);
@@ -542,7 +577,7 @@ int32_t orc_migrate_range(const orc_layout* Lo, const orc_layout* Ln, const int3
     int32_t lt, pc; int64_t row, col; orc_holder s;
     if (orc_global_of(Ln, n, kind, l, &lt, &pc, &row, &col)) { rc = ORC_ERR_ARG; break; }
     int how = orc_pick_source(Lo, Ln, n, p, kind, lt, pc, row, col, h, &s);
-    if (how < 0) { rc = ORC_ERR_ARG; break; }
+    if (how < 0) { rc = how == -2 ? ORC_ERR_UNRECOVERABLE : ORC_ERR_ARG; break; }
     if (dst) memcpy((char*)dst + l * es, (const char*)src_bufs[s.dev * 4 + kind] + s.l * es, (size_t)es);
     if (T) T[(size_t)s.dev * P + p] += es;
     if (written) written[l]++;

@@ -46,6 +46,8 @@ def lib():
         L.orc_layout_new.argtypes = [P(Model), P(Cfg), P(vp)]
         L.orc_layout_free.argtypes = [vp]
         L.orc_layout_free.restype = None
+        L.orc_layout_set_failed.argtypes = [vp, vp]
+        L.orc_layout_set_failed.restype = None
         L.orc_num_devices.restype = i32
         L.orc_num_devices.argtypes = [vp]
         L.orc_buffer_elems.restype = i64
@@ -124,6 +126,17 @@ class Layout:
         if getattr(self, "h", None):
             lib().orc_layout_free(self.h)
             self.h = None
+
+    def set_failed(self, failed):
+        """Mark devices of this (old) layout as failed (reading A26); None clears the mask."""
+        if failed is None:
+            lib().orc_layout_set_failed(self.h, None)
+            self.failed = None
+        else:
+            f = np.ascontiguousarray(failed, np.uint8)
+            assert f.shape == (self.n_dev,)
+            lib().orc_layout_set_failed(self.h, _ptr(f))
+            self.failed = f.copy()
 
     def kinds(self):
         return [k for k in range(4) if (self.model["kinds"] >> k) & 1]
