@@ -49,7 +49,8 @@ enum {
   ETC_ERR_BAD_MAP = -4,      /* device_map not injective or out of [0,P) */
   ETC_ERR_WORKSPACE = -5,    /* problem larger than the kernel's on-chip workspace (sketch: P > ETC_SKETCH_MAX_P) */
   ETC_ERR_UNSUPPORTED = -6,  /* tp > n_kv_heads (KV-head replication, reading A10) */
-  ETC_ERR_CUDA = -7          /* a CUDA call failed, or no CUDA device */
+  ETC_ERR_CUDA = -7,         /* a CUDA call failed, or no CUDA device */
+  ETC_ERR_UNRECOVERABLE = -8 /* some needed bytes have no surviving source (every replica failed, reading A26) */
 };
 
 enum { ETC_GPT = 0, ETC_LLAMA = 1 };                 /* etc_model_desc.style */
@@ -131,6 +132,20 @@ enum { ETC_LOCAL_DIRECT = 0, ETC_ALL_STAGED = 1, ETC_KIND_MAJOR = 2 };
 etc_status etc_plan_create(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
                            int32_t flags, etc_plan** out, void* stream);
 void etc_plan_destroy(etc_plan* plan);
+
+/* (f4) Failure-aware sourcing ("Fault-tolerance through DP": "the workload on the failed device can be
+ * obtained from other DP groups via the PP/TP ranks"; reading A26).  failed: [n_old] uint8, host OR device
+ * pointer, nonzero = old device lost with everything it held (NULL = no failures = etc_plan_create).  A failed device is
+ * never a source (not even a local one: its physical slot may host a new rank, which then receives everything); where
+ * the designated holder (d,s,r) of reading A6 failed, the source is the next surviving DP replica (d+1, d+2, ... mod
+ * dp_old, same s and r).  With dp_old = d this survives any d-1 failures.  ETC_ERR_UNRECOVERABLE if some needed element
+ * has no surviving holder (all replicas failed, or a DP-sharded distributed-optimizer range whose only holder failed).
+ * etc_mask_failed zeroes the failed devices' columns of d_overlap [n_new][P] and entries of d_hold [P] (may be NULL),
+ * so that etc_sketch counts nothing as local on them; d_failed is a DEVICE pointer [n_old].  Enqueues on `stream`. */
+etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
+                                  const uint8_t* failed, int32_t flags, etc_plan** out, void* stream);
+etc_status etc_mask_failed(int64_t* d_overlap, int64_t* d_hold, int32_t n_new, int32_t n_old, int32_t P,
+                           const uint8_t* d_failed, void* stream);
 
 typedef struct {
   int64_t staging_bytes;   /* size the caller must allocate for `staging` (payload + alignment padding) */

@@ -22,7 +22,7 @@ EXPORTED_SYMBOLS = (
     "etc_layout_buffer_bytes", "etc_cost_matrix", "etc_sketch", "etc_plan_create", "etc_plan_destroy",
     "etc_plan_get_stats", "etc_plan_get_traffic", "etc_plan_get_slices", "etc_migrate", "etc_migrate_phase",
     "etc_status_string", "etc_last_error_detail", "etc_kernel_launches", "etc_defrag",
-    "etc_plan_set_rounds", "etc_plan_get_round", "etc_migrate_round",
+    "etc_plan_set_rounds", "etc_plan_get_round", "etc_migrate_round", "etc_plan_create_failed", "etc_mask_failed",
 )
 
 
@@ -81,6 +81,9 @@ def lib():
         L.etc_sketch.restype = i32; L.etc_sketch.argtypes = [vp, i32, i32, vp, i32, vp, vp, vp]
         L.etc_defrag.restype = i32; L.etc_defrag.argtypes = [vp, i32, i32, i32, i32, vp, vp, vp, vp]
         L.etc_plan_create.restype = i32; L.etc_plan_create.argtypes = [vp, vp, vp, i32, C.POINTER(vp), vp]
+        L.etc_plan_create_failed.restype = i32
+        L.etc_plan_create_failed.argtypes = [vp, vp, vp, vp, i32, C.POINTER(vp), vp]
+        L.etc_mask_failed.restype = i32; L.etc_mask_failed.argtypes = [vp, vp, i32, i32, i32, vp, vp]
         L.etc_plan_destroy.restype = None; L.etc_plan_destroy.argtypes = [vp]
         L.etc_plan_get_stats.restype = i32; L.etc_plan_get_stats.argtypes = [vp, C.POINTER(_PlanStats)]
         L.etc_plan_get_traffic.restype = i32; L.etc_plan_get_traffic.argtypes = [vp, vp]
@@ -264,8 +267,21 @@ class Plan:
             self.h = None
 
 
-def etc_plan_create(old: Layout, new: Layout, device_map, flags: int = ETC_LOCAL_DIRECT, stream=None) -> Plan:
-    """(a4) device_map: CUDA int32 tensor (e.g. from etc_sketch) or a host sequence.  Synchronises the stream once."""
+def etc_mask_failed(overlap, hold, failed, n_old: int, stream=None):
+    """(f4) zero the failed old devices' columns of overlap [n_new][P] and entries of hold [P] in place.
+    failed: CUDA uint8 tensor [n_old]."""
+    import torch
+    n_new, P = overlap.shape
+    assert failed.is_cuda and failed.dtype == torch.uint8 and failed.numel() == n_old
+    _check(lib().etc_mask_failed(overlap.data_ptr(), 0 if hold is None else hold.data_ptr(), n_new, n_old, P,
+                                 failed.data_ptr(), _stream(stream)))
+    return overlap, hold
+
+
+def etc_plan_create(old: Layout, new: Layout, device_map, flags: int = ETC_LOCAL_DIRECT, stream=None,
+                    failed=None) -> Plan:
+    """(a4) device_map: CUDA int32 tensor (e.g. from etc_sketch) or a host sequence.  Synchronises the stream once.
+    failed (f4): optional [n_old] uint8 mask, CUDA tensor or host sequence (include/etc.h etc_plan_create_failed)."""
     import numpy as np
     import torch
     if isinstance(device_map, torch.Tensor):
@@ -276,9 +292,18 @@ def etc_plan_create(old: Layout, new: Layout, device_map, flags: int = ETC_LOCAL
         keep = np.ascontiguousarray(device_map, np.int32)
         assert keep.shape == (new.n_dev,)
         ptr = keep.ctypes.data
+    fptr, fkeep = None, None
+    if failed is not None:
+        if isinstance(failed, torch.Tensor):
+            assert failed.dtype == torch.uint8 and failed.numel() == old.n_dev and failed.is_contiguous()
+            fkeep = failed; fptr = failed.data_ptr()
+        else:
+            fkeep = np.ascontiguousarray(failed, np.uint8)
+            assert fkeep.shape == (old.n_dev,)
+            fptr = fkeep.ctypes.data
     h = C.c_void_p()
-    _check(lib().etc_plan_create(old.h, new.h, ptr, flags, C.byref(h), _stream(stream)))
-    del keep
+    _check(lib().etc_plan_create_failed(old.h, new.h, ptr, fptr, flags, C.byref(h), _stream(stream)))
+    del keep, fkeep
     return Plan(h)
 
 

@@ -122,3 +122,28 @@ extern "C" etc_status etc_cost_matrix(const etc_layout* old_l, const etc_layout*
   old_l->last_stream = new_l->last_stream = (cudaStream_t)stream;
   return ETC_OK;
 }
+
+// (f4) reading A26: a failed old device holds nothing — zero its column of the overlap matrix and its
+// hold entry, so the sketch keeps nothing "local" on it.
+namespace etc {
+__global__ void mask_failed_kernel(int64_t* __restrict__ overlap, int64_t* __restrict__ hold, int n_new, int n_old, int P,
+                                   const uint8_t* __restrict__ failed) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (long long)(n_new + 1) * n_old) return;
+  const int o = (int)(i % n_old), n = (int)(i / n_old);
+  if (!failed[o]) return;
+  if (n < n_new) overlap[(size_t)n * P + o] = 0; else if (hold) hold[o] = 0;
+}
+}  // namespace etc
+
+extern "C" etc_status etc_mask_failed(int64_t* d_overlap, int64_t* d_hold, int32_t n_new, int32_t n_old, int32_t P,
+                                      const uint8_t* d_failed, void* stream) {
+  etc::clear_error_detail();
+  if (!d_overlap || !d_failed || n_new < 1 || n_old < 1 || P < n_old || P < n_new) return ETC_ERR_INVALID_ARG;
+  const long long total = (long long)(n_new + 1) * n_old;
+  etc::mask_failed_kernel<<<(unsigned)((total + 255) / 256), 256, 0, (cudaStream_t)stream>>>(d_overlap, d_hold, n_new,
+                                                                                              n_old, P, d_failed);
+  ETC_CUDA_TRY(cudaGetLastError());
+  etc::count_launch();
+  return ETC_OK;
+}

@@ -299,6 +299,7 @@ extern "C" const char* etc_status_string(etc_status s) {
     case ETC_ERR_WORKSPACE: return "ETC_ERR_WORKSPACE";
     case ETC_ERR_UNSUPPORTED: return "ETC_ERR_UNSUPPORTED";
     case ETC_ERR_CUDA: return "ETC_ERR_CUDA";
+    case ETC_ERR_UNRECOVERABLE: return "ETC_ERR_UNRECOVERABLE";
     default: return "ETC_ERR_UNKNOWN";
   }
 }

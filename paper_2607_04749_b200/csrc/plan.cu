@@ -28,12 +28,25 @@ __device__ __forceinline__ bool rect_isect(const Piece& a, const Piece& b, Rect&
   return r1 > r0 && c1 > c0;
 }
 
-// Is old piece o the designated holder for new piece q (reading A6 (ii))?
-__device__ __forceinline__ bool designated(const Piece& o, const Piece& q, int tp_old, int dp_old) {
+// Is old piece o the designated holder for new piece q (reading A6 (ii))?  With a failure mask (reading A26,
+// PAPER.md:173-177) the designated DP rank is the first SURVIVING replica in cyclic DP order starting at d' mod dp_old,
+// with the same PP/TP ranks; the caller has already skipped pieces of failed devices.
+__device__ __forceinline__ bool designated(const Piece& o, const Piece& q, int tp_old, int dp_old,
+                                           const uint8_t* __restrict__ failed) {
   const bool stage_ok = (o.flags & PF_SOLE_INST) || ((o.flags & PF_POST_COPY) == (q.flags & PF_POST_COPY));
   const bool r_ok = (o.flags & PF_TP_SHARDED) || o.r == q.r % tp_old;
-  const bool d_ok = (o.flags & PF_DP_SHARDED) || o.d == q.d % dp_old;
-  return stage_ok && r_ok && d_ok;
+  if (!(stage_ok && r_ok)) return false;
+  if (o.flags & PF_DP_SHARDED) return true;
+  int d_des = q.d % dp_old;
+  if (failed) {
+    int j = 0;
+    for (; j < dp_old; ++j) {
+      const int d = (d_des + j) % dp_old;
+      if (!failed[o.r + tp_old * (d + dp_old * o.s)]) { d_des = d; break; }
+    }
+    if (j == dp_old) return false;
+  }
+  return o.d == d_des;
 }
 
 // I minus the flat interval [b0,b1) of the shard (row pitch W) that I lives in.  I's first element is local
@@ -83,7 +96,8 @@ __device__ __forceinline__ int64_t slice_padded(const SliceGeom& s) { return (s.
 // Enumerate, in canonical order, the slices that new piece q receives from source device od.
 template <typename F>
 __device__ __forceinline__ void for_each_slice(const DeviceTables& oldT, const Piece& q, int od, int p, bool local_unit,
-                                               int es, int kind, F&& f) {
+                                               int es, int kind, const uint8_t* __restrict__ failed, F&& f) {
+  if (failed && failed[od]) return;                                              // a failed device sources nothing
   int j = oldT.first[(size_t)od * oldT.n_grp + q.grp];
   if (j < 0) return;
   const int oe = oldT.dev_start[od + 1];
@@ -93,9 +107,9 @@ __device__ __forceinline__ void for_each_slice(const DeviceTables& oldT, const P
     Rect I;
     if (!rect_isect(q, o, I)) continue;
     if (local_unit) { f(make_slice(I, o, q, es, kind)); continue; }              // (i) local first
-    if (!designated(o, q, oldT.tp, oldT.dp)) continue;                           // (ii) designated holder only
+    if (!designated(o, q, oldT.tp, oldT.dp, failed)) continue;                   // (ii) designated holder only
     Rect parts[4]; int np = 1; parts[0] = I;
-    if (p >= 0 && p < oldT.n_dev) {                                              // minus what the destination device holds
+    if (p >= 0 && p < oldT.n_dev && !(failed && failed[p])) {                    // minus what the destination device holds
       const int pj = oldT.first[(size_t)p * oldT.n_grp + q.grp];
       if (pj >= 0) {
         const Piece& h = oldT.pieces[pj];
@@ -134,7 +148,8 @@ __device__ __forceinline__ void sub_range(const DeviceTables& newT, int n, int k
 
 // pass 1: per-(unit, sub-block) counts; unit totals accumulated with integer atomics (order-independent sums).
 __global__ void __launch_bounds__(PLAN_WARPS * 32)
-plan_count_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict__ device_map, int K, int B,
+plan_count_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict__ device_map,
+                  const uint8_t* __restrict__ failed, int K, int B,
                   UnitCount* __restrict__ units, BlockCount* __restrict__ blocks) {
   const int lane = threadIdx.x & 31;
   const long long w = (long long)blockIdx.x * PLAN_WARPS + (threadIdx.x >> 5);
@@ -153,7 +168,7 @@ plan_count_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restric
     for (int i = i0 + lane; i < i1; i += 32) {
       const Piece q = newT.pieces[i];
       const int kind = q.grp / newT.n_tensors, es = newT.elem_bytes[kind];
-      for_each_slice(oldT, q, od, p, local_unit, es, kind, [&](const SliceGeom& s) {
+      for_each_slice(oldT, q, od, p, local_unit, es, kind, failed, [&](const SliceGeom& s) {
         n_sl += 1; n_ch += slice_chunks(s); bytes += s.nrows * s.row_bytes; padded += slice_padded(s);
       });
     }
@@ -270,7 +285,8 @@ __device__ __forceinline__ int vec_of(int64_t a) {
 // pass 2: recompute the slices of each (unit, sub-block) and write slice records (+ first chunk index) at their final
 // positions: unit base (scan) + earlier sub-blocks of the unit + warp-level prefix inside the sub-block.
 __global__ void __launch_bounds__(PLAN_WARPS * 32)
-plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict__ device_map, int flags, int K, int B,
+plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict__ device_map,
+                 const uint8_t* __restrict__ failed, int flags, int K, int B,
                  const BlockCount* __restrict__ blocks, const UnitBase* __restrict__ bases,
                  etc_slice* __restrict__ sl_staged, etc_slice* __restrict__ sl_local,
                  int64_t* __restrict__ c0_staged, int64_t* __restrict__ c0_local) {
@@ -297,7 +313,7 @@ plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict
     int64_t my_sl = 0, my_ch = 0, my_pad = 0;
     if (i < i1) {
       q = newT.pieces[i]; kind = q.grp / newT.n_tensors; es = newT.elem_bytes[kind];
-      for_each_slice(oldT, q, od, p, local_unit, es, kind, [&](const SliceGeom& s) {
+      for_each_slice(oldT, q, od, p, local_unit, es, kind, failed, [&](const SliceGeom& s) {
         my_sl += 1; my_ch += slice_chunks(s); my_pad += slice_padded(s);
       });
     }
@@ -307,7 +323,7 @@ plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict
     int64_t o_stg = run_stg + warp_excl_scan64(my_pad, lane, tot_pad);
     run_sl += tot_sl; run_ch += tot_ch; run_stg += tot_pad;
     if (i < i1 && my_sl) {
-      for_each_slice(oldT, q, od, p, local_unit, es, kind, [&](const SliceGeom& s) {
+      for_each_slice(oldT, q, od, p, local_unit, es, kind, failed, [&](const SliceGeom& s) {
         etc_slice r;
         r.src_off = s.src_off; r.dst_off = s.dst_off; r.stg_off = staged ? o_stg : -1; r.row_bytes = s.row_bytes;
         r.src_stride = s.src_stride; r.dst_stride = s.dst_stride; r.nrows = s.nrows;
@@ -363,8 +379,19 @@ static PlanTotals* g_pinned_totals = nullptr;
 static unsigned g_pinned_next = 0;
 constexpr unsigned N_PINNED_TOTALS = 64;
 
+static bool on_device_ptr(const void* p) {
+  cudaPointerAttributes attr{};
+  if (cudaPointerGetAttributes(&attr, p) != cudaSuccess) { (void)cudaGetLastError(); return false; }
+  return attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged;
+}
+
 extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
                                       int32_t flags, etc_plan** out, void* stream) {
+  return etc_plan_create_failed(old_l, new_l, device_map, nullptr, flags, out, stream);
+}
+
+extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
+                                             const uint8_t* failed, int32_t flags, etc_plan** out, void* stream) {
   clear_error_detail();
   if (!old_l || !new_l || !device_map || !out) return ETC_ERR_INVALID_ARG;
   if (flags < 0 || flags > (ETC_ALL_STAGED | ETC_KIND_MAJOR)) return ETC_ERR_INVALID_ARG;
@@ -390,10 +417,7 @@ extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout*
   PlanTotals* h_tot = &g_pinned_totals[__atomic_fetch_add(&g_pinned_next, 1u, __ATOMIC_RELAXED) % N_PINNED_TOTALS];
 
   // device_map may live on the host or on the device
-  cudaPointerAttributes attr{};
-  cudaError_t pe = cudaPointerGetAttributes(&attr, device_map);
-  if (pe != cudaSuccess) { (void)cudaGetLastError(); attr.type = cudaMemoryTypeUnregistered; }
-  const bool on_device = attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged;
+  const bool on_device = on_device_ptr(device_map);
   if (!on_device) {
     std::vector<char> seen((size_t)P, 0);
     for (int n = 0; n < n_new; ++n) {
@@ -409,7 +433,8 @@ extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout*
                o_traffic = o_blocks + al(sizeof(BlockCount) * (size_t)U * B),
                o_totals = o_traffic + al(sizeof(int64_t) * (size_t)P * P), o_map = o_totals + al(sizeof(PlanTotals)),
                o_ptrs = o_map + al(sizeof(int32_t) * (size_t)n_new),
-               ws_bytes = o_ptrs + al(sizeof(void*) * (size_t)(n_old + n_new) * ETC_NUM_KINDS);
+               o_failed = o_ptrs + al(sizeof(void*) * (size_t)(n_old + n_new) * ETC_NUM_KINDS),
+               ws_bytes = o_failed + al((size_t)n_old);
   PLAN_TRY(cudaMallocAsync(&pl->d_ws, ws_bytes, st));
   char* ws = static_cast<char*>(pl->d_ws);
   pl->d_units = reinterpret_cast<UnitCount*>(ws + o_units); pl->d_bases = reinterpret_cast<UnitBase*>(ws + o_bases);
@@ -419,9 +444,16 @@ extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout*
   PLAN_TRY(cudaMemcpyAsync(pl->d_map, device_map, sizeof(int32_t) * (size_t)n_new,
                            on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
   PLAN_TRY(cudaMemsetAsync(pl->d_units, 0, sizeof(UnitCount) * (size_t)U, st));
+  const uint8_t* d_failed = nullptr;
+  if (failed) {                                                 // reading A26: host or device mask [n_old]
+    PLAN_TRY(cudaMemcpyAsync(ws + o_failed, failed, (size_t)n_old,
+                             on_device_ptr(failed) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+    d_failed = reinterpret_cast<const uint8_t*>(ws + o_failed);
+  }
 
   const unsigned grid = (unsigned)((U * B + PLAN_WARPS - 1) / PLAN_WARPS);
-  plan_count_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, K, B, pl->d_units, pl->d_blocks);
+  plan_count_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, d_failed, K, B, pl->d_units,
+                                                      pl->d_blocks);
   PLAN_TRY(cudaGetLastError());
   plan_scan_kernel<<<1, SCAN_THREADS, 0, st>>>(pl->d_units, U, K, n_old, n_new, P, flags, pl->d_map, pl->d_bases,
                                                pl->d_traffic, pl->d_totals);
@@ -431,6 +463,11 @@ extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout*
   PLAN_TRY(cudaStreamSynchronize(st));                          // the one host sync: sizes must come back
   pl->totals = *h_tot;
   if (pl->totals.bad_map) return fail(ETC_ERR_BAD_MAP);
+  {                                                             // every needed byte must have found its one source
+    int64_t need = 0;
+    for (int64_t b : pl->new_bytes) need += b;
+    if (pl->totals.local_bytes + pl->totals.remote_bytes != need) return fail(ETC_ERR_UNRECOVERABLE);
+  }
 
   // blob 2: slice records | first-chunk indices | chunk descriptors
   const PlanTotals& t = pl->totals;
@@ -447,7 +484,7 @@ extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout*
     pl->d_ch_staged = reinterpret_cast<Chunk*>(tb + o_chs); pl->d_ch_local = reinterpret_cast<Chunk*>(tb + o_chl);
   }
   if (t.n_slices_staged + t.n_slices_local) {
-    plan_fill_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, flags, K, B, pl->d_blocks, pl->d_bases,
+    plan_fill_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, d_failed, flags, K, B, pl->d_blocks, pl->d_bases,
                                                        pl->d_sl_staged, pl->d_sl_local, pl->d_c0_staged, pl->d_c0_local);
     PLAN_TRY(cudaGetLastError());
     count_launch();
