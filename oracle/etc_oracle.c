@@ -43,7 +43,8 @@ typedef struct {
   int32_t kinds;       /* bitmask over kinds 0..3 = PARAM, MASTER, ADAM_M, ADAM_V */
 } orc_model;
 
-typedef struct { int32_t tp, pp, dp, dist_opt; } orc_cfg;
+/* pp_first / pp_last: layers on the first / last pipeline stage (0 = not set), reading A27 (uneven pipeline split) */
+typedef struct { int32_t tp, pp, dp, dist_opt, pp_first, pp_last; } orc_cfg;
 
 typedef struct { int64_t rows, cols; int32_t split, where, layer; } orc_lt;   /* one logical tensor */
 
@@ -124,6 +125,25 @@ int32_t orc_logical_info(const orc_model* m, int64_t* rows, int64_t* cols, int32
 static int orc_elem_bytes(const orc_model* m, int kind) { return kind == 0 ? m->param_bytes : 4; }
 int32_t orc_kind_bytes(const orc_model* m, int32_t kind) { return orc_elem_bytes(m, kind); }
 
+/* First layer of pipeline stage s (s = pp gives n_layers).  Even split ("divisible by PP sizes") unless
+ * pp_first / pp_last fix the layer count of the first / last stage (reading A27, as Megatron-LM's
+ * --decoder-first/last-pipeline-num-layers): the remaining layers are split evenly over the remaining stages.
+ * Returns -1 if the split is impossible (indivisible, or a stage would be empty), -2 on nonsense arguments. */
+static int orc_stage_begin(int n_layers, const orc_cfg* c, int s) {
+  int first = c->pp_first, last = c->pp_last, pp = c->pp;
+  if (first < 0 || last < 0) return -2;
+  if ((first || last) && pp < 2) return -2;
+  int mid_stages = pp - (first ? 1 : 0) - (last ? 1 : 0), mid_layers = n_layers - first - last;
+  if (mid_stages < 0 || mid_layers < 0) return -1;
+  if (mid_stages == 0) { if (mid_layers != 0) return -1; }
+  else if (mid_layers % mid_stages || mid_layers / mid_stages < 1) return -1;
+  int per = mid_stages ? mid_layers / mid_stages : 0;
+  if (s <= 0) return 0;
+  if (s >= pp) return n_layers;
+  if (first) return first + (s - 1) * per;
+  return s * per;
+}
+
 /* divisibility rules (layers divisible by PP, hidden by TP; A7, A10, A12) */
 static int orc_validate(const orc_model* m, const orc_cfg* c) {
   if (!m || !c) return ORC_ERR_ARG;
@@ -134,7 +154,7 @@ static int orc_validate(const orc_model* m, const orc_cfg* c) {
   if (m->kinds <= 0 || m->kinds > 15) return ORC_ERR_ARG;
   if (m->n_q_heads % m->n_kv_heads) return ORC_ERR_ARG;
   if (c->tp > m->n_kv_heads) return ORC_ERR_UNSUPPORTED;       /* KV-head replication is out of scope (A10) */
-  if (m->n_layers % c->pp) return ORC_ERR_INDIVISIBLE;
+  if (orc_stage_begin(m->n_layers, c, 0) < 0) return orc_stage_begin(m->n_layers, c, 0) == -2 ? ORC_ERR_ARG : ORC_ERR_INDIVISIBLE;
   if (m->n_kv_heads % c->tp) return ORC_ERR_INDIVISIBLE;
   if (m->ffn_hidden % c->tp) return ORC_ERR_INDIVISIBLE;
   if (m->vocab % c->tp) return ORC_ERR_INDIVISIBLE;
@@ -190,8 +210,8 @@ int32_t orc_layout_new(const orc_model* m, const orc_cfg* c, orc_layout** out) {
   L->tied_idx = (int32_t*)malloc(sizeof(int32_t) * (size_t)c->pp);
   for (int i = 0; i < c->pp * L->n_lt; i++) L->idx[i] = -1;
   for (int i = 0; i < c->pp; i++) L->tied_idx[i] = -1;
-  int per = m->n_layers / c->pp;
   for (int s = 0; s < c->pp; s++) for (int r = 0; r < c->tp; r++) {
+    int l_begin = orc_stage_begin(m->n_layers, c, s), l_end = orc_stage_begin(m->n_layers, c, s + 1);
     orc_shard* v = (orc_shard*)malloc(sizeof(orc_shard) * (size_t)(L->n_lt + 1));
     int k = 0; int64_t pos = 0;
     /* local order: pre tensors (stage 0), the stage's layers ascending, post tensors (last stage), tied replica */
@@ -199,7 +219,7 @@ int32_t orc_layout_new(const orc_model* m, const orc_cfg* c, orc_layout** out) {
       const orc_lt* t = &L->lt[i];
       if (t->where != pass) continue;
       if (pass == ORC_PRE && s != 0) continue;
-      if (pass == ORC_LAYER && (t->layer < s * per || t->layer >= (s + 1) * per)) continue;
+      if (pass == ORC_LAYER && (t->layer < l_begin || t->layer >= l_end)) continue;
       if (pass == ORC_POST && s != c->pp - 1) continue;
       orc_make_shard(t, i, 0, c->tp, r, &v[k]); v[k].start = pos; pos += v[k].n;
       L->idx[s * L->n_lt + i] = k; k++;
