@@ -70,8 +70,11 @@ typedef struct {
 } etc_model_desc;
 
 /* Megatron-style parallel configuration.  dist_opt = 1: MASTER/ADAM_M/ADAM_V are sharded over DP as
- * contiguous flat ranges of each (stage, tp-rank) local parameter space (reading A14); PARAM stays replicated. */
-typedef struct { int32_t tp, pp, dp, dist_opt; } etc_parallel_cfg;
+ * contiguous flat ranges of each (stage, tp-rank) local parameter space (reading A14); PARAM stays replicated.
+ * pp_first / pp_last (f3, reading A27): number of layers on the first / last pipeline stage, 0 = not set (as
+ * Megatron-LM's --decoder-first/last-pipeline-num-layers); the remaining layers are split evenly over the remaining
+ * stages.  Both 0 = the even split the paper requires. */
+typedef struct { int32_t tp, pp, dp, dist_opt, pp_first, pp_last; } etc_parallel_cfg;
 
 typedef struct etc_layout etc_layout;   /* opaque, immutable after create */
 typedef struct etc_plan etc_plan;       /* opaque, immutable after create */

@@ -56,6 +56,20 @@ static std::vector<LTensor> logical_tensors(const etc_model_desc& m) {
   return v;
 }
 
+// First layer of pipeline stage s (s = pp -> n_layers); even split unless pp_first / pp_last are set (reading A27).
+// -1: impossible split, -2: invalid arguments.
+static int stage_begin(int n_layers, const etc_parallel_cfg& c, int s) {
+  if (c.pp_first < 0 || c.pp_last < 0 || ((c.pp_first || c.pp_last) && c.pp < 2)) return -2;
+  const int fixed_stages = (c.pp_first ? 1 : 0) + (c.pp_last ? 1 : 0);
+  const int free_stages = c.pp - fixed_stages, free_layers = n_layers - c.pp_first - c.pp_last;
+  if (free_stages < 0 || free_layers < 0) return -1;
+  if (free_stages == 0 ? free_layers != 0 : (free_layers % free_stages != 0 || free_layers < free_stages)) return -1;
+  const int per = free_stages ? free_layers / free_stages : 0;
+  if (s <= 0) return 0;
+  if (s >= c.pp) return n_layers;
+  return c.pp_first ? c.pp_first + (s - 1) * per : s * per;
+}
+
 static etc_status validate(const etc_model_desc* m, const etc_parallel_cfg* c) {
   if (!m || !c) return ETC_ERR_INVALID_ARG;
   if (c->tp < 1 || c->pp < 1 || c->dp < 1 || (c->dist_opt != 0 && c->dist_opt != 1)) return ETC_ERR_INVALID_ARG;
@@ -68,8 +82,8 @@ static etc_status validate(const etc_model_desc* m, const etc_parallel_cfg* c) {
   if (m->n_q_heads % m->n_kv_heads) return ETC_ERR_INVALID_ARG;
   if (int64_t(c->tp) * c->pp * c->dp > 32767) return ETC_ERR_INVALID_ARG;
   if (c->tp > m->n_kv_heads) return ETC_ERR_UNSUPPORTED;
-  if (m->n_layers % c->pp || m->n_kv_heads % c->tp || m->ffn_hidden % c->tp || m->vocab % c->tp)
-    return ETC_ERR_INDIVISIBLE;
+  { const int sb = stage_begin(m->n_layers, *c, 0); if (sb < 0) return sb == -2 ? ETC_ERR_INVALID_ARG : ETC_ERR_INDIVISIBLE; }
+  if (m->n_kv_heads % c->tp || m->ffn_hidden % c->tp || m->vocab % c->tp) return ETC_ERR_INDIVISIBLE;
   return ETC_OK;
 }
 
@@ -122,14 +136,15 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   const int n_dev = tp * pp * dp;
   const std::vector<LTensor> lts = logical_tensors(m);
   const int nT = (int)lts.size(), nG = nT * ETC_NUM_KINDS;
-  const int per_stage = m.n_layers / pp;
+  int max_stage_layers = 0;
+  for (int s = 0; s < pp; ++s) max_stage_layers = std::max(max_stage_layers, stage_begin(m.n_layers, *cfg, s + 1) - stage_begin(m.n_layers, *cfg, s));
   const bool two_inst = m.tied_embeddings && pp > 1;     // word_embeddings held by first AND last stage
   const int mask_words = (nT + 31) / 32;
   int n_kinds = 0; for (int k = 0; k < ETC_NUM_KINDS; ++k) n_kinds += (m.kinds >> k) & 1;
 
   // blob: dev_start | first | ltmask | kind_start | pieces (pieces last: their count is known only after the build)
   auto al = [](size_t x) { return (x + 255) & ~size_t(255); };
-  const size_t max_inst = (size_t)per_stage * (m.style == ETC_GPT ? 12 : 6) + 6;
+  const size_t max_inst = (size_t)max_stage_layers * (m.style == ETC_GPT ? 12 : 6) + 6;
   const size_t o_start = 0, o_first = al((size_t)(n_dev + 1) * 4), o_mask = o_first + al((size_t)n_dev * nG * 4),
                o_kstart = o_mask + al((size_t)n_dev * mask_words * 4),
                o_pieces = o_kstart + al((size_t)n_dev * (ETC_NUM_KINDS + 1) * 4);
@@ -152,6 +167,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
 
   std::vector<std::vector<Sh>> shr(tp);     // shards of (stage, tp-rank r), in GROUP order: tied replica first
   for (int s = 0; s < pp; ++s) {
+    const int l_begin = stage_begin(m.n_layers, *cfg, s), l_end = stage_begin(m.n_layers, *cfg, s + 1);
     // the stage's tensor instances in LOCAL order: pre, layers ascending, post, tied replica (reading A11)
     std::vector<std::pair<int32_t, bool>> inst;
     for (int pass = 0; pass < 3; ++pass)
@@ -159,7 +175,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
         const LTensor& T = lts[t];
         if (T.where != pass) continue;
         if (pass == 0 && s != 0) continue;
-        if (pass == 1 && (T.layer < s * per_stage || T.layer >= (s + 1) * per_stage)) continue;
+        if (pass == 1 && (T.layer < l_begin || T.layer >= l_end)) continue;
         if (pass == 2 && s != pp - 1) continue;
         inst.push_back({t, false});
       }

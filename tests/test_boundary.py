@@ -49,6 +49,11 @@ def test_layout_validation_without_gpu(lib):
     assert lib.etc_layout_create(C.byref(m), C.byref(_ParallelCfg(4, 1, 1, 0)), C.byref(h)) == -6   # tp > kv heads
     assert lib.etc_layout_create(C.byref(m), C.byref(_ParallelCfg(0, 1, 1, 0)), C.byref(h)) == -1
     assert lib.etc_layout_create(None, C.byref(_ParallelCfg(1, 1, 1, 0)), C.byref(h)) == -1
+    # uneven pipeline splits (f3, reading A27): validated on the host as well
+    assert lib.etc_layout_create(C.byref(m), C.byref(_ParallelCfg(1, 3, 1, 0, 1, 0)), C.byref(h)) == -2   # 3 layers / 2 stages
+    assert lib.etc_layout_create(C.byref(m), C.byref(_ParallelCfg(1, 2, 1, 0, 1, 1)), C.byref(h)) == -2   # 2 layers unassigned
+    assert lib.etc_layout_create(C.byref(m), C.byref(_ParallelCfg(1, 1, 1, 0, 4, 0)), C.byref(h)) == -1   # pp = 1
+    assert lib.etc_layout_create(C.byref(m), C.byref(_ParallelCfg(1, 2, 1, 0, -1, 0)), C.byref(h)) == -1
     m.param_dtype = 3
     assert lib.etc_layout_create(C.byref(m), C.byref(_ParallelCfg(1, 1, 1, 0)), C.byref(h)) == -1
     assert h.value is None
