@@ -53,7 +53,7 @@ def test_uneven_pipeline_scaled_preemption(E):
 
 def test_uneven_validation_codes_match_oracle(E):
     m = dict(tiny_models())["gpt_t"]
-    for cfg in (_cfg(1, 3, 1, 0, 1, 0), _cfg(1, 2, 1, 0, 1, 1), _cfg(1, 1, 1, 0, 4, 0), _cfg(4, 3, 1, 0, 2, 0)):
+    for cfg in (_cfg(1, 3, 1, 0, 1, 0), _cfg(1, 2, 1, 0, 1, 1), _cfg(1, 1, 1, 0, 4, 0), _cfg(8, 3, 1, 0, 2, 0)):
         with pytest.raises(O.OracleError) as oe:
             O.Layout(m, cfg)
         with pytest.raises(E.EtcError) as ge:
