@@ -119,7 +119,7 @@ extern "C" etc_status etc_cost_matrix(const etc_layout* old_l, const etc_layout*
         old_l->t, new_l->t, P, d_overlap, d_need, d_hold);
   ETC_CUDA_TRY(cudaGetLastError());
   count_launch();
-  old_l->last_stream = new_l->last_stream = (cudaStream_t)stream;
+  old_l->streams.note((cudaStream_t)stream); new_l->streams.note((cudaStream_t)stream);
   return ETC_OK;
 }
 

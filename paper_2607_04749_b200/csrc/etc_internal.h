@@ -2,6 +2,7 @@
 // Nothing here is shared with oracle/ (the CPU oracle is written separately from the paper).
 #pragma once
 #include <cstdint>
+#include <vector>
 #include <cuda_runtime.h>
 #include "../../include/etc.h"
 
@@ -47,6 +48,31 @@ struct DeviceTables {            // device memory
   int32_t elem_bytes[ETC_NUM_KINDS];
 };
 
+// The streams on which kernels reading an object's device tables have been enqueued.  The tables are released with a
+// stream-ordered free; join() returns the most recently used stream after making it wait (by event) for everything
+// enqueued so far on every other noted stream, so the free is ordered after all readers.  A NULL cudaStream_t is the
+// legacy default stream and is a stream like any other here (it must not be mistaken for "never used").
+struct StreamSet {
+  std::vector<cudaStream_t> used;
+  void note(cudaStream_t st) {
+    for (size_t i = 0; i < used.size(); ++i)
+      if (used[i] == st) { used.erase(used.begin() + (long)i); break; }
+    used.push_back(st);
+  }
+  cudaStream_t join(cudaStream_t fallback) const {
+    if (used.empty()) return fallback;
+    cudaStream_t last = used.back();
+    for (size_t i = 0; i + 1 < used.size(); ++i) {
+      cudaEvent_t e;
+      if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) { (void)cudaGetLastError(); continue; }
+      if (cudaEventRecord(e, used[i]) == cudaSuccess) cudaStreamWaitEvent(last, e, 0);
+      cudaEventDestroy(e);
+      (void)cudaGetLastError();
+    }
+    return last;
+  }
+};
+
 }  // namespace etc
 
 struct etc_layout {
@@ -56,7 +82,7 @@ struct etc_layout {
   int64_t* h_buffer_bytes = nullptr;      // [n_dev][4] host
   int32_t max_dev_pieces = 0;             // largest piece count of one device
   void* d_blob = nullptr;                 // one allocation holding all device tables
-  mutable cudaStream_t last_stream = nullptr;   // last stream a kernel reading the tables was enqueued on
+  mutable etc::StreamSet streams;         // streams that kernels reading the tables were enqueued on
 };
 
 // ---- error plumbing

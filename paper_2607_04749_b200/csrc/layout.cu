@@ -292,8 +292,8 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
 
 extern "C" void etc_layout_destroy(etc_layout* L) {
   if (!L) return;
-  // stream-ordered free on the last stream that used the tables: kernels already enqueued there finish first
-  if (L->d_blob) cudaFreeAsync(L->d_blob, L->last_stream ? L->last_stream : g_up_stream);
+  // stream-ordered free, ordered after every kernel already enqueued on any stream that read the tables
+  if (L->d_blob) cudaFreeAsync(L->d_blob, L->streams.join(g_up_stream));
   delete[] L->h_buffer_bytes;
   delete L;
 }

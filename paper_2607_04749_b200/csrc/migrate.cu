@@ -116,7 +116,7 @@ static etc_status launch_migrate(const etc_plan* pl, const void* const* src_bufs
     if (pl->new_bytes[i] > 0 && !dst_bufs[i]) return ETC_ERR_INVALID_ARG;
     if (reinterpret_cast<uintptr_t>(dst_bufs[i]) & 15) return ETC_ERR_INVALID_ARG;
   }
-  pl->last_stream = st;
+  pl->streams.note(st);
   // pointer tables: source pointers then destination pointers
   ETC_CUDA_TRY(cudaMemcpyAsync(d_ptrs, src_bufs, sizeof(void*) * ns, cudaMemcpyHostToDevice, st));
   ETC_CUDA_TRY(cudaMemcpyAsync(d_ptrs + ns, dst_bufs, sizeof(void*) * nd, cudaMemcpyHostToDevice, st));

@@ -399,7 +399,7 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
   const int n_old = old_l->t.n_dev, n_new = new_l->t.n_dev, P = n_old > n_new ? n_old : n_new;
   if ((long long)P * ETC_NUM_KINDS > 65535) return ETC_ERR_WORKSPACE;
   cudaStream_t st = (cudaStream_t)stream;
-  old_l->last_stream = new_l->last_stream = st;
+  old_l->streams.note(st); new_l->streams.note(st);
   const int K = (flags & ETC_KIND_MAJOR) ? ETC_NUM_KINDS : 1;
   const long long U = (long long)K * n_old * n_new;
   // sub-blocks per unit: enough warps to fill the machine when there are few units, 1 when there are many
@@ -408,6 +408,7 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
 
   etc_plan* pl = new etc_plan();
   pl->n_old = n_old; pl->n_new = n_new; pl->P = P; pl->flags = flags; pl->stream_created_on = st;
+  pl->streams.note(st);
   pl->old_bytes.assign(old_l->h_buffer_bytes, old_l->h_buffer_bytes + (size_t)n_old * ETC_NUM_KINDS);
   pl->new_bytes.assign(new_l->h_buffer_bytes, new_l->h_buffer_bytes + (size_t)n_new * ETC_NUM_KINDS);
   auto fail = [&](etc_status s) { etc_plan_destroy(pl); return s; };
@@ -508,7 +509,7 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
 
 extern "C" void etc_plan_destroy(etc_plan* pl) {
   if (!pl) return;
-  cudaStream_t st = pl->last_stream ? pl->last_stream : pl->stream_created_on;
+  cudaStream_t st = pl->streams.join(pl->stream_created_on);
   if (pl->d_ws) cudaFreeAsync(pl->d_ws, st);
   if (pl->d_tb) cudaFreeAsync(pl->d_tb, st);
   if (pl->d_rounds_ws) cudaFreeAsync(pl->d_rounds_ws, st);

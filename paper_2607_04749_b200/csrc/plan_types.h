@@ -42,7 +42,7 @@ struct RoundRec {
 struct etc_plan {
   int32_t n_old = 0, n_new = 0, P = 0, flags = 0;
   cudaStream_t stream_created_on = nullptr;
-  mutable cudaStream_t last_stream = nullptr;      // last stream a migrate was enqueued on (frees are ordered after it)
+  mutable etc::StreamSet streams;                  // streams the plan's tables were written / read on (frees are ordered after them)
   etc::PlanTotals totals{};
   void* d_ws = nullptr;                            // blob 1: the tables below up to d_ptrs
   void* d_tb = nullptr;                            // blob 2: slices, first-chunk indices, chunks

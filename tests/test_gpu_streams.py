@@ -1,0 +1,67 @@
+"""-m gpu: object lifetime across streams.  bench.py plans step i+1 on a side stream while the copy kernels of step i
+still run on another stream and drops each plan / layout as soon as the next one exists.  The library frees its tables
+with stream-ordered frees, so the free must be ordered after EVERY stream that still reads the tables (the legacy
+default stream, a NULL cudaStream_t, included): otherwise the next plan reuses the memory under a running copy kernel.
+The result must stay bit-identical to the oracle's element-wise migration."""
+from __future__ import annotations
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from etc_inputs import workload
+from oracle import oracle as O
+from helpers import make_logical, shard_all
+from gpu_helpers import upload, download
+
+
+@pytest.fixture(scope="module")
+def E():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_2607_04749_b200 as E
+    E.init()
+    return E
+
+
+@pytest.mark.parametrize("copy_on_default_stream", [True, False])
+@pytest.mark.parametrize("name,flags", [("s3", 0), ("s5", 1)])
+def test_pipelined_plans_dropped_early(E, name, flags, copy_on_default_stream):
+    w = workload(name)
+    model = w["model"]
+    oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
+    src_np = shard_all(oo, make_logical(model, w["seed"], "stamp"))
+    src = upload(src_np)
+    lay_new = E.etc_layout_create(model, w["new"])
+    dst = E.alloc_buffers(lay_new, fill=0x3C)
+    plan_stream = torch.cuda.Stream(priority=-1)
+    copy_stream = torch.cuda.default_stream() if copy_on_default_stream else torch.cuda.Stream()
+    # a big dummy copy keeps the copy stream busy so that the planning of later steps runs far ahead of it
+    big_a = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")
+    big_b = torch.empty_like(big_a)
+    staging = None
+    dmap = None
+    for it in range(12):
+        with torch.cuda.stream(plan_stream):
+            lo, ln = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])
+            ov, _, _ = E.etc_cost_matrix(lo, ln, stream=plan_stream)
+            dm, _ = E.etc_sketch(ov, stream=plan_stream)
+            plan = E.etc_plan_create(lo, ln, dm, flags, stream=plan_stream)
+            done = torch.cuda.Event()
+            done.record(plan_stream)
+        if staging is None:
+            staging = torch.empty(max(plan.stats.staging_bytes, 16), dtype=torch.uint8, device="cuda")
+            dmap = dm.cpu().numpy().copy()
+        assert plan.stats.staging_bytes <= staging.numel()
+        with torch.cuda.stream(copy_stream):
+            for _ in range(3):
+                big_b.copy_(big_a, non_blocking=True)
+            copy_stream.wait_event(done)
+            E.etc_migrate(plan, src, dst, staging, stream=copy_stream)
+        del plan, lo, ln            # dropped while the copy stream is still far behind
+    torch.cuda.synchronize()
+    exp, _, _ = O.migrate(oo, on, dmap, src_np)
+    for key, e in exp.items():
+        if e.shape[0]:
+            assert np.array_equal(download(dst[key], on.elem_bytes(key[1])), e), key
