@@ -44,7 +44,9 @@ typedef struct {
 } orc_model;
 
 /* pp_first / pp_last: layers on the first / last pipeline stage (0 = not set), reading A27 (uneven pipeline split) */
-typedef struct { int32_t tp, pp, dp, dist_opt, pp_first, pp_last; } orc_cfg;
+/* dist_opt_align (reading A28, f3): the DP shard size of the distributed optimizer is rounded up to a multiple of this
+ * many elements (0 or 1 = no rounding), as Megatron-LM pads its buffers so that every DP shard is aligned */
+typedef struct { int32_t tp, pp, dp, dist_opt, pp_first, pp_last, dist_opt_align; } orc_cfg;
 
 typedef struct { int64_t rows, cols; int32_t split, where, layer; } orc_lt;   /* one logical tensor */
 
@@ -147,7 +149,7 @@ static int orc_stage_begin(int n_layers, const orc_cfg* c, int s) {
 /* divisibility rules (layers divisible by PP, hidden by TP; A7, A10, A12) */
 static int orc_validate(const orc_model* m, const orc_cfg* c) {
   if (!m || !c) return ORC_ERR_ARG;
-  if (c->tp < 1 || c->pp < 1 || c->dp < 1) return ORC_ERR_ARG;
+  if (c->tp < 1 || c->pp < 1 || c->dp < 1 || c->dist_opt_align < 0) return ORC_ERR_ARG;
   if (m->n_layers < 1 || m->hidden < 1 || m->n_q_heads < 1 || m->n_kv_heads < 1 || m->head_dim < 1 ||
       m->ffn_hidden < 1 || m->vocab < 1 || m->max_pos < 0) return ORC_ERR_ARG;
   if (m->param_bytes != 2 && m->param_bytes != 4) return ORC_ERR_ARG;
@@ -252,7 +254,9 @@ static void orc_flat_range(const orc_layout* L, int d, int s, int r, int kind, i
   int64_t n = L->Lloc[s * L->c.tp + r];
   if (!orc_has_kind(L, kind)) { *lo = 0; *hi = 0; return; }
   if (orc_dp_sharded(L, kind)) {
-    int64_t chunk = (n + L->c.dp - 1) / L->c.dp;
+    /* A14: chunk = ceil(n / dp); A28: rounded up to a multiple of `align` elements: chunk = ceil(n / (dp*align)) * align */
+    int64_t align = L->c.dist_opt_align > 1 ? L->c.dist_opt_align : 1;
+    int64_t chunk = (n + (int64_t)L->c.dp * align - 1) / ((int64_t)L->c.dp * align) * align;
     int64_t a = (int64_t)d * chunk, b = (int64_t)(d + 1) * chunk;
     *lo = a < n ? a : n; *hi = b < n ? b : n;
   } else { *lo = 0; *hi = n; }

@@ -23,7 +23,7 @@ class Model(C.Structure):
 
 
 class Cfg(C.Structure):
-    _fields_ = [(n, C.c_int32) for n in ("tp", "pp", "dp", "dist_opt", "pp_first", "pp_last")]
+    _fields_ = [(n, C.c_int32) for n in ("tp", "pp", "dp", "dist_opt", "pp_first", "pp_last", "dist_opt_align")]
 
 
 def build(force: bool = False) -> str:

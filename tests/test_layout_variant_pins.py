@@ -86,3 +86,62 @@ def test_uneven_reconfigurations_full_battery():
         na, nb = a["tp"] * a["pp"] * a["dp"], b["tp"] * b["pp"] * b["dp"]
         dm = rng.permutation(max(na, nb))[:nb].astype(np.int32)
         assert _check_reconfiguration(TINY[name], a, b, 950 + i, device_map=dm)
+
+
+# ---------------------------------------------------------------------------------------------- A28: aligned dist-opt
+GOLD_ALIGN = read_golden("distopt_align_handcomputed.txt")
+
+
+def _cfga(tp, pp, dp, align, dist_opt=1):
+    return dict(tp=tp, pp=pp, dp=dp, dist_opt=dist_opt, dist_opt_align=align)
+
+
+@pytest.mark.parametrize("row", GOLD_ALIGN, ids=lambda r: "-".join(r[1:7]))
+def test_aligned_distopt_ranges_handcomputed(row):
+    name, tp, pp, dp, align = row[1], int(row[2]), int(row[3]), int(row[4]), int(row[5])
+    L = O.Layout(TINY[name], _cfga(tp, pp, dp, align))
+    got = [L.buffer_elems(0 + tp * d, 1) for d in range(dp)]            # device id = r + tp*(d + dp*s), r = s = 0
+    assert got == [int(x) for x in row[7:]]
+    # PARAM stays replicated (BASELINE.json config 4), M and V follow MASTER
+    assert len({L.buffer_elems(tp * d, 0) for d in range(dp)}) == 1
+    assert all(L.buffer_elems(tp * d, 2) == got[d] and L.buffer_elems(tp * d, 3) == got[d] for d in range(dp))
+
+
+def test_aligned_distopt_invariants():
+    """Every shard boundary is a multiple of the alignment, shards tile the local space exactly once, and alignment
+    changes nothing when the kind is not DP-sharded."""
+    for name, model in TINY.items():
+        for tp, pp, dp, align in [(1, 2, 2, 16), (2, 1, 4, 8), (1, 1, 3, 100), (2, 2, 2, 7)]:
+            try:
+                L = O.Layout(model, _cfga(tp, pp, dp, align))
+                R = O.Layout(model, _cfga(tp, pp, dp, align, dist_opt=0))
+            except O.OracleError:
+                continue
+            for s in range(pp):
+                for r in range(tp):
+                    sizes = [L.buffer_elems(r + tp * (d + dp * s), 2) for d in range(dp)]
+                    assert sum(sizes) == R.buffer_elems(r + tp * dp * s, 2)
+                    full = [x for x in sizes if x and x != sizes[0]]
+                    assert sizes[0] % align == 0 or sum(sizes) == sizes[0]
+                    assert len(full) <= 1                                  # only one ragged shard
+                    lts = [L.global_of(r + tp * (d + dp * s), 2) for d in range(dp) if sizes[d]]
+                    ref = R.global_of(r + tp * dp * s, 2)
+                    for j in range(4):
+                        assert np.array_equal(np.concatenate([x[j] for x in lts]), ref[j])
+    with pytest.raises(O.OracleError):
+        O.Layout(TINY["gpt_t"], _cfga(1, 1, 2, -4))
+
+
+def test_aligned_distopt_full_battery():
+    """P2-P5, P8-P10 on reconfigurations between differently aligned distributed-optimizer layouts."""
+    cases = [("gpt_t", _cfga(1, 1, 4, 128), _cfga(2, 1, 2, 64)),
+             ("gpt_t", _cfga(2, 2, 2, 32), _cfga(1, 2, 2, 0, dist_opt=0)),
+             ("gpt_np", _cfga(1, 2, 2, 0), _cfga(2, 2, 2, 48)),
+             ("llama_u", _cfga(2, 1, 4, 24), _cfga(1, 2, 3, 40)),
+             ("llama_t", _cfga(1, 2, 3, 1000), _cfga(2, 2, 2, 8))]
+    rng = np.random.default_rng(11)
+    for i, (name, a, b) in enumerate(cases):
+        assert _check_reconfiguration(TINY[name], a, b, 1200 + i)
+        na, nb = a["tp"] * a["pp"] * a["dp"], b["tp"] * b["pp"] * b["dp"]
+        dm = rng.permutation(max(na, nb))[:nb].astype(np.int32)
+        assert _check_reconfiguration(TINY[name], a, b, 1250 + i, device_map=dm)
