@@ -73,8 +73,12 @@ typedef struct {
  * contiguous flat ranges of each (stage, tp-rank) local parameter space (reading A14); PARAM stays replicated.
  * pp_first / pp_last (f3, reading A27): number of layers on the first / last pipeline stage, 0 = not set (as
  * Megatron-LM's --decoder-first/last-pipeline-num-layers); the remaining layers are split evenly over the remaining
- * stages.  Both 0 = the even split the paper requires. */
-typedef struct { int32_t tp, pp, dp, dist_opt, pp_first, pp_last; } etc_parallel_cfg;
+ * stages.  Both 0 = the even split the paper requires.
+ * dist_opt_align (f3, reading A28): with dist_opt = 1 the DP shard size is rounded up to a multiple of this many
+ * elements, chunk = ceil(Lloc / (dp*align)) * align (Megatron-LM pads its distributed-optimizer buffers so that every
+ * DP shard is aligned); 0 or 1 = no rounding (reading A14); negative -> ETC_ERR_INVALID_ARG.  Padding is not stored:
+ * a buffer holds only the real elements of its range. */
+typedef struct { int32_t tp, pp, dp, dist_opt, pp_first, pp_last, dist_opt_align; } etc_parallel_cfg;
 
 typedef struct etc_layout etc_layout;   /* opaque, immutable after create */
 typedef struct etc_plan etc_plan;       /* opaque, immutable after create */

@@ -39,7 +39,7 @@ class _ModelDesc(C.Structure):
 
 
 class _ParallelCfg(C.Structure):
-    _fields_ = [(n, C.c_int32) for n in ("tp", "pp", "dp", "dist_opt", "pp_first", "pp_last")]
+    _fields_ = [(n, C.c_int32) for n in ("tp", "pp", "dp", "dist_opt", "pp_first", "pp_last", "dist_opt_align")]
 
 
 class _PlanStats(C.Structure):
@@ -163,7 +163,8 @@ def etc_layout_create(model: dict, cfg: dict) -> Layout:
                    ffn_hidden=model["ffn_hidden"], vocab=model["vocab"], max_pos=model["max_pos"],
                    tied_embeddings=model["tied"], param_dtype=model["param_bytes"], kinds=model["kinds"])
     c = _ParallelCfg(tp=cfg["tp"], pp=cfg["pp"], dp=cfg["dp"], dist_opt=cfg.get("dist_opt", 0),
-                     pp_first=cfg.get("pp_first", 0), pp_last=cfg.get("pp_last", 0))
+                     pp_first=cfg.get("pp_first", 0), pp_last=cfg.get("pp_last", 0),
+                     dist_opt_align=cfg.get("dist_opt_align", 0))
     h = C.c_void_p()
     _check(lib().etc_layout_create(C.byref(m), C.byref(c), C.byref(h)))
     return Layout(h, model, cfg)

@@ -72,7 +72,7 @@ static int stage_begin(int n_layers, const etc_parallel_cfg& c, int s) {
 
 static etc_status validate(const etc_model_desc* m, const etc_parallel_cfg* c) {
   if (!m || !c) return ETC_ERR_INVALID_ARG;
-  if (c->tp < 1 || c->pp < 1 || c->dp < 1 || (c->dist_opt != 0 && c->dist_opt != 1)) return ETC_ERR_INVALID_ARG;
+  if (c->tp < 1 || c->pp < 1 || c->dp < 1 || (c->dist_opt != 0 && c->dist_opt != 1) || c->dist_opt_align < 0) return ETC_ERR_INVALID_ARG;
   if (m->style != ETC_GPT && m->style != ETC_LLAMA) return ETC_ERR_INVALID_ARG;
   if (m->n_layers < 1 || m->hidden < 1 || m->n_q_heads < 1 || m->n_kv_heads < 1 || m->head_dim < 1 ||
       m->ffn_hidden < 1 || m->vocab < 1 || m->max_pos < 0) return ETC_ERR_INVALID_ARG;
@@ -214,8 +214,9 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
           const int64_t es = kind == 0 ? m.param_dtype : 4;
           const bool dp_sharded = cfg->dist_opt && dp > 1 && kind >= 1;
           int64_t lo = 0, hi = Lloc;
-          if (dp_sharded) {                                  // reading A14: contiguous flat range, chunk = ceil(Lloc/dp)
-            const int64_t chunk = (Lloc + dp - 1) / dp;
+          if (dp_sharded) {                                  // readings A14 / A28: contiguous flat range of `chunk` elements
+            const int64_t unit = (int64_t)dp * std::max(1, cfg->dist_opt_align);
+            const int64_t chunk = (Lloc + unit - 1) / unit * std::max(1, cfg->dist_opt_align);
             lo = std::min<int64_t>(Lloc, (int64_t)d * chunk); hi = std::min<int64_t>(Lloc, (int64_t)(d + 1) * chunk);
           }
           bufbytes[(size_t)dev * ETC_NUM_KINDS + kind] = (hi - lo) * es;

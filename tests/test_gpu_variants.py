@@ -59,3 +59,39 @@ def test_uneven_validation_codes_match_oracle(E):
         with pytest.raises(E.EtcError) as ge:
             E.etc_layout_create(m, cfg)
         assert ge.value.code == oe.value.code, cfg
+
+
+# ---------------------------------------------------------------------------------------------- A28: aligned dist-opt
+def _cfga(tp, pp, dp, align, dist_opt=1):
+    return dict(tp=tp, pp=pp, dp=dp, dist_opt=dist_opt, dist_opt_align=align)
+
+
+def test_aligned_distopt_tiny(E):
+    T = dict(tiny_models())
+    cases = [("gpt_t", _cfga(1, 1, 4, 128), _cfga(2, 1, 2, 64)),
+             ("gpt_t", _cfga(2, 2, 2, 32), _cfga(1, 2, 2, 0, dist_opt=0)),
+             ("gpt_np", _cfga(1, 2, 2, 0), _cfga(2, 2, 2, 48)),
+             ("llama_u", _cfga(2, 1, 4, 24), _cfga(1, 2, 3, 40)),
+             ("llama_t", _cfga(1, 2, 3, 1000), _cfga(2, 2, 2, 8)),
+             ("gpt_t", _cfga(1, 1, 4, 1024), _cfga(1, 1, 4, 128))]         # a DP rank that holds nothing
+    rng = np.random.default_rng(41)
+    for i, (name, a, b) in enumerate(cases):
+        for flags in (0, 3):
+            _check_migration(E, T[name], a, b, 800 + i, flags=flags)
+        na, nb = a["tp"] * a["pp"] * a["dp"], b["tp"] * b["pp"] * b["dp"]
+        _check_migration(E, T[name], a, b, 850 + i, device_map=rng.permutation(max(na, nb))[:nb].astype(np.int32))
+    la = E.etc_layout_create(T["gpt_t"], _cfga(1, 1, 4, 128))
+    assert [la.buffer_bytes(d, 1) for d in range(4)] == [640 * 4, 640 * 4, 640 * 4, 592 * 4]   # tests/golden, hand-computed
+    with pytest.raises(E.EtcError) as ge:
+        E.etc_layout_create(T["gpt_t"], _cfga(1, 1, 2, -4))
+    assert ge.value.code == -1
+
+
+def test_aligned_distopt_scaled_c4(E):
+    """s4 (config 4's reconfiguration, TP2 PP4 DP2 -> TP4 PP2 DP4, distributed optimizer on both sides) with 128-element
+    aligned DP shards on the old side and 256-element aligned shards on the new side."""
+    w = workload("s4")
+    old, new = dict(w["old"], dist_opt_align=128), dict(w["new"], dist_opt_align=256)
+    for flags in (0, 1):
+        g = _check_migration(E, w["model"], old, new, w["seed"], flags=flags)
+    assert g["plan"].stats.remote_bytes > 0
