@@ -31,7 +31,7 @@
 #endif
 
 #define ORC_MAX_KINDS 4
-enum { ORC_REPL = 0, ORC_COL = 1, ORC_ROW = 2, ORC_COL2 = 3 };
+enum { ORC_REPL = 0, ORC_COL = 1, ORC_ROW = 2, ORC_COL2 = 3, ORC_QKV = 4 };
 enum { ORC_PRE = 0, ORC_LAYER = 1, ORC_POST = 2 };
 enum { ORC_OK = 0, ORC_ERR_ARG = -1, ORC_ERR_INDIVISIBLE = -2, ORC_ERR_UNSUPPORTED = -6, ORC_ERR_UNRECOVERABLE = -8 };
 
@@ -41,6 +41,8 @@ typedef struct {
   int32_t tied;        /* 1: output layer shares word_embeddings (replica on the last PP stage when pp > 1) */
   int32_t param_bytes; /* element size of kind PARAM: 2 (bf16) or 4 (fp32) */
   int32_t kinds;       /* bitmask over kinds 0..3 = PARAM, MASTER, ADAM_M, ADAM_V */
+  int32_t qkv_order;   /* logical row order of the fused QKV tensor (readings A10, A29): 0 = KV-group order (per group:
+                          its q heads, K, V); 1 = [Q; K; V] (all q heads, then all k heads, then all v heads) */
 } orc_model;
 
 /* pp_first / pp_last: layers on the first / last pipeline stage (0 = not set), reading A27 (uneven pipeline split) */
@@ -55,8 +57,9 @@ typedef struct {
   int32_t lt;          /* logical tensor id */
   int32_t post_copy;   /* 1: this is the tied replica of word_embeddings held by the last stage */
   int64_t start, n;    /* position and element count inside the local flat space */
-  int32_t nblk;        /* row blocks (2 for COL2: gate block then up block) */
-  int64_t rb[2], nrb;  /* first logical row of each block, rows per block */
+  int32_t nblk;        /* row blocks, stored one after the other (COL2: gate, up; QKV: up to 3, readings A29/A30) */
+  int64_t rb[3], nr[3]; /* first logical row and number of rows of each block */
+  int32_t rep[3];      /* how many TP ranks hold each element of the block (1 = TP-sharded, tp = replicated) */
   int64_t c0, W;       /* first logical column, local row length */
 } orc_shard;
 
@@ -83,8 +86,8 @@ static int orc_logical(const orc_model* m, orc_lt* out) {
     if (m->style == 0) {
       ADD(1, h, ORC_REPL, ORC_LAYER, l);      /* ln1.weight */
       ADD(1, h, ORC_REPL, ORC_LAYER, l);      /* ln1.bias */
-      ADD(qkv, h, ORC_COL, ORC_LAYER, l);     /* qkv.weight, rows in KV-group order (A10) */
-      ADD(qkv, 1, ORC_COL, ORC_LAYER, l);     /* qkv.bias */
+      ADD(qkv, h, ORC_QKV, ORC_LAYER, l);     /* qkv.weight (A10, A29, A30) */
+      ADD(qkv, 1, ORC_QKV, ORC_LAYER, l);     /* qkv.bias */
       ADD(h, qd, ORC_ROW, ORC_LAYER, l);      /* proj.weight */
       ADD(1, h, ORC_REPL, ORC_LAYER, l);      /* proj.bias */
       ADD(1, h, ORC_REPL, ORC_LAYER, l);      /* ln2.weight */
@@ -95,7 +98,7 @@ static int orc_logical(const orc_model* m, orc_lt* out) {
       ADD(1, h, ORC_REPL, ORC_LAYER, l);      /* fc2.bias */
     } else {
       ADD(1, h, ORC_REPL, ORC_LAYER, l);      /* ln1.weight */
-      ADD(qkv, h, ORC_COL, ORC_LAYER, l);     /* qkv.weight */
+      ADD(qkv, h, ORC_QKV, ORC_LAYER, l);     /* qkv.weight */
       ADD(h, qd, ORC_ROW, ORC_LAYER, l);      /* proj.weight */
       ADD(1, h, ORC_REPL, ORC_LAYER, l);      /* ln2.weight */
       ADD(2 * f, h, ORC_COL2, ORC_LAYER, l);  /* fc1.weight = [gate; up] */
@@ -155,26 +158,83 @@ static int orc_validate(const orc_model* m, const orc_cfg* c) {
   if (m->param_bytes != 2 && m->param_bytes != 4) return ORC_ERR_ARG;
   if (m->kinds <= 0 || m->kinds > 15) return ORC_ERR_ARG;
   if (m->n_q_heads % m->n_kv_heads) return ORC_ERR_ARG;
-  if (c->tp > m->n_kv_heads) return ORC_ERR_UNSUPPORTED;       /* KV-head replication is out of scope (A10) */
+  if (m->qkv_order != 0 && m->qkv_order != 1) return ORC_ERR_ARG;
+  if (c->tp > m->n_kv_heads) {                                 /* KV-head replication (reading A30) */
+    int rep = c->tp / m->n_kv_heads;
+    if (c->tp % m->n_kv_heads || (m->n_q_heads / m->n_kv_heads) % rep) return ORC_ERR_UNSUPPORTED;
+  }
   if (orc_stage_begin(m->n_layers, c, 0) < 0) return orc_stage_begin(m->n_layers, c, 0) == -2 ? ORC_ERR_ARG : ORC_ERR_INDIVISIBLE;
-  if (m->n_kv_heads % c->tp) return ORC_ERR_INDIVISIBLE;
+  if (c->tp <= m->n_kv_heads && m->n_kv_heads % c->tp) return ORC_ERR_INDIVISIBLE;
   if (m->ffn_hidden % c->tp) return ORC_ERR_INDIVISIBLE;
   if (m->vocab % c->tp) return ORC_ERR_INDIVISIBLE;
   return ORC_OK;
 }
 
 /* ---------------------------------------------------------------- layout */
-static void orc_make_shard(const orc_lt* t, int lt, int post_copy, int tp, int r, orc_shard* s) {
-  s->lt = lt; s->post_copy = post_copy; s->nblk = 1; s->rb[0] = 0; s->rb[1] = 0;
-  s->nrb = t->rows; s->c0 = 0; s->W = t->cols;
+/* TP shard of logical tensor t on TP rank r: an ordered list of row blocks x a column range.
+ * QKV (readings A10, A29, A30): with q = n_q heads, k = n_kv heads, d rows per head, qpg = q/k q heads per KV group.
+ *   tp <= k (each rank holds whole groups, kpr = k/tp of them):
+ *     order 0 (group order, group g = rows [g*(qpg+2)*d, (g+1)*(qpg+2)*d)): one block, groups [r*kpr, (r+1)*kpr)
+ *     order 1 ([Q;K;V]): three blocks: q heads [r*q/tp, (r+1)*q/tp), k heads [r*kpr, (r+1)*kpr), v heads likewise
+ *   tp > k (KV-head replication, rep = tp/k ranks share group g = r/rep; rank r holds qpr = qpg/rep q heads of it,
+ *           the j-th share with j = r % rep, and the WHOLE K and V head of the group):
+ *     order 0: two blocks: q rows [g*(qpg+2)*d + j*qpr*d, +qpr*d), then the K,V rows [g*(qpg+2)*d + qpg*d, +2d)
+ *     order 1: three blocks: q heads [r*qpr, (r+1)*qpr), k head g, v head g
+ *   K and V blocks of the replicated case are held by rep ranks (rep[] = tp/k), everything else by one. */
+static void orc_make_shard(const orc_model* m, const orc_lt* t, int lt, int post_copy, int tp, int r, orc_shard* s) {
+  s->lt = lt; s->post_copy = post_copy; s->nblk = 1; s->c0 = 0; s->W = t->cols;
+  for (int b = 0; b < 3; b++) { s->rb[b] = 0; s->nr[b] = 0; s->rep[b] = 1; }
+  s->nr[0] = t->rows;
   switch (t->split) {
-    case ORC_REPL: break;                                                       /* whole tensor on every rank */
-    case ORC_COL:  s->nrb = t->rows / tp; s->rb[0] = r * s->nrb; break;         /* rows / tp */
+    case ORC_REPL: s->rep[0] = tp; break;                                       /* whole tensor on every rank */
+    case ORC_COL:  s->nr[0] = t->rows / tp; s->rb[0] = r * s->nr[0]; break;     /* rows / tp */
     case ORC_ROW:  s->W = t->cols / tp; s->c0 = r * s->W; break;                /* cols / tp */
-    case ORC_COL2: { int64_t F = t->rows / 2; s->nblk = 2; s->nrb = F / tp;     /* gate block, then up block */
-                     s->rb[0] = r * s->nrb; s->rb[1] = F + r * s->nrb; break; }
+    case ORC_COL2: { int64_t F = t->rows / 2; s->nblk = 2; s->nr[0] = s->nr[1] = F / tp;   /* gate block, then up block */
+                     s->rb[0] = r * s->nr[0]; s->rb[1] = F + r * s->nr[0]; break; }
+    case ORC_QKV: {
+      int64_t q = m->n_q_heads, k = m->n_kv_heads, d = m->head_dim, qpg = q / k;
+      if (tp <= k) {
+        int64_t kpr = k / tp;
+        if (m->qkv_order == 0) { s->nr[0] = kpr * (qpg + 2) * d; s->rb[0] = r * s->nr[0]; }
+        else {
+          s->nblk = 3;
+          s->nr[0] = q / tp * d; s->rb[0] = r * s->nr[0];
+          s->nr[1] = kpr * d;    s->rb[1] = q * d + r * s->nr[1];
+          s->nr[2] = kpr * d;    s->rb[2] = (q + k) * d + r * s->nr[2];
+        }
+      } else {
+        int64_t rep = tp / k, g = r / rep, j = r % rep, qpr = qpg / rep;
+        if (m->qkv_order == 0) {
+          int64_t base = g * (qpg + 2) * d;
+          s->nblk = 2;
+          s->nr[0] = qpr * d; s->rb[0] = base + j * qpr * d;
+          s->nr[1] = 2 * d;   s->rb[1] = base + qpg * d;  s->rep[1] = (int32_t)rep;
+        } else {
+          s->nblk = 3;
+          s->nr[0] = qpr * d; s->rb[0] = (int64_t)r * qpr * d;
+          s->nr[1] = d;       s->rb[1] = q * d + g * d;        s->rep[1] = (int32_t)rep;
+          s->nr[2] = d;       s->rb[2] = (q + k) * d + g * d;  s->rep[2] = (int32_t)rep;
+        }
+      }
+      break;
+    }
   }
-  s->n = (int64_t)s->nblk * s->nrb * s->W;
+  s->n = 0;
+  for (int b = 0; b < s->nblk; b++) s->n += s->nr[b] * s->W;
+}
+
+/* local row i of a shard -> (block, row inside the block); blocks are stored one after the other */
+static int orc_block_of(const orc_shard* q, int64_t i, int64_t* within) {
+  int b = 0;
+  while (b + 1 < q->nblk && i >= q->nr[b]) { i -= q->nr[b]; b++; }
+  *within = i;
+  return b;
+}
+/* first local row of block b */
+static int64_t orc_block_start(const orc_shard* q, int b) {
+  int64_t x = 0;
+  for (int i = 0; i < b; i++) x += q->nr[i];
+  return x;
 }
 
 void orc_layout_free(orc_layout* L) {
@@ -223,11 +283,11 @@ int32_t orc_layout_new(const orc_model* m, const orc_cfg* c, orc_layout** out) {
       if (pass == ORC_PRE && s != 0) continue;
       if (pass == ORC_LAYER && (t->layer < l_begin || t->layer >= l_end)) continue;
       if (pass == ORC_POST && s != c->pp - 1) continue;
-      orc_make_shard(t, i, 0, c->tp, r, &v[k]); v[k].start = pos; pos += v[k].n;
+      orc_make_shard(m, t, i, 0, c->tp, r, &v[k]); v[k].start = pos; pos += v[k].n;
       L->idx[s * L->n_lt + i] = k; k++;
     }
     if (m->tied && c->pp > 1 && s == c->pp - 1) {                  /* A11: replica of word_embeddings (tensor 0) */
-      orc_make_shard(&L->lt[0], 0, 1, c->tp, r, &v[k]); v[k].start = pos; pos += v[k].n;
+      orc_make_shard(m, &L->lt[0], 0, 1, c->tp, r, &v[k]); v[k].start = pos; pos += v[k].n;
       L->tied_idx[s] = k; k++;
     }
     L->sh[s * c->tp + r] = v; L->n_sh[s * c->tp + r] = k; L->Lloc[s * c->tp + r] = pos;
@@ -280,8 +340,8 @@ int32_t orc_global_of(const orc_layout* L, int32_t dev, int32_t kind, int64_t l,
   while (a < b) { int mid = (a + b + 1) / 2; if (v[mid].start <= g) a = mid; else b = mid - 1; }
   const orc_shard* q = &v[a];
   int64_t x = g - q->start, i = x / q->W, j = x % q->W;
-  int blk = (int)(i / q->nrb);
-  *lt = q->lt; *post_copy = q->post_copy; *row = q->rb[blk] + i % q->nrb; *col = q->c0 + j;
+  int64_t within; int blk = orc_block_of(q, i, &within);
+  *lt = q->lt; *post_copy = q->post_copy; *row = q->rb[blk] + within; *col = q->c0 + j;
   return ORC_OK;
 }
 
@@ -309,9 +369,9 @@ static int orc_holders(const orc_layout* L, int kind, int lt, int64_t row, int64
       const orc_shard* q = &L->sh[s * L->c.tp + r][k];
       if (col < q->c0 || col >= q->c0 + q->W) continue;
       int blk = -1;
-      for (int b = 0; b < q->nblk; b++) if (row >= q->rb[b] && row < q->rb[b] + q->nrb) blk = b;
+      for (int b = 0; b < q->nblk; b++) if (row >= q->rb[b] && row < q->rb[b] + q->nr[b]) blk = b;
       if (blk < 0) continue;
-      int64_t g = q->start + ((int64_t)blk * q->nrb + (row - q->rb[blk])) * q->W + (col - q->c0);
+      int64_t g = q->start + (orc_block_start(q, blk) + (row - q->rb[blk])) * q->W + (col - q->c0);
       for (int d = 0; d < L->c.dp; d++) {
         int64_t lo, hi; orc_flat_range(L, d, s, r, kind, &lo, &hi);
         if (g < lo || g >= hi) continue;
@@ -397,8 +457,8 @@ static int64_t orc_isect(int64_t a0, int64_t a1, int64_t b0, int64_t b1) {
 /* columns [*c0,*c1) of logical row `row` that buffer range [lo,hi) of shard q holds; returns 0 if none */
 static int orc_row_cols(const orc_shard* q, int64_t lo, int64_t hi, int64_t row, int64_t* c0, int64_t* c1) {
   for (int b = 0; b < q->nblk; b++) {
-    if (row < q->rb[b] || row >= q->rb[b] + q->nrb) continue;
-    int64_t g0 = q->start + ((int64_t)b * q->nrb + (row - q->rb[b])) * q->W, g1 = g0 + q->W;
+    if (row < q->rb[b] || row >= q->rb[b] + q->nr[b]) continue;
+    int64_t g0 = q->start + (orc_block_start(q, b) + (row - q->rb[b])) * q->W, g1 = g0 + q->W;
     int64_t a = g0 > lo ? g0 : lo, e = g1 < hi ? g1 : hi;
     if (e <= a) return 0;
     *c0 = q->c0 + (a - g0); *c1 = q->c0 + (e - g0);
@@ -439,7 +499,7 @@ int32_t orc_overlap_ranges(const orc_layout* Lo, const orc_layout* Ln, int64_t* 
           if (!cols) continue;
           for (int ba = 0; ba < A->nblk; ba++) for (int bb = 0; bb < B->nblk; bb++) {
             int64_t r0 = A->rb[ba] > B->rb[bb] ? A->rb[ba] : B->rb[bb];
-            int64_t r1a = A->rb[ba] + A->nrb, r1b = B->rb[bb] + B->nrb, r1 = r1a < r1b ? r1a : r1b;
+            int64_t r1a = A->rb[ba] + A->nr[ba], r1b = B->rb[bb] + B->nr[bb], r1 = r1a < r1b ? r1a : r1b;
             if (r1 <= r0) continue;
             if (wholeA && wholeB) { acc += (r1 - r0) * cols * es; continue; }
             for (int64_t row = r0; row < r1; row++) {            /* a held range cuts through rows: go row by row */
@@ -527,7 +587,8 @@ int32_t orc_sketch_hungarian(const int64_t* overlap, int32_t n_new, int32_t P, c
  *   (i)  local first: if old device p holds the element, the source is p (paper's Refer: stays in place);
  *   (ii) else the designated holder (d, s, r): s = the old stage holding the tensor (tied word_embeddings held by two
  *        stages: stage 0 for the `pre` copy, the last stage for the `post` copy); r = the unique TP rank holding it
- *        if the tensor is TP-sharded in old, else r' mod tp_old; d = the unique DP rank whose flat range holds it if
+ *        if the tensor is TP-sharded in old, else r' mod tp_old (in general: round-robin by r' over the ranks of that
+ *        stage holding the element, A30); d = the unique DP rank whose flat range holds it if
  *        the kind is DP-sharded in old, else d' mod dp_old (round-robin over source groups). */
 static int orc_pick_source(const orc_layout* Lo, const orc_layout* Ln, int n, int p, int kind,
                            int lt, int post_copy, int64_t row, int64_t col, orc_holder* h, orc_holder* src) {
@@ -539,8 +600,19 @@ static int orc_pick_source(const orc_layout* Lo, const orc_layout* Ln, int n, in
   for (int i = 1; i < nh; i++) { if (h[i].s < smin) smin = h[i].s; if (h[i].s > smax) smax = h[i].s; }
   int s_des = (smin == smax) ? smin : (post_copy ? smax : smin);
   int r_des = -1, d_first = -1, d_des;
-  if (Lo->lt[lt].split == ORC_REPL) r_des = rn % Lo->c.tp;                 /* replicated over TP: round-robin */
-  else for (int i = 0; i < nh; i++) if (h[i].s == s_des) r_des = h[i].r;   /* TP-sharded: the one rank holding it */
+  {
+    /* the TP ranks of stage s_des holding the element, ascending: one if the element is TP-sharded, all tp if the
+     * tensor is replicated, the tp/n_kv ranks of a KV group for a replicated K/V head (A30).  Round-robin over them
+     * by the new TP rank: r = ranks[r' mod count]  (for a replicated tensor this is r' mod tp_old, A6) */
+    int cnt = 0, last = -1;
+    for (int i = 0; i < nh; i++) if (h[i].s == s_des && h[i].r != last) { last = h[i].r; cnt++; }
+    int want = rn % cnt, seen = 0; last = -1;
+    for (int i = 0; i < nh; i++) if (h[i].s == s_des && h[i].r != last) {
+      last = h[i].r;
+      if (seen == want) r_des = h[i].r;
+      seen++;
+    }
+  }
   if (orc_dp_sharded(Lo, kind)) {
     for (int i = 0; i < nh; i++) if (h[i].s == s_des && h[i].r == r_des) d_first = h[i].d;
     d_des = d_first;

@@ -19,7 +19,7 @@ _lib = None
 
 class Model(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("style", "n_layers", "hidden", "n_q_heads", "n_kv_heads", "head_dim",
-                                          "ffn_hidden", "vocab", "max_pos", "tied", "param_bytes", "kinds")]
+                                          "ffn_hidden", "vocab", "max_pos", "tied", "param_bytes", "kinds", "qkv_order")]
 
 
 class Cfg(C.Structure):
@@ -82,7 +82,7 @@ class OracleError(RuntimeError):
 
 
 def _model(m: dict) -> Model:
-    return Model(**{k: int(m[k]) for k, _ in Model._fields_})
+    return Model(**{k: int(m.get(k, 0)) for k, _ in Model._fields_})
 
 
 def _ptr(a):

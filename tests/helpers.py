@@ -76,3 +76,23 @@ def replication_factor(layout: O.Layout, kind: int, split: int, t: int) -> int:
     if m["tied"] and c["pp"] > 1 and t == 0:
         f *= 2
     return f
+
+
+def replication_map(layout: O.Layout, kind: int, lt_info, t: int) -> np.ndarray:
+    """R(t) of pin P3 per ELEMENT: how many buffers of `kind` hold each element of logical tensor t, written from the
+    definitions (readings A6, A10, A11, A14, A29, A30), not from the oracle: replicated tensors are on every TP
+    rank, a kind that is not DP-sharded is on every DP rank, the tied embedding is on two stages, and under KV-head
+    replication (tp > n_kv) the rows of a K or V head are on tp/n_kv TP ranks."""
+    rows, cols, split = lt_info[t][0], lt_info[t][1], lt_info[t][2]
+    c, m = layout.cfg, layout.model
+    R = np.full((rows, cols), replication_factor(layout, kind, split, t), np.int64)
+    if split == 4 and c["tp"] > m["n_kv_heads"]:                 # fused QKV (weight or bias) with replicated KV heads
+        rep = c["tp"] // m["n_kv_heads"]
+        d, q, k = m["head_dim"], m["n_q_heads"], m["n_kv_heads"]
+        r = np.arange(rows)
+        if m.get("qkv_order", 0) == 0:
+            is_kv = (r % ((q // k + 2) * d)) >= (q // k) * d     # inside a group: q heads first, then K, then V
+        else:
+            is_kv = r >= q * d                                   # [Q; K; V]
+        R[is_kv, :] *= rep
+    return R

@@ -7,7 +7,7 @@ import pytest
 
 from etc_inputs import workload, tiny_models, tiny_parallel_cfgs, position_stamp, STYLE_GPT
 from oracle import oracle as O
-from helpers import read_golden, make_logical, shard_all, stamp_all, reassemble, replication_factor
+from helpers import read_golden, make_logical, shard_all, stamp_all, reassemble, replication_factor, replication_map
 
 TINY = dict(tiny_models())
 
@@ -219,23 +219,19 @@ def _check_reconfiguration(model, old_cfg, new_cfg, seed, device_map=None, paylo
     P = O.P_of(old, new)
     ov, need, hold = O.overlap(old, new)
     lts = O.logical_tensors(model)
-    # --- P3 sum identities with replication factors
+    # --- P3 sum identities with replication factors (per element: KV-head replication makes them vary inside a tensor)
+    def weighted(layout_mine, dev, layout_other):
+        tot = 0
+        for k in layout_mine.kinds():
+            lt, _, row, col = layout_mine.global_of(dev, k)
+            for t in np.unique(lt):
+                sel = lt == t
+                tot += int(replication_map(layout_other, k, lts, int(t))[row[sel], col[sel]].sum()) * O.kind_bytes(model, k)
+        return tot
     for n in range(new.n_dev):
-        exp = 0
-        for k in new.kinds():
-            lt, _, _, _ = new.global_of(n, k)
-            cnt = np.bincount(lt, minlength=len(lts))
-            exp += sum(int(cnt[t]) * O.kind_bytes(model, k) * replication_factor(old, k, lts[t][2], t)
-                       for t in range(len(lts)))
-        assert ov[n].sum() == exp, ("row sum", n)
+        assert ov[n].sum() == weighted(new, n, old), ("row sum", n)
     for o in range(old.n_dev):
-        exp = 0
-        for k in old.kinds():
-            lt, _, _, _ = old.global_of(o, k)
-            cnt = np.bincount(lt, minlength=len(lts)) if lt.shape[0] else np.zeros(len(lts), int)
-            exp += sum(int(cnt[t]) * O.kind_bytes(model, k) * replication_factor(new, k, lts[t][2], t)
-                       for t in range(len(lts)))
-        assert ov[:, o].sum() == exp, ("col sum", o)
+        assert ov[:, o].sum() == weighted(old, o, new), ("col sum", o)
     assert (ov <= need[:, None]).all() and (ov <= hold[None, :]).all()
     # --- P5 sketch
     if device_map is None:
@@ -257,7 +253,7 @@ def _check_reconfiguration(model, old_cfg, new_cfg, seed, device_map=None, paylo
     for k in logical:
         for t in range(len(lts)):
             assert np.array_equal(rebuilt[k][t], logical[k][t]), ("P4", k, t)
-            assert (cover[k][t] == replication_factor(new, k, lts[t][2], t)).all(), ("P4 cover", k, t)
+            assert np.array_equal(cover[k][t], replication_map(new, k, lts, t)), ("P4 cover", k, t)
     # --- P3 on T
     for n in range(new.n_dev):
         assert T[:, device_map[n]].sum() == need[n]
