@@ -44,17 +44,20 @@ typedef int32_t etc_status;
 enum {
   ETC_OK = 0,
   ETC_ERR_INVALID_ARG = -1,  /* null pointer, non-positive size, unknown enum, misaligned buffer */
-  ETC_ERR_INDIVISIBLE = -2,  /* n_layers % pp, n_kv_heads % tp, ffn_hidden % tp or vocab % tp != 0 */
+  ETC_ERR_INDIVISIBLE = -2,  /* n_layers % pp, n_kv_heads % tp (tp <= n_kv_heads), ffn_hidden % tp or vocab % tp != 0
+                                 */
   ETC_ERR_MISMATCH = -3,     /* old and new layouts describe different models / kinds */
   ETC_ERR_BAD_MAP = -4,      /* device_map not injective or out of [0,P) */
   ETC_ERR_WORKSPACE = -5,    /* problem larger than the kernel's on-chip workspace (sketch: P > ETC_SKETCH_MAX_P) */
-  ETC_ERR_UNSUPPORTED = -6,  /* tp > n_kv_heads (KV-head replication, reading A10) */
+  ETC_ERR_UNSUPPORTED = -6,  /* tp > n_kv_heads where KV-head replication (reading A30) cannot be formed: tp is not a
+                                multiple of n_kv_heads, or tp/n_kv_heads does not divide the q heads of a KV group */
   ETC_ERR_CUDA = -7,         /* a CUDA call failed, or no CUDA device */
   ETC_ERR_UNRECOVERABLE = -8 /* some needed bytes have no surviving source (every replica failed, reading A26) */
 };
 
 enum { ETC_GPT = 0, ETC_LLAMA = 1 };                 /* etc_model_desc.style */
 enum { ETC_BF16 = 2, ETC_FP32 = 4 };                 /* etc_model_desc.param_dtype = element size in bytes */
+enum { ETC_QKV_GROUPED = 0, ETC_QKV_BLOCKED = 1 };   /* etc_model_desc.qkv_order */
 enum { ETC_K_PARAM = 1, ETC_K_MASTER = 2, ETC_K_ADAM_M = 4, ETC_K_ADAM_V = 8 };   /* kinds bitmask; kind index 0..3 */
 #define ETC_NUM_KINDS 4
 #define ETC_SKETCH_MAX_P 2048
@@ -67,6 +70,12 @@ typedef struct {
   int32_t tied_embeddings;   /* 1: the output layer shares word_embeddings (replica on the last PP stage if pp > 1) */
   int32_t param_dtype;       /* ETC_BF16 | ETC_FP32: element size of kind PARAM; MASTER / ADAM_M / ADAM_V are fp32 */
   int32_t kinds;             /* bitmask of state kinds present */
+  int32_t qkv_order;         /* logical row order of the fused QKV weight / bias (f3, readings A10, A29):
+                                ETC_QKV_GROUPED: per KV group its q heads, then K, then V (Megatron's fused layout);
+                                ETC_QKV_BLOCKED: [Q; K; V], all q heads, then all k heads, then all v heads — a TP shard
+                                is then [Q_r; K_r; V_r], three row blocks stored one after the other.
+                                With tp > n_kv_heads (KV-head replication, reading A30) the tp/n_kv_heads ranks of a KV
+                                group each hold their share of the group's q heads and the WHOLE K and V head */
 } etc_model_desc;
 
 /* Megatron-style parallel configuration.  dist_opt = 1: MASTER/ADAM_M/ADAM_V are sharded over DP as

@@ -35,7 +35,8 @@ class EtcError(RuntimeError):
 
 class _ModelDesc(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("style", "n_layers", "hidden", "n_q_heads", "n_kv_heads", "head_dim",
-                                          "ffn_hidden", "vocab", "max_pos", "tied_embeddings", "param_dtype", "kinds")]
+                                          "ffn_hidden", "vocab", "max_pos", "tied_embeddings", "param_dtype", "kinds",
+                                          "qkv_order")]
 
 
 class _ParallelCfg(C.Structure):
@@ -161,7 +162,8 @@ def etc_layout_create(model: dict, cfg: dict) -> Layout:
     m = _ModelDesc(style=model["style"], n_layers=model["n_layers"], hidden=model["hidden"],
                    n_q_heads=model["n_q_heads"], n_kv_heads=model["n_kv_heads"], head_dim=model["head_dim"],
                    ffn_hidden=model["ffn_hidden"], vocab=model["vocab"], max_pos=model["max_pos"],
-                   tied_embeddings=model["tied"], param_dtype=model["param_bytes"], kinds=model["kinds"])
+                   tied_embeddings=model["tied"], param_dtype=model["param_bytes"], kinds=model["kinds"],
+                   qkv_order=model.get("qkv_order", 0))
     c = _ParallelCfg(tp=cfg["tp"], pp=cfg["pp"], dp=cfg["dp"], dist_opt=cfg.get("dist_opt", 0),
                      pp_first=cfg.get("pp_first", 0), pp_last=cfg.get("pp_last", 0),
                      dist_opt_align=cfg.get("dist_opt_align", 0))

@@ -100,7 +100,7 @@ static bool same_model(const etc_layout* a, const etc_layout* b) {
   return x.style == y.style && x.n_layers == y.n_layers && x.hidden == y.hidden && x.n_q_heads == y.n_q_heads &&
          x.n_kv_heads == y.n_kv_heads && x.head_dim == y.head_dim && x.ffn_hidden == y.ffn_hidden &&
          x.vocab == y.vocab && x.max_pos == y.max_pos && x.tied_embeddings == y.tied_embeddings &&
-         x.param_dtype == y.param_dtype && x.kinds == y.kinds;
+         x.param_dtype == y.param_dtype && x.kinds == y.kinds && x.qkv_order == y.qkv_order;
 }
 bool etc_same_model(const etc_layout* a, const etc_layout* b) { return same_model(a, b); }
 

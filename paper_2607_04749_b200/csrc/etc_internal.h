@@ -9,13 +9,12 @@
 namespace etc {
 
 // Split type of a logical tensor (PAPER.md:199 replaced by an explicit type, reading A8).
-enum Split : int32_t { REPL = 0, COL = 1, ROW = 2, COL2 = 3 };
+enum Split : int32_t { REPL = 0, COL = 1, ROW = 2, COL2 = 3, QKV = 4 };
 
 // Piece flags
 enum : uint16_t {
   PF_POST_COPY = 1,   // tied word_embeddings replica held by the last PP stage (reading A11)
   PF_SOLE_INST = 2,   // the tensor is held by exactly one PP stage in this layout
-  PF_TP_SHARDED = 4,  // split != REPL: exactly one TP rank holds each element
   PF_DP_SHARDED = 8,  // kind is sharded over DP (distributed optimizer, reading A14)
 };
 
@@ -31,6 +30,8 @@ struct Piece {
   int32_t W;          // row pitch in elements inside the buffer
   int16_t s, r, d;    // PP stage, TP rank, DP rank of dev
   uint16_t flags;
+  int16_t rep, rbase; // the TP ranks [rbase, rbase + rep) of stage s hold these elements: rep = 1 TP-sharded, rep = tp
+                      // replicated tensor, rep = tp / n_kv K or V head under KV-head replication (reading A30)
   int64_t boff;       // byte offset of element (r0,c0) inside the buffer of (dev, kind)
   int64_t f0, f1;
 };

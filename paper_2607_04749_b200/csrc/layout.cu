@@ -25,8 +25,8 @@ int current_device() { return g_device; }
 
 struct LTensor { int64_t rows, cols; int32_t split, where, layer; };   // where: 0 pre, 1 layer, 2 post
 
-// Logical tensor list in id order.  QKV rows are in KV-group order, so an equal row split
-// is the GQA-aware split as long as n_kv_heads % tp == 0 (reading A10); SwiGLU fc1 = [gate; up] is COL2.
+// Logical tensor list in id order.  The fused QKV weight / bias has its own split type
+// (readings A10, A29, A30: row order and KV-head replication, see qkv_blocks); SwiGLU fc1 = [gate; up] is COL2.
 static std::vector<LTensor> logical_tensors(const etc_model_desc& m) {
   std::vector<LTensor> v;
   const int64_t h = m.hidden, d = m.head_dim, f = m.ffn_hidden;
@@ -36,14 +36,14 @@ static std::vector<LTensor> logical_tensors(const etc_model_desc& m) {
   for (int l = 0; l < m.n_layers; ++l) {
     if (m.style == ETC_GPT) {
       v.push_back({1, h, REPL, 1, l}); v.push_back({1, h, REPL, 1, l});          // ln1 w,b
-      v.push_back({qkv, h, COL, 1, l}); v.push_back({qkv, 1, COL, 1, l});        // qkv w,b
+      v.push_back({qkv, h, QKV, 1, l}); v.push_back({qkv, 1, QKV, 1, l});        // qkv w,b
       v.push_back({h, qd, ROW, 1, l}); v.push_back({1, h, REPL, 1, l});          // proj w,b
       v.push_back({1, h, REPL, 1, l}); v.push_back({1, h, REPL, 1, l});          // ln2 w,b
       v.push_back({f, h, COL, 1, l}); v.push_back({f, 1, COL, 1, l});            // fc1 w,b
       v.push_back({h, f, ROW, 1, l}); v.push_back({1, h, REPL, 1, l});           // fc2 w,b
     } else {
       v.push_back({1, h, REPL, 1, l});                                           // ln1 w
-      v.push_back({qkv, h, COL, 1, l});                                          // qkv w
+      v.push_back({qkv, h, QKV, 1, l});                                          // qkv w
       v.push_back({h, qd, ROW, 1, l});                                           // proj w
       v.push_back({1, h, REPL, 1, l});                                           // ln2 w
       v.push_back({2 * f, h, COL2, 1, l});                                       // fc1 w = [gate; up]
@@ -81,9 +81,13 @@ static etc_status validate(const etc_model_desc* m, const etc_parallel_cfg* c) {
   if (m->tied_embeddings != 0 && m->tied_embeddings != 1) return ETC_ERR_INVALID_ARG;
   if (m->n_q_heads % m->n_kv_heads) return ETC_ERR_INVALID_ARG;
   if (int64_t(c->tp) * c->pp * c->dp > 32767) return ETC_ERR_INVALID_ARG;
-  if (c->tp > m->n_kv_heads) return ETC_ERR_UNSUPPORTED;
+  if (m->qkv_order != ETC_QKV_GROUPED && m->qkv_order != ETC_QKV_BLOCKED) return ETC_ERR_INVALID_ARG;
+  if (c->tp > m->n_kv_heads) {                               // KV-head replication (reading A30)
+    const int rep = c->tp / m->n_kv_heads;
+    if (c->tp % m->n_kv_heads || (m->n_q_heads / m->n_kv_heads) % rep) return ETC_ERR_UNSUPPORTED;
+  }
   { const int sb = stage_begin(m->n_layers, *c, 0); if (sb < 0) return sb == -2 ? ETC_ERR_INVALID_ARG : ETC_ERR_INDIVISIBLE; }
-  if (m->n_kv_heads % c->tp || m->ffn_hidden % c->tp || m->vocab % c->tp) return ETC_ERR_INDIVISIBLE;
+  if ((c->tp <= m->n_kv_heads && m->n_kv_heads % c->tp) || m->ffn_hidden % c->tp || m->vocab % c->tp) return ETC_ERR_INDIVISIBLE;
   return ETC_OK;
 }
 
@@ -123,7 +127,39 @@ static cudaError_t upload_prepare(size_t bytes) {
   }
   return cudaSuccess;
 }
-struct Sh { int64_t start, n, rb[2], nrb, c0, W; int nblk; int32_t lt; uint16_t flags; };
+// TP shard of one tensor instance: up to 3 row blocks (first logical row rb, rows nr, first local row ls) stored one
+// after the other, times a column range.  rep / rbase per block: the TP ranks [rbase, rbase + rep) hold its elements.
+struct Sh { int64_t start, n, rb[3], nr[3], ls[3], c0, W; int nblk; int16_t rep[3], rbase[3]; int32_t lt; uint16_t flags; };
+
+// Row blocks of the fused QKV tensor on TP rank r (q = n_q heads, k = n_kv heads, d rows per head, qpg = q/k):
+//   tp <= k: the rank holds kpr = k/tp whole KV groups.  GROUPED order: they are one contiguous row range (reading
+//            A10).  BLOCKED order ([Q;K;V], reading A29): [Q_r; K_r; V_r], three blocks.
+//   tp >  k: rep = tp/k ranks share KV group g = r/rep (reading A30); rank r holds the (r % rep)-th share of the group's
+//            q heads and the whole K and V head of the group, which are therefore held by rep ranks.
+static void qkv_blocks(const etc_model_desc& m, int tp, int r, Sh& s) {
+  const int64_t q = m.n_q_heads, k = m.n_kv_heads, d = m.head_dim, qpg = q / k;
+  if (tp <= k) {
+    const int64_t kpr = k / tp;
+    if (m.qkv_order == ETC_QKV_GROUPED) { s.nr[0] = kpr * (qpg + 2) * d; s.rb[0] = r * s.nr[0]; return; }
+    s.nblk = 3;
+    s.nr[0] = q / tp * d; s.rb[0] = r * s.nr[0];
+    s.nr[1] = s.nr[2] = kpr * d; s.rb[1] = q * d + r * kpr * d; s.rb[2] = (q + k) * d + r * kpr * d;
+    return;
+  }
+  const int64_t rep = tp / k, g = r / rep, share = r % rep, qpr = qpg / rep;
+  if (m.qkv_order == ETC_QKV_GROUPED) {
+    const int64_t g0 = g * (qpg + 2) * d;
+    s.nblk = 2;
+    s.nr[0] = qpr * d; s.rb[0] = g0 + share * qpr * d;
+    s.nr[1] = 2 * d;   s.rb[1] = g0 + qpg * d;
+    s.rep[1] = (int16_t)rep; s.rbase[1] = (int16_t)(g * rep);
+  } else {
+    s.nblk = 3;
+    s.nr[0] = qpr * d; s.rb[0] = r * qpr * d;
+    s.nr[1] = s.nr[2] = d; s.rb[1] = q * d + g * d; s.rb[2] = (q + k) * d + g * d;
+    s.rep[1] = s.rep[2] = (int16_t)rep; s.rbase[1] = s.rbase[2] = (int16_t)(g * rep);
+  }
+}
 }  // namespace etc
 
 extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_parallel_cfg* cfg, etc_layout** out) {
@@ -148,7 +184,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   const size_t o_start = 0, o_first = al((size_t)(n_dev + 1) * 4), o_mask = o_first + al((size_t)n_dev * nG * 4),
                o_kstart = o_mask + al((size_t)n_dev * mask_words * 4),
                o_pieces = o_kstart + al((size_t)n_dev * (ETC_NUM_KINDS + 1) * 4);
-  const size_t max_total = o_pieces + (size_t)n_dev * n_kinds * max_inst * 4 * sizeof(Piece);
+  const size_t max_total = o_pieces + (size_t)n_dev * n_kinds * max_inst * 5 * sizeof(Piece);   // <= 5 rectangles / instance
 
   std::lock_guard<std::mutex> lock(g_up_mu);
   cudaError_t e = cudaSetDevice(current_device());
@@ -189,16 +225,21 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
         const LTensor& T = lts[inst[i].first];
         // start offsets follow LOCAL order; the slot order is GROUP order (the replica, tensor 0, goes first)
         Sh& q = sh[inst[i].second ? 0 : i + (has_replica ? 1 : 0)];
-        q.nblk = 1; q.rb[0] = q.rb[1] = 0; q.nrb = T.rows; q.c0 = 0; q.W = T.cols; q.lt = inst[i].first;
+        q.nblk = 1; q.c0 = 0; q.W = T.cols; q.lt = inst[i].first;
+        for (int b = 0; b < 3; ++b) { q.rb[b] = q.nr[b] = 0; q.rep[b] = 1; q.rbase[b] = (int16_t)r; }
+        q.nr[0] = T.rows;
         switch (T.split) {
-          case COL: q.nrb = T.rows / tp; q.rb[0] = r * q.nrb; break;
+          case REPL: q.rep[0] = (int16_t)tp; q.rbase[0] = 0; break;
+          case COL: q.nr[0] = T.rows / tp; q.rb[0] = r * q.nr[0]; break;
           case ROW: q.W = T.cols / tp; q.c0 = r * q.W; break;
-          case COL2: { const int64_t F = T.rows / 2; q.nblk = 2; q.nrb = F / tp; q.rb[0] = r * q.nrb; q.rb[1] = F + r * q.nrb; break; }
+          case COL2: { const int64_t F = T.rows / 2; q.nblk = 2; q.nr[0] = q.nr[1] = F / tp; q.rb[0] = r * q.nr[0]; q.rb[1] = F + r * q.nr[0]; break; }
+          case QKV: qkv_blocks(m, tp, r, q); break;
           default: break;
         }
-        q.n = (int64_t)q.nblk * q.nrb * q.W; q.start = pos; pos += q.n;
-        q.flags = (inst[i].second ? PF_POST_COPY : 0) | ((two_inst && inst[i].first == 0) ? 0 : PF_SOLE_INST) |
-                  (T.split != REPL ? PF_TP_SHARDED : 0);
+        int64_t rows = 0;
+        for (int b = 0; b < q.nblk; ++b) { q.ls[b] = rows; rows += q.nr[b]; }
+        q.n = rows * q.W; q.start = pos; pos += q.n;
+        q.flags = (inst[i].second ? PF_POST_COPY : 0) | ((two_inst && inst[i].first == 0) ? 0 : PF_SOLE_INST);
       }
     }
     for (int d = 0; d < dp; ++d)
@@ -227,32 +268,37 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
             const int32_t grp = kind * nT + q.lt;
             first[(size_t)dev * nG + grp] = (int32_t)np;
             // decompose the held flat range [a,b) of the shard into rectangles of local rows x local cols
-            int64_t rect[4][4]; int nr = 0;
+            // (head partial row, whole rows cut at the block boundaries, tail partial row: <= 5)
+            int64_t rect[5][4]; int nr = 0;
             auto add = [&](int64_t i0, int64_t i1, int64_t j0, int64_t j1) { rect[nr][0] = i0; rect[nr][1] = i1; rect[nr][2] = j0; rect[nr][3] = j1; ++nr; };
-            if (a == 0 && b == q.n) {                        // whole shard (the common case)
-              if (q.nblk == 2) { add(0, q.nrb, 0, q.W); add(q.nrb, 2 * q.nrb, 0, q.W); } else add(0, q.nrb, 0, q.W);
-            } else {
+            auto add_rows = [&](int64_t i0, int64_t i1) {    // whole local rows [i0,i1), one rectangle per row block
+              for (int blk = 0; blk < q.nblk; ++blk) {
+                const int64_t x0 = std::max(i0, q.ls[blk]), x1 = std::min(i1, q.ls[blk] + q.nr[blk]);
+                if (x1 > x0) add(x0, x1, 0, q.W);
+              }
+            };
+            if (a == 0 && b == q.n) add_rows(0, q.n / q.W);  // whole shard (the common case)
+            else {
               const int64_t ia = a / q.W, ja = a % q.W, ib = b / q.W, jb = b % q.W;
               if (ia == ib) add(ia, ia + 1, ja, jb);
               else {
                 int64_t body0 = ia;
                 if (ja > 0) { add(ia, ia + 1, ja, q.W); body0 = ia + 1; }
-                if (ib > body0) {
-                  if (q.nblk == 2 && body0 < q.nrb && ib > q.nrb) { add(body0, q.nrb, 0, q.W); add(q.nrb, ib, 0, q.W); }
-                  else add(body0, ib, 0, q.W);
-                }
+                if (ib > body0) add_rows(body0, ib);
                 if (jb > 0) add(ib, ib + 1, 0, jb);
               }
             }
             for (int k = 0; k < nr; ++k) {
               const int64_t i0 = rect[k][0], i1 = rect[k][1], j0 = rect[k][2], j1 = rect[k][3];
-              const int blk = (int)(i0 / q.nrb);
+              int blk = 0;
+              while (blk + 1 < q.nblk && i0 >= q.ls[blk] + q.nr[blk]) ++blk;
               Piece& p = pieces[np++];
               p.dev = dev; p.grp = grp;
-              p.r0 = (int32_t)(q.rb[blk] + i0 % q.nrb); p.nr = (int32_t)(i1 - i0);
+              p.r0 = (int32_t)(q.rb[blk] + (i0 - q.ls[blk])); p.nr = (int32_t)(i1 - i0);
               p.c0 = (int32_t)(q.c0 + j0); p.nc = (int32_t)(j1 - j0);
               p.lrow0 = (int32_t)i0; p.lcol0 = (int32_t)j0; p.W = (int32_t)q.W;
               p.s = (int16_t)s; p.r = (int16_t)r; p.d = (int16_t)d; p.flags = flags;
+              p.rep = q.rep[blk]; p.rbase = q.rbase[blk];
               p.boff = (q.start + i0 * q.W + j0 - lo) * es;
               p.f0 = a; p.f1 = b;
             }

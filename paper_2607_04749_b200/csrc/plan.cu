@@ -34,7 +34,7 @@ __device__ __forceinline__ bool rect_isect(const Piece& a, const Piece& b, Rect&
 __device__ __forceinline__ bool designated(const Piece& o, const Piece& q, int tp_old, int dp_old,
                                            const uint8_t* __restrict__ failed) {
   const bool stage_ok = (o.flags & PF_SOLE_INST) || ((o.flags & PF_POST_COPY) == (q.flags & PF_POST_COPY));
-  const bool r_ok = (o.flags & PF_TP_SHARDED) || o.r == q.r % tp_old;
+  const bool r_ok = o.r == o.rbase + q.r % o.rep;      // round-robin by r' over the TP ranks holding it (A6, A30)
   if (!(stage_ok && r_ok)) return false;
   if (o.flags & PF_DP_SHARDED) return true;
   int d_des = q.d % dp_old;
@@ -113,7 +113,9 @@ __device__ __forceinline__ void for_each_slice(const DeviceTables& oldT, const P
       const int pj = oldT.first[(size_t)p * oldT.n_grp + q.grp];
       if (pj >= 0) {
         const Piece& h = oldT.pieces[pj];
-        if (!(o.flags & PF_TP_SHARDED) || h.r == o.r)                            // same TP shard: subtract its held range
+        // p holds these elements only if its TP rank is one of those holding them; all such ranks store them at the
+        // same shard-local position (same shard, or the K/V block of one KV group, A30): subtract p's held flat range
+        if (h.r >= o.rbase && h.r < o.rbase + o.rep)
           np = subtract_interval(I, (int64_t)o.lrow0 + (I.r0 - o.r0), (int64_t)o.lcol0 + (I.c0 - o.c0), o.W, h.f0, h.f1, parts);
       }
     }
