@@ -129,3 +129,23 @@ def test_all_replicas_failed_is_unrecoverable(E):
     assert e.value.code == -8
     f[3] = 0
     E.etc_plan_create(old, new, np.array([0, 2], np.int32), failed=f)
+
+
+def test_dp_growth_round_robin_balance_on_device(E):
+    """PAPER.md:171 (DP growth: counterpart sends its whole state, source groups round-robin): the plan's traffic matrix
+    equals the closed form of tests/test_dp_growth_pins.py and the device sketch finds a map that keeps every existing
+    group local; s2's model, TP2 PP2, DP 2 -> 5."""
+    from test_dp_growth_pins import growth_map, closed_form_T
+    from test_gpu_parity import _check_migration
+    w = workload("s2")
+    old_c, new_c = dict(tp=2, pp=2, dp=2, dist_opt=0), dict(tp=2, pp=2, dp=5, dist_opt=0)
+    dm = growth_map(old_c, new_c)
+    g = _check_migration(E, w["model"], old_c, new_c, w["seed"], device_map=dm)
+    T = g["plan"].traffic()
+    assert np.array_equal(T, closed_form_T(old_c, new_c, g["hold"], dm))
+    sent = [(int(T[o].sum() - T[o, o]) // int(g["hold"][o])) for o in range(8)]        # whole states sent per old device
+    per_group = [sum(sent[o] for o in range(8) if (o // 2) % 2 == d) // 4 for d in range(2)]
+    assert sorted(per_group) == [1, 2]                                                   # 3 new groups over 2 old ones
+    ov, _, _ = E.etc_cost_matrix(g["old"], g["new"])
+    _, lb = E.etc_sketch(ov)
+    assert int(lb.item()) == int(g["hold"][:8].sum())
