@@ -48,7 +48,10 @@ typedef struct {
 /* pp_first / pp_last: layers on the first / last pipeline stage (0 = not set), reading A27 (uneven pipeline split) */
 /* dist_opt_align (reading A28, f3): the DP shard size of the distributed optimizer is rounded up to a multiple of this
  * many elements (0 or 1 = no rounding), as Megatron-LM pads its buffers so that every DP shard is aligned */
-typedef struct { int32_t tp, pp, dp, dist_opt, pp_first, pp_last, dist_opt_align; } orc_cfg;
+/* vocab_divisor (reading A31, f3): > 0 pads the vocabulary dimension of word_embeddings / lm_head to a multiple of
+ * vocab_divisor * tp rows (Megatron-LM's --make-vocab-size-divisible-by); the padding rows are stored like any other
+ * row.  0 = no padding: vocab % tp == 0 is required (reading A12) */
+typedef struct { int32_t tp, pp, dp, dist_opt, pp_first, pp_last, dist_opt_align, vocab_divisor; } orc_cfg;
 
 typedef struct { int64_t rows, cols; int32_t split, where, layer; } orc_lt;   /* one logical tensor */
 
@@ -73,14 +76,23 @@ typedef struct {
 } orc_layout;
 
 /* ---------------------------------------------------------------- logical model */
-static int orc_logical(const orc_model* m, orc_lt* out) {
+/* rows of the embedding tensors in a layout: the padded vocabulary (reading A31) */
+static int64_t orc_vocab_rows(const orc_model* m, const orc_cfg* c) {
+  if (!c || c->vocab_divisor <= 0) return m->vocab;
+  int64_t unit = (int64_t)c->vocab_divisor * c->tp;
+  return ((int64_t)m->vocab + unit - 1) / unit * unit;
+}
+
+/* c == NULL: the unpadded logical model */
+static int orc_logical(const orc_model* m, const orc_cfg* c, orc_lt* out) {
   int n = 0;
+  const int64_t V = orc_vocab_rows(m, c);
   const int64_t h = m->hidden, d = m->head_dim;
   const int64_t qkv = ((int64_t)m->n_q_heads + 2 * (int64_t)m->n_kv_heads) * d;
   const int64_t qd = (int64_t)m->n_q_heads * d, f = m->ffn_hidden;
 #define ADD(R, C, S, WH, LY) do { if (out) { out[n].rows = (R); out[n].cols = (C); out[n].split = (S); \
                                   out[n].where = (WH); out[n].layer = (LY); } n++; } while (0)
-  ADD(m->vocab, h, ORC_COL, ORC_PRE, -1);                        /* word_embeddings */
+  ADD(V, h, ORC_COL, ORC_PRE, -1);                               /* word_embeddings */
   if (m->style == 0 && m->max_pos > 0) ADD(m->max_pos, h, ORC_REPL, ORC_PRE, -1);   /* position_embeddings */
   for (int l = 0; l < m->n_layers; l++) {
     if (m->style == 0) {
@@ -107,19 +119,26 @@ static int orc_logical(const orc_model* m, orc_lt* out) {
   }
   ADD(1, h, ORC_REPL, ORC_POST, -1);                             /* final_ln.weight */
   if (m->style == 0) ADD(1, h, ORC_REPL, ORC_POST, -1);          /* final_ln.bias */
-  if (!m->tied) ADD(m->vocab, h, ORC_COL, ORC_POST, -1);         /* lm_head */
+  if (!m->tied) ADD(V, h, ORC_COL, ORC_POST, -1);                /* lm_head */
 #undef ADD
   return n;
 }
 
-int32_t orc_num_logical(const orc_model* m) { return orc_logical(m, NULL); }
+int32_t orc_num_logical(const orc_model* m) { return orc_logical(m, NULL, NULL); }
 
 /* rows[i], cols[i], split[i], where[i], layer[i] for every logical tensor */
+int32_t orc_logical_info_cfg(const orc_model* m, const orc_cfg* c, int64_t* rows, int64_t* cols, int32_t* split,
+                             int32_t* where, int32_t* layer);
 int32_t orc_logical_info(const orc_model* m, int64_t* rows, int64_t* cols, int32_t* split, int32_t* where,
                          int32_t* layer) {
-  int n = orc_logical(m, NULL);
+  return orc_logical_info_cfg(m, NULL, rows, cols, split, where, layer);
+}
+/* the same with the embedding rows of a given parallel configuration (padded vocabulary, reading A31) */
+int32_t orc_logical_info_cfg(const orc_model* m, const orc_cfg* c, int64_t* rows, int64_t* cols, int32_t* split,
+                             int32_t* where, int32_t* layer) {
+  int n = orc_logical(m, c, NULL);
   orc_lt* t = (orc_lt*)malloc(sizeof(orc_lt) * (size_t)n);
-  orc_logical(m, t);
+  orc_logical(m, c, t);
   for (int i = 0; i < n; i++) {
     rows[i] = t[i].rows; cols[i] = t[i].cols; split[i] = t[i].split; where[i] = t[i].where; layer[i] = t[i].layer;
   }
@@ -152,7 +171,7 @@ static int orc_stage_begin(int n_layers, const orc_cfg* c, int s) {
 /* divisibility rules (layers divisible by PP, hidden by TP; A7, A10, A12) */
 static int orc_validate(const orc_model* m, const orc_cfg* c) {
   if (!m || !c) return ORC_ERR_ARG;
-  if (c->tp < 1 || c->pp < 1 || c->dp < 1 || c->dist_opt_align < 0) return ORC_ERR_ARG;
+  if (c->tp < 1 || c->pp < 1 || c->dp < 1 || c->dist_opt_align < 0 || c->vocab_divisor < 0) return ORC_ERR_ARG;
   if (m->n_layers < 1 || m->hidden < 1 || m->n_q_heads < 1 || m->n_kv_heads < 1 || m->head_dim < 1 ||
       m->ffn_hidden < 1 || m->vocab < 1 || m->max_pos < 0) return ORC_ERR_ARG;
   if (m->param_bytes != 2 && m->param_bytes != 4) return ORC_ERR_ARG;
@@ -166,7 +185,7 @@ static int orc_validate(const orc_model* m, const orc_cfg* c) {
   if (orc_stage_begin(m->n_layers, c, 0) < 0) return orc_stage_begin(m->n_layers, c, 0) == -2 ? ORC_ERR_ARG : ORC_ERR_INDIVISIBLE;
   if (c->tp <= m->n_kv_heads && m->n_kv_heads % c->tp) return ORC_ERR_INDIVISIBLE;
   if (m->ffn_hidden % c->tp) return ORC_ERR_INDIVISIBLE;
-  if (m->vocab % c->tp) return ORC_ERR_INDIVISIBLE;
+  if (c->vocab_divisor == 0 && m->vocab % c->tp) return ORC_ERR_INDIVISIBLE;   /* A12; with padding (A31) it always divides */
   return ORC_OK;
 }
 
@@ -261,9 +280,9 @@ int32_t orc_layout_new(const orc_model* m, const orc_cfg* c, orc_layout** out) {
   if (!out) return ORC_ERR_ARG;
   orc_layout* L = (orc_layout*)calloc(1, sizeof(orc_layout));
   L->m = *m; L->c = *c;
-  L->n_lt = orc_logical(m, NULL);
+  L->n_lt = orc_logical(m, c, NULL);
   L->lt = (orc_lt*)malloc(sizeof(orc_lt) * (size_t)L->n_lt);
-  orc_logical(m, L->lt);
+  orc_logical(m, c, L->lt);
   int nsr = c->pp * c->tp;
   L->n_sh = (int32_t*)calloc((size_t)nsr, sizeof(int32_t));
   L->sh = (orc_shard**)calloc((size_t)nsr, sizeof(orc_shard*));
@@ -593,7 +612,13 @@ int32_t orc_sketch_hungarian(const int64_t* overlap, int32_t n_new, int32_t P, c
 static int orc_pick_source(const orc_layout* Lo, const orc_layout* Ln, int n, int p, int kind,
                            int lt, int post_copy, int64_t row, int64_t col, orc_holder* h, orc_holder* src) {
   int nh = orc_holders(Lo, kind, lt, row, col, h);
-  if (nh == 0) return -1;
+  if (nh == 0) {
+    /* reading A31: a padding row of the new layout's padded vocabulary that lies beyond the old layout's padded
+     * vocabulary is held by no old device: it has no source and is zero-filled.  Anything else without a holder is
+     * an error. */
+    if (Lo->lt[lt].rows != Ln->lt[lt].rows && row >= Lo->lt[lt].rows && row < Ln->lt[lt].rows) return 2;
+    return -1;
+  }
   for (int i = 0; i < nh; i++) if (h[i].dev == p && !orc_is_failed(Lo, p)) { *src = h[i]; return 0; }   /* (i) */
   int dn, sn, rn; orc_coords(Ln, n, &dn, &sn, &rn);
   int smin = h[0].s, smax = h[0].s;
@@ -641,6 +666,7 @@ int32_t orc_source_of(const orc_layout* Lo, const orc_layout* Ln, const int32_t*
     if (orc_global_of(Ln, n, kind, l_list[i], &lt, &pc, &row, &col)) { rc = ORC_ERR_ARG; break; }
     int how = orc_pick_source(Lo, Ln, n, device_map[n], kind, lt, pc, row, col, h, &s);
     if (how < 0) { rc = how == -2 ? ORC_ERR_UNRECOVERABLE : ORC_ERR_ARG; break; }
+    if (how == 2) { src_dev[i] = -1; src_l[i] = -1; continue; }      /* zero-filled: no source (A31) */
     src_dev[i] = s.dev; src_l[i] = s.l;
   }
   free(h);
@@ -659,10 +685,19 @@ static int orc_check_map(const int32_t* map, int nn, int P) {
  * src_bufs: array [n_old*4] of host pointers; dst: the new buffer (n, kind) (NULL = count traffic only).
  * T (optional, [P][P] row-major, ADDED to): T[o][p] += elem bytes.  overrides (optional, ADDED to): number of
  * elements whose local-first source differs from the designated holder.  written (optional): per-element write
- * count of the destination buffer, incremented (pin P10). */
+ * count of the destination buffer, incremented (pin P10).  fill (optional, ADDED to): bytes of this range that have
+ * no source and are zero-filled (padding rows of a grown padded vocabulary, reading A31). */
+int32_t orc_migrate_range_fill(const orc_layout* Lo, const orc_layout* Ln, const int32_t* device_map, int32_t n,
+                               int32_t kind, int64_t l0, int64_t l1, const void* const* src_bufs, void* dst,
+                               int64_t* T, int64_t* overrides, uint8_t* written, int64_t* fill);
 int32_t orc_migrate_range(const orc_layout* Lo, const orc_layout* Ln, const int32_t* device_map, int32_t n,
                           int32_t kind, int64_t l0, int64_t l1, const void* const* src_bufs, void* dst,
                           int64_t* T, int64_t* overrides, uint8_t* written) {
+  return orc_migrate_range_fill(Lo, Ln, device_map, n, kind, l0, l1, src_bufs, dst, T, overrides, written, NULL);
+}
+int32_t orc_migrate_range_fill(const orc_layout* Lo, const orc_layout* Ln, const int32_t* device_map, int32_t n,
+                               int32_t kind, int64_t l0, int64_t l1, const void* const* src_bufs, void* dst,
+                               int64_t* T, int64_t* overrides, uint8_t* written, int64_t* fill) {
   if (!orc_same_model(Lo, Ln)) return ORC_ERR_ARG;
   int no = orc_num_devices(Lo), nn = orc_num_devices(Ln), P = no > nn ? no : nn;
   if (orc_check_map(device_map, nn, P)) return ORC_ERR_ARG;
@@ -674,6 +709,12 @@ int32_t orc_migrate_range(const orc_layout* Lo, const orc_layout* Ln, const int3
     if (orc_global_of(Ln, n, kind, l, &lt, &pc, &row, &col)) { rc = ORC_ERR_ARG; break; }
     int how = orc_pick_source(Lo, Ln, n, p, kind, lt, pc, row, col, h, &s);
     if (how < 0) { rc = how == -2 ? ORC_ERR_UNRECOVERABLE : ORC_ERR_ARG; break; }
+    if (how == 2) {                          /* A31: no source, zero-fill; moves no bytes between devices */
+      if (dst) memset((char*)dst + l * es, 0, (size_t)es);
+      if (written) written[l]++;
+      if (fill) *fill += es;
+      continue;
+    }
     if (dst) memcpy((char*)dst + l * es, (const char*)src_bufs[s.dev * 4 + kind] + s.l * es, (size_t)es);
     if (T) T[(size_t)s.dev * P + p] += es;
     if (written) written[l]++;
@@ -688,11 +729,21 @@ int32_t orc_migrate_range(const orc_layout* Lo, const orc_layout* Ln, const int3
 }
 
 /* Whole migration: every (n, kind), all elements.  dst_bufs [n_new*4] may be NULL (traffic only). */
+int32_t orc_migrate_fill(const orc_layout* Lo, const orc_layout* Ln, const int32_t* device_map,
+                         const void* const* src_bufs, void* const* dst_bufs, int64_t* T, int64_t* overrides,
+                         int64_t* fill);
 int32_t orc_migrate(const orc_layout* Lo, const orc_layout* Ln, const int32_t* device_map,
                     const void* const* src_bufs, void* const* dst_bufs, int64_t* T, int64_t* overrides) {
+  return orc_migrate_fill(Lo, Ln, device_map, src_bufs, dst_bufs, T, overrides, NULL);
+}
+/* fill (optional, [n_new], overwritten): bytes of each new rank that are zero-filled (reading A31) */
+int32_t orc_migrate_fill(const orc_layout* Lo, const orc_layout* Ln, const int32_t* device_map,
+                         const void* const* src_bufs, void* const* dst_bufs, int64_t* T, int64_t* overrides,
+                         int64_t* fill) {
   int no = orc_num_devices(Lo), nn = orc_num_devices(Ln), P = no > nn ? no : nn;
   if (T) memset(T, 0, sizeof(int64_t) * (size_t)P * (size_t)P);
   if (overrides) *overrides = 0;
+  if (fill) memset(fill, 0, sizeof(int64_t) * (size_t)nn);
   if (orc_check_map(device_map, nn, P)) return ORC_ERR_ARG;
   int rc_all = ORC_OK;
 #pragma omp parallel for schedule(dynamic, 1)
@@ -702,8 +753,8 @@ int32_t orc_migrate(const orc_layout* Lo, const orc_layout* Ln, const int32_t* d
     for (int k = 0; k < 4; k++) {
       int64_t cnt = orc_buffer_elems(Ln, n, k);
       if (!cnt) continue;
-      int rc = orc_migrate_range(Lo, Ln, device_map, n, k, 0, cnt, src_bufs, dst_bufs ? dst_bufs[n * 4 + k] : NULL,
-                                 T, overrides ? &ovr : NULL, NULL);
+      int rc = orc_migrate_range_fill(Lo, Ln, device_map, n, k, 0, cnt, src_bufs, dst_bufs ? dst_bufs[n * 4 + k] : NULL,
+                                      T, overrides ? &ovr : NULL, NULL, fill ? &fill[n] : NULL);
       if (rc) {
 #pragma omp critical
         rc_all = rc;

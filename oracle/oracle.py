@@ -23,7 +23,8 @@ class Model(C.Structure):
 
 
 class Cfg(C.Structure):
-    _fields_ = [(n, C.c_int32) for n in ("tp", "pp", "dp", "dist_opt", "pp_first", "pp_last", "dist_opt_align")]
+    _fields_ = [(n, C.c_int32) for n in ("tp", "pp", "dp", "dist_opt", "pp_first", "pp_last", "dist_opt_align",
+                                          "vocab_divisor")]
 
 
 def build(force: bool = False) -> str:
@@ -70,6 +71,10 @@ def lib():
         L.orc_migrate_range.argtypes = [vp, vp, vp, i32, i32, i64, i64, vp, vp, vp, vp, vp]
         L.orc_migrate.restype = i32
         L.orc_migrate.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+        L.orc_migrate_fill.restype = i32
+        L.orc_migrate_fill.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
+        L.orc_logical_info_cfg.restype = i32
+        L.orc_logical_info_cfg.argtypes = [P(Model), P(Cfg), vp, vp, vp, vp, vp]
         L.orc_max_threads.restype = i32
         _lib = L
     return _lib
@@ -93,13 +98,20 @@ def max_threads() -> int:
     return int(lib().orc_max_threads())
 
 
-def logical_tensors(model: dict):
-    """[(rows, cols, split, where, layer)] for every logical tensor, in id order."""
+def _cfg(cfg: dict) -> Cfg:
+    return Cfg(**{k: int(cfg.get(k, 0)) for k, _ in Cfg._fields_})
+
+
+def logical_tensors(model: dict, cfg: dict | None = None):
+    """[(rows, cols, split, where, layer)] for every logical tensor, in id order.  With cfg: the embedding tensors have
+    that parallel configuration's padded vocabulary rows (reading A31); without: the unpadded model."""
     m = _model(model)
     n = lib().orc_num_logical(C.byref(m))
     rows = np.zeros(n, np.int64); cols = np.zeros(n, np.int64)
     split = np.zeros(n, np.int32); where = np.zeros(n, np.int32); layer = np.zeros(n, np.int32)
-    lib().orc_logical_info(C.byref(m), _ptr(rows), _ptr(cols), _ptr(split), _ptr(where), _ptr(layer))
+    c = _cfg(cfg) if cfg is not None else None
+    lib().orc_logical_info_cfg(C.byref(m), C.byref(c) if c is not None else None, _ptr(rows), _ptr(cols), _ptr(split),
+                               _ptr(where), _ptr(layer))
     return [(int(rows[i]), int(cols[i]), int(split[i]), int(where[i]), int(layer[i])) for i in range(n)]
 
 
@@ -114,7 +126,7 @@ class Layout:
     def __init__(self, model: dict, cfg: dict):
         self.model, self.cfg = dict(model), dict(cfg)
         m = _model(model)
-        c = Cfg(**{k: int(cfg.get(k, 0)) for k, _ in Cfg._fields_})
+        c = _cfg(cfg)
         h = C.c_void_p()
         rc = lib().orc_layout_new(C.byref(m), C.byref(c), C.byref(h))
         if rc:
@@ -140,6 +152,10 @@ class Layout:
 
     def kinds(self):
         return [k for k in range(4) if (self.model["kinds"] >> k) & 1]
+
+    def logical_tensors(self):
+        """the logical tensor list as this layout sees it (padded vocabulary rows, reading A31)"""
+        return logical_tensors(self.model, self.cfg)
 
     def elem_bytes(self, kind):
         return kind_bytes(self.model, kind)
@@ -231,9 +247,11 @@ def _ptr_table(bufs, n_dev):
     return tab
 
 
-def migrate(old: Layout, new: Layout, device_map, src_bufs: dict | None, want_overrides=False):
+def migrate(old: Layout, new: Layout, device_map, src_bufs: dict | None, want_overrides=False, fill_out=None):
     """Element-wise migration.  src_bufs: {(old_dev, kind): 1-D uint16/uint32 array} or None (traffic only).
-    Returns (dst_bufs {(n, kind): array} or None, T[P][P], overrides)."""
+    Returns (dst_bufs {(n, kind): array} or None, T[P][P], overrides).  fill_out: optional int64 array [n_new] that
+    receives the bytes of each new rank that have no source and are zero-filled (reading A31).  The destination buffers
+    start out poisoned, so a zero in them was written."""
     P = P_of(old, new)
     dm = np.ascontiguousarray(device_map, np.int32)
     T = np.zeros((P, P), np.int64); ovr = C.c_int64(0)
@@ -244,9 +262,12 @@ def migrate(old: Layout, new: Layout, device_map, src_bufs: dict | None, want_ov
         for n in range(new.n_dev):
             for k in new.kinds():
                 cnt = new.buffer_elems(n, k)
-                dst[(n, k)] = np.zeros(cnt, np.uint16 if new.elem_bytes(k) == 2 else np.uint32)
+                dst[(n, k)] = np.full(cnt, 0xA5A5, np.uint16) if new.elem_bytes(k) == 2 else np.full(cnt, 0xA5A5A5A5, np.uint32)
         dt = _ptr_table(dst, new.n_dev)
-    rc = lib().orc_migrate(old.h, new.h, _ptr(dm), st, dt, _ptr(T), C.byref(ovr) if want_overrides else None)
+    if fill_out is not None:
+        assert fill_out.dtype == np.int64 and fill_out.shape == (new.n_dev,) and fill_out.flags.c_contiguous
+    rc = lib().orc_migrate_fill(old.h, new.h, _ptr(dm), st, dt, _ptr(T), C.byref(ovr) if want_overrides else None,
+                                _ptr(fill_out))
     if rc:
         raise OracleError(rc)
     return dst, T, int(ovr.value)

@@ -18,9 +18,10 @@ def read_golden(name):
     return rows
 
 
-def make_logical(model: dict, seed: int, payload: str = "values"):
-    """{kind: [2-D array per logical tensor]} in logical space (uint16 / uint32 bit patterns)."""
-    lts = O.logical_tensors(model)
+def make_logical(model: dict, seed: int, payload: str = "values", lts=None):
+    """{kind: [2-D array per logical tensor]} in logical space (uint16 / uint32 bit patterns).  lts: the tensor list to
+    use instead of the unpadded model's (a layout's own list when the vocabulary is padded, reading A31)."""
+    lts = O.logical_tensors(model) if lts is None else lts
     out = {}
     for k in range(4):
         if not (model["kinds"] >> k) & 1:
@@ -96,3 +97,19 @@ def replication_map(layout: O.Layout, kind: int, lt_info, t: int) -> np.ndarray:
             is_kv = r >= q * d                                   # [Q; K; V]
         R[is_kv, :] *= rep
     return R
+
+
+def resize_logical(logical: dict, lts_to) -> dict:
+    """Reading A31 stated on logical tensors: going to a layout whose embedding tensors have another padded row count,
+    rows present on both sides are kept, rows beyond the new count are dropped, rows beyond the old count are zero."""
+    out = {}
+    for k, arrs in logical.items():
+        new = []
+        for a, (rows, cols, *_r) in zip(arrs, lts_to):
+            assert a.shape[1] == cols
+            b = np.zeros((rows, cols), a.dtype)
+            m = min(rows, a.shape[0])
+            b[:m] = a[:m]
+            new.append(b)
+        out[k] = new
+    return out
