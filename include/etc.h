@@ -86,8 +86,15 @@ typedef struct {
  * dist_opt_align (f3, reading A28): with dist_opt = 1 the DP shard size is rounded up to a multiple of this many
  * elements, chunk = ceil(Lloc / (dp*align)) * align (Megatron-LM pads its distributed-optimizer buffers so that every
  * DP shard is aligned); 0 or 1 = no rounding (reading A14); negative -> ETC_ERR_INVALID_ARG.  Padding is not stored:
- * a buffer holds only the real elements of its range. */
-typedef struct { int32_t tp, pp, dp, dist_opt, pp_first, pp_last, dist_opt_align; } etc_parallel_cfg;
+ * a buffer holds only the real elements of its range.
+ * vocab_divisor (f3, reading A31): > 0 pads the vocabulary dimension of word_embeddings / lm_head in this layout to
+ * Vp = ceil(vocab / (vocab_divisor*tp)) * vocab_divisor*tp rows (Megatron-LM's --make-vocab-size-divisible-by, default
+ * there 128); the padding rows [vocab, Vp) are stored in the shards like any other row.  0 = no padding, vocab % tp == 0
+ * required (reading A12); negative -> ETC_ERR_INVALID_ARG.  Migration between layouts with different Vp: rows present on
+ * both sides are moved (old padding rows included, so an identity reconfiguration is the identity), old rows beyond
+ * the new Vp are dropped, new rows beyond the old Vp have no source and are ZERO-FILLED (`Fill`, next to the paper's
+ * Send / Recv / Refer of PAPER.md:193-195); they count in need[] but in no traffic cell (etc_plan_stats.fill_bytes). */
+typedef struct { int32_t tp, pp, dp, dist_opt, pp_first, pp_last, dist_opt_align, vocab_divisor; } etc_parallel_cfg;
 
 typedef struct etc_layout etc_layout;   /* opaque, immutable after create */
 typedef struct etc_plan etc_plan;       /* opaque, immutable after create */
@@ -171,6 +178,9 @@ typedef struct {
   int64_t n_slices_local, n_slices_staged;   /* 2-D strided copy descriptors */
   int64_t n_chunks_local, n_chunks_staged;   /* copy work items (<= ETC_CHUNK_BYTES each) */
   int32_t n_old, n_new, P, flags;
+  int64_t fill_bytes;      /* destination bytes with no source, zero-filled (grown padded vocabulary, reading A31);
+                              local_bytes + remote_bytes + fill_bytes = sum of need[] */
+  int64_t n_fills;         /* zero-fill descriptors */
 } etc_plan_stats;
 etc_status etc_plan_get_stats(const etc_plan* plan, etc_plan_stats* out);
 /* traffic matrix T [P][P] row-major, int64, copied to HOST memory: T[o][p] = payload bytes whose source is old device
@@ -188,11 +198,15 @@ typedef struct {
   int32_t pad;
 } etc_slice;
 etc_status etc_plan_get_slices(const etc_plan* plan, int32_t which, etc_slice* h_out);
+/* The zero-fill descriptors (reading A31) as etc_slice records with no source: src_dev = -1, src_off = stg_off = -1,
+ * src_stride = 0; h_out must hold etc_plan_stats.n_fills entries (order unspecified).  Copied to HOST memory. */
+etc_status etc_plan_get_fills(const etc_plan* plan, etc_slice* h_out);
 
 /* (a5,a6) Migrate.  src_bufs[old_dev*4 + kind], dst_bufs[new_rank*4 + kind]: HOST arrays of DEVICE pointers (NULL
  * where the buffer has 0 bytes), each 16-byte aligned and at least etc_layout_buffer_bytes() long.  staging: device
  * pointer, >= staging_bytes (may be NULL if staging_bytes == 0).  Enqueues on `stream`:
- *   ETC_PHASE_PACK   : pack staged slices old buffers -> staging, and copy local slices old -> new directly
+ *   ETC_PHASE_PACK   : pack staged slices old buffers -> staging, copy local slices old -> new directly, and zero-fill
+ *                      the destination bytes that have no source (reading A31; none unless the padded vocabulary grew)
  *   ETC_PHASE_UNPACK : unpack staged slices staging -> new buffers
  * etc_migrate runs both phases.  No allocation, no host synchronisation.  Every destination byte is written exactly
  * once. */
@@ -211,7 +225,8 @@ etc_status etc_migrate_phase(const etc_plan* plan, const void* const* src_bufs, 
  * many rounds as it takes for every round to use at most max_staging_bytes (>= 2*ETC_CHUNK_BYTES) of staging.
  * Synchronises `stream` once (round sizes come back to the host).  May be called again with another bound.
  * etc_migrate_round enqueues round `round` (pack + local, unpack; `phases` as in etc_migrate_phase).  It reads only the
- * source buffers and writes only the destination buffers of the round's kind: pointers of other kinds are not looked
+ * source buffers and writes only the destination buffers of the round's kind (the kind's zero-fills, reading A31, go
+ * with its first round): pointers of other kinds are not looked
  * at (they may be NULL: already released, or not yet allocated).  `staging` needs only etc_round_info.staging_bytes
  * bytes and may be reused by the next round on the same stream.  After all rounds every destination byte has been
  * written exactly once, bit-identical to etc_migrate. */

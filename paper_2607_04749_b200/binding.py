@@ -20,7 +20,8 @@ ETC_DEFRAG_OCCUPANCY, ETC_DEFRAG_EFFICIENCY, ETC_DEFRAG_BOTH = 1, 2, 3
 EXPORTED_SYMBOLS = (
     "etc_init", "etc_layout_create", "etc_layout_destroy", "etc_layout_num_devices", "etc_layout_num_pieces",
     "etc_layout_buffer_bytes", "etc_cost_matrix", "etc_sketch", "etc_plan_create", "etc_plan_destroy",
-    "etc_plan_get_stats", "etc_plan_get_traffic", "etc_plan_get_slices", "etc_migrate", "etc_migrate_phase",
+    "etc_plan_get_stats", "etc_plan_get_traffic", "etc_plan_get_slices", "etc_plan_get_fills", "etc_migrate",
+    "etc_migrate_phase",
     "etc_status_string", "etc_last_error_detail", "etc_kernel_launches", "etc_defrag",
     "etc_plan_set_rounds", "etc_plan_get_round", "etc_migrate_round", "etc_plan_create_failed", "etc_mask_failed",
 )
@@ -40,13 +41,15 @@ class _ModelDesc(C.Structure):
 
 
 class _ParallelCfg(C.Structure):
-    _fields_ = [(n, C.c_int32) for n in ("tp", "pp", "dp", "dist_opt", "pp_first", "pp_last", "dist_opt_align")]
+    _fields_ = [(n, C.c_int32) for n in ("tp", "pp", "dp", "dist_opt", "pp_first", "pp_last", "dist_opt_align",
+                                          "vocab_divisor")]
 
 
 class _PlanStats(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("staging_bytes", "local_bytes", "remote_bytes", "staged_bytes",
                                           "n_slices_local", "n_slices_staged", "n_chunks_local", "n_chunks_staged")] + \
-               [(n, C.c_int32) for n in ("n_old", "n_new", "P", "flags")]
+               [(n, C.c_int32) for n in ("n_old", "n_new", "P", "flags")] + \
+               [(n, C.c_int64) for n in ("fill_bytes", "n_fills")]
 
 
 class _RoundInfo(C.Structure):
@@ -89,6 +92,7 @@ def lib():
         L.etc_plan_get_stats.restype = i32; L.etc_plan_get_stats.argtypes = [vp, C.POINTER(_PlanStats)]
         L.etc_plan_get_traffic.restype = i32; L.etc_plan_get_traffic.argtypes = [vp, vp]
         L.etc_plan_get_slices.restype = i32; L.etc_plan_get_slices.argtypes = [vp, i32, vp]
+        L.etc_plan_get_fills.restype = i32; L.etc_plan_get_fills.argtypes = [vp, vp]
         L.etc_migrate.restype = i32; L.etc_migrate.argtypes = [vp, vp, vp, vp, vp]
         L.etc_migrate_phase.restype = i32; L.etc_migrate_phase.argtypes = [vp, vp, vp, vp, i32, vp]
         L.etc_plan_set_rounds.restype = i32; L.etc_plan_set_rounds.argtypes = [vp, i64, C.POINTER(i32), vp]
@@ -166,7 +170,7 @@ def etc_layout_create(model: dict, cfg: dict) -> Layout:
                    qkv_order=model.get("qkv_order", 0))
     c = _ParallelCfg(tp=cfg["tp"], pp=cfg["pp"], dp=cfg["dp"], dist_opt=cfg.get("dist_opt", 0),
                      pp_first=cfg.get("pp_first", 0), pp_last=cfg.get("pp_last", 0),
-                     dist_opt_align=cfg.get("dist_opt_align", 0))
+                     dist_opt_align=cfg.get("dist_opt_align", 0), vocab_divisor=cfg.get("vocab_divisor", 0))
     h = C.c_void_p()
     _check(lib().etc_layout_create(C.byref(m), C.byref(c), C.byref(h)))
     return Layout(h, model, cfg)
@@ -233,6 +237,8 @@ class PlanStats:
     n_new: int
     P: int
     flags: int
+    fill_bytes: int = 0
+    n_fills: int = 0
 
     @property
     def hbm_bytes(self) -> int:
@@ -263,6 +269,15 @@ class Plan:
         assert dt.itemsize == C.sizeof(_Slice)
         arr = np.zeros(max(n, 1), dt)
         _check(lib().etc_plan_get_slices(self.h, which, arr.ctypes.data))
+        return arr[:n]
+
+    def fills(self):
+        """zero-fill descriptors (reading A31) as etc_slice records with src_dev = -1."""
+        import numpy as np
+        n = self.stats.n_fills
+        dt = np.dtype([(f, np.int64 if t is C.c_int64 else np.int32) for f, t in _Slice._fields_], align=True)
+        arr = np.zeros(max(n, 1), dt)
+        _check(lib().etc_plan_get_fills(self.h, arr.ctypes.data))
         return arr[:n]
 
     def __del__(self):

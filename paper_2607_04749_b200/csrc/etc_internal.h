@@ -82,6 +82,9 @@ struct etc_layout {
   etc::DeviceTables t;                    // device pointers + sizes
   int64_t* h_buffer_bytes = nullptr;      // [n_dev][4] host
   int32_t max_dev_pieces = 0;             // largest piece count of one device
+  int32_t vocab_rows = 0;                 // rows of the embedding tensors in this layout (padded vocabulary, reading A31)
+  int32_t lm_head_id = -1;                // logical tensor id of lm_head (-1: tied); word_embeddings is tensor 0
+  int32_t n_emb_pieces = 0;               // pieces of the embedding tensors (upper bound of the zero-fill list)
   void* d_blob = nullptr;                 // one allocation holding all device tables
   mutable etc::StreamSet streams;         // streams that kernels reading the tables were enqueued on
 };

@@ -27,11 +27,19 @@ struct LTensor { int64_t rows, cols; int32_t split, where, layer; };   // where:
 
 // Logical tensor list in id order.  The fused QKV weight / bias has its own split type
 // (readings A10, A29, A30: row order and KV-head replication, see qkv_blocks); SwiGLU fc1 = [gate; up] is COL2.
-static std::vector<LTensor> logical_tensors(const etc_model_desc& m) {
+// rows of the embedding tensors: the vocabulary padded to a multiple of vocab_divisor * tp (reading A31)
+static int64_t vocab_rows(const etc_model_desc& m, const etc_parallel_cfg& c) {
+  if (c.vocab_divisor <= 0) return m.vocab;
+  const int64_t unit = (int64_t)c.vocab_divisor * c.tp;
+  return ((int64_t)m.vocab + unit - 1) / unit * unit;
+}
+
+static std::vector<LTensor> logical_tensors(const etc_model_desc& m, const etc_parallel_cfg& c) {
   std::vector<LTensor> v;
+  const int64_t V = vocab_rows(m, c);
   const int64_t h = m.hidden, d = m.head_dim, f = m.ffn_hidden;
   const int64_t qkv = (int64_t(m.n_q_heads) + 2 * int64_t(m.n_kv_heads)) * d, qd = int64_t(m.n_q_heads) * d;
-  v.push_back({m.vocab, h, COL, 0, -1});
+  v.push_back({V, h, COL, 0, -1});
   if (m.style == ETC_GPT && m.max_pos > 0) v.push_back({m.max_pos, h, REPL, 0, -1});
   for (int l = 0; l < m.n_layers; ++l) {
     if (m.style == ETC_GPT) {
@@ -52,7 +60,7 @@ static std::vector<LTensor> logical_tensors(const etc_model_desc& m) {
   }
   v.push_back({1, h, REPL, 2, -1});                                              // final_ln w
   if (m.style == ETC_GPT) v.push_back({1, h, REPL, 2, -1});                      // final_ln b
-  if (!m.tied_embeddings) v.push_back({m.vocab, h, COL, 2, -1});                 // lm_head
+  if (!m.tied_embeddings) v.push_back({V, h, COL, 2, -1});                       // lm_head
   return v;
 }
 
@@ -72,7 +80,8 @@ static int stage_begin(int n_layers, const etc_parallel_cfg& c, int s) {
 
 static etc_status validate(const etc_model_desc* m, const etc_parallel_cfg* c) {
   if (!m || !c) return ETC_ERR_INVALID_ARG;
-  if (c->tp < 1 || c->pp < 1 || c->dp < 1 || (c->dist_opt != 0 && c->dist_opt != 1) || c->dist_opt_align < 0) return ETC_ERR_INVALID_ARG;
+  if (c->tp < 1 || c->pp < 1 || c->dp < 1 || (c->dist_opt != 0 && c->dist_opt != 1) || c->dist_opt_align < 0 ||
+      c->vocab_divisor < 0) return ETC_ERR_INVALID_ARG;
   if (m->style != ETC_GPT && m->style != ETC_LLAMA) return ETC_ERR_INVALID_ARG;
   if (m->n_layers < 1 || m->hidden < 1 || m->n_q_heads < 1 || m->n_kv_heads < 1 || m->head_dim < 1 ||
       m->ffn_hidden < 1 || m->vocab < 1 || m->max_pos < 0) return ETC_ERR_INVALID_ARG;
@@ -87,7 +96,8 @@ static etc_status validate(const etc_model_desc* m, const etc_parallel_cfg* c) {
     if (c->tp % m->n_kv_heads || (m->n_q_heads / m->n_kv_heads) % rep) return ETC_ERR_UNSUPPORTED;
   }
   { const int sb = stage_begin(m->n_layers, *c, 0); if (sb < 0) return sb == -2 ? ETC_ERR_INVALID_ARG : ETC_ERR_INDIVISIBLE; }
-  if ((c->tp <= m->n_kv_heads && m->n_kv_heads % c->tp) || m->ffn_hidden % c->tp || m->vocab % c->tp) return ETC_ERR_INDIVISIBLE;
+  if ((c->tp <= m->n_kv_heads && m->n_kv_heads % c->tp) || m->ffn_hidden % c->tp ||
+      (c->vocab_divisor == 0 && m->vocab % c->tp)) return ETC_ERR_INDIVISIBLE;
   return ETC_OK;
 }
 
@@ -170,7 +180,8 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   const etc_model_desc& m = *model;
   const int tp = cfg->tp, pp = cfg->pp, dp = cfg->dp;
   const int n_dev = tp * pp * dp;
-  const std::vector<LTensor> lts = logical_tensors(m);
+  const std::vector<LTensor> lts = logical_tensors(m, *cfg);
+  if (vocab_rows(m, *cfg) > INT32_MAX) return ETC_ERR_INVALID_ARG;
   const int nT = (int)lts.size(), nG = nT * ETC_NUM_KINDS;
   int max_stage_layers = 0;
   for (int s = 0; s < pp; ++s) max_stage_layers = std::max(max_stage_layers, stage_begin(m.n_layers, *cfg, s + 1) - stage_begin(m.n_layers, *cfg, s));
@@ -200,6 +211,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   memset(ltmask, 0, (size_t)n_dev * mask_words * 4);
   int64_t* bufbytes = new int64_t[(size_t)n_dev * ETC_NUM_KINDS]();
   size_t np = 0;
+  int32_t n_emb_pieces = 0;
 
   std::vector<std::vector<Sh>> shr(tp);     // shards of (stage, tp-rank r), in GROUP order: tied replica first
   for (int s = 0; s < pp; ++s) {
@@ -267,6 +279,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
             const uint16_t flags = q.flags | (dp_sharded ? PF_DP_SHARDED : 0);
             const int32_t grp = kind * nT + q.lt;
             first[(size_t)dev * nG + grp] = (int32_t)np;
+            const size_t np_before = np;
             // decompose the held flat range [a,b) of the shard into rectangles of local rows x local cols
             // (head partial row, whole rows cut at the block boundaries, tail partial row: <= 5)
             int64_t rect[5][4]; int nr = 0;
@@ -302,6 +315,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
               p.boff = (q.start + i0 * q.W + j0 - lo) * es;
               p.f0 = a; p.f1 = b;
             }
+            if (q.lt == 0 || (!m.tied_embeddings && q.lt == nT - 1)) n_emb_pieces += (int32_t)(np - np_before);
           }
         }
         kind_start[(size_t)dev * (ETC_NUM_KINDS + 1) + ETC_NUM_KINDS] = (int32_t)np;
@@ -314,6 +328,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
 
   etc_layout* L = new etc_layout();
   L->model = m; L->cfg = *cfg; L->h_buffer_bytes = bufbytes; L->max_dev_pieces = max_dev_pieces;
+  L->vocab_rows = (int32_t)vocab_rows(m, *cfg); L->lm_head_id = m.tied_embeddings ? -1 : nT - 1; L->n_emb_pieces = n_emb_pieces;
   e = cudaMallocAsync(&L->d_blob, total, g_up_stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync(L->d_blob, host, total, cudaMemcpyHostToDevice, g_up_stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(g_up_stream);

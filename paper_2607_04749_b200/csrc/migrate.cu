@@ -151,6 +151,36 @@ migrate_copy_kernel(const Chunk* __restrict__ chA, long long nA, const Chunk* __
   copy_dispatch(c.vec, src, dst, c.nrows, (uint32_t)c.row_bytes, sp, dp);
 }
 
+// Zero-fill (reading A31): blockIdx.x = descriptor, blockIdx.y = one of FILL_SPLIT CTAs sharing its rows x row_bytes.
+// only_kind >= 0 restricts the launch to one state kind (rounds of state chunking).  Padding rows are a sliver of the
+// state, so this is the plain vector store loop, not a tuned kernel.
+constexpr int FILL_SPLIT = 16;
+template <typename V>
+__device__ __forceinline__ void fill_rows(char* dst, int nrows, uint32_t row_bytes, uint32_t pitch) {
+  const uint32_t vpr = row_bytes / (uint32_t)sizeof(V);
+  const unsigned long long total = (unsigned long long)vpr * (unsigned)nrows;
+  V z; memset(&z, 0, sizeof(V));
+  for (unsigned long long i = (unsigned long long)blockIdx.y * blockDim.x + threadIdx.x; i < total;
+       i += (unsigned long long)gridDim.y * blockDim.x) {
+    const unsigned long long row = i / vpr, col = i - row * vpr;
+    reinterpret_cast<V*>(dst + row * pitch)[col] = z;
+  }
+}
+__global__ void __launch_bounds__(CP_THREADS)
+migrate_fill_kernel(const etc_slice* __restrict__ fills, void* const* __restrict__ dst_tab, int only_kind) {
+  const etc_slice f = fills[blockIdx.x];
+  if (only_kind >= 0 && f.kind != only_kind) return;
+  char* dst = static_cast<char*>(dst_tab[f.dst_rank * ETC_NUM_KINDS + f.kind]) + f.dst_off;
+  int64_t al = f.dst_off | f.row_bytes;
+  if (f.nrows > 1) al |= (int64_t)f.dst_stride;
+  const int64_t low = al & -al;
+  // one contiguous run longer than 2^32 bytes cannot occur (a buffer row is < 2^31 elements); rows are < 4 GiB
+  if (low >= 16 || al == 0) fill_rows<uint4>(dst, f.nrows, (uint32_t)f.row_bytes, (uint32_t)f.dst_stride);
+  else if (low >= 4) fill_rows<unsigned int>(dst, f.nrows, (uint32_t)f.row_bytes, (uint32_t)f.dst_stride);
+  else if (low >= 2) fill_rows<unsigned short>(dst, f.nrows, (uint32_t)f.row_bytes, (uint32_t)f.dst_stride);
+  else fill_rows<unsigned char>(dst, f.nrows, (uint32_t)f.row_bytes, (uint32_t)f.dst_stride);
+}
+
 // the TMA path stages one chunk per CTA in dynamic shared memory
 static cudaError_t copy_kernel_attrs() {
   static bool done = false;
@@ -172,7 +202,7 @@ using namespace etc;
 // chunk ranges.  `staging` is addressed relative to stg_base.
 static etc_status launch_migrate(const etc_plan* pl, const void* const* src_bufs, void* const* dst_bufs, void* staging,
                                  int32_t phases, cudaStream_t st, void** d_ptrs, int only_kind, long long ca, long long nA,
-                                 long long la, long long nB, int64_t stg_base, int64_t stg_need) {
+                                 long long la, long long nB, int64_t stg_base, int64_t stg_need, bool with_fills) {
   if (!pl || !src_bufs || !dst_bufs || phases < 1 || phases > ETC_PHASE_ALL) return ETC_ERR_INVALID_ARG;
   if (stg_need > 0 && !staging) return ETC_ERR_INVALID_ARG;
   if (reinterpret_cast<uintptr_t>(staging) & 15) return ETC_ERR_INVALID_ARG;
@@ -200,6 +230,11 @@ static etc_status launch_migrate(const etc_plan* pl, const void* const* src_bufs
     ETC_CUDA_TRY(cudaGetLastError());
     count_launch();
   }
+  if ((phases & ETC_PHASE_PACK) && with_fills && pl->totals.n_fills > 0) {      // reading A31: bytes with no source
+    migrate_fill_kernel<<<dim3((unsigned)pl->totals.n_fills, FILL_SPLIT), CP_THREADS, 0, st>>>(pl->d_fills, d_dst, only_kind);
+    ETC_CUDA_TRY(cudaGetLastError());
+    count_launch();
+  }
   if ((phases & ETC_PHASE_UNPACK) && nA > 0) {
     migrate_copy_kernel<true><<<(unsigned)nA, CP_THREADS, ETC_CHUNK_BYTES, st>>>(pl->d_ch_staged + ca, nA, nullptr, d_src, d_dst, stg);
     ETC_CUDA_TRY(cudaGetLastError());
@@ -214,7 +249,7 @@ extern "C" etc_status etc_migrate_phase(const etc_plan* pl, const void* const* s
   if (!pl) return ETC_ERR_INVALID_ARG;
   const PlanTotals& t = pl->totals;
   return launch_migrate(pl, src_bufs, dst_bufs, staging, phases, (cudaStream_t)stream, pl->d_ptrs, -1, 0,
-                        t.n_chunks_staged, 0, t.n_chunks_local, 0, t.staging_bytes);
+                        t.n_chunks_staged, 0, t.n_chunks_local, 0, t.staging_bytes, true);
 }
 
 extern "C" etc_status etc_migrate(const etc_plan* pl, const void* const* src_bufs, void* const* dst_bufs, void* staging,
@@ -231,5 +266,5 @@ extern "C" etc_status etc_migrate_round(const etc_plan* pl, int32_t round, const
   const size_t n_ptrs = ((size_t)(pl->n_old + pl->n_new) * ETC_NUM_KINDS * sizeof(void*) + 255) / 256 * 256 / sizeof(void*);
   return launch_migrate(pl, src_bufs, dst_bufs, staging, phases, (cudaStream_t)stream,
                         pl->d_round_ptrs + n_ptrs * (size_t)round, r.kind, r.ca, r.cb - r.ca, r.la, r.lb - r.la,
-                        r.stg_base, r.stg_span);
+                        r.stg_base, r.stg_span, r.sub == 0);
 }

@@ -271,6 +271,7 @@ plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int K, int n_
       t.n_slices_staged = s_carry[0]; t.n_chunks_staged = s_carry[1]; t.staging_bytes = s_carry[2];
       t.n_slices_local = s_carry[3]; t.n_chunks_local = s_carry[4];
       t.local_bytes = loc; t.remote_bytes = rem; t.bad_map = bad ? 1 : 0;
+      t.fill_bytes = 0; t.n_fills = 0;                          // plan_fills_kernel adds to these
       for (int k = 0; k < ETC_NUM_KINDS; ++k) for (int j = 0; j < 3; ++j) t.kind_base[k][j] = s_kind[k][j];
       t.kind_base[ETC_NUM_KINDS][0] = s_carry[1]; t.kind_base[ETC_NUM_KINDS][1] = s_carry[2];
       t.kind_base[ETC_NUM_KINDS][2] = s_carry[4];
@@ -335,6 +336,31 @@ plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict
       });
     }
   }
+}
+
+// Zero-fill list (reading A31): a row of an embedding tensor of the new layout that lies beyond the old layout's padded
+// vocabulary (rows >= old_rows) is held by no old device.  One thread per new piece; a piece's rows beyond old_rows are
+// one descriptor (an etc_slice with no source).  Runs only when the padded vocabulary grew.
+__global__ void __launch_bounds__(256)
+plan_fills_kernel(DeviceTables newT, const int32_t* __restrict__ device_map, int old_rows, int lm_head_id,
+                  etc_slice* __restrict__ fills, PlanTotals* __restrict__ totals) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= newT.n_pieces) return;
+  const Piece q = newT.pieces[i];
+  const int t = q.grp % newT.n_tensors, kind = q.grp / newT.n_tensors;
+  if (t != 0 && t != lm_head_id) return;
+  const int r0 = max(q.r0, old_rows), r1 = q.r0 + q.nr;
+  if (r1 <= r0) return;
+  const int es = newT.elem_bytes[kind];
+  etc_slice f;
+  f.src_off = -1; f.stg_off = -1; f.src_stride = 0; f.src_dev = -1; f.pad = 0;
+  f.dst_off = q.boff + (int64_t)(r0 - q.r0) * q.W * es;
+  f.row_bytes = (int64_t)q.nc * es; f.dst_stride = q.W * es; f.nrows = r1 - r0;
+  if (f.nrows > 1 && f.row_bytes == f.dst_stride) { f.row_bytes *= f.nrows; f.nrows = 1; }
+  f.dst_rank = q.dev; f.dst_phys = device_map[q.dev]; f.kind = kind;
+  const unsigned long long slot = atomicAdd(reinterpret_cast<unsigned long long*>(&totals->n_fills), 1ull);
+  fills[slot] = f;
+  atomicAdd(reinterpret_cast<unsigned long long*>(&totals->fill_bytes), (unsigned long long)((int64_t)(r1 - r0) * q.nc * es));
 }
 
 // pass 3: one thread per chunk: find its slice by binary search over the slices' first-chunk indices, cut the chunk out
@@ -429,7 +455,9 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
       seen[p] = 1;
     }
   }
-  // workspace blob 1: units | bases | blocks | traffic | totals | map | pointer tables
+  // reading A31: the new layout's padded vocabulary has rows the old one lacks -> those are zero-filled
+  const bool grows = new_l->vocab_rows > old_l->vocab_rows && new_l->n_emb_pieces > 0;
+  // workspace blob 1: units | bases | blocks | traffic | totals | map | pointer tables | failure mask | zero-fill list
   auto al = [](size_t x) { return (x + 255) & ~size_t(255); };
   const size_t o_units = 0, o_bases = o_units + al(sizeof(UnitCount) * (size_t)U),
                o_blocks = o_bases + al(sizeof(UnitBase) * (size_t)U),
@@ -437,7 +465,8 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
                o_totals = o_traffic + al(sizeof(int64_t) * (size_t)P * P), o_map = o_totals + al(sizeof(PlanTotals)),
                o_ptrs = o_map + al(sizeof(int32_t) * (size_t)n_new),
                o_failed = o_ptrs + al(sizeof(void*) * (size_t)(n_old + n_new) * ETC_NUM_KINDS),
-               ws_bytes = o_failed + al((size_t)n_old);
+               o_fills = o_failed + al((size_t)n_old),
+               ws_bytes = o_fills + (grows ? al(sizeof(etc_slice) * (size_t)new_l->n_emb_pieces) : 0);
   PLAN_TRY(cudaMallocAsync(&pl->d_ws, ws_bytes, st));
   char* ws = static_cast<char*>(pl->d_ws);
   pl->d_units = reinterpret_cast<UnitCount*>(ws + o_units); pl->d_bases = reinterpret_cast<UnitBase*>(ws + o_bases);
@@ -462,6 +491,13 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
                                                pl->d_traffic, pl->d_totals);
   PLAN_TRY(cudaGetLastError());
   count_launch(2);
+  if (grows) {
+    pl->d_fills = reinterpret_cast<etc_slice*>(ws + o_fills);
+    plan_fills_kernel<<<(unsigned)((new_l->t.n_pieces + 255) / 256), 256, 0, st>>>(new_l->t, pl->d_map, old_l->vocab_rows,
+                                                                                   new_l->lm_head_id, pl->d_fills, pl->d_totals);
+    PLAN_TRY(cudaGetLastError());
+    count_launch();
+  }
   PLAN_TRY(cudaMemcpyAsync(h_tot, pl->d_totals, sizeof(PlanTotals), cudaMemcpyDeviceToHost, st));
   PLAN_TRY(cudaStreamSynchronize(st));                          // the one host sync: sizes must come back
   pl->totals = *h_tot;
@@ -469,7 +505,7 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
   {                                                             // every needed byte must have found its one source
     int64_t need = 0;
     for (int64_t b : pl->new_bytes) need += b;
-    if (pl->totals.local_bytes + pl->totals.remote_bytes != need) return fail(ETC_ERR_UNRECOVERABLE);
+    if (pl->totals.local_bytes + pl->totals.remote_bytes + pl->totals.fill_bytes != need) return fail(ETC_ERR_UNRECOVERABLE);
   }
 
   // blob 2: slice records | first-chunk indices | chunk descriptors
@@ -526,6 +562,7 @@ extern "C" etc_status etc_plan_get_stats(const etc_plan* pl, etc_plan_stats* out
   out->n_slices_local = t.n_slices_local; out->n_slices_staged = t.n_slices_staged;
   out->n_chunks_local = t.n_chunks_local; out->n_chunks_staged = t.n_chunks_staged;
   out->n_old = pl->n_old; out->n_new = pl->n_new; out->P = pl->P; out->flags = pl->flags;
+  out->fill_bytes = t.fill_bytes; out->n_fills = t.n_fills;
   return ETC_OK;
 }
 
@@ -544,5 +581,13 @@ extern "C" etc_status etc_plan_get_slices(const etc_plan* pl, int32_t which, etc
   const etc_slice* src = which == 0 ? pl->d_sl_staged : pl->d_sl_local;
   ETC_CUDA_TRY(cudaStreamSynchronize(pl->stream_created_on));
   if (n) ETC_CUDA_TRY(cudaMemcpy(h_out, src, sizeof(etc_slice) * (size_t)n, cudaMemcpyDeviceToHost));
+  return ETC_OK;
+}
+
+extern "C" etc_status etc_plan_get_fills(const etc_plan* pl, etc_slice* h_out) {
+  clear_error_detail();
+  if (!pl || !h_out) return ETC_ERR_INVALID_ARG;
+  ETC_CUDA_TRY(cudaStreamSynchronize(pl->stream_created_on));
+  if (pl->totals.n_fills) ETC_CUDA_TRY(cudaMemcpy(h_out, pl->d_fills, sizeof(etc_slice) * (size_t)pl->totals.n_fills, cudaMemcpyDeviceToHost));
   return ETC_OK;
 }

@@ -11,6 +11,7 @@ struct UnitBase { int64_t slice0, chunk0, stg0; };
 struct PlanTotals {
   int64_t n_slices_staged, n_chunks_staged, staging_bytes, n_slices_local, n_chunks_local;
   int64_t local_bytes, remote_bytes, bad_map;
+  int64_t fill_bytes, n_fills;           // zero-filled destination bytes / descriptors (reading A31); added after the scan
   // kind-major plans: [kind][0] first staged chunk, [1] first staging byte, [2] first local chunk of the kind;
   // entry [ETC_NUM_KINDS] = the totals
   int64_t kind_base[ETC_NUM_KINDS + 1][3];
@@ -55,6 +56,7 @@ struct etc_plan {
   etc_slice* d_sl_staged = nullptr; etc_slice* d_sl_local = nullptr;
   etc::Chunk* d_ch_staged = nullptr; etc::Chunk* d_ch_local = nullptr;
   int64_t* d_c0_staged = nullptr; int64_t* d_c0_local = nullptr;
+  etc_slice* d_fills = nullptr;                    // zero-fill descriptors (in d_ws; totals.n_fills of them), reading A31
   std::vector<int64_t> old_bytes, new_bytes;       // buffer sizes [dev*4+kind], for argument checks in migrate
   void** d_ptrs = nullptr;                         // [n_old*4] source pointers then [n_new*4] destination pointers
   // state chunking (f2): rounds of bounded staging, set by etc_plan_set_rounds
