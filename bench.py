@@ -412,9 +412,12 @@ def extras(E, torch, w, dev, src, dst, lay_old, lay_new, peak):
 
 
 def e2e(E, torch, args, w, dev, src, dst, hbm_bytes, world, barrier):
-    """The same metric through the public API with HOST buffers: old shards in pinned host memory -> H2D -> whole path
-    (a1-a6, as kind-by-kind rounds of a kind-major plan) -> D2H -> new shards in pinned host memory, every copy inside
-    the timed region.  Uploads, rounds and downloads of different kinds overlap on three streams (host_pipeline.py)."""
+    """The same metric through the public API with HOST buffers: old shards in pinned host memory -> whole path (a1-a6,
+    as kind-by-kind rounds of a kind-major plan) -> new shards in pinned host memory, everything inside the timed region.
+    Headline: zero-copy (host_pipeline.HostMigration(zero_copy=True)): the pinned host buffers ARE the source and
+    destination tables of the C-ABI call, the copy kernels move every byte over PCIe, no device copy of any shard exists.
+    Beside it: the DMA pipelines (cudaMemcpyAsync of every old shard byte / of only the regions the plan reads, rounds
+    on device buffers, cudaMemcpyAsync of the new shards; three streams)."""
     from paper_2607_04749_b200.host_pipeline import HostMigration
     h_src = {k: torch.empty(t.shape, dtype=t.dtype, pin_memory=True) for k, t in src.items()}
     h_dst = {k: torch.empty(t.shape, dtype=t.dtype, pin_memory=True) for k, t in dst.items()}
@@ -423,22 +426,38 @@ def e2e(E, torch, args, w, dev, src, dst, hbm_bytes, world, barrier):
     torch.cuda.synchronize()
     n = max(1, min(args.steps, args.e2e_steps))
     flags = E.ETC_ALL_STAGED if args.all_staged else E.ETC_LOCAL_DIRECT
-    warm = HostMigration(w["model"], w["old"], w["new"], h_src, h_dst, dev, args.e2e_staging, flags, d_src=src, d_dst=dst)
-    warm.run(); barrier()
-    hm = HostMigration(w["model"], w["old"], w["new"], h_src, h_dst, dev, args.e2e_staging, flags, d_src=src, d_dst=dst)
-    del warm
-    barrier()
-    for _ in range(n):
-        plan = hm.run()
-    barrier()
-    ms = hm.begin.elapsed_time(hm.done) / n
-    ms = max_over_ranks(ms, world, dev)
-    return {"value": job_value(world, hbm_bytes, ms), "unit": UNIT, "ms_per_step": ms, "steps": n,
-            "h2d_bytes_per_step": hm.h2d_bytes, "d2h_bytes_per_step": hm.d2h_bytes,
-            "pcie_GBs_each_way": [hm.h2d_bytes / ms / 1e6, hm.d2h_bytes / ms / 1e6],
-            "rounds": len(plan.rounds), "staging_bytes": args.e2e_staging,
-            "note": "host-pinned old shards -> H2D -> whole path (kind-major rounds) -> D2H of new shards, all inside "
-                    "the timed region; upload, rounds and download of different kinds overlap on three streams"}
+
+    def leg(**kw):
+        mk = lambda: HostMigration(w["model"], w["old"], w["new"], h_src, h_dst, dev, args.e2e_staging, flags, **kw)
+        warm = mk(); warm.run(); barrier()
+        hm = mk()
+        del warm
+        barrier()
+        for _ in range(n):
+            plan = hm.run()
+        barrier()
+        ms = max_over_ranks(hm.begin.elapsed_time(hm.done) / n, world, dev)
+        return {"value": job_value(world, hbm_bytes, ms), "unit": UNIT, "ms_per_step": ms, "steps": n,
+                "h2d_bytes_per_step": hm.h2d_bytes, "d2h_bytes_per_step": hm.d2h_bytes,
+                "pcie_GBs_each_way": [hm.h2d_bytes / ms / 1e6, hm.d2h_bytes / ms / 1e6],
+                "rounds": len(plan.rounds), "staging_bytes": args.e2e_staging}
+
+    out = leg(zero_copy=True)
+    out["note"] = ("zero-copy: pinned host old shards -> [copy kernels read them over PCIe, only the bytes their chunks "
+                   "name] -> whole path (kind-major rounds, staging on the device) -> [copy kernels write over PCIe] -> "
+                   "pinned host new shards; h2d / d2h = bytes the kernels read from / write to host memory")
+    for key, kw, note in (
+            ("dma_full_upload", dict(d_src=src, d_dst=dst),
+             "cudaMemcpyAsync of EVERY old shard byte -> rounds on device buffers -> cudaMemcpyAsync of the new shards; "
+             "upload, rounds and download of different kinds overlap on three streams"),
+            ("dma_needed_only", dict(d_src=src, d_dst=dst, needed_only=True),
+             "plan first, then cudaMemcpy2DAsync of only the source regions the plan's slices read (etc_upload_sources)")):
+        try:
+            out[key] = leg(**kw)
+            out[key]["note"] = note
+        except Exception as ex:
+            out[key] = {"error": repr(ex)[:200]}
+    return out
 
 
 def chunked(E, torch, w, dev, src, lay_old, lay_new, cap):

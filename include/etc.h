@@ -203,7 +203,10 @@ etc_status etc_plan_get_slices(const etc_plan* plan, int32_t which, etc_slice* h
 etc_status etc_plan_get_fills(const etc_plan* plan, etc_slice* h_out);
 
 /* (a5,a6) Migrate.  src_bufs[old_dev*4 + kind], dst_bufs[new_rank*4 + kind]: HOST arrays of DEVICE pointers (NULL
- * where the buffer has 0 bytes), each 16-byte aligned and at least etc_layout_buffer_bytes() long.  staging: device
+ * where the buffer has 0 bytes), each 16-byte aligned and at least etc_layout_buffer_bytes() long.  A buffer may also
+ * live in PINNED HOST memory (cudaMallocHost / cudaHostAlloc: device-addressable at the same address): the copy kernels
+ * then read or write it over PCIe themselves ("zero-copy"), touching only the bytes their chunks name, and no device
+ * copy of that shard is needed.  staging: device
  * pointer, >= staging_bytes (may be NULL if staging_bytes == 0).  Enqueues on `stream`:
  *   ETC_PHASE_PACK   : pack staged slices old buffers -> staging, copy local slices old -> new directly, and zero-fill
  *                      the destination bytes that have no source (reading A31; none unless the padded vocabulary grew)
@@ -240,6 +243,18 @@ etc_status etc_plan_set_rounds(etc_plan* plan, int64_t max_staging_bytes, int32_
 etc_status etc_plan_get_round(const etc_plan* plan, int32_t round, etc_round_info* out);
 etc_status etc_migrate_round(const etc_plan* plan, int32_t round, const void* const* src_bufs, void* const* dst_bufs,
                              void* staging, int32_t phases, void* stream);
+
+/* Host-resident old shards: upload exactly the source bytes the plan reads (only the slices named by
+ * the migration instructions move).  h_src_bufs / d_src_bufs: HOST arrays [n_old*4] of pointers to the host copy
+ * (pinned memory, or the copies are not asynchronous) and the device copy of each old shard buffer; every region a
+ * slice of the plan reads (rows x row_bytes at the buffer's pitch) is copied from the host buffer to the same offset
+ * of the device buffer with cudaMemcpyAsync / cudaMemcpy2DAsync on `stream`; regions read by several slices are
+ * copied once; bytes no slice reads are not transferred and stay undefined on the device (etc_migrate never reads
+ * them).  only_kind = 0..3 restricts the call to one state kind (pipelining with rounds), -1 = all kinds.
+ * *bytes_out (optional) receives the bytes enqueued.  The first call on a plan synchronises the stream the plan was
+ * created on (the slice table comes back to the host once). */
+etc_status etc_upload_sources(const etc_plan* plan, const void* const* h_src_bufs, void* const* d_src_bufs,
+                              int32_t only_kind, int64_t* bytes_out, void* stream);
 
 const char* etc_status_string(etc_status s);   /* static strings */
 const char* etc_last_error_detail(void);       /* thread-local; CUDA error text after ETC_ERR_CUDA, else "" */

@@ -24,6 +24,7 @@ EXPORTED_SYMBOLS = (
     "etc_migrate_phase",
     "etc_status_string", "etc_last_error_detail", "etc_kernel_launches", "etc_defrag",
     "etc_plan_set_rounds", "etc_plan_get_round", "etc_migrate_round", "etc_plan_create_failed", "etc_mask_failed",
+    "etc_upload_sources",
 )
 
 
@@ -98,6 +99,7 @@ def lib():
         L.etc_plan_set_rounds.restype = i32; L.etc_plan_set_rounds.argtypes = [vp, i64, C.POINTER(i32), vp]
         L.etc_plan_get_round.restype = i32; L.etc_plan_get_round.argtypes = [vp, i32, C.POINTER(_RoundInfo)]
         L.etc_migrate_round.restype = i32; L.etc_migrate_round.argtypes = [vp, i32, vp, vp, vp, i32, vp]
+        L.etc_upload_sources.restype = i32; L.etc_upload_sources.argtypes = [vp, vp, vp, i32, C.POINTER(i64), vp]
         L.etc_status_string.restype = C.c_char_p; L.etc_status_string.argtypes = [i32]
         L.etc_last_error_detail.restype = C.c_char_p
         L.etc_kernel_launches.restype = i64
@@ -347,6 +349,20 @@ def etc_migrate(plan: Plan, src_bufs: dict, dst_bufs: dict, staging, phases: int
         assert staging.numel() * staging.element_size() >= st.staging_bytes
         sp = staging.data_ptr()
     _check(lib().etc_migrate_phase(plan.h, src_bufs, dst_bufs, sp, phases, _stream(stream)))
+
+
+def etc_upload_sources(plan: Plan, h_src_bufs, d_src_bufs, only_kind: int = -1, stream=None) -> int:
+    """Host-resident old shards: copy exactly the regions the plan reads from the pinned host buffers to the same offsets
+    of the device buffers (include/etc.h etc_upload_sources).  Dicts {(old_dev, kind): tensor} or pointer tables.
+    Returns the bytes enqueued."""
+    st = plan.stats
+    if isinstance(h_src_bufs, dict):
+        h_src_bufs = _ptr_table(h_src_bufs, st.n_old)
+    if isinstance(d_src_bufs, dict):
+        d_src_bufs = _ptr_table(d_src_bufs, st.n_old)
+    n = C.c_int64(0)
+    _check(lib().etc_upload_sources(plan.h, h_src_bufs, d_src_bufs, only_kind, C.byref(n), _stream(stream)))
+    return int(n.value)
 
 
 @dataclass

@@ -64,4 +64,8 @@ struct etc_plan {
   int64_t round_staging_cap = 0;
   void* d_rounds_ws = nullptr;                     // round records + one pointer table per round
   void** d_round_ptrs = nullptr;
+  // host_io.cu: de-duplicated source regions per state kind (src_dev = buffer index), built on first use
+  mutable std::vector<etc_slice> h_regions[ETC_NUM_KINDS];
+  mutable int64_t h_region_bytes[ETC_NUM_KINDS] = {0, 0, 0, 0};
+  mutable bool h_regions_ready = false;
 };

@@ -6,6 +6,13 @@ with on-demand buffer allocation, and eager release of source-side state"; :378 
 * `HostMigration`   old shards in pinned host memory -> H2D -> whole path -> D2H -> new shards in pinned host memory.
                     Kinds are pipelined over three streams, so the upload of kind k+1, the migration of kind k and the
                     download of kind k-1 overlap (PCIe is full duplex; the copy kernels need a few % of HBM time).
+                    With `needed_only=True` the plan is made first and only the source regions its slices read cross
+                    PCIe (etc_upload_sources: PAPER.md:193-197, only the workload named by the instructions moves).
+                    With `zero_copy=True` there are no device-side shard buffers and no DMA copies at all: the pinned
+                    host buffers are handed to etc_migrate_round as they are (pinned memory is device-addressable), so
+                    the copy kernels themselves read the old shards over PCIe — only the bytes their chunks name — and
+                    write the new shards back over PCIe; slices that stay on their device go host -> shared memory ->
+                    host in one hop, using both PCIe directions at once.
 * `migrate_chunked` device-resident: for each kind, allocate its new buffers, run its rounds through one bounded
                     staging buffer, release its old buffers.  Returns the peak of live bytes, the quantity Fig. 12 of
                     the paper plots.
@@ -31,7 +38,7 @@ class HostMigration:
 
     def __init__(self, model: dict, old_cfg: dict, new_cfg: dict, h_src: dict, h_dst: dict, device=None,
                  max_staging_bytes: int = 1 << 30, flags: int = B.ETC_LOCAL_DIRECT, device_map=None,
-                 d_src: dict | None = None, d_dst: dict | None = None):
+                 d_src: dict | None = None, d_dst: dict | None = None, needed_only: bool = False, zero_copy: bool = False):
         import torch
         self.torch = torch
         self.model, self.old_cfg, self.new_cfg = model, old_cfg, new_cfg
@@ -40,15 +47,24 @@ class HostMigration:
         self.flags = flags | B.ETC_KIND_MAJOR
         self.cap = int(max_staging_bytes)
         self.device_map = device_map
+        self.needed_only = needed_only
+        self.zero_copy = zero_copy
         lo, ln = B.etc_layout_create(model, old_cfg), B.etc_layout_create(model, new_cfg)
-        self.d_src = d_src if d_src is not None else B.alloc_buffers(lo, self.device)     # device-side shard buffers
-        self.d_dst = d_dst if d_dst is not None else B.alloc_buffers(ln, self.device)
+        if zero_copy:
+            self.d_src = self.d_dst = {}                           # no device-side shard buffers
+        else:
+            self.d_src = d_src if d_src is not None else B.alloc_buffers(lo, self.device)
+            self.d_dst = d_dst if d_dst is not None else B.alloc_buffers(ln, self.device)
         self.n_old, self.n_new = lo.n_dev, ln.n_dev
         self.kinds = lo.kinds()
         eb = {k: (model["param_bytes"] if k == 0 else 4) for k in self.kinds}
         self.order = kind_order(self.kinds, eb)
         self.staging = torch.empty(self.cap, dtype=torch.uint8, device=self.device)
         self.s_h2d, self.s_run, self.s_d2h = (torch.cuda.Stream(self.device) for _ in range(3))
+        # planning has its own stream: etc_plan_create synchronises the stream it runs on (sizes come back to the host),
+        # and on s_run that would block the host until the previous pass's rounds are done
+        self.s_plan = torch.cuda.Stream(self.device)
+        self.ev_plan = torch.cuda.Event()
         mk = lambda: {k: torch.cuda.Event() for k in self.kinds}
         self.ev_up, self.ev_run, self.ev_down = mk(), mk(), mk()
         self.begin, self.done = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -57,8 +73,29 @@ class HostMigration:
         self.d2h_bytes = sum(t.numel() for t in h_dst.values())
         self.src_tab = B._ptr_table(self.d_src, self.n_old)
         self.dst_tab = B._ptr_table(self.d_dst, self.n_new)
+        self.h_src_tab = B._ptr_table(self.h_src, self.n_old)
+        self.h_dst_tab = B._ptr_table(self.h_dst, self.n_new)
+
+    def _plan(self):
+        """(a1)-(a4) on the planning stream; s_run is made to wait for it."""
+        with self.torch.cuda.stream(self.s_plan):
+            lo, ln = B.etc_layout_create(self.model, self.old_cfg), B.etc_layout_create(self.model, self.new_cfg)
+            if self.device_map is None:
+                ov, _, _ = B.etc_cost_matrix(lo, ln, stream=self.s_plan)
+                dm, _ = B.etc_sketch(ov, stream=self.s_plan)
+            else:
+                dm = self.device_map
+            plan = B.etc_plan_create(lo, ln, dm, self.flags, stream=self.s_plan)
+            rounds = B.etc_plan_set_rounds(plan, self.cap, stream=self.s_plan)
+            self.ev_plan.record(self.s_plan)
+        self.s_run.wait_event(self.ev_plan)
+        return plan, rounds
 
     def run(self):
+        if self.zero_copy:
+            return self._run_zero_copy()
+        if self.needed_only:
+            return self._run_needed_only()
         torch = self.torch
         # uploads: kind by kind; a buffer may be overwritten only after the previous pass's rounds have read it
         with torch.cuda.stream(self.s_h2d):
@@ -72,15 +109,8 @@ class HostMigration:
                         t.copy_(self.h_src[(d, kk)], non_blocking=True)
                 self.ev_up[k].record(self.s_h2d)
         # planning (metadata only) overlaps the first upload
+        plan, rounds = self._plan()
         with torch.cuda.stream(self.s_run):
-            lo, ln = B.etc_layout_create(self.model, self.old_cfg), B.etc_layout_create(self.model, self.new_cfg)
-            if self.device_map is None:
-                ov, _, _ = B.etc_cost_matrix(lo, ln, stream=self.s_run)
-                dm, _ = B.etc_sketch(ov, stream=self.s_run)
-            else:
-                dm = self.device_map
-            plan = B.etc_plan_create(lo, ln, dm, self.flags, stream=self.s_run)
-            rounds = B.etc_plan_set_rounds(plan, self.cap, stream=self.s_run)
             for k in self.order:
                 self.s_run.wait_event(self.ev_up[k])
                 if not self.first:
@@ -97,6 +127,56 @@ class HostMigration:
                         self.h_dst[(n, kk)].copy_(t, non_blocking=True)
                 self.ev_down[k].record(self.s_d2h)
             self.done.record(self.s_d2h)
+        self.first = False
+        self.plan = plan
+        return plan
+
+
+    def _run_zero_copy(self):
+        """Plan, then the rounds with the pinned HOST buffers as source and destination tables: every byte is moved by
+        the copy kernels, over PCIe; the device holds only the plan's tables and the bounded staging buffer."""
+        if self.first:
+            self.begin.record(self.s_plan)
+        plan, rounds = self._plan()
+        for i in range(len(rounds)):
+            B.etc_migrate_round(plan, i, self.h_src_tab, self.h_dst_tab, self.staging, stream=self.s_run)
+        self.done.record(self.s_run)
+        st = plan.stats
+        self.h2d_bytes = st.local_bytes + st.remote_bytes          # payload bytes the kernels read from host memory
+        self.d2h_bytes = st.local_bytes + st.remote_bytes + st.fill_bytes
+        self.first = False
+        self.plan = plan
+        return plan
+
+    def _run_needed_only(self):
+        """Plan first (metadata, < 1 ms), then per kind: upload the regions the plan reads -> rounds -> download.
+        The three queues are fed kind by kind: a stream accepts only so many pending copies before the enqueueing call
+        blocks, and an upload is thousands of region copies, so the rounds and the download of kind k must be queued
+        before the upload of kind k+1 is."""
+        torch = self.torch
+        if self.first:
+            self.begin.record(self.s_plan)
+        plan, rounds = self._plan()
+        self.h2d_bytes = 0
+        for k in self.order:
+            if not self.first:
+                self.s_h2d.wait_event(self.ev_run[k])              # the previous pass's rounds have read these buffers
+            self.h2d_bytes += B.etc_upload_sources(plan, self.h_src_tab, self.src_tab, k, stream=self.s_h2d)
+            self.ev_up[k].record(self.s_h2d)
+            self.s_run.wait_event(self.ev_up[k])
+            if not self.first:
+                self.s_run.wait_event(self.ev_down[k])             # the previous pass's download of these buffers
+            for i, r in enumerate(rounds):
+                if r.kind == k:
+                    B.etc_migrate_round(plan, i, self.src_tab, self.dst_tab, self.staging, stream=self.s_run)
+            self.ev_run[k].record(self.s_run)
+            self.s_d2h.wait_event(self.ev_run[k])
+            with torch.cuda.stream(self.s_d2h):
+                for (n, kk), t in self.d_dst.items():
+                    if kk == k:
+                        self.h_dst[(n, kk)].copy_(t, non_blocking=True)
+            self.ev_down[k].record(self.s_d2h)
+        self.done.record(self.s_d2h)
         self.first = False
         self.plan = plan
         return plan

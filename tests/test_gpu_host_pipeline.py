@@ -93,3 +93,83 @@ def test_chunked_migration_releases_and_matches(E, name):
     for k in sorted(on.kinds()):
         live += per_kind_new[k]; peak = max(peak, live); live -= per_kind_old[k]
     assert info["peak_live_bytes"] == peak
+
+
+@pytest.mark.parametrize("name", ["c1", "s2", "s3", "s4", "s5"])
+def test_host_migration_uploads_only_what_the_plan_reads(E, name):
+    """etc_upload_sources: the device copies of the old shards start poisoned and only the regions the plan's slices
+    read are uploaded; the new shards still equal the oracle's, and the bytes that crossed PCIe are bounded below by
+    the number of DISTINCT source elements the oracle's source rule reads (counted from O.source_of alone) and above by
+    the whole old state."""
+    from paper_2607_04749_b200.host_pipeline import HostMigration
+    w = workload(name)
+    model = w["model"]
+    oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
+    payloads = [shard_all(oo, make_logical(model, w["seed"] + i, "stamp" if i == 0 else "values")) for i in range(2)]
+    h_src = _pinned(payloads[0])
+    h_dst = {(n, k): torch.full((on.buffer_elems(n, k) * on.elem_bytes(k),), 0x77, dtype=torch.uint8).pin_memory()
+             for n in range(on.n_dev) for k in on.kinds() if on.buffer_elems(n, k)}
+    old = E.etc_layout_create(model, w["old"])
+    d_src = E.alloc_buffers(old, fill=0xEE)
+    hm = HostMigration(model, w["old"], w["new"], h_src, h_dst, max_staging_bytes=1 << 22, d_src=d_src, needed_only=True)
+    for i in range(2):
+        for key, a in payloads[i].items():
+            if a.shape[0]:
+                h_src[key].numpy()[:] = a.view(np.uint8)
+        plan = hm.run()
+        torch.cuda.synchronize()
+        new = E.etc_layout_create(model, w["new"])
+        ov, _, _ = E.etc_cost_matrix(old, new)
+        dm = E.etc_sketch(ov)[0].cpu().numpy()
+        exp, T, _ = O.migrate(oo, on, dm, payloads[i])
+        assert np.array_equal(plan.traffic(), T)
+        for key, e in exp.items():
+            if e.shape[0]:
+                assert np.array_equal(h_dst[key].numpy().view(e.dtype), e), (i, key)
+    distinct = 0
+    for k in on.kinds():
+        seen = {o: np.zeros(oo.buffer_elems(o, k), bool) for o in range(oo.n_dev)}
+        for n in range(on.n_dev):
+            cnt = on.buffer_elems(n, k)
+            if cnt:
+                sd, sl = O.source_of(oo, on, dm, n, k, np.arange(cnt))
+                for o in np.unique(sd):
+                    seen[int(o)][sl[sd == o]] = True
+        distinct += sum(int(v.sum()) for v in seen.values()) * on.elem_bytes(k)
+    total_old = sum(a.nbytes for a in payloads[0].values())
+    assert distinct <= hm.h2d_bytes <= total_old, (distinct, hm.h2d_bytes, total_old)
+    print(f"{name}: uploaded {hm.h2d_bytes} of {total_old} old bytes; distinct source bytes {distinct}")
+    if name in ("s2", "s3", "s5"):
+        assert hm.h2d_bytes == distinct
+
+
+@pytest.mark.parametrize("name", ["c1", "s2", "s3", "s4", "s4odd", "s5"])
+@pytest.mark.parametrize("flags", [0, 1])
+def test_host_migration_zero_copy(E, name, flags):
+    """zero_copy=True: the pinned host shards are the source and destination tables of the copy kernels; there is no
+    device copy of any shard.  New shards equal the oracle's; h2d / d2h byte counts are the payload."""
+    from paper_2607_04749_b200.host_pipeline import HostMigration
+    w = workload(name)
+    model = w["model"]
+    oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
+    payloads = [shard_all(oo, make_logical(model, w["seed"] + i, "stamp" if i == 0 else "values")) for i in range(2)]
+    h_src = _pinned(payloads[0])
+    h_dst = {(n, k): torch.full((on.buffer_elems(n, k) * on.elem_bytes(k),), 0x77, dtype=torch.uint8).pin_memory()
+             for n in range(on.n_dev) for k in on.kinds() if on.buffer_elems(n, k)}
+    before = torch.cuda.memory_allocated()
+    hm = HostMigration(model, w["old"], w["new"], h_src, h_dst, max_staging_bytes=4 * 65536, flags=flags, zero_copy=True)
+    assert torch.cuda.memory_allocated() - before <= 4 * 65536 + 4096      # only the staging buffer lives on the device
+    for i in range(2):
+        for key, a in payloads[i].items():
+            if a.shape[0]:
+                h_src[key].numpy()[:] = a.view(np.uint8)
+        plan = hm.run()
+        torch.cuda.synchronize()
+        old, new = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])
+        dm = E.etc_sketch(E.etc_cost_matrix(old, new)[0])[0].cpu().numpy()
+        exp, T, _ = O.migrate(oo, on, dm, payloads[i])
+        assert np.array_equal(plan.traffic(), T)
+        for key, e in exp.items():
+            if e.shape[0]:
+                assert np.array_equal(h_dst[key].numpy().view(e.dtype), e), (i, key)
+    assert hm.h2d_bytes == int(T.sum()) == hm.d2h_bytes
