@@ -198,6 +198,11 @@ typedef struct {
   int32_t pad;
 } etc_slice;
 etc_status etc_plan_get_slices(const etc_plan* plan, int32_t which, etc_slice* h_out);
+/* Bounds check of a finished plan, on the device: counts the copy work items whose source, destination or staging
+ * extent does not lie inside the buffer it addresses (sizes from the layouts the plan was made from), or whose declared
+ * access width does not divide its addresses.  *n_bad (HOST) = 0 for every plan this library makes; a debugging and
+ * test aid (one thread per work item, synchronises `stream`). */
+etc_status etc_plan_validate(const etc_plan* plan, int64_t* n_bad, void* stream);
 /* The zero-fill descriptors (reading A31) as etc_slice records with no source: src_dev = -1, src_off = stg_off = -1,
  * src_stride = 0; h_out must hold etc_plan_stats.n_fills entries (order unspecified).  Copied to HOST memory. */
 etc_status etc_plan_get_fills(const etc_plan* plan, etc_slice* h_out);

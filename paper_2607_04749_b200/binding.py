@@ -24,7 +24,7 @@ EXPORTED_SYMBOLS = (
     "etc_migrate_phase",
     "etc_status_string", "etc_last_error_detail", "etc_kernel_launches", "etc_defrag",
     "etc_plan_set_rounds", "etc_plan_get_round", "etc_migrate_round", "etc_plan_create_failed", "etc_mask_failed",
-    "etc_upload_sources",
+    "etc_upload_sources", "etc_plan_validate",
 )
 
 
@@ -94,6 +94,7 @@ def lib():
         L.etc_plan_get_traffic.restype = i32; L.etc_plan_get_traffic.argtypes = [vp, vp]
         L.etc_plan_get_slices.restype = i32; L.etc_plan_get_slices.argtypes = [vp, i32, vp]
         L.etc_plan_get_fills.restype = i32; L.etc_plan_get_fills.argtypes = [vp, vp]
+        L.etc_plan_validate.restype = i32; L.etc_plan_validate.argtypes = [vp, C.POINTER(i64), vp]
         L.etc_migrate.restype = i32; L.etc_migrate.argtypes = [vp, vp, vp, vp, vp]
         L.etc_migrate_phase.restype = i32; L.etc_migrate_phase.argtypes = [vp, vp, vp, vp, i32, vp]
         L.etc_plan_set_rounds.restype = i32; L.etc_plan_set_rounds.argtypes = [vp, i64, C.POINTER(i32), vp]
@@ -272,6 +273,12 @@ class Plan:
         arr = np.zeros(max(n, 1), dt)
         _check(lib().etc_plan_get_slices(self.h, which, arr.ctypes.data))
         return arr[:n]
+
+    def validate(self, stream=None) -> int:
+        """device-side bounds check of every copy work item; returns the number of bad ones (0 for a sound plan)"""
+        n = C.c_int64(-1)
+        _check(lib().etc_plan_validate(self.h, C.byref(n), _stream(stream)))
+        return int(n.value)
 
     def fills(self):
         """zero-fill descriptors (reading A31) as etc_slice records with src_dev = -1."""

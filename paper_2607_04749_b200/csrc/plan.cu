@@ -398,6 +398,29 @@ plan_chunks_kernel(const etc_slice* __restrict__ slices, const int64_t* __restri
   out[c] = ch;
 }
 
+// Bounds check of the finished plan (a safety net of our own: compute-sanitizer is not available everywhere): every
+// chunk's source, destination and staging extent must lie inside the buffer it addresses.  One thread per chunk.
+__global__ void __launch_bounds__(256)
+plan_validate_kernel(const Chunk* __restrict__ ch, long long n, int staged, const int64_t* __restrict__ old_bytes,
+                     const int64_t* __restrict__ new_bytes, int64_t staging_bytes, unsigned long long* __restrict__ bad) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const Chunk c = ch[i];
+  const int64_t span_src = (int64_t)(c.nrows - 1) * c.src_stride + c.row_bytes;
+  const int64_t span_dst = (int64_t)(c.nrows - 1) * c.dst_stride + c.row_bytes;
+  bool ok = c.nrows >= 1 && c.row_bytes >= 1 && (int64_t)c.nrows * c.row_bytes <= ETC_CHUNK_BYTES;
+  ok = ok && c.src_off >= 0 && c.src_off + span_src <= old_bytes[c.src_buf];
+  ok = ok && c.dst_off >= 0 && c.dst_off + span_dst <= new_bytes[c.dst_buf];
+  ok = ok && (c.nrows == 1 || (c.src_stride >= c.row_bytes && c.dst_stride >= c.row_bytes));
+  if (staged) ok = ok && c.stg_off >= 0 && c.stg_off + (int64_t)c.nrows * c.row_bytes <= staging_bytes;
+  if (c.vec > 1) {
+    int64_t al = c.src_off | c.dst_off | c.row_bytes | (staged ? c.stg_off : 0);
+    if (c.nrows > 1) al |= (int64_t)c.src_stride | (int64_t)c.dst_stride;
+    ok = ok && (al & (c.vec - 1)) == 0;
+  }
+  if (!ok) atomicAdd(bad, 1ull);
+}
+
 }  // namespace etc
 
 using namespace etc;
@@ -590,4 +613,37 @@ extern "C" etc_status etc_plan_get_fills(const etc_plan* pl, etc_slice* h_out) {
   ETC_CUDA_TRY(cudaStreamSynchronize(pl->stream_created_on));
   if (pl->totals.n_fills) ETC_CUDA_TRY(cudaMemcpy(h_out, pl->d_fills, sizeof(etc_slice) * (size_t)pl->totals.n_fills, cudaMemcpyDeviceToHost));
   return ETC_OK;
+}
+
+extern "C" etc_status etc_plan_validate(const etc_plan* pl, int64_t* n_bad, void* stream) {
+  clear_error_detail();
+  if (!pl || !n_bad) return ETC_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  pl->streams.note(st);
+  const size_t ns = pl->old_bytes.size(), nd = pl->new_bytes.size();
+  int64_t* d_sizes = nullptr;
+  ETC_CUDA_TRY(cudaMallocAsync(&d_sizes, sizeof(int64_t) * (ns + nd + 1), st));
+  auto done = [&](etc_status rc) { cudaFreeAsync(d_sizes, st); return rc; };
+#define VAL_TRY(expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) { set_error_detail(#expr, _e); return done(ETC_ERR_CUDA); } } while (0)
+  VAL_TRY(cudaMemcpyAsync(d_sizes, pl->old_bytes.data(), sizeof(int64_t) * ns, cudaMemcpyHostToDevice, st));
+  VAL_TRY(cudaMemcpyAsync(d_sizes + ns, pl->new_bytes.data(), sizeof(int64_t) * nd, cudaMemcpyHostToDevice, st));
+  unsigned long long* d_bad = reinterpret_cast<unsigned long long*>(d_sizes + ns + nd);
+  VAL_TRY(cudaMemsetAsync(d_bad, 0, sizeof(unsigned long long), st));
+  const PlanTotals& t = pl->totals;
+  if (t.n_chunks_staged) {
+    plan_validate_kernel<<<(unsigned)((t.n_chunks_staged + 255) / 256), 256, 0, st>>>(pl->d_ch_staged, t.n_chunks_staged, 1, d_sizes,
+                                                                                     d_sizes + ns, t.staging_bytes, d_bad);
+    VAL_TRY(cudaGetLastError()); count_launch();
+  }
+  if (t.n_chunks_local) {
+    plan_validate_kernel<<<(unsigned)((t.n_chunks_local + 255) / 256), 256, 0, st>>>(pl->d_ch_local, t.n_chunks_local, 0, d_sizes,
+                                                                                    d_sizes + ns, t.staging_bytes, d_bad);
+    VAL_TRY(cudaGetLastError()); count_launch();
+  }
+  unsigned long long h_bad = 0;
+  VAL_TRY(cudaMemcpyAsync(&h_bad, d_bad, sizeof(h_bad), cudaMemcpyDeviceToHost, st));
+  VAL_TRY(cudaStreamSynchronize(st));
+#undef VAL_TRY
+  *n_bad = (int64_t)h_bad;
+  return done(ETC_OK);
 }

@@ -30,6 +30,7 @@ def run_gpu_migration(w_model, old_cfg, new_cfg, src_np: dict, device_map=None, 
         dm = torch.tensor(np.asarray(device_map, np.int32)).cuda()
         lb = None
     plan = E.etc_plan_create(old, new, dm, flags)
+    assert plan.validate() == 0                    # every work item inside its buffers (device-side bounds check)
     src = upload(src_np) if src_np is not None else None
     dst = E.alloc_buffers(new, fill=poison)
     staging = torch.full((max(plan.stats.staging_bytes, 16),), poison, dtype=torch.uint8, device="cuda")

@@ -47,6 +47,7 @@ def _run(E, name, flags, poison_runs):
     assert np.array_equal(ov.cpu().numpy(), o_ov) and np.array_equal(need.cpu().numpy(), o_need)
     assert int(lb.item()) == O.sketch_hungarian(o_ov)[1]
     plan = E.etc_plan_create(old, new, dm, flags)
+    assert plan.validate() == 0
     st = plan.stats
     dmap = dm.cpu().numpy()
     T = plan.traffic()
