@@ -2,6 +2,7 @@
 // Nothing here is shared with oracle/ (the CPU oracle is written separately from the paper).
 #pragma once
 #include <cstdint>
+#include <mutex>
 #include <vector>
 #include <cuda_runtime.h>
 #include "../../include/etc.h"
@@ -95,6 +96,11 @@ void set_error_detail(const char* what, cudaError_t e);
 void clear_error_detail();
 void count_launch(int n = 1);
 int current_device();
+// xfer.cu: metadata transfers as kernels on the caller's stream, so that they never queue behind bulk DMA transfers
+cudaError_t write_small(void* d_dst, const void* h_src, size_t bytes, cudaStream_t st);      // host -> device via kernel parameters
+cudaError_t copy_by_kernel(void* dst, const void* src, size_t bytes, cudaStream_t st);       // device / pinned host, either way
+std::mutex& pinned_scratch_mutex();                   // hold it while the scratch is in use
+void* pinned_scratch(size_t bytes);                   // grow-only pinned buffer (nullptr on failure)
 }
 #define ETC_CUDA_TRY(expr)                                          \
   do {                                                              \

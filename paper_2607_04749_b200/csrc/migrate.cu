@@ -220,8 +220,13 @@ static etc_status launch_migrate(const etc_plan* pl, const void* const* src_bufs
   ETC_CUDA_TRY(copy_kernel_attrs());
   pl->streams.note(st);
   // pointer tables: source pointers then destination pointers
-  ETC_CUDA_TRY(cudaMemcpyAsync(d_ptrs, src_bufs, sizeof(void*) * ns, cudaMemcpyHostToDevice, st));
-  ETC_CUDA_TRY(cudaMemcpyAsync(d_ptrs + ns, dst_bufs, sizeof(void*) * nd, cudaMemcpyHostToDevice, st));
+  // (as kernel parameters, not as DMA copies: a copy would queue behind bulk transfers pending in the copy engines)
+  {
+    std::vector<const void*> both(ns + nd);
+    for (size_t i = 0; i < ns; ++i) both[i] = src_bufs[i];
+    for (size_t i = 0; i < nd; ++i) both[ns + i] = dst_bufs[i];
+    ETC_CUDA_TRY(write_small(d_ptrs, both.data(), sizeof(void*) * (ns + nd), st));
+  }
   const void* const* d_src = d_ptrs; void* const* d_dst = d_ptrs + ns;
   char* stg = static_cast<char*>(staging) - stg_base;          // chunk records carry offsets of the full staging layout
   if ((phases & ETC_PHASE_PACK) && nA + nB > 0) {

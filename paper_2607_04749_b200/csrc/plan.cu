@@ -496,13 +496,14 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
   pl->d_blocks = reinterpret_cast<BlockCount*>(ws + o_blocks); pl->d_traffic = reinterpret_cast<int64_t*>(ws + o_traffic);
   pl->d_totals = reinterpret_cast<PlanTotals*>(ws + o_totals); pl->d_map = reinterpret_cast<int32_t*>(ws + o_map);
   pl->d_ptrs = reinterpret_cast<void**>(ws + o_ptrs);
-  PLAN_TRY(cudaMemcpyAsync(pl->d_map, device_map, sizeof(int32_t) * (size_t)n_new,
-                           on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+  // metadata moves as kernels on `st`, never through the copy engines (xfer.cu)
+  if (on_device) PLAN_TRY(copy_by_kernel(pl->d_map, device_map, sizeof(int32_t) * (size_t)n_new, st));
+  else PLAN_TRY(write_small(pl->d_map, device_map, sizeof(int32_t) * (size_t)n_new, st));
   PLAN_TRY(cudaMemsetAsync(pl->d_units, 0, sizeof(UnitCount) * (size_t)U, st));
   const uint8_t* d_failed = nullptr;
   if (failed) {                                                 // reading A26: host or device mask [n_old]
-    PLAN_TRY(cudaMemcpyAsync(ws + o_failed, failed, (size_t)n_old,
-                             on_device_ptr(failed) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+    if (on_device_ptr(failed)) PLAN_TRY(copy_by_kernel(ws + o_failed, failed, (size_t)n_old, st));
+    else PLAN_TRY(write_small(ws + o_failed, failed, (size_t)n_old, st));
     d_failed = reinterpret_cast<const uint8_t*>(ws + o_failed);
   }
 
@@ -521,7 +522,7 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
     PLAN_TRY(cudaGetLastError());
     count_launch();
   }
-  PLAN_TRY(cudaMemcpyAsync(h_tot, pl->d_totals, sizeof(PlanTotals), cudaMemcpyDeviceToHost, st));
+  PLAN_TRY(copy_by_kernel(h_tot, pl->d_totals, sizeof(PlanTotals), st));      // h_tot is pinned: the kernel writes it
   PLAN_TRY(cudaStreamSynchronize(st));                          // the one host sync: sizes must come back
   pl->totals = *h_tot;
   if (pl->totals.bad_map) return fail(ETC_ERR_BAD_MAP);

@@ -13,6 +13,7 @@
 // Window boundaries are found independently per round by binary search over the (monotone) staging offsets of the
 // chunk table: one CTA per round, which then reduces the round's payload bytes.
 #include <algorithm>
+#include <cstring>
 #include <vector>
 #include "etc_internal.h"
 #include "plan_types.h"
@@ -101,15 +102,24 @@ extern "C" etc_status etc_plan_set_rounds(etc_plan* pl, int64_t max_staging_byte
   ETC_CUDA_TRY(cudaMallocAsync(&pl->d_rounds_ws, bytes, st));
   char* ws = static_cast<char*>(pl->d_rounds_ws);
   pl->d_round_ptrs = reinterpret_cast<void**>(ws + o_ptrs);
-  ETC_CUDA_TRY(cudaMemcpyAsync(ws + o_specs, specs.data(), sizeof(RoundSpec) * R, cudaMemcpyHostToDevice, st));
+  // metadata moves as kernels on `st` while it is small (xfer.cu); a very long round list falls back to DMA copies
+  const bool small = R <= 512;
+  if (small) ETC_CUDA_TRY(write_small(ws + o_specs, specs.data(), sizeof(RoundSpec) * R, st));
+  else ETC_CUDA_TRY(cudaMemcpyAsync(ws + o_specs, specs.data(), sizeof(RoundSpec) * R, cudaMemcpyHostToDevice, st));
   plan_rounds_kernel<<<(unsigned)R, 256, 0, st>>>(pl->d_ch_staged, pl->d_ch_local,
                                                   reinterpret_cast<const RoundSpec*>(ws + o_specs),
                                                   reinterpret_cast<RoundRec*>(ws + o_recs));
   ETC_CUDA_TRY(cudaGetLastError());
   count_launch();
   std::vector<RoundRec> got(R);
-  ETC_CUDA_TRY(cudaMemcpyAsync(got.data(), ws + o_recs, sizeof(RoundRec) * R, cudaMemcpyDeviceToHost, st));
-  ETC_CUDA_TRY(cudaStreamSynchronize(st));                     // plan-time: round sizes must come back to the host
+  {
+    std::lock_guard<std::mutex> lock(pinned_scratch_mutex());
+    void* pin = small ? pinned_scratch(sizeof(RoundRec) * R) : nullptr;
+    if (pin) ETC_CUDA_TRY(copy_by_kernel(pin, ws + o_recs, sizeof(RoundRec) * R, st));
+    else ETC_CUDA_TRY(cudaMemcpyAsync(got.data(), ws + o_recs, sizeof(RoundRec) * R, cudaMemcpyDeviceToHost, st));
+    ETC_CUDA_TRY(cudaStreamSynchronize(st));                   // plan-time: round sizes must come back to the host
+    if (pin) memcpy(got.data(), pin, sizeof(RoundRec) * R);
+  }
   for (size_t i = 0; i < R; ++i) { got[i].kind = recs[i].kind; got[i].sub = recs[i].sub; got[i].n_sub = recs[i].n_sub; }
   pl->rounds = std::move(got);
   return ETC_OK;
