@@ -113,3 +113,35 @@ def resize_logical(logical: dict, lts_to) -> dict:
             new.append(b)
         out[k] = new
     return out
+
+
+def random_variant_case(rng, max_devices=12):
+    """A random tiny (model, old cfg, new cfg) drawing on EVERY layout variant at once (both styles, GQA ratios, both QKV
+    row orders, KV-head replication, tied / untied, uneven pipeline splits, distributed optimizer with and without
+    alignment, padded and unpadded vocabularies, any subset of state kinds), both configurations valid for the oracle."""
+    while True:
+        n_kv = int(rng.choice([1, 2, 4])); qpg = int(rng.choice([1, 2, 4]))
+        style = int(rng.integers(0, 2))
+        model = dict(style=style, n_layers=int(rng.choice([2, 3, 4, 6])), hidden=int(rng.choice([8, 12])),
+                     n_q_heads=n_kv * qpg, n_kv_heads=n_kv, head_dim=int(rng.choice([2, 3])),
+                     ffn_hidden=int(rng.choice([16, 24])), vocab=int(rng.choice([8, 11, 13, 16])),
+                     max_pos=int(rng.choice([0, 5])) if style == 0 else 0, tied=int(rng.integers(0, 2)),
+                     param_bytes=int(rng.choice([2, 4])), kinds=int(rng.integers(1, 16)), qkv_order=int(rng.integers(0, 2)))
+        cfgs = []
+        for _ in range(2):
+            pp = int(rng.choice([1, 2, 3]))
+            c = dict(tp=int(rng.choice([1, 2, 4, 8])), pp=pp, dp=int(rng.choice([1, 2, 3])), dist_opt=int(rng.integers(0, 2)),
+                     pp_first=0, pp_last=0, dist_opt_align=int(rng.choice([0, 0, 8, 24])),
+                     vocab_divisor=int(rng.choice([0, 0, 1, 3, 4])))
+            if pp >= 2 and rng.integers(0, 3) == 0:
+                c["pp_first"] = int(rng.integers(1, 3))
+            if pp >= 2 and rng.integers(0, 4) == 0:
+                c["pp_last"] = int(rng.integers(1, 3))
+            cfgs.append(c)
+        if any(c["tp"] * c["pp"] * c["dp"] > max_devices for c in cfgs):
+            continue
+        try:
+            O.Layout(model, cfgs[0]); O.Layout(model, cfgs[1])
+        except O.OracleError:
+            continue
+        return model, cfgs[0], cfgs[1]

@@ -34,7 +34,7 @@ def _survivable_mask(cfg, rng):
 
 def _run(E, model, old_c, new_c, f, seed, flags=0, device_map=None, avoid_failed=True, payload="stamp"):
     oo, on = O.Layout(model, old_c), O.Layout(model, new_c)
-    src_np = stamp_all(oo) if payload == "position" else shard_all(oo, make_logical(model, seed, payload))
+    src_np = stamp_all(oo) if payload == "position" else shard_all(oo, make_logical(model, seed, payload, lts=oo.logical_tensors()))
     for key in src_np:                                   # the failed devices' state is lost
         if f[key[0]]:
             src_np[key] = np.full_like(src_np[key], 0xDEAD)
@@ -149,3 +149,36 @@ def test_dp_growth_round_robin_balance_on_device(E):
     ov, _, _ = E.etc_cost_matrix(g["old"], g["new"])
     _, lb = E.etc_sketch(ov)
     assert int(lb.item()) == int(g["hold"][:8].sum())
+
+
+@pytest.mark.parametrize("seed", range(3))
+def test_failures_with_every_layout_variant(E, seed):
+    """Failure masks on random reconfigurations that draw on every layout variant at once (helpers.random_variant_case):
+    the device either reproduces the oracle's result bit for bit or reports the same ETC_ERR_UNRECOVERABLE."""
+    from helpers import random_variant_case
+    rng = np.random.default_rng(6000 + seed)
+    done = unrec = 0
+    while done - unrec < 5:                                  # five recoverable cases per seed, plus the unrecoverable ones met on the way
+        m, a, b = random_variant_case(rng)
+        if a["dp"] < 2:
+            continue
+        f = _survivable_mask(a, rng)
+        if not f.any():
+            continue
+        na, nb = a["tp"] * a["pp"] * a["dp"], b["tp"] * b["pp"] * b["dp"]
+        dm = rng.permutation(max(na, nb))[:nb].astype(np.int32)
+        oo, on = O.Layout(m, a), O.Layout(m, b)
+        oo.set_failed(f)
+        try:
+            O.migrate(oo, on, dm, None)
+        except O.OracleError as oe:
+            assert oe.code == -8
+            old, new = E.etc_layout_create(m, a), E.etc_layout_create(m, b)
+            with pytest.raises(E.EtcError) as ge:
+                E.etc_plan_create(old, new, dm, failed=f)
+            assert ge.value.code == -8
+            unrec += 1; done += 1
+            continue
+        _run(E, m, a, b, f, 6100 + done, flags=int(rng.integers(0, 2)), device_map=dm)
+        done += 1
+    print("unrecoverable cases:", unrec)

@@ -123,3 +123,20 @@ def test_padding_validation_codes_match_oracle(E):
             E.etc_layout_create(m, cfg)
         assert ge.value.code == oe.value.code
     assert E.etc_layout_create(m, _cfg(2, div=1)).buffer_bytes(0, 1) == O.Layout(m, _cfg(2, div=1)).buffer_elems(0, 1) * 4
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_all_variants_combined_random_sweep(E, seed):
+    """Every layout variant at once (helpers.random_variant_case): 10 random reconfigurations per seed through the whole
+    CUDA path against the oracle, optimal and random device maps, LOCAL_DIRECT and ALL_STAGED | KIND_MAJOR."""
+    from helpers import random_variant_case
+    rng = np.random.default_rng(4000 + seed)
+    filled = 0
+    for i in range(10):
+        m, a, b = random_variant_case(rng)
+        na, nb = a["tp"] * a["pp"] * a["dp"], b["tp"] * b["pp"] * b["dp"]
+        _, f = _check(E, m, a, b, 5000 + 100 * seed + i, flags=int(rng.choice([0, 1, 2, 3])))
+        dm = rng.permutation(max(na, nb))[:nb].astype(np.int32)
+        _, f2 = _check(E, m, a, b, 5050 + 100 * seed + i, device_map=dm, payload="values")
+        filled += (f > 0) + (f2 > 0)
+    print("cases with zero-fill:", filled)

@@ -11,7 +11,8 @@ import pytest
 from etc_inputs.workloads import STYLE_GPT, STYLE_LLAMA
 from etc_inputs import position_stamp
 from oracle import oracle as O
-from helpers import read_golden, make_logical, shard_all, stamp_all, reassemble, resize_logical, replication_factor
+from helpers import (read_golden, make_logical, shard_all, stamp_all, reassemble, resize_logical, replication_factor,
+                     replication_map, random_variant_case)
 
 GOLD = read_golden("vocab_padding_handcomputed.txt")
 
@@ -82,10 +83,11 @@ def check_padded_reconfiguration(model, old_cfg, new_cfg, seed, device_map=None)
     def weighted(mine, dev, other, lts_other):
         tot = 0
         for k in mine.kinds():
-            lt, _, row, _c = mine.global_of(dev, k)
+            lt, _, row, col = mine.global_of(dev, k)
             for t in np.unique(lt):
                 sel = (lt == t) & (row < lts_other[t][0])
-                tot += int(sel.sum()) * replication_factor(other, k, lts_other[t][2], int(t)) * O.kind_bytes(model, k)
+                R = replication_map(other, k, lts_other, int(t))          # per element: KV-head replication varies it
+                tot += int(R[row[sel], col[sel]].sum()) * O.kind_bytes(model, k)
         return tot
     for n in range(new.n_dev):
         assert ov[n].sum() == weighted(new, n, old, lts_o)
@@ -105,7 +107,7 @@ def check_padded_reconfiguration(model, old_cfg, new_cfg, seed, device_map=None)
     for k in logical_n:
         for t in range(len(lts_n)):
             assert np.array_equal(rebuilt[k][t], logical_n[k][t]), ("P4", k, t)
-            assert (cover[k][t] == replication_factor(new, k, lts_n[t][2], t)).all()
+            assert np.array_equal(cover[k][t], replication_map(new, k, lts_n, t))
     # --- fill: counted from global_of alone (elements of embedding tensors whose row lies beyond the old padded rows)
     for n in range(new.n_dev):
         want = 0
@@ -191,3 +193,15 @@ def test_padding_validation():
         O.Layout(m, _cfg(2, div=-1))
     assert e.value.code == -1
     assert O.Layout(m, _cfg(2, div=1)).n_dev == 2               # divisor 1: pad to a multiple of tp only
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_all_variants_combined_random_sweep(seed):
+    """Every layout variant at once (helpers.random_variant_case): the whole battery on 12 random reconfigurations per
+    seed with optimal and random device maps."""
+    rng = np.random.default_rng(3000 + seed)
+    for i in range(12):
+        m, a, b = random_variant_case(rng, max_devices=8)
+        check_padded_reconfiguration(m, a, b, 2000 + 100 * seed + i)
+        na, nb = a["tp"] * a["pp"] * a["dp"], b["tp"] * b["pp"] * b["dp"]
+        check_padded_reconfiguration(m, a, b, 2050 + 100 * seed + i, device_map=rng.permutation(max(na, nb))[:nb].astype(np.int32))
