@@ -163,6 +163,31 @@ def oracle_sample(w, budget_elems=6_000_000, threads=1):
                 elems_per_buffer=m, n_buffers=len(bufs), local_opt=val, threads=O.max_threads(), migrate_threads=threads)
 
 
+def oracle_metadata(w):
+    """CPU side of cost matrix + sketch on the full layout of workload w: the oracle's plain range-overlap routine, its
+    plain O(k^3) Hungarian, and (where SciPy is installed) linear_sum_assignment, the routine the paper itself calls
+    (PAPER.md:134)."""
+    from oracle import oracle as O
+    oo, on = O.Layout(w["model"], w["old"]), O.Layout(w["model"], w["new"])
+    O.overlap(oo, on, method="ranges")                      # untimed: starts the OpenMP thread pool
+    t0 = time.perf_counter()
+    ov, need, hold = O.overlap(oo, on, method="ranges")
+    t1 = time.perf_counter()
+    dm, val = O.sketch_hungarian(ov)
+    t2 = time.perf_counter()
+    out = {"devices": [oo.n_dev, on.n_dev], "cost_matrix_ms": (t1 - t0) * 1e3, "cost_matrix_threads": O.max_threads(),
+           "hungarian_ms": (t2 - t1) * 1e3, "local_bytes": int(val)}
+    try:
+        from scipy.optimize import linear_sum_assignment
+        t3 = time.perf_counter()
+        r, c = linear_sum_assignment(ov, maximize=True)
+        out["scipy_linear_sum_assignment_ms"] = (time.perf_counter() - t3) * 1e3
+        out["scipy_agrees"] = bool(int(ov[r, c].sum()) == int(val))
+    except ImportError:
+        pass
+    return out
+
+
 def run_reference(args, w):
     rank, _, world = dist_env()
     if rank != 0:
@@ -359,6 +384,11 @@ def run_cuda(args, w):
                 "single_thread_value": 2 * o1["payload_bytes"] / o1["migrate_s"] / 1e9,
                 "single_thread_sample": f"first {o1['elems_per_buffer']} elements of each buffer, 1 thread",
                 "cost_matrix_ms": o["cost_ms"], "sketch_ms": o["sketch_ms"], "cost_matrix_threads": o["threads"]}
+            try:
+                from etc_inputs import workload as _wl
+                line["cpu_baseline"]["metadata"] = {w["name"]: oracle_metadata(w), "c5b": oracle_metadata(_wl("c5b"))}
+            except Exception as ex:
+                line["cpu_baseline"]["metadata"] = {"error": repr(ex)[:200]}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

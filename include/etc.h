@@ -1,6 +1,6 @@
 /*
  * etc.h — C ABI of libetc.so: the data-parallel hot path of ETC's checkpoint-free model-state migration
- * (arxiv/paper_2607_04749, "ETC"; citations below are PAPER.md line numbers and DESIGN.md readings A1-A24).
+ * (arxiv/paper_2607_04749, "ETC"; citations below are PAPER.md line numbers and DESIGN.md readings A1-A31).
  *
  * The paper's primitive takes the previous parallel configuration, the current one and the model state, and
  * returns the migrated state.  Here that is four steps, each a call:
