@@ -356,7 +356,7 @@ plan_fills_kernel(DeviceTables newT, const int32_t* __restrict__ device_map, int
   f.src_off = -1; f.stg_off = -1; f.src_stride = 0; f.src_dev = -1; f.pad = 0;
   f.dst_off = q.boff + (int64_t)(r0 - q.r0) * q.W * es;
   f.row_bytes = (int64_t)q.nc * es; f.dst_stride = q.W * es; f.nrows = r1 - r0;
-  if (f.nrows > 1 && f.row_bytes == f.dst_stride) { f.row_bytes *= f.nrows; f.nrows = 1; }
+  if (f.nrows > 1 && f.row_bytes == f.dst_stride && f.row_bytes * f.nrows < (1ll << 31)) { f.row_bytes *= f.nrows; f.nrows = 1; }   // the fill kernel counts a row in 32 bits
   f.dst_rank = q.dev; f.dst_phys = device_map[q.dev]; f.kind = kind;
   const unsigned long long slot = atomicAdd(reinterpret_cast<unsigned long long*>(&totals->n_fills), 1ull);
   fills[slot] = f;
