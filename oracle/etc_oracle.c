@@ -467,6 +467,23 @@ int32_t orc_overlap_elementwise(const orc_layout* Lo, const orc_layout* Ln, int3
   return ORC_OK;
 }
 
+/* The paper's own treatment of DP ("DP Dimension"; reading A5): "we isolate the PP/TP processes
+ * under different DP ranks.  If two processes have different DP ranks, even if their workloads on PP/TP are the same, we
+ * regard the difference between the workloads to be infinite."  In the overlap form used here: a new rank and an old
+ * device with different DP ranks share nothing that counts, so their cell is zero and the sketch never keeps bytes
+ * local across DP groups.  Device id = r + tp*(d + dp*s) (A9).  Applied in place to overlap [n_new][P]. */
+int32_t orc_mask_cross_dp(const orc_layout* Lo, const orc_layout* Ln, int64_t* overlap) {
+  int no = orc_num_devices(Lo), nn = orc_num_devices(Ln), P = no > nn ? no : nn;
+  for (int n = 0; n < nn; n++) {
+    int dn, sn, rn; orc_coords(Ln, n, &dn, &sn, &rn);
+    for (int o = 0; o < no; o++) {
+      int dd, so, ro; orc_coords(Lo, o, &dd, &so, &ro);
+      if (dd != dn) overlap[(size_t)n * P + o] = 0;
+    }
+  }
+  return ORC_OK;
+}
+
 /* Second, separately written routine for layouts too large for element enumeration (config 5b): per pair of
  * tensor shards, count common elements row by row from the row/column ranges and the held flat ranges.
  * Validated against orc_overlap_elementwise on the tiny sweeps and on configs 1-2 (tests). */

@@ -210,6 +210,17 @@ def overlap(old: Layout, new: Layout, only_layers: bool = False, method: str = "
     return ov, need, hold
 
 
+def mask_cross_dp(old: Layout, new: Layout, ov: np.ndarray) -> np.ndarray:
+    """The paper's DP isolation (reading A5): a copy of `ov` with every cross-DP cell zeroed."""
+    out = np.ascontiguousarray(ov, np.int64).copy()
+    lib().orc_mask_cross_dp.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    lib().orc_mask_cross_dp.restype = C.c_int32
+    rc = lib().orc_mask_cross_dp(old.h, new.h, _ptr(out))
+    if rc:
+        raise OracleError(rc)
+    return out
+
+
 def sketch_bruteforce(ov: np.ndarray, avail=None):
     ov = np.ascontiguousarray(ov, np.int64)
     n, P = ov.shape
