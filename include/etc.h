@@ -170,6 +170,12 @@ etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_layout* new
 etc_status etc_mask_failed(int64_t* d_overlap, int64_t* d_hold, int32_t n_new, int32_t n_old, int32_t P,
                            const uint8_t* d_failed, void* stream);
 
+/* The paper's own treatment of the DP dimension ("we isolate the PP/TP processes under different DP
+ * ranks ... the difference between the workloads to be infinite"; reading A5 explains why the default matrix
+ * spans all DP x PP x TP devices instead): zero, in place, every cell of d_overlap [n_new][P] whose new rank and old
+ * device have different DP ranks, so that etc_sketch keeps no bytes local across DP groups.  Enqueues on `stream`. */
+etc_status etc_mask_cross_dp(const etc_layout* old_l, const etc_layout* new_l, int64_t* d_overlap, void* stream);
+
 typedef struct {
   int64_t staging_bytes;   /* size the caller must allocate for `staging` (payload + alignment padding) */
   int64_t local_bytes;     /* payload bytes whose source device is their destination device */

@@ -24,7 +24,7 @@ EXPORTED_SYMBOLS = (
     "etc_migrate_phase",
     "etc_status_string", "etc_last_error_detail", "etc_kernel_launches", "etc_defrag",
     "etc_plan_set_rounds", "etc_plan_get_round", "etc_migrate_round", "etc_plan_create_failed", "etc_mask_failed",
-    "etc_upload_sources", "etc_plan_validate",
+    "etc_upload_sources", "etc_plan_validate", "etc_mask_cross_dp",
 )
 
 
@@ -89,6 +89,7 @@ def lib():
         L.etc_plan_create_failed.restype = i32
         L.etc_plan_create_failed.argtypes = [vp, vp, vp, vp, i32, C.POINTER(vp), vp]
         L.etc_mask_failed.restype = i32; L.etc_mask_failed.argtypes = [vp, vp, i32, i32, i32, vp, vp]
+        L.etc_mask_cross_dp.restype = i32; L.etc_mask_cross_dp.argtypes = [vp, vp, vp, vp]
         L.etc_plan_destroy.restype = None; L.etc_plan_destroy.argtypes = [vp]
         L.etc_plan_get_stats.restype = i32; L.etc_plan_get_stats.argtypes = [vp, C.POINTER(_PlanStats)]
         L.etc_plan_get_traffic.restype = i32; L.etc_plan_get_traffic.argtypes = [vp, vp]
@@ -304,6 +305,12 @@ def etc_mask_failed(overlap, hold, failed, n_old: int, stream=None):
     _check(lib().etc_mask_failed(overlap.data_ptr(), 0 if hold is None else hold.data_ptr(), n_new, n_old, P,
                                  failed.data_ptr(), _stream(stream)))
     return overlap, hold
+
+
+def etc_mask_cross_dp(old: Layout, new: Layout, overlap, stream=None):
+    """The paper's DP isolation (reading A5): zero the cross-DP cells of overlap [n_new][P] in place."""
+    _check(lib().etc_mask_cross_dp(old.h, new.h, overlap.data_ptr(), _stream(stream)))
+    return overlap
 
 
 def etc_plan_create(old: Layout, new: Layout, device_map, flags: int = ETC_LOCAL_DIRECT, stream=None,

@@ -147,3 +147,28 @@ extern "C" etc_status etc_mask_failed(int64_t* d_overlap, int64_t* d_hold, int32
   etc::count_launch();
   return ETC_OK;
 }
+
+// The paper's own treatment of the DP dimension (reading A5): processes under different DP ranks
+// are isolated, "the difference between the workloads [is] infinite" — a cross-DP cell keeps nothing local.
+namespace etc {
+__global__ void mask_cross_dp_kernel(int64_t* __restrict__ overlap, int n_new, int n_old, int P, int tp_o, int dp_o,
+                                     int tp_n, int dp_n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (long long)n_new * n_old) return;
+  const int o = (int)(i % n_old), n = (int)(i / n_old);
+  if ((o / tp_o) % dp_o != (n / tp_n) % dp_n) overlap[(size_t)n * P + o] = 0;      // device id = r + tp*(d + dp*s)
+}
+}  // namespace etc
+
+extern "C" etc_status etc_mask_cross_dp(const etc_layout* old_l, const etc_layout* new_l, int64_t* d_overlap, void* stream) {
+  etc::clear_error_detail();
+  if (!old_l || !new_l || !d_overlap) return ETC_ERR_INVALID_ARG;
+  if (!same_model(old_l, new_l)) return ETC_ERR_MISMATCH;
+  const int n_old = old_l->t.n_dev, n_new = new_l->t.n_dev, P = n_old > n_new ? n_old : n_new;
+  const long long total = (long long)n_new * n_old;
+  etc::mask_cross_dp_kernel<<<(unsigned)((total + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
+      d_overlap, n_new, n_old, P, old_l->t.tp, old_l->t.dp, new_l->t.tp, new_l->t.dp);
+  ETC_CUDA_TRY(cudaGetLastError());
+  etc::count_launch();
+  return ETC_OK;
+}

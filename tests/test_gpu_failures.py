@@ -182,3 +182,33 @@ def test_failures_with_every_layout_variant(E, seed):
         _run(E, m, a, b, f, 6100 + done, flags=int(rng.integers(0, 2)), device_map=dm)
         done += 1
     print("unrecoverable cases:", unrec)
+
+
+def test_dp_isolated_matrix_on_device(E):
+    """etc_mask_cross_dp == the oracle's DP-isolated matrix (the paper's formulation, reading A5); on
+    config 2 at full size the isolated sketch keeps 2 899 197 952 B local against 5 798 395 904 B for the full matrix
+    (SURVEY.md A5 [scratch]); the plan made from the isolated sketch still migrates bit-exactly (s2)."""
+    from test_gpu_parity import _check_migration
+    w = workload("c2")
+    old, new = E.etc_layout_create(w["model"], w["old"]), E.etc_layout_create(w["model"], w["new"])
+    ov, _, _ = E.etc_cost_matrix(old, new)
+    assert int(E.etc_sketch(ov)[1].item()) == 5798395904
+    oo, on = O.Layout(w["model"], w["old"]), O.Layout(w["model"], w["new"])
+    o_iso = O.mask_cross_dp(oo, on, O.overlap(oo, on, method="ranges")[0])
+    E.etc_mask_cross_dp(old, new, ov)
+    assert np.array_equal(ov.cpu().numpy(), o_iso)
+    dm, lb = E.etc_sketch(ov)
+    assert int(lb.item()) == 2899197952
+    rng = np.random.default_rng(3)
+    for name, a, b in [("gpt_t", dict(tp=2, pp=2, dp=2, dist_opt=0), dict(tp=1, pp=2, dp=3, dist_opt=0)),
+                       ("llama_u", dict(tp=1, pp=2, dp=4, dist_opt=0), dict(tp=2, pp=2, dp=2, dist_opt=1))]:
+        m = dict(tiny_models())[name]
+        go, gn = E.etc_layout_create(m, a), E.etc_layout_create(m, b)
+        g = E.etc_cost_matrix(go, gn)[0]
+        E.etc_mask_cross_dp(go, gn, g)
+        lo, ln = O.Layout(m, a), O.Layout(m, b)
+        iso = O.mask_cross_dp(lo, ln, O.overlap(lo, ln)[0])
+        assert np.array_equal(g.cpu().numpy(), iso)
+        dmi, lbi = E.etc_sketch(g)
+        assert int(lbi.item()) == O.sketch_hungarian(iso)[1]
+        _check_migration(E, m, a, b, 77, device_map=dmi.cpu().numpy())     # the isolated sketch is just another map
