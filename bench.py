@@ -552,7 +552,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-extras", action="store_true")
-    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-steps", type=int, default=6)
     ap.add_argument("--e2e-staging", type=int, default=1 << 30, help="staging bound (bytes) of the e2e / chunked legs")
     ap.add_argument("--ref-elems", type=int, default=48_000_000, help="--impl reference: oracle sample (elements) per step")
     ap.add_argument("--cpu-elems", type=int, default=300_000_000, help="cpu_baseline leg: oracle sample (elements), ~10 s")

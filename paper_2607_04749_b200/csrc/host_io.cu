@@ -71,13 +71,17 @@ extern "C" etc_status etc_upload_sources(const etc_plan* pl, const void* const* 
   etc_status rc = source_regions(pl);
   if (rc != ETC_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
+  for (int k = 0; k < ETC_NUM_KINDS; ++k) {                   // every buffer a region names must exist on both sides
+    if (only_kind >= 0 && k != only_kind) continue;
+    for (const etc_slice& e : pl->h_regions[k])
+      if (!h_src_bufs[e.src_dev] || !d_src_bufs[e.src_dev]) return ETC_ERR_INVALID_ARG;
+  }
   int64_t total = 0;
   for (int k = 0; k < ETC_NUM_KINDS; ++k) {
     if (only_kind >= 0 && k != only_kind) continue;
     for (const etc_slice& e : pl->h_regions[k]) {
       const char* h = static_cast<const char*>(h_src_bufs[e.src_dev]);
       char* d = static_cast<char*>(d_src_bufs[e.src_dev]);
-      if (!h || !d) return ETC_ERR_INVALID_ARG;
       if (e.nrows == 1) ETC_CUDA_TRY(cudaMemcpyAsync(d + e.src_off, h + e.src_off, (size_t)e.row_bytes, cudaMemcpyHostToDevice, st));
       else ETC_CUDA_TRY(cudaMemcpy2DAsync(d + e.src_off, (size_t)e.src_stride, h + e.src_off, (size_t)e.src_stride,
                                           (size_t)e.row_bytes, (size_t)e.nrows, cudaMemcpyHostToDevice, st));
