@@ -80,7 +80,9 @@ sketch_exhaustive_kernel(const int64_t* __restrict__ overlap, int N, int P, cons
 // Shortest augmenting path with potentials (the O(k^3) method Algorithm 1 calls through SciPy, ref [39]).
 // cost(i,j) = -overlap[i][j]; columns masked by `avail` are never entered.  Per-column state lives in registers
 // (CPT columns per thread), row potentials / matching / back-pointers in shared memory.
-constexpr int SK_CPT = ETC_SKETCH_MAX_P / SK_THREADS;   // columns per thread
+// The block is sized to the matrix: T threads x CPT columns per thread >= P (fewer warps = cheaper barriers and a
+// shorter second reduction level); row i+1 is prefetched into registers while row i is being matched, so the first
+// Dijkstra step of every augmentation — in a structured overlap matrix usually the only one — waits for no load.
 
 struct ArgMin { int64_t v; int j; int matched; };
 __device__ __forceinline__ bool argmin_less(const ArgMin& a, const ArgMin& b) {
@@ -88,16 +90,29 @@ __device__ __forceinline__ bool argmin_less(const ArgMin& a, const ArgMin& b) {
   if (a.matched != b.matched) return a.matched < b.matched;     // prefer a free column: the path ends at once
   return a.j < b.j;
 }
-__device__ __forceinline__ ArgMin argmin_shfl(const ArgMin& a, int o) {
-  ArgMin b;
-  b.v = __shfl_xor_sync(0xffffffffu, a.v, o); b.j = __shfl_xor_sync(0xffffffffu, a.j, o);
-  b.matched = __shfl_xor_sync(0xffffffffu, a.matched, o);
-  return b;
+// Warp arg-min of (v, matched, lane) in a handful of instructions instead of five rounds of four shuffles: the 64-bit
+// minimum is two redux.sync ops (signed high word, then unsigned low word among the lanes that tie on the high word),
+// the tie-break (a free column first, then the lowest lane) two ballots, and one shuffle fetches the winner's column.
+__device__ __forceinline__ ArgMin warp_argmin(const ArgMin& a) {
+  const int hi = (int)(a.v >> 32);
+  const int mh = __reduce_min_sync(0xffffffffu, hi);
+  const unsigned lo = hi == mh ? (unsigned)(a.v & 0xffffffffll) : 0xffffffffu;
+  const unsigned ml = __reduce_min_sync(0xffffffffu, lo);
+  const bool win = hi == mh && lo == ml;
+  const unsigned m_all = __ballot_sync(0xffffffffu, win), m_free = __ballot_sync(0xffffffffu, win && !a.matched);
+  const int src = __ffs(m_free ? m_free : m_all) - 1;
+  ArgMin r;
+  r.v = (int64_t)(((uint64_t)(uint32_t)mh << 32) | ml);
+  r.j = __shfl_sync(0xffffffffu, a.j, src);
+  r.matched = m_free ? 0 : 1;
+  return r;
 }
 
-__global__ void __launch_bounds__(SK_THREADS)
+template <int SK_T, int SK_CPT>
+__global__ void __launch_bounds__(SK_T)
 sketch_hungarian_kernel(const int64_t* __restrict__ overlap, int N, int P, const uint8_t* __restrict__ avail,
                         int32_t* __restrict__ device_map, int64_t* __restrict__ local_bytes) {
+  constexpr int SK_THREADS = SK_T, SK_NW = SK_T / 32;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   int64_t* u = reinterpret_cast<int64_t*>(smem_raw);            // [N] row potentials
   int32_t* rowof = reinterpret_cast<int32_t*>(u + N);           // [P] column -> matched row or -1
@@ -115,10 +130,19 @@ sketch_hungarian_kernel(const int64_t* __restrict__ overlap, int N, int P, const
   for (int i = tid; i < N; i += SK_THREADS) u[i] = 0;
   __syncthreads();
 
+  int64_t ahead[SK_CPT], row_i[SK_CPT];                         // row i+1 (in flight) and row i of the matrix
+#pragma unroll
+  for (int c = 0; c < SK_CPT; ++c) { const int j = tid + c * SK_THREADS; ahead[c] = j < P ? overlap[j] : 0; }
+
   bool fail = false;                                            // uniform across the block
   for (int i = 0; i < N; ++i) {
 #pragma unroll
-    for (int c = 0; c < SK_CPT; ++c) { minv[c] = SK_INF; used[c] = !usable[c]; }
+    for (int c = 0; c < SK_CPT; ++c) {
+      const int j = tid + c * SK_THREADS;
+      minv[c] = SK_INF; used[c] = !usable[c];
+      row_i[c] = ahead[c];
+      if (i + 1 < N && j < P) ahead[c] = overlap[(size_t)(i + 1) * P + j];
+    }
     int i0 = i, j0 = -1;
     while (true) {
       // relax the edges of row i0, then block-wide arg-min of minv over the columns not yet on the tree
@@ -128,19 +152,16 @@ sketch_hungarian_kernel(const int64_t* __restrict__ overlap, int N, int P, const
       for (int c = 0; c < SK_CPT; ++c) {
         const int j = tid + c * SK_THREADS;
         if (!used[c]) {
-          const int64_t cur = -overlap[(size_t)i0 * P + j] - ui0 - v[c];
+          const int64_t cur = -(j0 < 0 ? row_i[c] : overlap[(size_t)i0 * P + j]) - ui0 - v[c];
           if (cur < minv[c]) { minv[c] = cur; way[j] = j0; }
           ArgMin a{minv[c], j, rowof[j] >= 0 ? 1 : 0};
           if (argmin_less(a, best)) best = a;
         }
       }
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) { ArgMin b = argmin_shfl(best, o); if (argmin_less(b, best)) best = b; }
+      best = warp_argmin(best);
       if (lane == 0) { s_v[wid] = best.v; s_j[wid] = best.j; s_m[wid] = best.matched; }
       __syncthreads();
-      best = ArgMin{s_v[lane], s_j[lane], s_m[lane]};
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) { ArgMin b = argmin_shfl(best, o); if (argmin_less(b, best)) best = b; }
+      best = warp_argmin(lane < SK_NW ? ArgMin{s_v[lane], s_j[lane], s_m[lane]} : ArgMin{SK_INF, 0x7fffffff, 1});
       if (best.v >= SK_INF) { fail = true; break; }                       // no column left: infeasible
       const int64_t delta = best.v; const int j1 = best.j;
       // dual update: tree rows gain delta, tree columns lose delta, the rest get closer by delta
@@ -184,7 +205,7 @@ sketch_hungarian_kernel(const int64_t* __restrict__ overlap, int N, int P, const
   if (lane == 0) s_v[wid] = acc;
   __syncthreads();
   if (wid == 0) {
-    acc = s_v[lane];
+    acc = lane < SK_NW ? s_v[lane] : 0;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
     if (lane == 0) *local_bytes = acc;
@@ -218,8 +239,7 @@ sketch_hungarian_warp_kernel(const int64_t* __restrict__ overlap, int N, int P, 
         if (cur < minv) { minv = cur; way[lane] = j0; }
         best = ArgMin{minv, lane, rowof >= 0 ? 1 : 0};
       }
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) { ArgMin b = argmin_shfl(best, o); if (argmin_less(b, best)) best = b; }
+      best = warp_argmin(best);
       if (best.v >= SK_INF) { fail = true; break; }
       const int64_t delta = best.v; const int j1 = best.j;
       // dual update: tree rows (the root i and the rows matched to tree columns) gain delta, tree columns lose it
@@ -275,14 +295,15 @@ extern "C" etc_status etc_sketch(const int64_t* d_overlap, int32_t n_new, int32_
       count_launch();
       return ETC_OK;
     }
-    const size_t smem = (size_t)n_new * 8 + (size_t)P * 8;
-    static bool attr_set = false;
-    if (!attr_set) {
-      ETC_CUDA_TRY(cudaFuncSetAttribute(sketch_hungarian_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                        ETC_SKETCH_MAX_P * 16));
-      attr_set = true;
-    }
-    sketch_hungarian_kernel<<<1, SK_THREADS, smem, st>>>(d_overlap, n_new, P, d_avail, d_device_map, d_local_bytes);
+    const size_t smem = (size_t)n_new * 8 + (size_t)P * 8;       // <= 32 KB: below the default dynamic limit
+#define SK_LAUNCH(T, CPT) sketch_hungarian_kernel<T, CPT><<<1, T, smem, st>>>(d_overlap, n_new, P, d_avail, d_device_map, d_local_bytes)
+    if (P <= 64) SK_LAUNCH(64, 1);
+    else if (P <= 128) SK_LAUNCH(128, 1);
+    else if (P <= 256) SK_LAUNCH(256, 1);
+    else if (P <= 512) SK_LAUNCH(512, 1);
+    else if (P <= 1024) SK_LAUNCH(1024, 1);
+    else SK_LAUNCH(1024, 2);
+#undef SK_LAUNCH
   } else {
     return ETC_ERR_INVALID_ARG;
   }
