@@ -449,6 +449,31 @@ def extras(E, torch, w, dev, src, dst, lay_old, lay_new, peak):
     except Exception as ex:
         out["one_shot"] = {"error": repr(ex)[:200]}
     try:
+        # (f1) virtual rank allocator on config 3's pre-emption (16 -> 12 devices, 4 per node), metadata only: bytes
+        # that change device under the sketch alone, under the sketch composed with Algorithm 2 (one hop: communication
+        # coalescing), and if the defragmentation were a second migration stage
+        w3 = workload("c3")
+        lo, ln = E.etc_layout_create(w3["model"], w3["old"]), E.etc_layout_create(w3["model"], w3["new"])
+        ov, need, _ = E.etc_cost_matrix(lo, ln)
+        dm, _ = E.etc_sketch(ov)
+        E.etc_defrag(dm, lo.n_dev, ln.n_dev, 4, E.ETC_DEFRAG_BOTH); torch.cuda.synchronize()     # untimed: loads the kernel
+        a, b = ev(), ev()
+        a.record(stream)
+        final, n_ops, _ = E.etc_defrag(dm, lo.n_dev, ln.n_dev, 4, E.ETC_DEFRAG_BOTH)
+        b.record(stream); torch.cuda.synchronize()
+        p0, p1 = E.etc_plan_create(lo, ln, dm), E.etc_plan_create(lo, ln, final)
+        dm_h, fin_h, need_h = dm.cpu().tolist(), final.cpu().tolist(), need.cpu().tolist()
+        moved = sum(need_h[r] for r in range(ln.n_dev) if dm_h[r] != fin_h[r])
+        out["defrag_c3_16_to_12"] = {"devices_per_node": 4, "sketch_map": dm_h, "final_map": fin_h,
+                                     "operators": [int(x) for x in n_ops.cpu().tolist()], "defrag_ms": a.elapsed_time(b),
+                                     "remote_bytes_sketch_only": p0.stats.remote_bytes,
+                                     "remote_bytes_coalesced": p1.stats.remote_bytes,
+                                     "remote_bytes_two_stage": p0.stats.remote_bytes + moved,
+                                     "nodes_occupied": [len({p // 4 for p in dm_h}), len({p // 4 for p in fin_h})]}
+        del p0, p1
+    except Exception as ex:
+        out["defrag_c3_16_to_12"] = {"error": repr(ex)[:200]}
+    try:
         wb = workload("c5b")
         lo, ln = E.etc_layout_create(wb["model"], wb["old"]), E.etc_layout_create(wb["model"], wb["new"])
         tc, ts = [], []
