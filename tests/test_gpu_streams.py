@@ -65,3 +65,41 @@ def test_pipelined_plans_dropped_early(E, name, flags, copy_on_default_stream):
     for key, e in exp.items():
         if e.shape[0]:
             assert np.array_equal(download(dst[key], on.elem_bytes(key[1])), e), key
+
+
+@pytest.mark.parametrize("name,flags", [("c1", 0), ("s4odd", 1), ("s5", 0)])
+def test_migrate_is_cuda_graph_capturable(E, name, flags):
+    """include/etc.h: etc_migrate does no allocation and no host synchronisation (its pointer tables travel as kernel
+    parameters, not as copies from pageable memory), so it can be captured into a CUDA graph and replayed: the replay
+    on fresh payloads must still equal the oracle's element-wise migration."""
+    w = workload(name)
+    model = w["model"]
+    oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
+    payloads = [shard_all(oo, make_logical(model, w["seed"] + i, "stamp" if i == 0 else "values")) for i in range(3)]
+    old, new = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])
+    dm, _ = E.etc_sketch(E.etc_cost_matrix(old, new)[0])
+    plan = E.etc_plan_create(old, new, dm, flags)
+    src = upload(payloads[0])
+    dst = E.alloc_buffers(new, fill=0x3C)
+    staging = torch.empty(max(plan.stats.staging_bytes, 16), dtype=torch.uint8, device="cuda")
+    E.etc_migrate(plan, src, dst, staging)                         # warm-up: kernel attributes are set outside capture
+    torch.cuda.synchronize()
+    launches0 = E.kernel_launches()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        E.etc_migrate(plan, src, dst, staging)
+    per_call = E.kernel_launches() - launches0
+    assert 1 <= per_call <= 4
+    dm_h = dm.cpu().numpy()
+    for i in (1, 2):
+        for key, a in payloads[i].items():
+            if a.shape[0]:
+                src[key].copy_(torch.from_numpy(a.view(np.uint8).copy()))
+        for t in dst.values():
+            t.fill_(0x3C)
+        graph.replay()
+        torch.cuda.synchronize()
+        exp, _, _ = O.migrate(oo, on, dm_h, payloads[i])
+        for key, e in exp.items():
+            if e.shape[0]:
+                assert np.array_equal(download(dst[key], e.itemsize), e), (i, key)
