@@ -499,8 +499,17 @@ def e2e(E, torch, args, w, dev, src, dst, hbm_bytes, world, barrier):
     Beside it: the DMA pipelines (cudaMemcpyAsync of every old shard byte / of only the regions the plan reads, rounds
     on device buffers, cudaMemcpyAsync of the new shards; three streams)."""
     from paper_2607_04749_b200.host_pipeline import HostMigration
-    h_src = {k: torch.empty(t.shape, dtype=t.dtype, pin_memory=True) for k, t in src.items()}
-    h_dst = {k: torch.empty(t.shape, dtype=t.dtype, pin_memory=True) for k, t in dst.items()}
+    # pinning the host copies is the step that can fail on one rank only (host memory): agree on it before any
+    # collective, so that no rank is left waiting in a barrier
+    ok, h_src, h_dst = 1.0, {}, {}
+    try:
+        h_src = {k: torch.empty(t.shape, dtype=t.dtype, pin_memory=True) for k, t in src.items()}
+        h_dst = {k: torch.empty(t.shape, dtype=t.dtype, pin_memory=True) for k, t in dst.items()}
+    except Exception:
+        ok = 0.0
+    if -max_over_ranks(-ok, world, dev) < 0.5:
+        h_src = h_dst = None
+        raise RuntimeError("pinned host buffers for the old and new shards could not be allocated on every rank")
     for k, t in src.items():
         h_src[k].copy_(t)
     torch.cuda.synchronize()
@@ -532,6 +541,8 @@ def e2e(E, torch, args, w, dev, src, dst, hbm_bytes, world, barrier):
              "upload, rounds and download of different kinds overlap on three streams"),
             ("dma_needed_only", dict(d_src=src, d_dst=dst, needed_only=True),
              "plan first, then cudaMemcpy2DAsync of only the source regions the plan's slices read (etc_upload_sources)")):
+        if world > 1:
+            continue                                            # context legs: single-GPU runs only
         try:
             out[key] = leg(**kw)
             out[key]["note"] = note
