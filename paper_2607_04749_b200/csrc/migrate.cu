@@ -8,8 +8,10 @@
 //     cp.async.bulk shared -> global for every row.  A row-parallel (strided) slice is thus gathered into a dense
 //     64 KB tile and written back out with the other side's pitch; three CTAs per SM keep ~192 KB in flight per SM.
 //     Measured 6.8-6.9 TB/s against 6.5-6.7 TB/s for the vector path on the same chunk lists.
-//   * everything else (rows < 512 B, or addresses not 16-byte aligned) takes the vector path: the widest aligned
-//     access (16/8/4/2/1 bytes), streaming loads/stores, four independent vectors in flight per thread.
+//   * chunks that are only 4- or 8-byte aligned are staged through the same tile with cp.async (LDGSTS): all loads of
+//     the chunk in flight at once, then narrow stores.
+//   * everything else (16-byte aligned rows < 512 B, or 1- / 2-byte alignment) takes the vector path: the widest
+//     aligned access, streaming loads/stores, four independent vectors in flight per thread.
 // Two launches per migration:
 //   launch 1: pack (old buffers -> staging segments)  +  local slices (old buffer -> new buffer directly)
 //   launch 2: unpack (staging segments -> new buffers)
@@ -61,6 +63,33 @@ __device__ __forceinline__ void copy_chunk(const char* __restrict__ src, char* _
     for (int k = 0; k < CP_UNROLL; ++k) st_stream(d[k], v[k]);
   }
   for (; i < total; i += CP_THREADS) { const V* s; V* d; addr(i, s, d); st_stream(d, ld_stream(s)); }
+}
+
+// ---- cp.async staged path for chunks that are only 4- or 8-byte aligned (odd hidden sizes, unaligned distributed-
+// optimizer cuts).  With register staging a thread keeps 4 narrow loads in flight and the CTA a few KB; here every
+// thread issues ALL its loads of the chunk as cp.async (LDGSTS) into the 64 KB tile, so the whole chunk is in flight,
+// as on the TMA path, and writes its own elements out again after its wait_group (no block barrier: a thread reads
+// back only what it loaded).  ncu on a layout with 52 % of the bytes misaligned: register path 27 % warps active,
+// stalled on long_scoreboard, 4.5 TB/s on the misaligned share.
+template <int VB> __device__ __forceinline__ void cp_async(void* smem, const void* g) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(g), "n"(VB) : "memory");
+}
+template <typename V>
+__device__ __forceinline__ void staged_copy_chunk(char* __restrict__ tile, const char* __restrict__ src, char* __restrict__ dst,
+                                                  int nrows, uint32_t row_bytes, uint32_t src_pitch, uint32_t dst_pitch) {
+  constexpr uint32_t VB = (uint32_t)sizeof(V);
+  const uint32_t vpr = row_bytes / VB, total = vpr * (uint32_t)nrows;
+  const uint32_t magic = (uint32_t)((0x100000000ull + vpr - 1) / vpr);
+  for (uint32_t i = threadIdx.x; i < total; i += CP_THREADS) {
+    const uint32_t row = (nrows == 1) ? 0 : (vpr == 1 ? i : __umulhi(i, magic)), col = i - row * vpr;
+    cp_async<(int)VB>(tile + (size_t)i * VB, src + (size_t)row * src_pitch + (size_t)col * VB);
+  }
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+  for (uint32_t i = threadIdx.x; i < total; i += CP_THREADS) {
+    const uint32_t row = (nrows == 1) ? 0 : (vpr == 1 ? i : __umulhi(i, magic)), col = i - row * vpr;
+    st_stream(reinterpret_cast<V*>(dst + (size_t)row * dst_pitch + (size_t)col * VB), *reinterpret_cast<const V*>(tile + (size_t)i * VB));
+  }
 }
 
 __device__ __forceinline__ void copy_dispatch(int vec, const char* src, char* dst, int nrows, uint32_t row_bytes,
@@ -128,7 +157,7 @@ __global__ void __launch_bounds__(CP_THREADS)
 migrate_copy_kernel(const Chunk* __restrict__ chA, long long nA, const Chunk* __restrict__ chB,
                     const void* const* __restrict__ src_tab, void* const* __restrict__ dst_tab,
                     char* __restrict__ staging) {
-  extern __shared__ __align__(128) char tile[];                 // ETC_CHUNK_BYTES, TMA path only
+  extern __shared__ __align__(128) char tile[];                 // ETC_CHUNK_BYTES: TMA path and cp.async staged path
   __shared__ uint64_t bar;
   const long long b = blockIdx.x;
   const bool staged = b < nA;
@@ -148,6 +177,10 @@ migrate_copy_kernel(const Chunk* __restrict__ chA, long long nA, const Chunk* __
     if (threadIdx.x < 32) tma_copy_chunk(tile, &bar, src, dst, c.nrows, (uint32_t)c.row_bytes, sp, dp);
     return;
   }
+  // 4- / 8-byte aligned chunks: cp.async staged (a 16-byte-store variant with per-row phase-aligned tile rows was
+  // measured slower, 5.73 vs 5.96 TB/s on the hidden-1026 layout: the narrow loads, not the stores, set the pace)
+  if (c.vec == 8) { staged_copy_chunk<uint2>(tile, src, dst, c.nrows, (uint32_t)c.row_bytes, sp, dp); return; }
+  if (c.vec == 4) { staged_copy_chunk<unsigned int>(tile, src, dst, c.nrows, (uint32_t)c.row_bytes, sp, dp); return; }
   copy_dispatch(c.vec, src, dst, c.nrows, (uint32_t)c.row_bytes, sp, dp);
 }
 
