@@ -72,13 +72,16 @@ _SCALED = {
     # odd sizes: rows that are not multiples of 16 bytes (exercises the scalar/unaligned copy path)
     "s4odd": ("c4", dict(n_layers=8, hidden=20, n_q_heads=4, n_kv_heads=4, head_dim=5, ffn_hidden=36,
                          vocab=52, max_pos=7)),
+    # rows of 388 B (bf16) / 776 B (fp32) at offsets that are only 4- / 8-byte aligned: the re-aligning staged copy path
+    "s2odd": ("c2", dict(n_layers=4, hidden=194, n_q_heads=12, n_kv_heads=12, head_dim=16, ffn_hidden=768,
+                         vocab=3000, max_pos=96)),
     "s5b": ("c5b", dict(n_layers=16, hidden=64, n_q_heads=16, n_kv_heads=8, head_dim=4, ffn_hidden=128,
                         vocab=256, max_pos=0)),
 }
 
 
 def workload(name: str) -> dict:
-    """Return a deep copy of the named workload ("c1".."c5", "c5b", "s2".."s5", "s4odd", "s5b")."""
+    """Return a deep copy of the named workload ("c1".."c5", "c5b", "s2".."s5", "s2odd", "s4odd", "s5b")."""
     if name in WORKLOADS:
         return copy.deepcopy(WORKLOADS[name])
     base, over = _SCALED[name]

@@ -8,8 +8,10 @@
 //     cp.async.bulk shared -> global for every row.  A row-parallel (strided) slice is thus gathered into a dense
 //     64 KB tile and written back out with the other side's pitch; three CTAs per SM keep ~192 KB in flight per SM.
 //     Measured 6.8-6.9 TB/s against 6.5-6.7 TB/s for the vector path on the same chunk lists.
-//   * chunks that are only 4- or 8-byte aligned are staged through the same tile with cp.async (LDGSTS): all loads of
-//     the chunk in flight at once, then narrow stores.
+//   * chunks that are only 4- or 8-byte aligned are staged through the same tile with cp.async (LDGSTS), all loads of
+//     the chunk in flight at once; rows >= 256 B are re-aligned on the way (16-byte loads into a tile row that starts at
+//     the source's phase modulo 16, 16-byte stores assembled from narrow shared-memory reads): 6.5 TB/s on a layout
+//     with half its bytes misaligned, against 5.4 TB/s with register staging.
 //   * everything else (16-byte aligned rows < 512 B, or 1- / 2-byte alignment) takes the vector path: the widest
 //     aligned access, streaming loads/stores, four independent vectors in flight per thread.
 // Two launches per migration:
@@ -92,6 +94,54 @@ __device__ __forceinline__ void staged_copy_chunk(char* __restrict__ tile, const
   }
 }
 
+// Re-aligning variant for rows >= 256 B: 16-byte loads AND 16-byte stores although source and destination disagree
+// modulo 16.  Row r of the tile starts at r*RP + (address of its SOURCE row mod 16), so every 16-byte slot of the tile
+// that lies wholly inside the row is one 16-byte cp.async from an aligned source address; on the way out every
+// 16-byte slot of the DESTINATION row is assembled from 16/sizeof(V) narrow shared-memory reads (the tile is V-aligned
+// there, not 16-byte aligned) and written with one 16-byte store.  Only the ragged ends of a row use the narrow width.
+// The per-row slack (<= 32 B) fits the tile's 8 KB margin because such a chunk has at most 256 rows.
+constexpr int TILE_BYTES = ETC_CHUNK_BYTES + 8192;
+constexpr uint32_t REALIGN_MIN_ROW = 256;
+template <typename V>
+__device__ __forceinline__ void staged_copy_realign(char* __restrict__ tile, const char* __restrict__ src, char* __restrict__ dst,
+                                                    int nrows, uint32_t row_bytes, uint32_t src_pitch, uint32_t dst_pitch) {
+  constexpr uint32_t VB = (uint32_t)sizeof(V);
+  const uint32_t RP = (row_bytes + 31u) & ~15u;                 // >= row_bytes + 16
+  const uint32_t S = RP / 16u, slots = S * (uint32_t)nrows;
+  const uint32_t magic_s = (uint32_t)((0x100000000ull + S - 1) / S);
+  const uint32_t sphase0 = (uint32_t)(reinterpret_cast<uintptr_t>(src) & 15), dphase0 = (uint32_t)(reinterpret_cast<uintptr_t>(dst) & 15);
+  for (uint32_t j = threadIdx.x; j < slots; j += CP_THREADS) {
+    const uint32_t row = nrows == 1 ? 0 : __umulhi(j, magic_s), k = j - row * S;
+    const uint32_t sphase = (sphase0 + row * src_pitch) & 15u;
+    const uint32_t lo = max(16u * k, sphase), hi = min(16u * k + 16u, sphase + row_bytes);
+    if (hi <= lo) continue;
+    const char* g = src + (size_t)row * src_pitch + (lo - sphase);
+    char* t = tile + (size_t)row * RP + lo;
+    if (hi - lo == 16u) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(t)), "l"(g) : "memory");
+    else for (uint32_t x = 0; x < hi - lo; x += VB) cp_async<(int)VB>(t + x, g + x);
+  }
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+  __syncthreads();
+  for (uint32_t j = threadIdx.x; j < slots; j += CP_THREADS) {
+    const uint32_t row = nrows == 1 ? 0 : __umulhi(j, magic_s), k = j - row * S;
+    const uint32_t sphase = (sphase0 + row * src_pitch) & 15u, dphase = (dphase0 + row * dst_pitch) & 15u;
+    const uint32_t lo = max(16u * k, dphase), hi = min(16u * k + 16u, dphase + row_bytes);
+    if (hi <= lo) continue;
+    const uint32_t x0 = lo - dphase;                             // offset inside the row
+    char* d = dst + (size_t)row * dst_pitch + x0;
+    const char* t = tile + (size_t)row * RP + sphase + x0;       // V-aligned
+    if (hi - lo == 16u) {
+      union { uint4 q; V v[16 / VB]; } u;
+#pragma unroll
+      for (uint32_t i = 0; i < 16 / VB; ++i) u.v[i] = reinterpret_cast<const V*>(t)[i];
+      st_stream(reinterpret_cast<uint4*>(d), u.q);
+    } else {
+      for (uint32_t x = 0; x < hi - lo; x += VB) st_stream(reinterpret_cast<V*>(d + x), *reinterpret_cast<const V*>(t + x));
+    }
+  }
+}
+
 __device__ __forceinline__ void copy_dispatch(int vec, const char* src, char* dst, int nrows, uint32_t row_bytes,
                                               uint32_t sp, uint32_t dp) {
   switch (vec) {
@@ -157,7 +207,7 @@ __global__ void __launch_bounds__(CP_THREADS)
 migrate_copy_kernel(const Chunk* __restrict__ chA, long long nA, const Chunk* __restrict__ chB,
                     const void* const* __restrict__ src_tab, void* const* __restrict__ dst_tab,
                     char* __restrict__ staging) {
-  extern __shared__ __align__(128) char tile[];                 // ETC_CHUNK_BYTES: TMA path and cp.async staged path
+  extern __shared__ __align__(128) char tile[];                 // TILE_BYTES: TMA path and cp.async staged paths
   __shared__ uint64_t bar;
   const long long b = blockIdx.x;
   const bool staged = b < nA;
@@ -177,10 +227,14 @@ migrate_copy_kernel(const Chunk* __restrict__ chA, long long nA, const Chunk* __
     if (threadIdx.x < 32) tma_copy_chunk(tile, &bar, src, dst, c.nrows, (uint32_t)c.row_bytes, sp, dp);
     return;
   }
-  // 4- / 8-byte aligned chunks: cp.async staged (a 16-byte-store variant with per-row phase-aligned tile rows was
-  // measured slower, 5.73 vs 5.96 TB/s on the hidden-1026 layout: the narrow loads, not the stores, set the pace)
-  if (c.vec == 8) { staged_copy_chunk<uint2>(tile, src, dst, c.nrows, (uint32_t)c.row_bytes, sp, dp); return; }
-  if (c.vec == 4) { staged_copy_chunk<unsigned int>(tile, src, dst, c.nrows, (uint32_t)c.row_bytes, sp, dp); return; }
+  if (c.vec == 8 || c.vec == 4) {
+    const bool wide = (uint32_t)c.row_bytes >= REALIGN_MIN_ROW;
+    if (c.vec == 8) { if (wide) staged_copy_realign<uint2>(tile, src, dst, c.nrows, (uint32_t)c.row_bytes, sp, dp);
+                      else staged_copy_chunk<uint2>(tile, src, dst, c.nrows, (uint32_t)c.row_bytes, sp, dp); }
+    else { if (wide) staged_copy_realign<unsigned int>(tile, src, dst, c.nrows, (uint32_t)c.row_bytes, sp, dp);
+           else staged_copy_chunk<unsigned int>(tile, src, dst, c.nrows, (uint32_t)c.row_bytes, sp, dp); }
+    return;
+  }
   copy_dispatch(c.vec, src, dst, c.nrows, (uint32_t)c.row_bytes, sp, dp);
 }
 
@@ -218,8 +272,8 @@ migrate_fill_kernel(const etc_slice* __restrict__ fills, void* const* __restrict
 static cudaError_t copy_kernel_attrs() {
   static bool done = false;
   if (done) return cudaSuccess;
-  cudaError_t e = cudaFuncSetAttribute(migrate_copy_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ETC_CHUNK_BYTES);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(migrate_copy_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ETC_CHUNK_BYTES);
+  cudaError_t e = cudaFuncSetAttribute(migrate_copy_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TILE_BYTES);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(migrate_copy_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TILE_BYTES);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(migrate_copy_kernel<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(migrate_copy_kernel<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
   done = e == cudaSuccess;
@@ -263,7 +317,7 @@ static etc_status launch_migrate(const etc_plan* pl, const void* const* src_bufs
   const void* const* d_src = d_ptrs; void* const* d_dst = d_ptrs + ns;
   char* stg = static_cast<char*>(staging) - stg_base;          // chunk records carry offsets of the full staging layout
   if ((phases & ETC_PHASE_PACK) && nA + nB > 0) {
-    migrate_copy_kernel<false><<<(unsigned)(nA + nB), CP_THREADS, ETC_CHUNK_BYTES, st>>>(pl->d_ch_staged + ca, nA, pl->d_ch_local + la,
+    migrate_copy_kernel<false><<<(unsigned)(nA + nB), CP_THREADS, TILE_BYTES, st>>>(pl->d_ch_staged + ca, nA, pl->d_ch_local + la,
                                                                            d_src, d_dst, stg);
     ETC_CUDA_TRY(cudaGetLastError());
     count_launch();
@@ -274,7 +328,7 @@ static etc_status launch_migrate(const etc_plan* pl, const void* const* src_bufs
     count_launch();
   }
   if ((phases & ETC_PHASE_UNPACK) && nA > 0) {
-    migrate_copy_kernel<true><<<(unsigned)nA, CP_THREADS, ETC_CHUNK_BYTES, st>>>(pl->d_ch_staged + ca, nA, nullptr, d_src, d_dst, stg);
+    migrate_copy_kernel<true><<<(unsigned)nA, CP_THREADS, TILE_BYTES, st>>>(pl->d_ch_staged + ca, nA, nullptr, d_src, d_dst, stg);
     ETC_CUDA_TRY(cudaGetLastError());
     count_launch();
   }

@@ -216,11 +216,26 @@ def test_migrate_config1(E, flags):
     _check_migration(E, w["model"], w["old"], w["new"], w["seed"], flags=flags, payload="stamp")
 
 
-@pytest.mark.parametrize("name", ["s2", "s3", "s4", "s4odd", "s5"])
+@pytest.mark.parametrize("name", ["s2", "s2odd", "s3", "s4", "s4odd", "s5"])
 @pytest.mark.parametrize("flags", [0, 1, 2, 3])              # 2, 3: + ETC_KIND_MAJOR (kind-major tables and staging)
 def test_migrate_scaled_configs(E, name, flags):
     w = workload(name)
     _check_migration(E, w["model"], w["old"], w["new"], w["seed"], flags=flags)
+
+
+@pytest.mark.parametrize("hidden", [66, 130, 258])
+def test_migrate_misaligned_wide_rows(E, hidden):
+    """Rows of 264 ... 1032 bytes whose addresses are only 4- or 8-byte aligned and whose pitches are not multiples of 16
+    (the source / destination phase modulo 16 changes from row to row), with distributed-optimizer cuts on both sides:
+    the re-aligning staged copy path (16-byte loads and stores through a phase-shifted tile) against the oracle."""
+    m = dict(workload("s2")["model"], hidden=hidden, n_q_heads=4, n_kv_heads=4, head_dim=16, ffn_hidden=4 * hidden,
+             vocab=516, max_pos=33, n_layers=4)
+    old_c, new_c = dict(tp=2, pp=2, dp=2, dist_opt=1), dict(tp=4, pp=1, dp=2, dist_opt=1)
+    rng = np.random.default_rng(hidden)
+    for flags in (0, 1):
+        _check_migration(E, m, old_c, new_c, 300 + hidden, flags=flags)
+    _check_migration(E, m, old_c, new_c, 301 + hidden, device_map=rng.permutation(8).astype(np.int32), flags=3, payload="values")
+    _check_migration(E, m, new_c, old_c, 302 + hidden, flags=1)
 
 
 def test_migrate_identity_map_and_arbitrary_maps(E):

@@ -72,7 +72,7 @@ def _run_rounds(E, model, old_cfg, new_cfg, seed, cap, flags, device_map=None, p
     return plan, rounds
 
 
-@pytest.mark.parametrize("name", ["c1", "s2", "s3", "s4", "s4odd", "s5"])
+@pytest.mark.parametrize("name", ["c1", "s2", "s2odd", "s3", "s4", "s4odd", "s5"])
 @pytest.mark.parametrize("cap", [2 * 65536, 1 << 20, 1 << 34])
 def test_rounds_vs_oracle(E, name, cap):
     w = workload(name)
