@@ -149,9 +149,12 @@ etc_status etc_defrag(const int32_t* d_device_map, int32_t pw, int32_t cw, int32
  * is the destination device are copied old buffer -> new buffer, never staged: the paper's Refer, reading A19) or
  * ETC_ALL_STAGED (every slice goes through pack/unpack: a measurement mode); OR-ed with ETC_KIND_MAJOR to order
  * slices, chunks and staging segments by state kind first (one segment per (kind, source, destination) instead of one
- * per (source, destination)): required for state chunking, etc_plan_set_rounds below.  Synchronises `stream` once
+ * per (source, destination)): required for state chunking, etc_plan_set_rounds below.  ETC_ALL_DIRECT (not with
+ * ETC_ALL_STAGED): NO slice is staged, every one is copied source buffer -> destination buffer in one hop — for shards
+ * that all live in one address space anyway (pinned host memory: the zero-copy pipeline), where a staging buffer
+ * stands for no message; the traffic matrix and remote_bytes are unchanged, staging_bytes = 0.  Synchronises `stream` once
  * (sizes must come back to the host).  Fails with ETC_ERR_BAD_MAP if the map is not injective into [0,P). */
-enum { ETC_LOCAL_DIRECT = 0, ETC_ALL_STAGED = 1, ETC_KIND_MAJOR = 2 };
+enum { ETC_LOCAL_DIRECT = 0, ETC_ALL_STAGED = 1, ETC_KIND_MAJOR = 2, ETC_ALL_DIRECT = 4 };
 etc_status etc_plan_create(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
                            int32_t flags, etc_plan** out, void* stream);
 void etc_plan_destroy(etc_plan* plan);

@@ -12,7 +12,7 @@ _LIB_PATH = os.path.join(_HERE, "libetc.so")
 _lib = None
 _inited = False
 
-ETC_LOCAL_DIRECT, ETC_ALL_STAGED, ETC_KIND_MAJOR = 0, 1, 2
+ETC_LOCAL_DIRECT, ETC_ALL_STAGED, ETC_KIND_MAJOR, ETC_ALL_DIRECT = 0, 1, 2, 4
 ETC_SKETCH_AUTO, ETC_SKETCH_EXHAUSTIVE, ETC_SKETCH_HUNGARIAN = 0, 1, 2
 ETC_PHASE_PACK, ETC_PHASE_UNPACK, ETC_PHASE_ALL = 1, 2, 3
 ETC_DEFRAG_OCCUPANCY, ETC_DEFRAG_EFFICIENCY, ETC_DEFRAG_BOTH = 1, 2, 3

@@ -222,7 +222,7 @@ plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int K, int n_
     if (u < U) {
       c = units[u];
       od = (int)((u / n_new) % n_old); p = device_map[(int)(u % n_new)];
-      staged = (od != p) || (flags & ETC_ALL_STAGED);
+      staged = !(flags & ETC_ALL_DIRECT) && ((od != p) || (flags & ETC_ALL_STAGED));
       c.padded = (c.padded + 511) & ~(int64_t)511;             // pair segments start 512-byte aligned
     }
     int64_t v[5];
@@ -302,7 +302,7 @@ plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict
   const UnitBase ub = bases[u];
   const int n = (int)(u % newT.n_dev), od = (int)((u / newT.n_dev) % oldT.n_dev), kq = (int)(u / newT.n_dev / oldT.n_dev);
   const int p = device_map[n];
-  const bool local_unit = (od == p), staged = !local_unit || (flags & ETC_ALL_STAGED);
+  const bool local_unit = (od == p), staged = !(flags & ETC_ALL_DIRECT) && (!local_unit || (flags & ETC_ALL_STAGED));
   etc_slice* sl_out = staged ? sl_staged : sl_local;
   int64_t* c0_out = staged ? c0_staged : c0_local;
   int64_t pre_sl = 0, pre_ch = 0, pre_pad = 0;                 // totals of the unit's earlier sub-blocks
@@ -445,7 +445,8 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
                                              const uint8_t* failed, int32_t flags, etc_plan** out, void* stream) {
   clear_error_detail();
   if (!old_l || !new_l || !device_map || !out) return ETC_ERR_INVALID_ARG;
-  if (flags < 0 || flags > (ETC_ALL_STAGED | ETC_KIND_MAJOR)) return ETC_ERR_INVALID_ARG;
+  if (flags < 0 || flags > (ETC_ALL_STAGED | ETC_KIND_MAJOR | ETC_ALL_DIRECT)) return ETC_ERR_INVALID_ARG;
+  if ((flags & ETC_ALL_STAGED) && (flags & ETC_ALL_DIRECT)) return ETC_ERR_INVALID_ARG;
   if (!etc_same_model(old_l, new_l)) return ETC_ERR_MISMATCH;
   const int n_old = old_l->t.n_dev, n_new = new_l->t.n_dev, P = n_old > n_new ? n_old : n_new;
   if ((long long)P * ETC_NUM_KINDS > 65535) return ETC_ERR_WORKSPACE;
@@ -582,7 +583,7 @@ extern "C" etc_status etc_plan_get_stats(const etc_plan* pl, etc_plan_stats* out
   if (!pl || !out) return ETC_ERR_INVALID_ARG;
   const PlanTotals& t = pl->totals;
   out->staging_bytes = t.staging_bytes; out->local_bytes = t.local_bytes; out->remote_bytes = t.remote_bytes;
-  out->staged_bytes = (pl->flags & ETC_ALL_STAGED) ? t.local_bytes + t.remote_bytes : t.remote_bytes;
+  out->staged_bytes = (pl->flags & ETC_ALL_STAGED) ? t.local_bytes + t.remote_bytes : ((pl->flags & ETC_ALL_DIRECT) ? 0 : t.remote_bytes);
   out->n_slices_local = t.n_slices_local; out->n_slices_staged = t.n_slices_staged;
   out->n_chunks_local = t.n_chunks_local; out->n_chunks_staged = t.n_chunks_staged;
   out->n_old = pl->n_old; out->n_new = pl->n_new; out->P = pl->P; out->flags = pl->flags;

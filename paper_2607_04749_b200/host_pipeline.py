@@ -45,6 +45,8 @@ class HostMigration:
         self.device = device or torch.device("cuda", torch.cuda.current_device())
         self.h_src, self.h_dst = h_src, h_dst
         self.flags = flags | B.ETC_KIND_MAJOR
+        if zero_copy and not (flags & B.ETC_ALL_STAGED):
+            self.flags |= B.ETC_ALL_DIRECT                         # one address space: a staging hop stands for nothing
         self.cap = int(max_staging_bytes)
         self.device_map = device_map
         self.needed_only = needed_only

@@ -185,7 +185,8 @@ def _check_migration(E, model, old_cfg, new_cfg, seed, device_map=None, flags=0,
     assert np.array_equal(g["plan"].traffic(), T)
     local = int(np.trace(T)); remote = int(T.sum() - np.trace(T))
     assert st.local_bytes == local and st.remote_bytes == remote and local + remote == int(need.sum())
-    assert st.staged_bytes == (local + remote if flags & E.ETC_ALL_STAGED else remote)
+    assert st.staged_bytes == (local + remote if flags & E.ETC_ALL_STAGED else (0 if flags & E.ETC_ALL_DIRECT else remote))
+    assert not (flags & E.ETC_ALL_DIRECT) or st.staging_bytes == 0
     for key, exp in dst.items():
         got = g["dst"][key]
         assert got.shape == exp.shape, key
@@ -217,7 +218,7 @@ def test_migrate_config1(E, flags):
 
 
 @pytest.mark.parametrize("name", ["s2", "s2odd", "s3", "s4", "s4odd", "s5"])
-@pytest.mark.parametrize("flags", [0, 1, 2, 3])              # 2, 3: + ETC_KIND_MAJOR (kind-major tables and staging)
+@pytest.mark.parametrize("flags", [0, 1, 2, 3, 4, 6])        # 2, 3: + ETC_KIND_MAJOR; 4, 6: ETC_ALL_DIRECT (nothing staged)
 def test_migrate_scaled_configs(E, name, flags):
     w = workload(name)
     _check_migration(E, w["model"], w["old"], w["new"], w["seed"], flags=flags)
