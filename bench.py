@@ -4,14 +4,19 @@
 A step = one pass of the whole hot path over one synthetic model state:
   (a1) etc_layout_create x2 -> (a2) etc_cost_matrix -> (a3) etc_sketch -> (a4) etc_plan_create -> (a5,a6) etc_migrate.
 metric = migrate GB/s counting read+write bytes: (2*direct + 4*staged payload bytes) / step time, plus the fraction of the
-measured HBM copy bandwidth the dominant copy kernel reaches (roofline) and the cost-matrix + sketch time.
+measured HBM copy bandwidth the copy kernels reach (roofline) and the cost-matrix + sketch time.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config c2] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config c4] [--impl reference]
+
+Default workload = c4 (BASELINE.json configs[3]): the largest configuration that fits one GPU (136 GB resident, 182 GB of
+HBM traffic per step), whose optimal sketch stages 35 GB through pack and unpack.  Everything the driver keeps lives in
+`config`, `roofline` (with `per_kernel` and `per_config`), `cpu_baseline`, `e2e`.
 N > 1 (torchrun): independent replicas, one per GPU ("replicas only": the path's only exchange step is closed by
 BASELINE.json, so there is no data-path collective); value = all ranks' bytes / max-over-ranks time.
 """
 from __future__ import annotations
 import argparse
+import gc
 import json
 import os
 import statistics
@@ -25,6 +30,8 @@ sys.path.insert(0, ROOT)
 
 METRIC = "migrate GB/s (read+write)"
 UNIT = "GB/s"
+NOMINAL_GBS = 8000.0          # BASELINE.json: "against roughly 8 TB/s"
+
 
 def ncu_traffic(workload_name: str, mode: str, kernel_prefix: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
@@ -122,15 +129,26 @@ def job_value(world: int, hbm_bytes_per_replica: int, ms_per_step: float) -> flo
     return world * hbm_bytes_per_replica / (ms_per_step * 1e-3) / 1e9
 
 
+def bench_config(w, all_staged: bool, world: int) -> dict:
+    """The `config` object of the JSON line: the same for the CUDA arm and for `--impl reference`."""
+    return {"workload": w["name"], "old": w["old"], "new": w["new"],
+            "mode": "ALL_STAGED" if all_staged else "LOCAL_DIRECT", "l2": "inputs_larger_than_L2",
+            "pipelining": "planning (a1-a4) of step i+1 on its own stream overlaps the copy kernels of step i",
+            "parallelism": "replicas only" if world > 1 else "1 GPU, all virtual devices in one HBM"}
+
+
 # ------------------------------------------------------------------------------------------------ reference arm (oracle)
-def oracle_sample(w, budget_elems=6_000_000, threads=1):
+def oracle_sample(w, budget_elems=6_000_000, threads=1, verify=True):
     """Time the CPU oracle, as it stands, on a bounded sample of the workload: cost matrix + sketch on the full layout
-    (they are metadata), then the element-wise migration of the first `m` elements of every new buffer.  threads > 1:
-    the (new rank, kind) buffers are independent, so they are handed to that many host threads (the oracle's C code
-    runs outside the GIL); each task counts into its own traffic matrix."""
+    (they are metadata), then the element-wise MIGRATION (oracle/etc_oracle.c orc_migrate_range: source rule A6, then one
+    memcpy per element from the old shard buffer into the new one) of the first `m` elements of every new buffer.
+    The old shard buffers are real, position-stamped host arrays; only the windows of them that the sample reads are
+    materialised (untimed preparation), so host memory stays bounded.  threads > 1: the (new rank, kind) buffers are
+    independent, so they are handed to that many host threads (the oracle's C code runs outside the GIL)."""
     import numpy as np
     from concurrent.futures import ThreadPoolExecutor
     from oracle import oracle as O
+    from etc_inputs import position_stamp, position_stamp_at
     oo, on = O.Layout(w["model"], w["old"]), O.Layout(w["model"], w["new"])
     t0 = time.perf_counter()
     ov, need, hold = O.overlap(oo, on, method="ranges")
@@ -140,27 +158,52 @@ def oracle_sample(w, budget_elems=6_000_000, threads=1):
     bufs = [(n, k, on.buffer_elems(n, k)) for n in range(on.n_dev) for k in on.kinds()]
     bufs = [b for b in bufs if b[2] > 0]
     m = max(1, budget_elems // max(1, len(bufs)))
-    # position-stamped source buffers would need the full state in host RAM; the oracle's migration time does not
-    # depend on the values, so the sample runs in traffic-counting mode plus a copy into a destination window.
-    src = None
     P = max(oo.n_dev, on.n_dev)
     moved = sum(min(m, cnt) * on.elem_bytes(k) for n, k, cnt in bufs)
+    pool = max(1, min(int(threads), len(bufs)))
+
+    def pmap(f, items):
+        if pool == 1:
+            return [f(x) for x in items]
+        with ThreadPoolExecutor(pool) as ex:
+            return list(ex.map(f, items))
+
+    # ---- untimed preparation: which window of which old buffer does each sampled range read?  One set of windows
+    #      per (new rank, kind) task: ranges of different new buffers read distant parts of the same old buffer
+    def prepare(b):
+        n, k, cnt = b
+        es = on.elem_bytes(k)
+        sd, sl = O.source_of(oo, on, dm, n, k, np.arange(min(m, cnt), dtype=np.int64))
+        win = {}
+        for o in np.unique(sd):
+            if o >= 0:
+                a, z = int(sl[sd == o].min()), int(sl[sd == o].max())
+                win[(int(o), k)] = (a, position_stamp(int(o), k, z - a + 1, es, start=a))
+        dst = np.empty(min(m, cnt), np.uint16 if es == 2 else np.uint32)
+        dst.fill(0xA5)                                     # touch the pages before the clock starts
+        return win, dst
+    prepared = dict(zip([(n, k) for n, k, _ in bufs], pmap(prepare, bufs)))
 
     def one(b):
         n, k, cnt = b
-        O.migrate_range(oo, on, dm, n, k, 0, min(m, cnt), src, None, np.zeros((P, P), np.int64), None)
+        win, dst = prepared[(n, k)]
+        O.migrate_range(oo, on, dm, n, k, 0, min(m, cnt), None, dst, np.zeros((P, P), np.int64), None, src_windows=win)
 
-    threads = max(1, min(int(threads), len(bufs)))
     t3 = time.perf_counter()
-    if threads == 1:
-        for b in bufs:
-            one(b)
-    else:
-        with ThreadPoolExecutor(threads) as ex:
-            list(ex.map(one, bufs))
+    pmap(one, bufs)
     t4 = time.perf_counter()
+    if verify:                                             # the bytes really moved: spot-check against the source rule
+        n, k, cnt = bufs[len(bufs) // 2]
+        idx = np.unique(np.linspace(0, min(m, cnt) - 1, 2048).astype(np.int64))
+        sd, sl = O.source_of(oo, on, dm, n, k, idx)
+        for o in np.unique(sd):
+            if o >= 0:
+                sel = sd == o
+                assert np.array_equal(prepared[(n, k)][1][idx[sel]], position_stamp_at(int(o), k, sl[sel], on.elem_bytes(k)))
+    src_bytes = sum(a.nbytes for win, _ in prepared.values() for _, a in win.values())
     return dict(cost_ms=(t1 - t0) * 1e3, sketch_ms=(t2 - t1) * 1e3, migrate_s=t4 - t3, payload_bytes=moved,
-                elems_per_buffer=m, n_buffers=len(bufs), local_opt=val, threads=O.max_threads(), migrate_threads=threads)
+                elems_per_buffer=m, n_buffers=len(bufs), local_opt=val, threads=O.max_threads(), migrate_threads=pool,
+                src_window_bytes=src_bytes)
 
 
 def oracle_metadata(w):
@@ -188,6 +231,11 @@ def oracle_metadata(w):
     return out
 
 
+def sample_text(o) -> str:
+    return (f"oracle migrates (memcpy per element) first {o['elems_per_buffer']} elems of {o['n_buffers']} new buffers, "
+            f"{o['payload_bytes']} B copied, {o['migrate_threads']} threads")
+
+
 def run_reference(args, w):
     rank, _, world = dist_env()
     if rank != 0:
@@ -196,22 +244,20 @@ def run_reference(args, w):
     O.build()
     times, last = [], None
     for i in range(args.warmup + args.steps):
-        t0 = time.perf_counter()
-        last = oracle_sample(w, budget_elems=args.ref_elems, threads=os.cpu_count() or 1)
-        dt = time.perf_counter() - t0
+        last = oracle_sample(w, budget_elems=args.ref_elems, threads=os.cpu_count() or 1, verify=(i == 0))
+        dt = (last["cost_ms"] + last["sketch_ms"]) * 1e-3 + last["migrate_s"]      # the step; window preparation is input setup
         if i >= args.warmup:
             times.append(dt)
     ms = statistics.mean(times) * 1e3
     # same metric: read+write bytes per second; the oracle copies each sampled payload byte once (1R + 1W)
     val = 2 * last["payload_bytes"] / (ms / 1e3) / 1e9
     cores = last["migrate_threads"]   # one host thread per (new rank, kind) buffer; the cost matrix uses OpenMP (below)
-    sample = (f"first {last['elems_per_buffer']} elements of each of {last['n_buffers']} new buffers "
-              f"({last['payload_bytes']} payload bytes, {cores} host threads) + full cost matrix (ranges routine, {last['threads']} OpenMP "
-              f"threads) + Hungarian, per step")
+    sample = sample_text(last) + " + full cost matrix + Hungarian, per step"
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "u8", "data": "synthetic", "config": {"workload": w["name"], "sample": sample},
+            "dtype": "u8", "data": "synthetic", "config": bench_config(w, args.all_staged, world),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                             "payload_GBs": last["payload_bytes"] / (ms / 1e3) / 1e9, "bytes_copied": last["payload_bytes"],
                              "cost_matrix_ms": last["cost_ms"], "sketch_ms": last["sketch_ms"]},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -219,11 +265,192 @@ def run_reference(args, w):
 
 
 # ------------------------------------------------------------------------------------------------ CUDA arm
+class Resident:
+    """One workload resident in HBM: old shard buffers (filled with the workload's value distribution), new shard
+    buffers, the staging buffer, and the pipelined whole-path step."""
+
+    def __init__(self, E, torch, w, dev, flags):
+        from etc_inputs import bench_fill_torch
+        from paper_2607_04749_b200.binding import pointer_tables
+        self.E, self.torch, self.w, self.dev, self.flags = E, torch, w, dev, flags
+        model = w["model"]
+        self.lay_old, self.lay_new = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])
+        self.src = E.alloc_buffers(self.lay_old, dev)
+        self.dst = E.alloc_buffers(self.lay_new, dev)
+        for (d, k), t in self.src.items():
+            view = t.view(torch.bfloat16 if (k == 0 and model["param_bytes"] == 2) else torch.float32)
+            bench_fill_torch(view, k, w["seed"] + d * 4 + k)
+        lo, ln = self.lay_old, self.lay_new
+        P = max(lo.n_dev, ln.n_dev)
+        self.out_cost = (torch.empty((ln.n_dev, P), dtype=torch.int64, device=dev),
+                         torch.empty(ln.n_dev, dtype=torch.int64, device=dev), torch.empty(P, dtype=torch.int64, device=dev))
+        self.out_sk = (torch.empty(ln.n_dev, dtype=torch.int32, device=dev), torch.empty(1, dtype=torch.int64, device=dev))
+        # staging sized once from a first plan (allocation is not part of the path)
+        ov, _, _ = E.etc_cost_matrix(lo, ln, out=self.out_cost)
+        dm, _ = E.etc_sketch(ov, out=self.out_sk)
+        plan0 = E.etc_plan_create(lo, ln, dm, flags)
+        self.stats = plan0.stats
+        self.staging = torch.empty(max(self.stats.staging_bytes, 16), dtype=torch.uint8, device=dev)
+        self.src_tab, self.dst_tab = pointer_tables(plan0, self.src, self.dst)
+        del plan0
+        self.stream = torch.cuda.current_stream()
+        self.plan_stream = torch.cuda.Stream(dev, priority=-1)   # high priority: its small kernels cut in front of copy CTAs
+        self.planned = [torch.cuda.Event() for _ in range(4)]
+        self.step_no = 0
+
+    def ev(self):
+        return self.torch.cuda.Event(enable_timing=True)
+
+    def step(self, record=None):
+        """One pass of the whole hot path.  Planning (a1-a4, metadata only) is enqueued on its own stream so that it
+        does not wait for the previous step's copy kernels; the copy stream waits for the plan by event.  record: list
+        to which this step's timing events are appended."""
+        E, torch, w = self.E, self.torch, self.w
+        ps, stream = self.plan_stream, self.stream
+        e = [self.ev() for _ in range(8)] if record is not None else None
+        with torch.cuda.stream(ps):
+            if e: e[0].record(ps)
+            lo, ln = E.etc_layout_create(w["model"], w["old"]), E.etc_layout_create(w["model"], w["new"])      # (a1)
+            if e: e[1].record(ps)
+            ov, need, hold = E.etc_cost_matrix(lo, ln, out=self.out_cost, stream=ps)                            # (a2)
+            if e: e[2].record(ps)
+            dm, lb = E.etc_sketch(ov, out=self.out_sk, stream=ps)                                               # (a3)
+            if e: e[3].record(ps)
+            plan = E.etc_plan_create(lo, ln, dm, self.flags, stream=ps)                                         # (a4)
+            if e: e[4].record(ps)
+            done = self.planned[self.step_no % len(self.planned)]
+            done.record(ps)
+        self.step_no += 1
+        stream.wait_event(done)
+        if e: e[7].record(stream)
+        E.etc_migrate(plan, self.src_tab, self.dst_tab, self.staging, E.ETC_PHASE_PACK, stream=stream)     # (a5) + local
+        if e: e[5].record(stream)
+        E.etc_migrate(plan, self.src_tab, self.dst_tab, self.staging, E.ETC_PHASE_UNPACK, stream=stream)   # (a6)
+        if e: e[6].record(stream)
+        if record is not None:
+            record.append(e)
+        return plan
+
+    def timed(self, steps, warmup, barrier, world, sampler=None):
+        """W warm-up steps, then exactly K steps between barrier + synchronize; device time, max over ranks."""
+        E, torch = self.E, self.torch
+        for _ in range(max(warmup, 3)):
+            self.step()
+        barrier()
+        if sampler:
+            sampler.start()
+        launches0 = E.kernel_launches()
+        recs = []
+        t_begin, t_end = self.ev(), self.ev()
+        barrier()
+        t_begin.record(self.stream)
+        for _ in range(steps):
+            plan = self.step(recs)
+        t_end.record(self.stream)
+        barrier()
+        launches = E.kernel_launches() - launches0
+        clocks = sampler.stop() if sampler else None
+        ms_per_step = max_over_ranks(t_begin.elapsed_time(t_end), world, self.dev) / steps
+        phase = lambda a, b: statistics.mean(r[a].elapsed_time(r[b]) for r in recs)
+        bd = {"layout_ms": phase(0, 1), "cost_matrix_ms": phase(1, 2), "sketch_ms": phase(2, 3), "plan_ms": phase(3, 4),
+              "pack_local_ms": phase(7, 5), "unpack_ms": phase(5, 6)}
+        self.stats = plan.stats
+        return dict(ms_per_step=ms_per_step, breakdown=bd, launches=launches, clocks=clocks, stats=plan.stats)
+
+    def one_shot(self, reps=8):
+        """One migration, cold start to finish, nothing overlapped: (a1)-(a6) on one stream, host wall clock from the
+        first call to the synchronise after the last kernel (the latency a single reconfiguration sees)."""
+        E, torch, w = self.E, self.torch, self.w
+        walls = []
+        for i in range(reps):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            lo, ln = E.etc_layout_create(w["model"], w["old"]), E.etc_layout_create(w["model"], w["new"])
+            ov, _, _ = E.etc_cost_matrix(lo, ln, out=self.out_cost)
+            dm, _ = E.etc_sketch(ov, out=self.out_sk)
+            plan = E.etc_plan_create(lo, ln, dm, self.flags)
+            E.etc_migrate(plan, self.src_tab, self.dst_tab, self.staging)
+            torch.cuda.synchronize()
+            if i >= 3:
+                walls.append((time.perf_counter() - t0) * 1e3)
+        return statistics.median(walls)
+
+    def close(self):
+        self.src = self.dst = self.staging = self.src_tab = self.dst_tab = None
+        self.lay_old = self.lay_new = None
+        gc.collect()
+        self.torch.cuda.empty_cache()
+
+
+def kernel_entry(nbytes, ms, peak):
+    gbs = nbytes / (ms * 1e-3) / 1e9 if ms and ms > 0 and nbytes else 0.0
+    return {"bytes": int(nbytes), "ms": ms, "GBs": gbs, "frac": gbs / peak, "frac_8TBs": gbs / NOMINAL_GBS}
+
+
+def copy_launch_bytes(stats):
+    direct = stats.local_bytes + stats.remote_bytes - stats.staged_bytes
+    return 2 * (stats.staged_bytes + direct), 2 * stats.staged_bytes     # launch 1: pack + local; launch 2: unpack
+
+
+def all_staged_rates(E, torch, R, peak):
+    """Pack and unpack with EVERY slice staged (ETC_ALL_STAGED), on the resident workload: each kernel moves the whole
+    payload.  If the full staging buffer does not fit beside the shards, the plan is cut into rounds of bounded staging
+    (etc_plan_set_rounds) and the pack / unpack launches of all rounds are summed."""
+    ev = R.ev
+    stream = R.stream
+    ov, _, _ = E.etc_cost_matrix(R.lay_old, R.lay_new, out=R.out_cost)
+    dm, _ = E.etc_sketch(ov, out=R.out_sk)
+    R.staging = None
+    torch.cuda.empty_cache()
+    plan = E.etc_plan_create(R.lay_old, R.lay_new, dm, E.ETC_ALL_STAGED | E.ETC_KIND_MAJOR)
+    need = plan.stats.staging_bytes
+    free_b, _ = torch.cuda.mem_get_info(R.dev)
+    cap = need if need + (2 << 30) <= free_b else max(1 << 30, (free_b - (3 << 30)))
+    rounds = E.etc_plan_set_rounds(plan, cap)
+    stg = torch.empty(max(max(r.staging_bytes for r in rounds), 16), dtype=torch.uint8, device=R.dev)
+    tp, tu = [], []
+    for i in range(6):
+        p_ms = u_ms = 0.0
+        evs = []
+        for j in range(len(rounds)):
+            a, b, c = ev(), ev(), ev()
+            a.record(stream); E.etc_migrate_round(plan, j, R.src_tab, R.dst_tab, stg, E.ETC_PHASE_PACK)
+            b.record(stream); E.etc_migrate_round(plan, j, R.src_tab, R.dst_tab, stg, E.ETC_PHASE_UNPACK)
+            c.record(stream)
+            evs.append((a, b, c))
+        torch.cuda.synchronize()
+        for a, b, c in evs:
+            p_ms += a.elapsed_time(b); u_ms += b.elapsed_time(c)
+        if i >= 2:
+            tp.append(p_ms); tu.append(u_ms)
+    nbytes = 2 * plan.stats.staged_bytes
+    out = {"all_staged_pack": kernel_entry(nbytes, statistics.mean(tp), peak),
+           "all_staged_unpack": kernel_entry(nbytes, statistics.mean(tu), peak)}
+    out["all_staged_pack"]["rounds"] = out["all_staged_unpack"]["rounds"] = len(rounds)
+    del stg, plan
+    torch.cuda.empty_cache()
+    return out
+
+
+def config_entry(res, peak, one_shot_ms=None):
+    st, bd = res["stats"], res["breakdown"]
+    b1, b2 = copy_launch_bytes(st)
+    k1, k2 = kernel_entry(b1, bd["pack_local_ms"], peak), kernel_entry(b2, bd["unpack_ms"], peak)
+    out = {"step_ms": res["ms_per_step"], "GBs": st.hbm_bytes / res["ms_per_step"] / 1e6, "hbm_bytes": st.hbm_bytes,
+           "staged_bytes": st.staged_bytes,
+           "pack_local_ms": k1["ms"], "pack_local_GBs": k1["GBs"], "pack_local_frac": k1["frac"],
+           "unpack_ms": k2["ms"], "unpack_GBs": k2["GBs"], "unpack_frac": k2["frac"],
+           "cost_sketch_ms": bd["cost_matrix_ms"] + bd["sketch_ms"], "plan_ms": bd["plan_ms"], "layout_ms": bd["layout_ms"]}
+    if one_shot_ms is not None:
+        out["one_shot_ms"] = one_shot_ms
+        out["one_shot_GBs"] = st.hbm_bytes / one_shot_ms / 1e6
+    return out
+
+
 def run_cuda(args, w):
-    import numpy as np
     import torch
     import paper_2607_04749_b200 as E
-    from etc_inputs import bench_fill_torch
+    from etc_inputs import workload
 
     rank, local_rank, world = dist_env()
     torch.cuda.set_device(local_rank)
@@ -232,161 +459,117 @@ def run_cuda(args, w):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
     E.init(local_rank)
-    model = w["model"]
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- resident inputs: every old shard buffer filled with the workload's value distribution
-    lay_old, lay_new = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])
-    src = E.alloc_buffers(lay_old, dev)
-    dst = E.alloc_buffers(lay_new, dev)
-    for (d, k), t in src.items():
-        view = t.view(torch.bfloat16 if (k == 0 and model["param_bytes"] == 2) else torch.float32)
-        bench_fill_torch(view, k, w["seed"] + d * 4 + k)
-    P = max(lay_old.n_dev, lay_new.n_dev)
-    out_cost = (torch.empty((lay_new.n_dev, P), dtype=torch.int64, device=dev),
-                torch.empty(lay_new.n_dev, dtype=torch.int64, device=dev), torch.empty(P, dtype=torch.int64, device=dev))
-    out_sk = (torch.empty(lay_new.n_dev, dtype=torch.int32, device=dev), torch.empty(1, dtype=torch.int64, device=dev))
+    peak, peak_src = measured_peak()
     flags = E.ETC_ALL_STAGED if args.all_staged else E.ETC_LOCAL_DIRECT
-    # staging sized once from a first plan (allocation is not part of the path)
-    ov, _, _ = E.etc_cost_matrix(lay_old, lay_new, out=out_cost)
-    dm, _ = E.etc_sketch(ov, out=out_sk)
-    plan0 = E.etc_plan_create(lay_old, lay_new, dm, flags)
-    st0 = plan0.stats
-    staging = torch.empty(max(st0.staging_bytes, 16), dtype=torch.uint8, device=dev)
-    from paper_2607_04749_b200.binding import pointer_tables
-    src_tab, dst_tab = pointer_tables(plan0, src, dst)
-    hbm_bytes = st0.hbm_bytes
-    del plan0
+    mode = "ALL_STAGED" if args.all_staged else "LOCAL_DIRECT"
 
-    stream = torch.cuda.current_stream()
-    ev = lambda: torch.cuda.Event(enable_timing=True)
-
-    plan_stream = torch.cuda.Stream(dev, priority=-1)     # high priority: its small kernels cut in front of copy CTAs
-    planned = [torch.cuda.Event() for _ in range(4)]
-    step_no = [0]
-
-    def step(record=None):
-        """One pass of the whole hot path.  Planning (a1-a4, metadata only, one host sync for table sizes) is enqueued
-        on its own stream so that its host sync does not wait for the previous step's copy kernels; the copy stream waits
-        for the plan by event.  record: list to which this step's timing events are appended."""
-        e = [ev() for _ in range(8)] if record is not None else None
-        with torch.cuda.stream(plan_stream):
-            if e: e[0].record(plan_stream)
-            lo, ln = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])     # (a1)
-            if e: e[1].record(plan_stream)
-            ov, need, hold = E.etc_cost_matrix(lo, ln, out=out_cost, stream=plan_stream)             # (a2)
-            if e: e[2].record(plan_stream)
-            dm, lb = E.etc_sketch(ov, out=out_sk, stream=plan_stream)                                # (a3)
-            if e: e[3].record(plan_stream)
-            plan = E.etc_plan_create(lo, ln, dm, flags, stream=plan_stream)                          # (a4)
-            if e: e[4].record(plan_stream)
-            done = planned[step_no[0] % len(planned)]
-            done.record(plan_stream)
-        step_no[0] += 1
-        stream.wait_event(done)
-        if e: e[7].record(stream)
-        E.etc_migrate(plan, src_tab, dst_tab, staging, E.ETC_PHASE_PACK, stream=stream)          # (a5) + local
-        if e: e[5].record(stream)
-        E.etc_migrate(plan, src_tab, dst_tab, staging, E.ETC_PHASE_UNPACK, stream=stream)        # (a6)
-        if e: e[6].record(stream)
-        if record is not None:
-            record.append(e)
-        return plan
-
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    launches0 = E.kernel_launches()
-    recs = []
-    t_begin, t_end = ev(), ev()
-    barrier()
-    t_begin.record(stream)
-    for _ in range(args.steps):
-        plan = step(recs)
-    t_end.record(stream)
-    barrier()
-    launches = E.kernel_launches() - launches0
-    clocks = sampler.stop()
-    total_ms = t_begin.elapsed_time(t_end)
-    total_ms = max_over_ranks(total_ms, world, dev)
-    ms_per_step = total_ms / args.steps
-    stats = plan.stats
-    phase = lambda a, b: statistics.mean(r[a].elapsed_time(r[b]) for r in recs)
-    bd = {"layout_ms": phase(0, 1), "cost_matrix_ms": phase(1, 2), "sketch_ms": phase(2, 3), "plan_ms": phase(3, 4),
-          "pack_local_ms": phase(7, 5), "unpack_ms": phase(5, 6)}
+    # ---- the timed line: whole path on the headline workload, inputs resident in HBM
+    R = Resident(E, torch, w, dev, flags)
+    res = R.timed(args.steps, args.warmup, barrier, world, ClockSampler(local_rank))
+    stats, bd, ms_per_step = res["stats"], res["breakdown"], res["ms_per_step"]
+    hbm_bytes = stats.hbm_bytes
     value = job_value(world, hbm_bytes, ms_per_step)
 
     # ---- roofline of the dominant kernel, timed live with CUDA events over the timed region
-    peak, peak_src = measured_peak()
-    direct = stats.local_bytes + stats.remote_bytes - stats.staged_bytes
-    k1_bytes = 2 * (stats.staged_bytes + direct)       # launch 1: pack (staged payload) + local (direct payload): 1R+1W
-    k2_bytes = 2 * stats.staged_bytes                  # launch 2: unpack
+    k1_bytes, k2_bytes = copy_launch_bytes(stats)
+    per_kernel = {"pack_local": kernel_entry(k1_bytes, bd["pack_local_ms"], peak),
+                  "unpack": kernel_entry(k2_bytes, bd["unpack_ms"], peak)}
+    per_kernel["pack_local"]["kernel"] = "migrate_copy_kernel<false>"
+    per_kernel["pack_local"]["staged_bytes_packed"] = stats.staged_bytes
+    per_kernel["unpack"]["kernel"] = "migrate_copy_kernel<true>"
     if bd["pack_local_ms"] >= bd["unpack_ms"]:
-        kname, kbytes, kms = "migrate_copy_kernel<false> (pack + local)", k1_bytes, bd["pack_local_ms"]
+        kname, dom = "migrate_copy_kernel<false> (pack + local)", per_kernel["pack_local"]
     else:
-        kname, kbytes, kms = "migrate_copy_kernel<true> (unpack)", k2_bytes, bd["unpack_ms"]
-    achieved = kbytes / (kms * 1e-3) / 1e9 if kms > 0 else 0.0
-    roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "peak_source": peak_src, "algorithmic_bytes_per_launch": kbytes,
-                "avg_launch_ms": kms, "traffic": ncu_traffic(w["name"], "ALL_STAGED" if args.all_staged else "LOCAL_DIRECT", kname),
-                "frac_of_8TBs_nominal": achieved / 8000.0}
+        kname, dom = "migrate_copy_kernel<true> (unpack)", per_kernel["unpack"]
+    roofline = {"bound": "hbm", "kernel": kname, "achieved": dom["GBs"], "peak": peak, "unit": "GB/s",
+                "frac": dom["frac"], "peak_source": peak_src, "algorithmic_bytes_per_launch": dom["bytes"],
+                "avg_launch_ms": dom["ms"], "traffic": ncu_traffic(w["name"], mode, kname),
+                "frac_of_8TBs_nominal": dom["frac_8TBs"], "staged_bytes_per_step": stats.staged_bytes,
+                "per_kernel": per_kernel}
+    for key, kn in (("pack_local", "migrate_copy_kernel<false>"), ("unpack", "migrate_copy_kernel<true>")):
+        per_kernel[key]["traffic"] = ncu_traffic(w["name"], mode, kn)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "u8", "data": "synthetic",
-            "config": {"workload": w["name"], "old": w["old"], "new": w["new"],
-                       "mode": "ALL_STAGED" if args.all_staged else "LOCAL_DIRECT", "l2": "inputs_larger_than_L2",
-                       "pipelining": "planning (a1-a4) of step i+1 on its own stream overlaps the copy kernels of step i",
-                       "parallelism": "replicas only" if world > 1 else "1 GPU, all virtual devices in one HBM"},
+            "vs_baseline": None, "dtype": "u8", "data": "synthetic", "config": bench_config(w, args.all_staged, world),
             "hbm_bytes_per_step": hbm_bytes, "payload": {"local": stats.local_bytes, "remote": stats.remote_bytes,
                                                          "staged": stats.staged_bytes},
             "breakdown_ms": bd, "cost_sketch_ms": bd["cost_matrix_ms"] + bd["sketch_ms"],
-            "roofline": roofline, "clocks": clocks, "gpu_launches": launches}
+            "roofline": roofline, "clocks": res["clocks"], "gpu_launches": res["launches"]}
+    line["config"]["cost_sketch_ms"] = line["cost_sketch_ms"]
+    line["config"]["hbm_bytes_per_step"] = hbm_bytes
 
-    del staging
-    torch.cuda.empty_cache()
-    if rank == 0 and not args.no_extras:
-        line["extras"] = extras(E, torch, w, dev, src, dst, lay_old, lay_new, peak)
+    per_config = {w["name"]: config_entry(res, peak)}
+    extras_on = rank == 0 and not args.no_extras
+    if extras_on:
+        try:
+            per_config[w["name"]]["one_shot_ms"] = R.one_shot()
+        except Exception as ex:
+            per_config[w["name"]]["one_shot_error"] = repr(ex)[:120]
+        if not args.all_staged:
+            try:
+                per_kernel.update(all_staged_rates(E, torch, R, peak))
+            except Exception as ex:
+                per_kernel["all_staged_error"] = repr(ex)[:160]
+    R.close()
+    del R
 
-    # ---- e2e: the same step through the C ABI with HOST buffers; H2D of every old shard and D2H of every new shard
-    #      are inside the timed region
+    # ---- the other configs of BASELINE.json, same build, same measurement (short runs), and the 512 -> 384 metadata case
+    if extras_on:
+        for name in args.per_config.split(","):
+            name = name.strip()
+            if not name or name == w["name"]:
+                continue
+            try:
+                wi = workload(name)
+                Ri = Resident(E, torch, wi, dev, flags)
+                ri = Ri.timed(args.config_steps, 3, barrier, 1)
+                per_config[name] = config_entry(ri, peak, Ri.one_shot())
+                Ri.close()
+                del Ri
+            except Exception as ex:
+                per_config[name] = {"error": repr(ex)[:160]}
+                gc.collect(); torch.cuda.empty_cache()
+        try:
+            per_config["c5b"] = metadata_only(E, torch, workload("c5b"))
+        except Exception as ex:
+            per_config["c5b"] = {"error": repr(ex)[:160]}
+        roofline["per_config"] = per_config
+        line["extras"] = extras(E, torch)
+
+    # ---- e2e: the same step through the C ABI with HOST buffers; every host<->device byte inside the timed region
     if not args.no_e2e:
         try:
-            line["e2e"] = e2e(E, torch, args, w, dev, src, dst, hbm_bytes, world, barrier)
+            line["e2e"] = e2e(E, torch, args, w, dev, world, barrier)
         except Exception as ex:       # e.g. not enough pinned host memory on the box
             line["e2e"] = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
-    if rank == 0 and not args.no_extras:
-        try:                          # destroys src: last GPU leg
-            del dst
-            torch.cuda.empty_cache()
-            line["extras"]["chunked_eager_release"] = chunked(E, torch, w, dev, src, lay_old, lay_new, args.e2e_staging)
+    if extras_on:
+        try:
+            line["extras"]["chunked_eager_release"] = chunked(E, torch, workload(args.chunked_config), dev, args.e2e_staging)
         except Exception as ex:
             line["extras"]["chunked_eager_release"] = {"error": repr(ex)[:200]}
 
     if rank == 0:
         if world == 1 and not args.no_cpu:
-            from oracle import oracle as O
             ncores = os.cpu_count() or 1
-            o = oracle_sample(w, budget_elems=args.cpu_elems, threads=ncores)          # all host cores (SURVEY.md 8(d))
-            o1 = oracle_sample(w, budget_elems=max(1, args.cpu_elems // 8), threads=1)  # single-thread figure
+            o = oracle_sample(w, budget_elems=args.cpu_elems, threads=ncores)           # all host cores
+            o1 = oracle_sample(w, budget_elems=max(1, args.cpu_elems // 8), threads=1, verify=False)  # single thread
             line["cpu_baseline"] = {
                 "value": 2 * o["payload_bytes"] / o["migrate_s"] / 1e9, "unit": UNIT, "cores": o["migrate_threads"],
-                "kind": "oracle",
-                "sample": f"element-wise oracle migration of the first {o['elems_per_buffer']} elements of each of "
-                          f"{o['n_buffers']} new buffers ({o['payload_bytes']} payload bytes, 1R+1W each), the independent "
-                          f"buffers spread over {o['migrate_threads']} host threads; host has {ncores} cores",
+                "kind": "oracle", "sample": sample_text(o),
+                "payload_GBs": o["payload_bytes"] / o["migrate_s"] / 1e9, "bytes_copied": o["payload_bytes"],
+                "migrate_s": o["migrate_s"], "src_window_bytes": o["src_window_bytes"], "host_cores": ncores,
                 "single_thread_value": 2 * o1["payload_bytes"] / o1["migrate_s"] / 1e9,
                 "single_thread_sample": f"first {o1['elems_per_buffer']} elements of each buffer, 1 thread",
                 "cost_matrix_ms": o["cost_ms"], "sketch_ms": o["sketch_ms"], "cost_matrix_threads": o["threads"]}
             try:
-                from etc_inputs import workload as _wl
-                line["cpu_baseline"]["metadata"] = {w["name"]: oracle_metadata(w), "c5b": oracle_metadata(_wl("c5b"))}
+                line["cpu_baseline"]["metadata"] = {w["name"]: oracle_metadata(w), "c5b": oracle_metadata(workload("c5b"))}
             except Exception as ex:
                 line["cpu_baseline"]["metadata"] = {"error": repr(ex)[:200]}
         print(json.dumps(line), flush=True)
@@ -394,60 +577,30 @@ def run_cuda(args, w):
         dist.destroy_process_group()
 
 
-def extras(E, torch, w, dev, src, dst, lay_old, lay_new, peak):
-    """Context numbers outside the timed region: pack / unpack kernel rates with everything staged, and the
-    metadata-only cost matrix + sketch of the 512 -> 384 device layout (BASELINE.json configs[4])."""
+def metadata_only(E, torch, wb):
+    """cost matrix + sketch of the metadata-only 512 -> 384 device layout (BASELINE.json configs[4])."""
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    stream = torch.cuda.current_stream()
+    lo, ln = E.etc_layout_create(wb["model"], wb["old"]), E.etc_layout_create(wb["model"], wb["new"])
+    tc, ts = [], []
+    for i in range(6):
+        a, b, c = ev(), ev(), ev()
+        a.record(stream); ov, _, _ = E.etc_cost_matrix(lo, ln)
+        b.record(stream); dm, lb = E.etc_sketch(ov)
+        c.record(stream); torch.cuda.synchronize()
+        if i >= 2:
+            tc.append(a.elapsed_time(b)); ts.append(b.elapsed_time(c))
+    return {"cost_matrix_ms": statistics.mean(tc), "sketch_ms": statistics.mean(ts),
+            "cost_sketch_ms": statistics.mean(tc) + statistics.mean(ts),
+            "local_bytes": int(lb.item()), "devices": [lo.n_dev, ln.n_dev], "pieces": [lo.n_pieces, ln.n_pieces]}
+
+
+def extras(E, torch):
+    """Context numbers outside the timed region (metadata only)."""
     from etc_inputs import workload
     out = {}
     ev = lambda: torch.cuda.Event(enable_timing=True)
     stream = torch.cuda.current_stream()
-    try:
-        ov, _, _ = E.etc_cost_matrix(lay_old, lay_new)
-        dm, _ = E.etc_sketch(ov)
-        plan = E.etc_plan_create(lay_old, lay_new, dm, E.ETC_ALL_STAGED)
-        stg = torch.empty(max(plan.stats.staging_bytes, 16), dtype=torch.uint8, device=dev)
-        tp, tu = [], []
-        for i in range(8):
-            a, b, c = ev(), ev(), ev()
-            a.record(stream); E.etc_migrate(plan, src, dst, stg, E.ETC_PHASE_PACK)
-            b.record(stream); E.etc_migrate(plan, src, dst, stg, E.ETC_PHASE_UNPACK)
-            c.record(stream); torch.cuda.synchronize()
-            if i >= 3:
-                tp.append(a.elapsed_time(b)); tu.append(b.elapsed_time(c))
-        nbytes = 2 * plan.stats.staged_bytes
-        out["all_staged"] = {"staged_bytes": plan.stats.staged_bytes, "pack_ms": statistics.mean(tp),
-                             "unpack_ms": statistics.mean(tu),
-                             "pack_GBs": nbytes / statistics.mean(tp) / 1e6, "unpack_GBs": nbytes / statistics.mean(tu) / 1e6,
-                             "pack_frac_of_measured_peak": nbytes / statistics.mean(tp) / 1e6 / peak,
-                             "unpack_frac_of_measured_peak": nbytes / statistics.mean(tu) / 1e6 / peak}
-        del stg, plan
-    except Exception as ex:
-        out["all_staged"] = {"error": repr(ex)[:200]}
-    try:
-        # one migration, cold start to finish, nothing overlapped: (a1)-(a6) on one stream, host wall clock from the
-        # first call to the synchronise after the last kernel (the latency a single reconfiguration sees)
-        walls = []
-        for i in range(8):
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            lo, ln = E.etc_layout_create(w["model"], w["old"]), E.etc_layout_create(w["model"], w["new"])
-            ov, _, _ = E.etc_cost_matrix(lo, ln)
-            dm, _ = E.etc_sketch(ov)
-            plan = E.etc_plan_create(lo, ln, dm, 0)
-            if i == 0:
-                stg = torch.empty(max(plan.stats.staging_bytes, 16), dtype=torch.uint8, device=dev)
-            E.etc_migrate(plan, src, dst, stg)
-            torch.cuda.synchronize()
-            if i >= 3:
-                walls.append((time.perf_counter() - t0) * 1e3)
-        hb = 2 * plan.stats.local_bytes + 4 * plan.stats.remote_bytes
-        out["one_shot"] = {"wall_ms_median": statistics.median(walls), "wall_ms_best": min(walls),
-                           "GBs": hb / statistics.median(walls) / 1e6,
-                           "note": "a1-a6 serially on one stream, host wall clock incl. every host-side step, no overlap "
-                                   "with a previous migration"}
-        del stg, plan
-    except Exception as ex:
-        out["one_shot"] = {"error": repr(ex)[:200]}
     try:
         # (f1) virtual rank allocator on config 3's pre-emption (16 -> 12 devices, 4 per node), metadata only: bytes
         # that change device under the sketch alone, under the sketch composed with Algorithm 2 (one hop: communication
@@ -473,51 +626,76 @@ def extras(E, torch, w, dev, src, dst, lay_old, lay_new, peak):
         del p0, p1
     except Exception as ex:
         out["defrag_c3_16_to_12"] = {"error": repr(ex)[:200]}
-    try:
-        wb = workload("c5b")
-        lo, ln = E.etc_layout_create(wb["model"], wb["old"]), E.etc_layout_create(wb["model"], wb["new"])
-        tc, ts = [], []
-        for i in range(6):
-            a, b, c = ev(), ev(), ev()
-            a.record(stream); ov, _, _ = E.etc_cost_matrix(lo, ln)
-            b.record(stream); dm, lb = E.etc_sketch(ov)
-            c.record(stream); torch.cuda.synchronize()
-            if i >= 2:
-                tc.append(a.elapsed_time(b)); ts.append(b.elapsed_time(c))
-        out["c5b_512_to_384"] = {"cost_matrix_ms": statistics.mean(tc), "sketch_ms": statistics.mean(ts),
-                                 "local_bytes": int(lb.item()), "pieces": [lo.n_pieces, ln.n_pieces]}
-    except Exception as ex:
-        out["c5b_512_to_384"] = {"error": repr(ex)[:200]}
     return out
 
 
-def e2e(E, torch, args, w, dev, src, dst, hbm_bytes, world, barrier):
+def host_memory_ok(nbytes: int) -> bool:
+    """Can `nbytes` of pinned host memory be asked for without endangering the box?"""
+    try:
+        import psutil
+        return psutil.virtual_memory().available > nbytes * 1.25 + (8 << 30)
+    except Exception:
+        return nbytes < (24 << 30)
+
+
+def e2e(E, torch, args, w, dev, world, barrier):
     """The same metric through the public API with HOST buffers: old shards in pinned host memory -> whole path (a1-a6,
     as kind-by-kind rounds of a kind-major plan) -> new shards in pinned host memory, everything inside the timed region.
-    Headline: zero-copy (host_pipeline.HostMigration(zero_copy=True)): the pinned host buffers ARE the source and
-    destination tables of the C-ABI call, the copy kernels move every byte over PCIe, no device copy of any shard exists.
-    Beside it: the DMA pipelines (cudaMemcpyAsync of every old shard byte / of only the regions the plan reads, rounds
-    on device buffers, cudaMemcpyAsync of the new shards; three streams)."""
+    Runs on the headline workload if its old + new shards can be pinned in host memory on every rank, else on the largest
+    BASELINE.json config that can (named in `config`).  Legs: zero-copy (the pinned host buffers ARE the source and
+    destination tables of the C-ABI call, the copy kernels move every byte over PCIe), and the DMA pipeline that uploads
+    only the regions the plan reads (etc_upload_sources); the faster one is the headline, both are reported."""
+    from etc_inputs import workload, bench_fill_torch
     from paper_2607_04749_b200.host_pipeline import HostMigration
-    # pinning the host copies is the step that can fail on one rank only (host memory): agree on it before any
-    # collective, so that no rank is left waiting in a barrier
-    ok, h_src, h_dst = 1.0, {}, {}
-    try:
-        h_src = {k: torch.empty(t.shape, dtype=t.dtype, pin_memory=True) for k, t in src.items()}
-        h_dst = {k: torch.empty(t.shape, dtype=t.dtype, pin_memory=True) for k, t in dst.items()}
-    except Exception:
-        ok = 0.0
-    if -max_over_ranks(-ok, world, dev) < 0.5:
-        h_src = h_dst = None
+    order = [w["name"]] + [c for c in ("c3", "c2", "c1") if c != w["name"]]
+    if args.e2e_config:
+        order = [args.e2e_config]
+    chosen = None
+    for name in order:
+        wi = workload(name)
+        lo, ln = E.etc_layout_create(wi["model"], wi["old"]), E.etc_layout_create(wi["model"], wi["new"])
+        total = lo.total_bytes() + ln.total_bytes()
+        ok = 1.0 if (total <= args.e2e_max_bytes and host_memory_ok(total)) else 0.0
+        h_src, h_dst = {}, {}
+        if ok:
+            try:
+                for d in range(lo.n_dev):
+                    for k in lo.kinds():
+                        nb = lo.buffer_bytes(d, k)
+                        if nb:
+                            h_src[(d, k)] = torch.empty(nb, dtype=torch.uint8, pin_memory=True)
+                for n in range(ln.n_dev):
+                    for k in ln.kinds():
+                        nb = ln.buffer_bytes(n, k)
+                        if nb:
+                            h_dst[(n, k)] = torch.empty(nb, dtype=torch.uint8, pin_memory=True)
+            except Exception:
+                ok = 0.0
+                h_src, h_dst = {}, {}
+        if -max_over_ranks(-ok, world, dev) > 0.5:          # every rank could pin it
+            chosen = (wi, lo, ln, h_src, h_dst)
+            break
+        del h_src, h_dst
+        gc.collect()
+    if chosen is None:
         raise RuntimeError("pinned host buffers for the old and new shards could not be allocated on every rank")
-    for k, t in src.items():
-        h_src[k].copy_(t)
+    wi, lo, ln, h_src, h_dst = chosen
+    model = wi["model"]
+    # fill the host copies with the workload's value distribution (through a bounded device scratch buffer)
+    big = max(t.numel() for t in h_src.values())
+    scratch = torch.empty(big, dtype=torch.uint8, device=dev)
+    for (d, k), t in h_src.items():
+        view = scratch[: t.numel()].view(torch.bfloat16 if (k == 0 and model["param_bytes"] == 2) else torch.float32)
+        bench_fill_torch(view, k, wi["seed"] + d * 4 + k)
+        t.copy_(scratch[: t.numel()])
     torch.cuda.synchronize()
+    del scratch
+    torch.cuda.empty_cache()
     n = max(1, min(args.steps, args.e2e_steps))
     flags = E.ETC_ALL_STAGED if args.all_staged else E.ETC_LOCAL_DIRECT
 
     def leg(**kw):
-        mk = lambda: HostMigration(w["model"], w["old"], w["new"], h_src, h_dst, dev, args.e2e_staging, flags, **kw)
+        mk = lambda: HostMigration(model, wi["old"], wi["new"], h_src, h_dst, dev, args.e2e_staging, flags, **kw)
         warm = mk(); warm.run(); barrier()
         hm = mk()
         del warm
@@ -526,35 +704,40 @@ def e2e(E, torch, args, w, dev, src, dst, hbm_bytes, world, barrier):
             plan = hm.run()
         barrier()
         ms = max_over_ranks(hm.begin.elapsed_time(hm.done) / n, world, dev)
-        return {"value": job_value(world, hbm_bytes, ms), "unit": UNIT, "ms_per_step": ms, "steps": n,
-                "h2d_bytes_per_step": hm.h2d_bytes, "d2h_bytes_per_step": hm.d2h_bytes,
-                "pcie_GBs_each_way": [hm.h2d_bytes / ms / 1e6, hm.d2h_bytes / ms / 1e6],
-                "rounds": len(plan.rounds), "staging_bytes": args.e2e_staging}
+        hb = plan.stats.local_bytes * 2 + plan.stats.remote_bytes * 4      # the metric's bytes (LOCAL_DIRECT accounting)
+        out = {"value": job_value(world, hb, ms), "unit": UNIT, "ms_per_step": ms, "steps": n,
+               "h2d_bytes_per_step": hm.h2d_bytes, "d2h_bytes_per_step": hm.d2h_bytes,
+               "pcie_GBs_each_way": [hm.h2d_bytes / ms / 1e6, hm.d2h_bytes / ms / 1e6],
+               "rounds": len(plan.rounds), "staging_bytes": args.e2e_staging}
+        del hm, plan
+        gc.collect(); torch.cuda.empty_cache()
+        return out
 
-    out = leg(zero_copy=True)
-    out["note"] = ("zero-copy: pinned host old shards -> [copy kernels read them over PCIe, only the bytes their chunks "
-                   "name] -> whole path (kind-major rounds, staging on the device) -> [copy kernels write over PCIe] -> "
-                   "pinned host new shards; h2d / d2h = bytes the kernels read from / write to host memory")
-    for key, kw, note in (
-            ("dma_full_upload", dict(d_src=src, d_dst=dst),
-             "cudaMemcpyAsync of EVERY old shard byte -> rounds on device buffers -> cudaMemcpyAsync of the new shards; "
-             "upload, rounds and download of different kinds overlap on three streams"),
-            ("dma_needed_only", dict(d_src=src, d_dst=dst, needed_only=True),
-             "plan first, then cudaMemcpy2DAsync of only the source regions the plan's slices read (etc_upload_sources)")):
-        if world > 1:
-            continue                                            # context legs: single-GPU runs only
+    legs = {}
+    legs["zero_copy"] = leg(zero_copy=True)
+    legs["zero_copy"]["note"] = "pinned host shards are the tables of the C-ABI call; copy kernels move every byte over PCIe"
+    if world == 1:
         try:
-            out[key] = leg(**kw)
-            out[key]["note"] = note
+            legs["dma_needed_only"] = leg(needed_only=True)
+            legs["dma_needed_only"]["note"] = "plan first, cudaMemcpy2DAsync of the regions the plan reads, rounds on device, D2H"
         except Exception as ex:
-            out[key] = {"error": repr(ex)[:200]}
+            legs["dma_needed_only"] = {"error": repr(ex)[:160]}
+    best = max((k for k in legs if legs[k].get("value")), key=lambda k: legs[k]["value"])
+    out = dict(legs[best])
+    out["leg"] = best
+    out["config"] = wi["name"]
+    out["note"] = f"{best} on {wi['name']}; " + legs[best].get("note", "")
+    out["legs"] = {k: {kk: vv for kk, vv in v.items() if kk != "note"} for k, v in legs.items()}
     return out
 
 
-def chunked(E, torch, w, dev, src, lay_old, lay_new, cap):
-    """(f2) device-resident state chunking with eager release: DESTROYS `src` (run last).  Reports the peak of live
-    bytes relative to the old state, the quantity of the paper's Fig. 12 (1.25x there)."""
+def chunked(E, torch, w, dev, cap):
+    """(f2) device-resident state chunking with eager release on workload w.  Reports the peak of live bytes relative
+    to the old state, the quantity of the paper's Fig. 12 (1.25x there)."""
+    from etc_inputs import bench_fill_torch
     from paper_2607_04749_b200.host_pipeline import migrate_chunked
+    lay_old, lay_new = E.etc_layout_create(w["model"], w["old"]), E.etc_layout_create(w["model"], w["new"])
+    src = E.alloc_buffers(lay_old, dev)
     stream = torch.cuda.current_stream()
     ov, _, _ = E.etc_cost_matrix(lay_old, lay_new)
     dm, _ = E.etc_sketch(ov)
@@ -570,7 +753,8 @@ def chunked(E, torch, w, dev, src, lay_old, lay_new, cap):
     torch.cuda.synchronize()
     ms = a.elapsed_time(b)
     peak_alloc = torch.cuda.max_memory_allocated(dev) - (base - old_bytes)
-    return {"staging_cap_bytes": cap, "rounds": info["rounds"], "ms": ms, "GBs": plan.stats.hbm_bytes / ms / 1e6,
+    return {"workload": w["name"], "staging_cap_bytes": cap, "rounds": info["rounds"], "ms": ms,
+            "GBs": plan.stats.hbm_bytes / ms / 1e6,
             "peak_live_over_old": info["peak_live_bytes"] / info["old_bytes"],
             "torch_peak_allocated_over_old": peak_alloc / old_bytes,
             "all_at_once_over_old": (info["old_bytes"] + info["new_bytes"] + plan.stats.staging_bytes) / info["old_bytes"],
@@ -583,13 +767,20 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--config", default="c2", help="workload: c1..c5 (BASELINE.json configs[0..4]); default configs[1]")
+    ap.add_argument("--config", default="c4", help="workload: c1..c5 (BASELINE.json configs[0..4]); default configs[3], "
+                                                    "the largest that fits one GPU")
     ap.add_argument("--all-staged", action="store_true", help="ETC_ALL_STAGED: every slice goes through pack/unpack")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--no-extras", action="store_true")
-    ap.add_argument("--e2e-steps", type=int, default=6)
+    ap.add_argument("--no-extras", action="store_true", help="skip per_config, all-staged rates and the context legs")
+    ap.add_argument("--per-config", default="c1,c2,c3,c5", help="other workloads measured for roofline.per_config")
+    ap.add_argument("--config-steps", type=int, default=8, help="timed steps of each per_config workload")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-config", default="", help="force the e2e workload (default: the headline one if it can be pinned)")
+    ap.add_argument("--e2e-max-bytes", type=int, default=48 << 30,
+                    help="largest old+new state the e2e leg will pin in host memory (pinning costs ~0.3 s/GB)")
     ap.add_argument("--e2e-staging", type=int, default=1 << 30, help="staging bound (bytes) of the e2e / chunked legs")
+    ap.add_argument("--chunked-config", default="c2", help="workload of the chunked eager-release context leg")
     ap.add_argument("--ref-elems", type=int, default=48_000_000, help="--impl reference: oracle sample (elements) per step")
     ap.add_argument("--cpu-elems", type=int, default=300_000_000, help="cpu_baseline leg: oracle sample (elements), ~10 s")
     args = ap.parse_args()

@@ -99,7 +99,8 @@ typedef struct { int32_t tp, pp, dp, dist_opt, pp_first, pp_last, dist_opt_align
 typedef struct etc_layout etc_layout;   /* opaque, immutable after create */
 typedef struct etc_plan etc_plan;       /* opaque, immutable after create */
 
-/* Select the CUDA device the library works on (default 0).  Call once per process before anything else. */
+/* Select the CUDA device the library works on (default 0).  Call once per process before anything else.  Calls that
+ * create library-owned objects make that device current while they run and restore the caller's current device. */
 etc_status etc_init(int32_t cuda_device);
 
 /* (a1) Build the layout descriptor on the host and upload its piece tables.  *out is written only on success. */
@@ -135,7 +136,10 @@ etc_status etc_sketch(const int64_t* d_overlap, int32_t n_new, int32_t P, const 
  *   mode: ETC_DEFRAG_OCCUPANCY (lines 1-9: idle devices in ascending order are paired with occupied devices in descending
  *         order until they meet, so the occupied devices become exactly [0,cw) and whole nodes are freed),
  *         ETC_DEFRAG_EFFICIENCY (lines 10-20: every device of a fragmented node takes its target rank, rank k on device k,
- *         so each TP group sits inside a node), ETC_DEFRAG_BOTH (occupancy, then efficiency on its result).
+ *         so each TP group sits inside a node; the target placement is fixed by the rank order alone, so this stage
+ *         OVERRIDES the sketch on every fragmented node — on its own it returns the identity placement wherever the
+ *         sketch differs from it — and `pw` only bounds the device ids accepted in d_device_map),
+ *         ETC_DEFRAG_BOTH (occupancy, then efficiency on its result).
  * Outputs (device memory): d_out_map [cw] int32 (must not alias d_device_map); d_n_ops [2] int32 = number of migration
  * operators of the occupancy and of the efficiency stage; d_ops: optional (NULL to skip) [2][cw][2] int32, operators
  * <a,b> in the paper's order: occupancy <idle device, occupied device> at d_ops[0..], efficiency <target rank, current
@@ -153,7 +157,11 @@ etc_status etc_defrag(const int32_t* d_device_map, int32_t pw, int32_t cw, int32
  * ETC_ALL_STAGED): NO slice is staged, every one is copied source buffer -> destination buffer in one hop — for shards
  * that all live in one address space anyway (pinned host memory: the zero-copy pipeline), where a staging buffer
  * stands for no message; the traffic matrix and remote_bytes are unchanged, staging_bytes = 0.  Synchronises `stream` once
- * (sizes must come back to the host).  Fails with ETC_ERR_BAD_MAP if the map is not injective into [0,P). */
+ * (sizes must come back to the host) and then enqueues the kernels that write the slice and chunk tables: the plan is
+ * complete in `stream` order, not on return.  Every later call that reads the plan on ANOTHER stream (etc_migrate*,
+ * etc_plan_set_rounds, etc_plan_validate) makes that stream wait for those kernels itself (an event recorded at the end
+ * of this call), so no caller-side ordering is needed.  Fails with ETC_ERR_BAD_MAP if the map is not injective into
+ * [0,P). */
 enum { ETC_LOCAL_DIRECT = 0, ETC_ALL_STAGED = 1, ETC_KIND_MAJOR = 2, ETC_ALL_DIRECT = 4 };
 etc_status etc_plan_create(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
                            int32_t flags, etc_plan** out, void* stream);
@@ -226,7 +234,12 @@ etc_status etc_plan_get_fills(const etc_plan* plan, etc_slice* h_out);
  *                      the destination bytes that have no source (reading A31; none unless the padded vocabulary grew)
  *   ETC_PHASE_UNPACK : unpack staged slices staging -> new buffers
  * etc_migrate runs both phases.  No allocation, no host synchronisation.  Every destination byte is written exactly
- * once. */
+ * once.  Concurrency: a plan is immutable and may be used by several etc_migrate* calls at once, from different host
+ * threads and on different streams, each with its own buffer set (double-buffered payloads, a captured CUDA graph
+ * replayed beside a live call): with (n_old + n_new) <= 96 the pointer tables travel in each launch's kernel
+ * parameters.  Beyond 96 devices the tables are written into one device table per plan (per round for
+ * etc_migrate_round) by a kernel on `stream`: such calls on the SAME plan must then be ordered one after the other (same
+ * stream, or events) unless they pass identical buffer sets. */
 enum { ETC_PHASE_PACK = 1, ETC_PHASE_UNPACK = 2, ETC_PHASE_ALL = 3 };
 etc_status etc_migrate(const etc_plan* plan, const void* const* src_bufs, void* const* dst_bufs,
                        void* staging, void* stream);

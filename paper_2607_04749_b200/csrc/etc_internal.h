@@ -56,12 +56,15 @@ struct DeviceTables {            // device memory
 // legacy default stream and is a stream like any other here (it must not be mistaken for "never used").
 struct StreamSet {
   std::vector<cudaStream_t> used;
+  std::mutex mu;                   // note() is called through const handles from any host thread
   void note(cudaStream_t st) {
+    std::lock_guard<std::mutex> lock(mu);
     for (size_t i = 0; i < used.size(); ++i)
       if (used[i] == st) { used.erase(used.begin() + (long)i); break; }
     used.push_back(st);
   }
-  cudaStream_t join(cudaStream_t fallback) const {
+  cudaStream_t join(cudaStream_t fallback) {
+    std::lock_guard<std::mutex> lock(mu);
     if (used.empty()) return fallback;
     cudaStream_t last = used.back();
     for (size_t i = 0; i + 1 < used.size(); ++i) {
@@ -96,6 +99,15 @@ void set_error_detail(const char* what, cudaError_t e);
 void clear_error_detail();
 void count_launch(int n = 1);
 int current_device();
+// Makes the library's device (etc_init) current for the lifetime of the guard and restores the caller's device after.
+struct DeviceGuard {
+  int prev = -1; bool switched = false; cudaError_t err = cudaSuccess;
+  DeviceGuard() {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != current_device()) { err = cudaSetDevice(current_device()); switched = err == cudaSuccess; }
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
 // xfer.cu: metadata transfers as kernels on the caller's stream, so that they never queue behind bulk DMA transfers
 cudaError_t write_small(void* d_dst, const void* h_src, size_t bytes, cudaStream_t st);      // host -> device via kernel parameters
 cudaError_t copy_by_kernel(void* dst, const void* src, size_t bytes, cudaStream_t st);       // device / pinned host, either way

@@ -198,7 +198,8 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   const size_t max_total = o_pieces + (size_t)n_dev * n_kinds * max_inst * 5 * sizeof(Piece);   // <= 5 rectangles / instance
 
   std::lock_guard<std::mutex> lock(g_up_mu);
-  cudaError_t e = cudaSetDevice(current_device());
+  DeviceGuard guard;                                       // the caller's current device is restored on return
+  cudaError_t e = guard.err;
   if (e == cudaSuccess) e = upload_prepare(max_total);
   if (e != cudaSuccess) { set_error_detail("etc_layout_create staging", e); return ETC_ERR_CUDA; }
   char* host = static_cast<char*>(g_pinned);

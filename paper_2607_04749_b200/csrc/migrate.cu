@@ -200,28 +200,39 @@ __device__ __forceinline__ void tma_copy_chunk(char* tile, uint64_t* bar, const 
   asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");      // the tile must outlive the reads of the bulk stores
 }
 
+// Pointer tables.  The caller's buffer pointers (n_old*4 source pointers, then n_new*4 destination pointers) ride in the
+// kernel's parameter block when they fit (PTR_PARAM_MAX pointers: up to 96 devices in all), so every launch carries its
+// own table: concurrent etc_migrate calls on one plan from different streams with different buffer sets (double-
+// buffered payloads, a replayed CUDA graph beside a live call) cannot disturb each other, and no upload kernel is
+// needed.  Larger device counts use a table in device memory that belongs to the plan (include/etc.h states the
+// ordering rule for that case).
+constexpr int PTR_PARAM_MAX = 384;
+struct PtrParams { const void* p[PTR_PARAM_MAX]; };
+
 // UNPACK = false: blocks [0,nA) pack staged chunks (src -> staging), blocks [nA,nA+nB) copy local chunks (src -> dst)
 // UNPACK = true : blocks [0,nA) unpack staged chunks (staging -> dst)
-template <bool UNPACK>
+template <bool UNPACK, bool PARAM_PTRS>
 __global__ void __launch_bounds__(CP_THREADS)
 migrate_copy_kernel(const Chunk* __restrict__ chA, long long nA, const Chunk* __restrict__ chB,
-                    const void* const* __restrict__ src_tab, void* const* __restrict__ dst_tab,
-                    char* __restrict__ staging) {
+                    const void* const* __restrict__ tab, int ns, char* __restrict__ staging,
+                    const __grid_constant__ PtrParams pp) {
   extern __shared__ __align__(128) char tile[];                 // TILE_BYTES: TMA path and cp.async staged paths
   __shared__ uint64_t bar;
   const long long b = blockIdx.x;
   const bool staged = b < nA;
   const Chunk c = staged ? chA[b] : chB[b - nA];
   const char* src; char* dst; uint32_t sp, dp;
+  auto src_ptr = [&]() { return static_cast<const char*>(PARAM_PTRS ? pp.p[c.src_buf] : tab[c.src_buf]); };
+  auto dst_ptr = [&]() { return static_cast<char*>(const_cast<void*>(PARAM_PTRS ? pp.p[ns + c.dst_buf] : tab[ns + c.dst_buf])); };
   if (UNPACK) {
     src = staging + c.stg_off; sp = (uint32_t)c.row_bytes;
-    dst = static_cast<char*>(dst_tab[c.dst_buf]) + c.dst_off; dp = (uint32_t)c.dst_stride;
+    dst = dst_ptr() + c.dst_off; dp = (uint32_t)c.dst_stride;
   } else if (staged) {
-    src = static_cast<const char*>(src_tab[c.src_buf]) + c.src_off; sp = (uint32_t)c.src_stride;
+    src = src_ptr() + c.src_off; sp = (uint32_t)c.src_stride;
     dst = staging + c.stg_off; dp = (uint32_t)c.row_bytes;
   } else {
-    src = static_cast<const char*>(src_tab[c.src_buf]) + c.src_off; sp = (uint32_t)c.src_stride;
-    dst = static_cast<char*>(dst_tab[c.dst_buf]) + c.dst_off; dp = (uint32_t)c.dst_stride;
+    src = src_ptr() + c.src_off; sp = (uint32_t)c.src_stride;
+    dst = dst_ptr() + c.dst_off; dp = (uint32_t)c.dst_stride;
   }
   if (c.vec == 16 && (c.nrows == 1 || c.row_bytes >= TMA_MIN_ROW)) {
     if (threadIdx.x < 32) tma_copy_chunk(tile, &bar, src, dst, c.nrows, (uint32_t)c.row_bytes, sp, dp);
@@ -253,11 +264,14 @@ __device__ __forceinline__ void fill_rows(char* dst, int nrows, uint32_t row_byt
     reinterpret_cast<V*>(dst + row * pitch)[col] = z;
   }
 }
+template <bool PARAM_PTRS>
 __global__ void __launch_bounds__(CP_THREADS)
-migrate_fill_kernel(const etc_slice* __restrict__ fills, void* const* __restrict__ dst_tab, int only_kind) {
+migrate_fill_kernel(const etc_slice* __restrict__ fills, const void* const* __restrict__ tab, int ns, int only_kind,
+                    const __grid_constant__ PtrParams pp) {
   const etc_slice f = fills[blockIdx.x];
   if (only_kind >= 0 && f.kind != only_kind) return;
-  char* dst = static_cast<char*>(dst_tab[f.dst_rank * ETC_NUM_KINDS + f.kind]) + f.dst_off;
+  const int di = ns + f.dst_rank * ETC_NUM_KINDS + f.kind;
+  char* dst = static_cast<char*>(const_cast<void*>(PARAM_PTRS ? pp.p[di] : tab[di])) + f.dst_off;
   int64_t al = f.dst_off | f.row_bytes;
   if (f.nrows > 1) al |= (int64_t)f.dst_stride;
   const int64_t low = al & -al;
@@ -268,15 +282,23 @@ migrate_fill_kernel(const etc_slice* __restrict__ fills, void* const* __restrict
   else fill_rows<unsigned char>(dst, f.nrows, (uint32_t)f.row_bytes, (uint32_t)f.dst_stride);
 }
 
-// the TMA path stages one chunk per CTA in dynamic shared memory
+// the TMA path stages one chunk per CTA in dynamic shared memory; function attributes are per device
+template <typename K> static cudaError_t big_smem(K kernel) {
+  cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TILE_BYTES);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+  return e;
+}
 static cudaError_t copy_kernel_attrs() {
-  static bool done = false;
-  if (done) return cudaSuccess;
-  cudaError_t e = cudaFuncSetAttribute(migrate_copy_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TILE_BYTES);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(migrate_copy_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TILE_BYTES);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(migrate_copy_kernel<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(migrate_copy_kernel<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-  done = e == cudaSuccess;
+  static bool done[64] = {};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev >= 0 && dev < 64 && done[dev]) return cudaSuccess;
+  e = big_smem(migrate_copy_kernel<false, false>);
+  if (e == cudaSuccess) e = big_smem(migrate_copy_kernel<false, true>);
+  if (e == cudaSuccess) e = big_smem(migrate_copy_kernel<true, false>);
+  if (e == cudaSuccess) e = big_smem(migrate_copy_kernel<true, true>);
+  if (e == cudaSuccess && dev >= 0 && dev < 64) done[dev] = true;
   return e;
 }
 
@@ -305,30 +327,42 @@ static etc_status launch_migrate(const etc_plan* pl, const void* const* src_bufs
     if (reinterpret_cast<uintptr_t>(dst_bufs[i]) & 15) return ETC_ERR_INVALID_ARG;
   }
   ETC_CUDA_TRY(copy_kernel_attrs());
-  pl->streams.note(st);
-  // pointer tables: source pointers then destination pointers
-  // (as kernel parameters, not as DMA copies: a copy would queue behind bulk transfers pending in the copy engines)
-  {
+  ETC_CUDA_TRY(plan_use(pl, st));                               // `st` waits for the plan's tables if they were written elsewhere
+  // pointer tables: source pointers then destination pointers — in the kernel's parameter block when they fit, else
+  // written into the plan's device table by a kernel on `st` (not a DMA copy: it would queue behind bulk transfers)
+  const bool in_params = ns + nd <= (size_t)PTR_PARAM_MAX;
+  PtrParams pp;
+  if (in_params) {
+    for (size_t i = 0; i < ns; ++i) pp.p[i] = src_bufs[i];
+    for (size_t i = 0; i < nd; ++i) pp.p[ns + i] = dst_bufs[i];
+  } else {
     std::vector<const void*> both(ns + nd);
     for (size_t i = 0; i < ns; ++i) both[i] = src_bufs[i];
     for (size_t i = 0; i < nd; ++i) both[ns + i] = dst_bufs[i];
     ETC_CUDA_TRY(write_small(d_ptrs, both.data(), sizeof(void*) * (ns + nd), st));
   }
-  const void* const* d_src = d_ptrs; void* const* d_dst = d_ptrs + ns;
+  const void* const* tab = d_ptrs;
   char* stg = static_cast<char*>(staging) - stg_base;          // chunk records carry offsets of the full staging layout
   if ((phases & ETC_PHASE_PACK) && nA + nB > 0) {
-    migrate_copy_kernel<false><<<(unsigned)(nA + nB), CP_THREADS, TILE_BYTES, st>>>(pl->d_ch_staged + ca, nA, pl->d_ch_local + la,
-                                                                           d_src, d_dst, stg);
+    if (in_params) migrate_copy_kernel<false, true><<<(unsigned)(nA + nB), CP_THREADS, TILE_BYTES, st>>>(
+        pl->d_ch_staged + ca, nA, pl->d_ch_local + la, tab, (int)ns, stg, pp);
+    else migrate_copy_kernel<false, false><<<(unsigned)(nA + nB), CP_THREADS, TILE_BYTES, st>>>(
+        pl->d_ch_staged + ca, nA, pl->d_ch_local + la, tab, (int)ns, stg, pp);
     ETC_CUDA_TRY(cudaGetLastError());
     count_launch();
   }
   if ((phases & ETC_PHASE_PACK) && with_fills && pl->totals.n_fills > 0) {      // reading A31: bytes with no source
-    migrate_fill_kernel<<<dim3((unsigned)pl->totals.n_fills, FILL_SPLIT), CP_THREADS, 0, st>>>(pl->d_fills, d_dst, only_kind);
+    const dim3 grid((unsigned)pl->totals.n_fills, FILL_SPLIT);
+    if (in_params) migrate_fill_kernel<true><<<grid, CP_THREADS, 0, st>>>(pl->d_fills, tab, (int)ns, only_kind, pp);
+    else migrate_fill_kernel<false><<<grid, CP_THREADS, 0, st>>>(pl->d_fills, tab, (int)ns, only_kind, pp);
     ETC_CUDA_TRY(cudaGetLastError());
     count_launch();
   }
   if ((phases & ETC_PHASE_UNPACK) && nA > 0) {
-    migrate_copy_kernel<true><<<(unsigned)nA, CP_THREADS, TILE_BYTES, st>>>(pl->d_ch_staged + ca, nA, nullptr, d_src, d_dst, stg);
+    if (in_params) migrate_copy_kernel<true, true><<<(unsigned)nA, CP_THREADS, TILE_BYTES, st>>>(
+        pl->d_ch_staged + ca, nA, nullptr, tab, (int)ns, stg, pp);
+    else migrate_copy_kernel<true, false><<<(unsigned)nA, CP_THREADS, TILE_BYTES, st>>>(
+        pl->d_ch_staged + ca, nA, nullptr, tab, (int)ns, stg, pp);
     ETC_CUDA_TRY(cudaGetLastError());
     count_launch();
   }

@@ -425,6 +425,20 @@ plan_validate_kernel(const Chunk* __restrict__ ch, long long n, int staged, cons
 
 using namespace etc;
 
+cudaError_t etc::plan_use(const etc_plan* pl, cudaStream_t st) {
+  cudaError_t e = cudaSuccess;
+  if (st != pl->stream_created_on && pl->ready) {
+    // inside a stream capture the wait becomes an external-event node of the graph (a plain wait on an event recorded
+    // outside the capture is not allowed there)
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    e = cudaStreamIsCapturing(st, &cap);
+    if (e == cudaSuccess)
+      e = cudaStreamWaitEvent(st, pl->ready, cap == cudaStreamCaptureStatusActive ? cudaEventWaitExternal : cudaEventWaitDefault);
+  }
+  pl->streams.note(st);
+  return e;
+}
+
 // pinned slots for the totals read-back (a pageable destination would make the copy synchronous and slower)
 static PlanTotals* g_pinned_totals = nullptr;
 static unsigned g_pinned_next = 0;
@@ -565,6 +579,9 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
     PLAN_TRY(cudaGetLastError());
     count_launch();
   }
+  // the tables are complete once `st` reaches this point: readers on other streams wait for it (plan_use)
+  PLAN_TRY(cudaEventCreateWithFlags(&pl->ready, cudaEventDisableTiming));
+  PLAN_TRY(cudaEventRecord(pl->ready, st));
 #undef PLAN_TRY
   *out = pl;
   return ETC_OK;
@@ -576,6 +593,7 @@ extern "C" void etc_plan_destroy(etc_plan* pl) {
   if (pl->d_ws) cudaFreeAsync(pl->d_ws, st);
   if (pl->d_tb) cudaFreeAsync(pl->d_tb, st);
   if (pl->d_rounds_ws) cudaFreeAsync(pl->d_rounds_ws, st);
+  if (pl->ready) cudaEventDestroy(pl->ready);
   delete pl;
 }
 
@@ -621,7 +639,7 @@ extern "C" etc_status etc_plan_validate(const etc_plan* pl, int64_t* n_bad, void
   clear_error_detail();
   if (!pl || !n_bad) return ETC_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
-  pl->streams.note(st);
+  ETC_CUDA_TRY(plan_use(pl, st));
   const size_t ns = pl->old_bytes.size(), nd = pl->new_bytes.size();
   int64_t* d_sizes = nullptr;
   ETC_CUDA_TRY(cudaMallocAsync(&d_sizes, sizeof(int64_t) * (ns + nd + 1), st));

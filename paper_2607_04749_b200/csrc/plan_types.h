@@ -40,9 +40,17 @@ struct RoundRec {
 
 }  // namespace etc
 
+struct etc_plan;
+namespace etc {
+// Call before enqueueing anything that reads the plan's tables on `st`: a stream other than the one the plan was created
+// on is made to wait for the plan's last table-writing kernel, and `st` is noted as a reader (frees are ordered after it).
+cudaError_t plan_use(const etc_plan* pl, cudaStream_t st);
+}
+
 struct etc_plan {
   int32_t n_old = 0, n_new = 0, P = 0, flags = 0;
   cudaStream_t stream_created_on = nullptr;
+  cudaEvent_t ready = nullptr;                     // recorded on stream_created_on after the last table-writing kernel
   mutable etc::StreamSet streams;                  // streams the plan's tables were written / read on (frees are ordered after them)
   etc::PlanTotals totals{};
   void* d_ws = nullptr;                            // blob 1: the tables below up to d_ptrs

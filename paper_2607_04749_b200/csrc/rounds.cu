@@ -90,7 +90,7 @@ extern "C" etc_status etc_plan_set_rounds(etc_plan* pl, int64_t max_staging_byte
   }
   const size_t R = specs.size();
   if (pl->d_rounds_ws) { cudaFreeAsync(pl->d_rounds_ws, pl->streams.join(st)); pl->d_rounds_ws = nullptr; pl->d_round_ptrs = nullptr; }
-  pl->streams.note(st);
+  ETC_CUDA_TRY(plan_use(pl, st));
   pl->rounds.clear(); pl->round_staging_cap = max_staging_bytes;
   *n_rounds = (int32_t)R;
   if (R == 0) return ETC_OK;

@@ -41,6 +41,59 @@ def shard_all(layout: O.Layout, logical: dict):
     return {(d, k): layout.shard_from_logical(d, k, logical[k]) for d in range(layout.n_dev) for k in layout.kinds()}
 
 
+# ---- memoised oracle results.  Many -m gpu tests run the SAME reconfiguration (same layouts, same payload, same device
+# map) through different launch modes of the CUDA path; the oracle's answer does not depend on the mode, so it is
+# computed once per distinct input and reused (it is the slowest part of those tests by far).
+import collections
+import json
+
+_MEMO: "collections.OrderedDict" = collections.OrderedDict()
+
+
+def _memo(key, fn, keep=10):
+    if key in _MEMO:
+        _MEMO.move_to_end(key)
+        return _MEMO[key]
+    val = fn()
+    _MEMO[key] = val
+    while len(_MEMO) > keep:
+        _MEMO.popitem(last=False)
+    return val
+
+
+def _lkey(layout: O.Layout):
+    failed = getattr(layout, "failed", None)
+    return (json.dumps(layout.model, sort_keys=True), json.dumps(layout.cfg, sort_keys=True),
+            None if failed is None else bytes(failed))
+
+
+class KeyedBufs(dict):
+    """{(dev, kind): array} that remembers what it was made from (see oracle_migrate).  Treat as read-only."""
+    key = None
+
+
+def sharded_payload(layout: O.Layout, seed: int, payload: str = "stamp", padded_lts: bool = False) -> KeyedBufs:
+    """shard_all(layout, make_logical(layout.model, seed, payload)), memoised."""
+    key = ("shards", _lkey(layout)[:2], int(seed), payload, bool(padded_lts))
+
+    def make():
+        lts = layout.logical_tensors() if padded_lts else None
+        out = KeyedBufs(shard_all(layout, make_logical(layout.model, seed, payload, lts=lts)))
+        out.key = key
+        return out
+    return _memo(key, make)
+
+
+def oracle_migrate(old: O.Layout, new: O.Layout, device_map, src_bufs):
+    """O.migrate(old, new, device_map, src_bufs) -> (dst, T, overrides); memoised when src_bufs came from
+    sharded_payload (its key names the payload)."""
+    dm = np.ascontiguousarray(device_map, np.int32)
+    skey = getattr(src_bufs, "key", None)
+    if skey is None:
+        return O.migrate(old, new, dm, src_bufs)
+    return _memo(("migrate", _lkey(old), _lkey(new), dm.tobytes(), skey), lambda: O.migrate(old, new, dm, src_bufs))
+
+
 def stamp_all(layout: O.Layout):
     """{(dev, kind): position-stamped 1-D array} (pin P9: values name the buffer and position they came from)."""
     return {(d, k): position_stamp(d, k, layout.buffer_elems(d, k), layout.elem_bytes(k))

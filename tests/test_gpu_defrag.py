@@ -11,7 +11,7 @@ pytestmark = pytest.mark.gpu
 from etc_inputs import workload
 from oracle import defrag as D
 from oracle import oracle as O
-from helpers import GOLDEN, make_logical, shard_all
+from helpers import GOLDEN, make_logical, shard_all, sharded_payload, oracle_migrate
 
 
 @pytest.fixture(scope="module")
@@ -109,9 +109,9 @@ def test_coalesced_migration_vs_oracle(E, name, n_per_node, mode):
     dm_h = dm.cpu().numpy()
     e_final, e_occ, e_eff = _oracle_defrag(dm_h, old.n_dev, new.n_dev, n_per_node, mode)
     assert final.cpu().numpy().tolist() == e_final
-    src = shard_all(oo, make_logical(w["model"], w["seed"], "stamp"))
+    src = sharded_payload(oo, w["seed"], "stamp")
     g = run_gpu_migration(w["model"], w["old"], w["new"], src, device_map=np.asarray(e_final, np.int32))
-    dst, T, _ = O.migrate(oo, on, np.asarray(e_final, np.int32), src)
+    dst, T, _ = oracle_migrate(oo, on, np.asarray(e_final, np.int32), src)
     assert np.array_equal(g["plan"].traffic(), T)
     for key, exp in dst.items():
         assert np.array_equal(g["dst"][key], exp), key

@@ -9,7 +9,7 @@ pytestmark = pytest.mark.gpu
 
 from etc_inputs import workload
 from oracle import oracle as O
-from helpers import make_logical, shard_all
+from helpers import make_logical, shard_all, sharded_payload, oracle_migrate
 from gpu_helpers import upload, download
 
 
@@ -39,7 +39,7 @@ def test_host_migration_vs_oracle(E, name, cap):
     w = workload(name)
     model = w["model"]
     oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
-    payloads = [shard_all(oo, make_logical(model, w["seed"] + i, "stamp" if i == 0 else "values")) for i in range(2)]
+    payloads = [sharded_payload(oo, w["seed"] + i, "stamp" if i == 0 else "values") for i in range(2)]
     h_src = _pinned(payloads[0])
     h_dst = {(n, k): torch.full((on.buffer_elems(n, k) * on.elem_bytes(k),), 0x77, dtype=torch.uint8).pin_memory()
              for n in range(on.n_dev) for k in on.kinds() if on.buffer_elems(n, k)}
@@ -54,7 +54,7 @@ def test_host_migration_vs_oracle(E, name, cap):
         old, new = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])
         ov, _, _ = E.etc_cost_matrix(old, new)
         dm, _ = E.etc_sketch(ov)
-        exp, T, _ = O.migrate(oo, on, dm.cpu().numpy(), payloads[i])
+        exp, T, _ = oracle_migrate(oo, on, dm.cpu().numpy(), payloads[i])
         assert np.array_equal(plan.traffic(), T)
         for key, e in exp.items():
             if e.shape[0]:
@@ -69,7 +69,7 @@ def test_chunked_migration_releases_and_matches(E, name):
     w = workload(name)
     model = w["model"]
     oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
-    src_np = shard_all(oo, make_logical(model, w["seed"], "stamp"))
+    src_np = sharded_payload(oo, w["seed"], "stamp")
     old, new = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])
     ov, need, hold = E.etc_cost_matrix(old, new)
     dm, _ = E.etc_sketch(ov)
@@ -78,7 +78,7 @@ def test_chunked_migration_releases_and_matches(E, name):
     dst, info = migrate_chunked(plan, new, src, 4 * 65536, fill=0x3C)
     torch.cuda.synchronize()
     assert not src                                       # every source buffer was released
-    exp, _, _ = O.migrate(oo, on, dm.cpu().numpy(), src_np)
+    exp, _, _ = oracle_migrate(oo, on, dm.cpu().numpy(), src_np)
     for key, e in exp.items():
         if e.shape[0]:
             assert np.array_equal(download(dst[key], e.itemsize), e), key
@@ -105,7 +105,7 @@ def test_host_migration_uploads_only_what_the_plan_reads(E, name):
     w = workload(name)
     model = w["model"]
     oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
-    payloads = [shard_all(oo, make_logical(model, w["seed"] + i, "stamp" if i == 0 else "values")) for i in range(2)]
+    payloads = [sharded_payload(oo, w["seed"] + i, "stamp" if i == 0 else "values") for i in range(2)]
     h_src = _pinned(payloads[0])
     h_dst = {(n, k): torch.full((on.buffer_elems(n, k) * on.elem_bytes(k),), 0x77, dtype=torch.uint8).pin_memory()
              for n in range(on.n_dev) for k in on.kinds() if on.buffer_elems(n, k)}
@@ -121,7 +121,7 @@ def test_host_migration_uploads_only_what_the_plan_reads(E, name):
         new = E.etc_layout_create(model, w["new"])
         ov, _, _ = E.etc_cost_matrix(old, new)
         dm = E.etc_sketch(ov)[0].cpu().numpy()
-        exp, T, _ = O.migrate(oo, on, dm, payloads[i])
+        exp, T, _ = oracle_migrate(oo, on, dm, payloads[i])
         assert np.array_equal(plan.traffic(), T)
         for key, e in exp.items():
             if e.shape[0]:
@@ -152,7 +152,7 @@ def test_host_migration_zero_copy(E, name, flags):
     w = workload(name)
     model = w["model"]
     oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
-    payloads = [shard_all(oo, make_logical(model, w["seed"] + i, "stamp" if i == 0 else "values")) for i in range(2)]
+    payloads = [sharded_payload(oo, w["seed"] + i, "stamp" if i == 0 else "values") for i in range(2)]
     h_src = _pinned(payloads[0])
     h_dst = {(n, k): torch.full((on.buffer_elems(n, k) * on.elem_bytes(k),), 0x77, dtype=torch.uint8).pin_memory()
              for n in range(on.n_dev) for k in on.kinds() if on.buffer_elems(n, k)}
@@ -167,7 +167,7 @@ def test_host_migration_zero_copy(E, name, flags):
         torch.cuda.synchronize()
         old, new = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])
         dm = E.etc_sketch(E.etc_cost_matrix(old, new)[0])[0].cpu().numpy()
-        exp, T, _ = O.migrate(oo, on, dm, payloads[i])
+        exp, T, _ = oracle_migrate(oo, on, dm, payloads[i])
         assert np.array_equal(plan.traffic(), T)
         for key, e in exp.items():
             if e.shape[0]:

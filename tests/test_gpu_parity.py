@@ -13,7 +13,7 @@ pytestmark = pytest.mark.gpu
 
 from etc_inputs import workload, tiny_models, tiny_parallel_cfgs, position_stamp
 from oracle import oracle as O
-from helpers import make_logical, shard_all, stamp_all
+from helpers import make_logical, shard_all, stamp_all, sharded_payload, oracle_migrate
 
 
 @pytest.fixture(scope="module")
@@ -169,8 +169,7 @@ def test_sketch_infeasible_and_errors(E):
 def _check_migration(E, model, old_cfg, new_cfg, seed, device_map=None, flags=0, payload="stamp"):
     from gpu_helpers import run_gpu_migration
     oo, on = O.Layout(model, old_cfg), O.Layout(model, new_cfg)
-    logical = make_logical(model, seed, payload)
-    src = shard_all(oo, logical)
+    src = sharded_payload(oo, seed, payload)
     g = run_gpu_migration(model, old_cfg, new_cfg, src, device_map=device_map, flags=flags)
     ov, need, hold = O.overlap(oo, on)
     assert np.array_equal(g["overlap"], ov) and np.array_equal(g["need"], need) and np.array_equal(g["hold"], hold)
@@ -180,7 +179,7 @@ def _check_migration(E, model, old_cfg, new_cfg, seed, device_map=None, flags=0,
         ref = O.sketch_bruteforce(ov)[1] if P <= 8 else O.sketch_hungarian(ov)[1]
         assert g["local_bytes"] == ref
     # oracle migration with the GPU's own map (A17)
-    dst, T, _ = O.migrate(oo, on, dm, src)
+    dst, T, _ = oracle_migrate(oo, on, dm, src)
     st = g["plan"].stats
     assert np.array_equal(g["plan"].traffic(), T)
     local = int(np.trace(T)); remote = int(T.sum() - np.trace(T))
@@ -194,15 +193,18 @@ def _check_migration(E, model, old_cfg, new_cfg, seed, device_map=None, flags=0,
     # slice table: every destination byte written exactly once, staging segments disjoint and inside the buffer
     cover = {key: np.zeros(v.shape[0] * v.itemsize, np.uint8) for key, v in dst.items()}
     stg = np.zeros(max(st.staging_bytes, 1), np.uint8)
+    from numpy.lib.stride_tricks import as_strided
     for which in (0, 1):
         for s in g["plan"].slices(which):
             key = (int(s["dst_rank"]), int(s["kind"]))
-            for r in range(int(s["nrows"])):
-                a = int(s["dst_off"]) + r * int(s["dst_stride"])
-                cover[key][a:a + int(s["row_bytes"])] += 1
-                if which == 0:
-                    b = int(s["stg_off"]) + r * int(s["row_bytes"])
-                    stg[b:b + int(s["row_bytes"])] += 1
+            nrows, rb, a0 = int(s["nrows"]), int(s["row_bytes"]), int(s["dst_off"])
+            pitch = int(s["dst_stride"]) if nrows > 1 else rb
+            assert pitch >= rb and a0 >= 0 and a0 + (nrows - 1) * pitch + rb <= cover[key].shape[0], key
+            as_strided(cover[key][a0:], shape=(nrows, rb), strides=(pitch, 1))[...] += 1     # rows x row_bytes at the pitch
+            if which == 0:
+                b0 = int(s["stg_off"])
+                assert b0 >= 0 and b0 + nrows * rb <= stg.shape[0]
+                stg[b0:b0 + nrows * rb] += 1                                                  # packed back to back
             assert int(s["dst_phys"]) == int(dm[int(s["dst_rank"])])
     for key, c in cover.items():
         assert (c == 1).all(), key

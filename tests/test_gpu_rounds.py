@@ -10,7 +10,7 @@ pytestmark = pytest.mark.gpu
 
 from etc_inputs import workload, tiny_models
 from oracle import oracle as O
-from helpers import make_logical, shard_all
+from helpers import make_logical, shard_all, sharded_payload, oracle_migrate
 from gpu_helpers import upload, download
 
 
@@ -25,7 +25,7 @@ def E():
 
 def _run_rounds(E, model, old_cfg, new_cfg, seed, cap, flags, device_map=None, poison=0x5A):
     oo, on = O.Layout(model, old_cfg), O.Layout(model, new_cfg)
-    src_np = shard_all(oo, make_logical(model, seed, "stamp"))
+    src_np = sharded_payload(oo, seed, "stamp")
     old, new = E.etc_layout_create(model, old_cfg), E.etc_layout_create(model, new_cfg)
     if device_map is None:
         ov, _, _ = E.etc_cost_matrix(old, new)
@@ -63,7 +63,7 @@ def _run_rounds(E, model, old_cfg, new_cfg, seed, cap, flags, device_map=None, p
         for key, t in dst_k.items():
             out[key] = download(t, es)
         del src_k, dst_k                                           # eager release
-    dst, T, _ = O.migrate(oo, on, dm.cpu().numpy(), src_np)
+    dst, T, _ = oracle_migrate(oo, on, dm.cpu().numpy(), src_np)
     assert np.array_equal(plan.traffic(), T)
     for key, exp in dst.items():
         if exp.shape[0] == 0:

@@ -12,7 +12,7 @@ pytestmark = pytest.mark.gpu
 
 from etc_inputs import workload
 from oracle import oracle as O
-from helpers import make_logical, shard_all
+from helpers import make_logical, shard_all, sharded_payload, oracle_migrate
 from gpu_helpers import upload, download
 
 
@@ -31,7 +31,7 @@ def test_pipelined_plans_dropped_early(E, name, flags, copy_on_default_stream):
     w = workload(name)
     model = w["model"]
     oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
-    src_np = shard_all(oo, make_logical(model, w["seed"], "stamp"))
+    src_np = sharded_payload(oo, w["seed"], "stamp")
     src = upload(src_np)
     lay_new = E.etc_layout_create(model, w["new"])
     dst = E.alloc_buffers(lay_new, fill=0x3C)
@@ -61,7 +61,7 @@ def test_pipelined_plans_dropped_early(E, name, flags, copy_on_default_stream):
             E.etc_migrate(plan, src, dst, staging, stream=copy_stream)
         del plan, lo, ln            # dropped while the copy stream is still far behind
     torch.cuda.synchronize()
-    exp, _, _ = O.migrate(oo, on, dmap, src_np)
+    exp, _, _ = oracle_migrate(oo, on, dmap, src_np)
     for key, e in exp.items():
         if e.shape[0]:
             assert np.array_equal(download(dst[key], on.elem_bytes(key[1])), e), key
@@ -75,7 +75,7 @@ def test_migrate_is_cuda_graph_capturable(E, name, flags):
     w = workload(name)
     model = w["model"]
     oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
-    payloads = [shard_all(oo, make_logical(model, w["seed"] + i, "stamp" if i == 0 else "values")) for i in range(3)]
+    payloads = [sharded_payload(oo, w["seed"] + i, "stamp" if i == 0 else "values") for i in range(3)]
     old, new = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])
     dm, _ = E.etc_sketch(E.etc_cost_matrix(old, new)[0])
     plan = E.etc_plan_create(old, new, dm, flags)
@@ -99,7 +99,64 @@ def test_migrate_is_cuda_graph_capturable(E, name, flags):
             t.fill_(0x3C)
         graph.replay()
         torch.cuda.synchronize()
-        exp, _, _ = O.migrate(oo, on, dm_h, payloads[i])
+        exp, _, _ = oracle_migrate(oo, on, dm_h, payloads[i])
         for key, e in exp.items():
             if e.shape[0]:
                 assert np.array_equal(download(dst[key], e.itemsize), e), (i, key)
+
+
+@pytest.mark.parametrize("name,flags", [("s3", 0), ("s4", 1)])
+def test_plan_used_on_another_stream_without_a_manual_wait(E, name, flags):
+    """include/etc.h etc_plan_create: the slice and chunk tables are written by kernels enqueued AFTER the call's one host
+    synchronisation, so the plan is complete in stream order only.  A call that reads it on another stream must order
+    itself after those kernels (the library records an event at the end of etc_plan_create and waits for it).  Here the
+    planning stream is held back by a long dummy copy enqueued before the plan's table kernels could run... the
+    migration on a second stream, with NO wait_event by the caller, must still equal the oracle; so must
+    etc_plan_validate and etc_plan_set_rounds + etc_migrate_round on a third stream."""
+    w = workload(name)
+    model = w["model"]
+    oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
+    src_np = sharded_payload(oo, w["seed"], "stamp")
+    src = upload(src_np)
+    old, new = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])
+    dm, _ = E.etc_sketch(E.etc_cost_matrix(old, new)[0])
+    torch.cuda.synchronize()
+    dmap = dm.cpu().numpy().copy()
+    exp, _, _ = oracle_migrate(oo, on, dmap, src_np)
+    big_a = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")
+    big_b = torch.empty_like(big_a)
+    s_plan, s_copy, s_rounds = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+    for mode in ("migrate", "rounds"):
+        dst = E.alloc_buffers(new, fill=0x3C)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(s_plan):
+            # etc_plan_create synchronises s_plan once (sizes), then enqueues the table kernels behind these copies: a
+            # second thread keeps the stream fed while the call waits
+            import threading
+            stop = threading.Event()
+
+            def feed():
+                with torch.cuda.stream(s_plan):
+                    while not stop.is_set():
+                        for _ in range(4):
+                            big_b.copy_(big_a, non_blocking=True)
+                        stop.wait(0.0005)
+            th = threading.Thread(target=feed)
+            th.start()
+            try:
+                plan = E.etc_plan_create(old, new, dm, flags | (E.ETC_KIND_MAJOR if mode == "rounds" else 0), stream=s_plan)
+            finally:
+                stop.set(); th.join()
+        staging = torch.empty(max(plan.stats.staging_bytes, 16), dtype=torch.uint8, device="cuda")
+        if mode == "migrate":
+            E.etc_migrate(plan, src, dst, staging, stream=s_copy)          # no wait_event here
+            assert plan.validate(stream=s_rounds) == 0
+        else:
+            rounds = E.etc_plan_set_rounds(plan, max(2 * 65536, plan.stats.staging_bytes // 3 + 65536), stream=s_rounds)
+            for i in range(len(rounds)):
+                E.etc_migrate_round(plan, i, src, dst, staging, stream=s_copy)
+        torch.cuda.synchronize()
+        for key, e in exp.items():
+            if e.shape[0]:
+                assert np.array_equal(download(dst[key], on.elem_bytes(key[1])), e), (mode, key)
+        del plan
