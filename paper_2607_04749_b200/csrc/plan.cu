@@ -85,10 +85,22 @@ __device__ __forceinline__ SliceGeom make_slice(const Rect& R, const Piece& o, c
   return s;
 }
 
+// widest power-of-two access (<= 16 bytes) that every address of a slice is aligned to.  Staging offsets of slices are
+// multiples of 16 and the staging pitch is row_bytes, so the staging side adds nothing.
+__device__ __forceinline__ int vec_of(int64_t a) {
+  const int64_t low = a & -a;
+  return a == 0 ? 16 : (low >= 16 ? 16 : (int)low);
+}
+__device__ __forceinline__ int slice_vec(int64_t src_off, int64_t dst_off, int64_t row_bytes, int32_t src_stride,
+                                         int32_t dst_stride, int32_t nrows) {
+  int64_t al = src_off | dst_off | row_bytes;
+  if (nrows > 1) al |= (int64_t)src_stride | (int64_t)dst_stride;
+  return vec_of(al);
+}
 __device__ __forceinline__ int64_t slice_chunks(const SliceGeom& s) {
   if (s.nrows == 1) return (s.row_bytes + ETC_CHUNK_BYTES - 1) / ETC_CHUNK_BYTES;
   if (s.row_bytes >= ETC_CHUNK_BYTES) return (int64_t)s.nrows * ((s.row_bytes + ETC_CHUNK_BYTES - 1) / ETC_CHUNK_BYTES);
-  const int rpc = (int)(ETC_CHUNK_BYTES / s.row_bytes);
+  const int rpc = rows_per_chunk(s.row_bytes, slice_vec(s.src_off, s.dst_off, s.row_bytes, s.src_stride, s.dst_stride, s.nrows) == 16);
   return (s.nrows + rpc - 1) / rpc;
 }
 __device__ __forceinline__ int64_t slice_padded(const SliceGeom& s) { return (s.nrows * s.row_bytes + 15) & ~(int64_t)15; }
@@ -280,11 +292,6 @@ plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int K, int n_
   }
 }
 
-__device__ __forceinline__ int vec_of(int64_t a) {
-  const int64_t low = a & -a;
-  return a == 0 ? 16 : (low >= 16 ? 16 : (int)low);
-}
-
 // pass 2: recompute the slices of each (unit, sub-block) and write slice records (+ first chunk index) at their final
 // positions: unit base (scan) + earlier sub-blocks of the unit + warp-level prefix inside the sub-block.
 __global__ void __launch_bounds__(PLAN_WARPS * 32)
@@ -377,9 +384,7 @@ plan_chunks_kernel(const etc_slice* __restrict__ slices, const int64_t* __restri
   ch.src_buf = (uint16_t)(s.src_dev * ETC_NUM_KINDS + s.kind); ch.dst_buf = (uint16_t)(s.dst_rank * ETC_NUM_KINDS + s.kind);
   ch.src_stride = s.src_stride; ch.dst_stride = s.dst_stride; ch.pad = 0;
   const int64_t stg = s.stg_off >= 0 ? s.stg_off : 0;
-  int64_t al = s.src_off | s.dst_off | stg | s.row_bytes;
-  if (s.nrows > 1) al |= (int64_t)s.src_stride | (int64_t)s.dst_stride;
-  ch.vec = (int16_t)vec_of(al);
+  ch.vec = (int16_t)slice_vec(s.src_off, s.dst_off, s.row_bytes, s.src_stride, s.dst_stride, s.nrows);
   if (s.nrows == 1 || s.row_bytes >= ETC_CHUNK_BYTES) {
     const long long cpr = (s.row_bytes + ETC_CHUNK_BYTES - 1) / ETC_CHUNK_BYTES;
     const long long row = k / cpr; const int64_t b = (k % cpr) * ETC_CHUNK_BYTES;
@@ -388,7 +393,7 @@ plan_chunks_kernel(const etc_slice* __restrict__ slices, const int64_t* __restri
     ch.stg_off = stg + row * s.row_bytes + b;
     ch.nrows = 1; ch.row_bytes = (int32_t)min((int64_t)ETC_CHUNK_BYTES, s.row_bytes - b);
   } else {
-    const int rpc = (int)(ETC_CHUNK_BYTES / s.row_bytes);
+    const int rpc = rows_per_chunk(s.row_bytes, ch.vec == 16);
     const long long row = k * rpc;
     ch.src_off = s.src_off + row * s.src_stride;
     ch.dst_off = s.dst_off + row * s.dst_stride;

@@ -17,6 +17,22 @@ struct PlanTotals {
   int64_t kind_base[ETC_NUM_KINDS + 1][3];
 };
 
+// Shared-memory tile of the copy kernels: one chunk of payload plus slack for the byte-phase re-aligning path, which
+// stores row r at r * realign_pitch(row_bytes) + (source address of the row mod 16).
+constexpr int TILE_BYTES = ETC_CHUNK_BYTES + 8192;
+// tile row pitch of the re-aligning path: the 16-byte slots that can overlap a row of row_bytes at any byte phase
+__host__ __device__ __forceinline__ uint32_t realign_pitch(uint32_t row_bytes) { return ((row_bytes + 30u) >> 4) << 4; }
+// Rows per chunk of a 2-D slice with rows shorter than ETC_CHUNK_BYTES.  aligned16: every address, pitch and the row
+// length are multiples of 16 (the chunk is then staged densely); otherwise the re-aligning path's padded rows must fit.
+__host__ __device__ __forceinline__ int rows_per_chunk(int64_t row_bytes, bool aligned16) {
+  int rpc = (int)(ETC_CHUNK_BYTES / row_bytes);
+  if (!aligned16) {
+    const int fit = (int)((TILE_BYTES - 16) / realign_pitch((uint32_t)row_bytes));
+    if (fit < rpc) rpc = fit;
+  }
+  return rpc < 1 ? 1 : rpc;
+}
+
 // One copy work item: nrows x row_bytes, at most ETC_CHUNK_BYTES in total (or one row segment of that size).
 struct Chunk {
   int64_t src_off, dst_off, stg_off;   // byte offsets inside the source buffer, destination buffer, staging buffer

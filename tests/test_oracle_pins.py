@@ -260,7 +260,10 @@ def _check_reconfiguration(model, old_cfg, new_cfg, seed, device_map=None, paylo
     assert T.sum() == need.sum()
     local = sum(int(T[device_map[n], device_map[n]]) for n in range(new.n_dev))
     assert local == sum(int(ov[n, device_map[n]]) for n in range(new.n_dev))      # local-first keeps overlap local
-    # --- P9 replica-stamped payload: the values name the source, the histogram is T
+    # --- P9 replica-stamped payload: the values name the source, the histogram is T.  orc_migrate and orc_source_of share
+    # the rule's code (orc_pick_source), so this block checks their CONSISTENCY and the histogram identity only; the rule
+    # itself is pinned by re-deriving every source from holders_of in test_megatron_geometry_pins.py
+    # (test_sources_rederived_from_holders) and, under failure masks, in test_failure_pins.py
     stamps = stamp_all(old)
     dst2, T2, _ = O.migrate(old, new, device_map, stamps)
     hist = np.zeros_like(T)
