@@ -357,23 +357,42 @@ class Resident:
         self.stats = plan.stats
         return dict(ms_per_step=ms_per_step, breakdown=bd, launches=launches, clocks=clocks, stats=plan.stats)
 
-    def one_shot(self, reps=8):
-        """One migration, cold start to finish, nothing overlapped: (a1)-(a6) on one stream, host wall clock from the
-        first call to the synchronise after the last kernel (the latency a single reconfiguration sees)."""
+    def one_shot(self, reps=10):
+        """One migration, cold start to finish, nothing overlapped, through the one-call primitive etc_migrate_state:
+        (a1)-(a6) enqueued by ONE C-ABI call without any host synchronisation (small plans: ETC_NO_SYNC), host wall
+        clock from the call to the return of the synchronise after the last kernel — the latency a single
+        reconfiguration sees.  Also the rate of back-to-back calls with no synchronise in between."""
         E, torch, w = self.E, self.torch, self.w
+        stg = self.staging
+        call = E.MigrateState(w["model"], w["old"], w["new"], self.src_tab, self.dst_tab, stg, self.flags)
+        try:
+            call(); torch.cuda.synchronize()
+        except E.EtcError as ex:                       # the exact-size staging buffer is below the no-sync bound
+            if ex.code != -5:
+                raise
+            self.staging = stg = None
+            torch.cuda.empty_cache()
+            stg = torch.empty(max(E.etc_staging_bound(self.lay_old, self.lay_new, self.flags), 16), dtype=torch.uint8, device=self.dev)
+            call = E.MigrateState(w["model"], w["old"], w["new"], self.src_tab, self.dst_tab, stg, self.flags)
+            call(); torch.cuda.synchronize()
         walls = []
         for i in range(reps):
             torch.cuda.synchronize()
             t0 = time.perf_counter()
-            lo, ln = E.etc_layout_create(w["model"], w["old"]), E.etc_layout_create(w["model"], w["new"])
-            ov, _, _ = E.etc_cost_matrix(lo, ln, out=self.out_cost)
-            dm, _ = E.etc_sketch(ov, out=self.out_sk)
-            plan = E.etc_plan_create(lo, ln, dm, self.flags)
-            E.etc_migrate(plan, self.src_tab, self.dst_tab, self.staging)
+            call()
             torch.cuda.synchronize()
             if i >= 3:
                 walls.append((time.perf_counter() - t0) * 1e3)
-        return statistics.median(walls)
+        n = 50 if self.stats.hbm_bytes < (1 << 32) else 6
+        a, b = self.ev(), self.ev()
+        torch.cuda.synchronize()
+        a.record(self.stream)
+        for _ in range(n):
+            call()
+        b.record(self.stream)
+        torch.cuda.synchronize()
+        self.staging = stg
+        return statistics.median(walls), a.elapsed_time(b) / n
 
     def close(self):
         self.src = self.dst = self.staging = self.src_tab = self.dst_tab = None
@@ -442,8 +461,9 @@ def config_entry(res, peak, one_shot_ms=None):
            "unpack_ms": k2["ms"], "unpack_GBs": k2["GBs"], "unpack_frac": k2["frac"],
            "cost_sketch_ms": bd["cost_matrix_ms"] + bd["sketch_ms"], "plan_ms": bd["plan_ms"], "layout_ms": bd["layout_ms"]}
     if one_shot_ms is not None:
-        out["one_shot_ms"] = one_shot_ms
-        out["one_shot_GBs"] = st.hbm_bytes / one_shot_ms / 1e6
+        out["one_shot_ms"], out["one_call_step_ms"] = one_shot_ms
+        out["one_shot_GBs"] = st.hbm_bytes / out["one_shot_ms"] / 1e6
+        out["one_call_step_GBs"] = st.hbm_bytes / out["one_call_step_ms"] / 1e6
     return out
 
 
@@ -502,16 +522,19 @@ def run_cuda(args, w):
                                                          "staged": stats.staged_bytes},
             "breakdown_ms": bd, "cost_sketch_ms": bd["cost_matrix_ms"] + bd["sketch_ms"],
             "roofline": roofline, "clocks": res["clocks"], "gpu_launches": res["launches"]}
-    line["config"]["cost_sketch_ms"] = line["cost_sketch_ms"]
-    line["config"]["hbm_bytes_per_step"] = hbm_bytes
+    roofline["cost_sketch_ms"] = line["cost_sketch_ms"]        # the metric's second half, where the driver keeps it
+    roofline["hbm_bytes_per_step"] = hbm_bytes
 
-    per_config = {w["name"]: config_entry(res, peak)}
     extras_on = rank == 0 and not args.no_extras
+    one = None
     if extras_on:
         try:
-            per_config[w["name"]]["one_shot_ms"] = R.one_shot()
+            one = R.one_shot()
         except Exception as ex:
-            per_config[w["name"]]["one_shot_error"] = repr(ex)[:120]
+            one = None
+            line["one_shot_error"] = repr(ex)[:160]
+    per_config = {w["name"]: config_entry(res, peak, one)}
+    if extras_on:
         if not args.all_staged:
             try:
                 per_kernel.update(all_staged_rates(E, torch, R, peak))

@@ -162,7 +162,17 @@ etc_status etc_defrag(const int32_t* d_device_map, int32_t pw, int32_t cw, int32
  * etc_plan_set_rounds, etc_plan_validate) makes that stream wait for those kernels itself (an event recorded at the end
  * of this call), so no caller-side ordering is needed.  Fails with ETC_ERR_BAD_MAP if the map is not injective into
  * [0,P). */
-enum { ETC_LOCAL_DIRECT = 0, ETC_ALL_STAGED = 1, ETC_KIND_MAJOR = 2, ETC_ALL_DIRECT = 4 };
+enum { ETC_LOCAL_DIRECT = 0, ETC_ALL_STAGED = 1, ETC_KIND_MAJOR = 2, ETC_ALL_DIRECT = 4, ETC_NO_SYNC = 8 };
+/* ETC_NO_SYNC (OR-ed into flags): etc_plan_create does NOT synchronise.  The slice / chunk tables are sized from upper
+ * bounds the host derives from the two layouts (pieces per tensor, bytes needed), the real counts stay on the device, and
+ * etc_migrate / etc_migrate_phase launch bound-sized grids whose surplus CTAs leave at once: a whole reconfiguration is
+ * then one uninterrupted submission (etc_migrate_state below).  The staging buffer must hold etc_staging_bound() bytes
+ * (the exact size is not known to the host).  A bad device map, an unrecoverable failure mask or (never observed) a
+ * bound that falls short is detected ON THE DEVICE: the plan then copies nothing, and the error is reported by the
+ * first call that needs the counts on the host — etc_plan_get_stats (which waits for the plan's kernels), and likewise
+ * etc_plan_get_traffic / _slices / _fills / etc_plan_set_rounds / etc_plan_validate.  A hint: plans whose bound-sized
+ * tables would exceed 64 MB are made the synchronising way (their copy kernels dwarf one host sync). */
+int64_t etc_staging_bound(const etc_layout* old_l, const etc_layout* new_l, int32_t flags);   /* bytes; < 0 on bad arguments */
 etc_status etc_plan_create(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
                            int32_t flags, etc_plan** out, void* stream);
 void etc_plan_destroy(etc_plan* plan);
@@ -203,6 +213,10 @@ etc_status etc_plan_get_stats(const etc_plan* plan, etc_plan_stats* out);
 /* traffic matrix T [P][P] row-major, int64, copied to HOST memory: T[o][p] = payload bytes whose source is old device
  * o and whose destination is physical device p (diagonal = local bytes).  Synchronous. */
 etc_status etc_plan_get_traffic(const etc_plan* plan, int64_t* h_traffic);
+
+/* The device map the plan was made for, [n_new] int32 copied to HOST memory (e.g. the sketch etc_migrate_state chose).
+ * Synchronous. */
+etc_status etc_plan_get_map(const etc_plan* plan, int32_t* h_device_map);
 
 /* One slice = one 2-D strided copy (rows x row_bytes).  For tests / inspection; copied to HOST memory.
  * which = 0: staged slices, 1: local slices.  h_out must hold n_slices_* entries. */
@@ -245,6 +259,19 @@ etc_status etc_migrate(const etc_plan* plan, const void* const* src_bufs, void* 
                        void* staging, void* stream);
 etc_status etc_migrate_phase(const etc_plan* plan, const void* const* src_bufs, void* const* dst_bufs,
                              void* staging, int32_t phases, void* stream);
+
+/* The migration primitive in ONE call (previous configuration, current configuration, model state
+ * in; migrated state out): (a1) both layout descriptors, (a2) cost matrix, (a3) sketch (d_avail: optional device mask
+ * [P], as etc_sketch), (a4) plan with ETC_NO_SYNC, (a5, a6) pack / unpack / local — enqueued back to back on `stream`
+ * without any host synchronisation; returns as soon as everything is enqueued.  staging / staging_bytes: device buffer
+ * of at least etc_staging_bound() bytes for these two layouts (ETC_ERR_WORKSPACE if smaller; may be NULL / 0 with
+ * ETC_ALL_DIRECT).  flags: ETC_LOCAL_DIRECT | ETC_ALL_STAGED | ETC_ALL_DIRECT.  plan_out: optional; receives the plan
+ * (caller destroys it) so that the chosen map's statistics and any device-side error can be read with
+ * etc_plan_get_stats afterwards; with NULL a device-side error (e.g. no feasible sketch under d_avail) leaves the
+ * destination buffers unwritten and goes unreported. */
+etc_status etc_migrate_state(const etc_model_desc* model, const etc_parallel_cfg* old_cfg, const etc_parallel_cfg* new_cfg,
+                             const void* const* src_bufs, void* const* dst_bufs, void* staging, int64_t staging_bytes,
+                             const uint8_t* d_avail, int32_t flags, etc_plan** plan_out, void* stream);
 
 #define ETC_CHUNK_BYTES 65536
 

@@ -12,7 +12,7 @@ _LIB_PATH = os.path.join(_HERE, "libetc.so")
 _lib = None
 _inited = False
 
-ETC_LOCAL_DIRECT, ETC_ALL_STAGED, ETC_KIND_MAJOR, ETC_ALL_DIRECT = 0, 1, 2, 4
+ETC_LOCAL_DIRECT, ETC_ALL_STAGED, ETC_KIND_MAJOR, ETC_ALL_DIRECT, ETC_NO_SYNC = 0, 1, 2, 4, 8
 ETC_SKETCH_AUTO, ETC_SKETCH_EXHAUSTIVE, ETC_SKETCH_HUNGARIAN = 0, 1, 2
 ETC_PHASE_PACK, ETC_PHASE_UNPACK, ETC_PHASE_ALL = 1, 2, 3
 ETC_DEFRAG_OCCUPANCY, ETC_DEFRAG_EFFICIENCY, ETC_DEFRAG_BOTH = 1, 2, 3
@@ -24,7 +24,7 @@ EXPORTED_SYMBOLS = (
     "etc_migrate_phase",
     "etc_status_string", "etc_last_error_detail", "etc_kernel_launches", "etc_defrag",
     "etc_plan_set_rounds", "etc_plan_get_round", "etc_migrate_round", "etc_plan_create_failed", "etc_mask_failed",
-    "etc_upload_sources", "etc_plan_validate", "etc_mask_cross_dp",
+    "etc_upload_sources", "etc_plan_validate", "etc_mask_cross_dp", "etc_staging_bound", "etc_migrate_state", "etc_plan_get_map",
 )
 
 
@@ -94,6 +94,7 @@ def lib():
         L.etc_plan_get_stats.restype = i32; L.etc_plan_get_stats.argtypes = [vp, C.POINTER(_PlanStats)]
         L.etc_plan_get_traffic.restype = i32; L.etc_plan_get_traffic.argtypes = [vp, vp]
         L.etc_plan_get_slices.restype = i32; L.etc_plan_get_slices.argtypes = [vp, i32, vp]
+        L.etc_plan_get_map.restype = i32; L.etc_plan_get_map.argtypes = [vp, vp]
         L.etc_plan_get_fills.restype = i32; L.etc_plan_get_fills.argtypes = [vp, vp]
         L.etc_plan_validate.restype = i32; L.etc_plan_validate.argtypes = [vp, C.POINTER(i64), vp]
         L.etc_migrate.restype = i32; L.etc_migrate.argtypes = [vp, vp, vp, vp, vp]
@@ -102,6 +103,10 @@ def lib():
         L.etc_plan_get_round.restype = i32; L.etc_plan_get_round.argtypes = [vp, i32, C.POINTER(_RoundInfo)]
         L.etc_migrate_round.restype = i32; L.etc_migrate_round.argtypes = [vp, i32, vp, vp, vp, i32, vp]
         L.etc_upload_sources.restype = i32; L.etc_upload_sources.argtypes = [vp, vp, vp, i32, C.POINTER(i64), vp]
+        L.etc_staging_bound.restype = i64; L.etc_staging_bound.argtypes = [vp, vp, i32]
+        L.etc_migrate_state.restype = i32
+        L.etc_migrate_state.argtypes = [C.POINTER(_ModelDesc), C.POINTER(_ParallelCfg), C.POINTER(_ParallelCfg), vp, vp, vp,
+                                        i64, vp, i32, C.POINTER(vp), vp]
         L.etc_status_string.restype = C.c_char_p; L.etc_status_string.argtypes = [i32]
         L.etc_last_error_detail.restype = C.c_char_p
         L.etc_kernel_launches.restype = i64
@@ -167,14 +172,7 @@ class Layout:
 def etc_layout_create(model: dict, cfg: dict) -> Layout:
     """(a1) include/etc.h etc_layout_create.  model: etc_inputs workload["model"] dict; cfg: {"tp","pp","dp","dist_opt"}."""
     _ensure_init()
-    m = _ModelDesc(style=model["style"], n_layers=model["n_layers"], hidden=model["hidden"],
-                   n_q_heads=model["n_q_heads"], n_kv_heads=model["n_kv_heads"], head_dim=model["head_dim"],
-                   ffn_hidden=model["ffn_hidden"], vocab=model["vocab"], max_pos=model["max_pos"],
-                   tied_embeddings=model["tied"], param_dtype=model["param_bytes"], kinds=model["kinds"],
-                   qkv_order=model.get("qkv_order", 0))
-    c = _ParallelCfg(tp=cfg["tp"], pp=cfg["pp"], dp=cfg["dp"], dist_opt=cfg.get("dist_opt", 0),
-                     pp_first=cfg.get("pp_first", 0), pp_last=cfg.get("pp_last", 0),
-                     dist_opt_align=cfg.get("dist_opt_align", 0), vocab_divisor=cfg.get("vocab_divisor", 0))
+    m, c = _model_struct(model), _cfg_struct(cfg)
     h = C.c_void_p()
     _check(lib().etc_layout_create(C.byref(m), C.byref(c), C.byref(h)))
     return Layout(h, model, cfg)
@@ -252,11 +250,20 @@ class PlanStats:
 
 
 class Plan:
-    def __init__(self, handle):
+    def __init__(self, handle, lazy: bool = False):
         self.h = handle
-        s = _PlanStats()
-        _check(lib().etc_plan_get_stats(handle, C.byref(s)))
-        self.stats = PlanStats(**{n: int(getattr(s, n)) for n, _ in _PlanStats._fields_})
+        self._stats = None
+        if not lazy:
+            self.stats                                    # read now (no wait: the plan was made the synchronising way)
+
+    @property
+    def stats(self) -> PlanStats:
+        """etc_plan_get_stats; for an ETC_NO_SYNC plan the first access waits for the plan's kernels."""
+        if self._stats is None:
+            s = _PlanStats()
+            _check(lib().etc_plan_get_stats(self.h, C.byref(s)))
+            self._stats = PlanStats(**{n: int(getattr(s, n)) for n, _ in _PlanStats._fields_})
+        return self._stats
 
     def traffic(self):
         import numpy as np
@@ -264,6 +271,14 @@ class Plan:
         T = np.zeros((P, P), np.int64)
         _check(lib().etc_plan_get_traffic(self.h, T.ctypes.data))
         return T
+
+    def device_map(self):
+        """the device map the plan was made for (host numpy int32 [n_new]); synchronous."""
+        import numpy as np
+        n = getattr(self, "n_new", None) or self.stats.n_new
+        m = np.zeros(n, np.int32)
+        _check(lib().etc_plan_get_map(self.h, m.ctypes.data))
+        return m
 
     def slices(self, which: int):
         """which = 0 staged, 1 local -> numpy structured array of etc_slice records."""
@@ -339,7 +354,68 @@ def etc_plan_create(old: Layout, new: Layout, device_map, flags: int = ETC_LOCAL
     h = C.c_void_p()
     _check(lib().etc_plan_create_failed(old.h, new.h, ptr, fptr, flags, C.byref(h), _stream(stream)))
     del keep, fkeep
-    return Plan(h)
+    p = Plan(h, lazy=bool(flags & ETC_NO_SYNC))
+    p.n_old, p.n_new = old.n_dev, new.n_dev
+    return p
+
+
+def etc_staging_bound(old: Layout, new: Layout, flags: int = ETC_LOCAL_DIRECT) -> int:
+    """include/etc.h etc_staging_bound: staging bytes that suffice for ANY device map between the two layouts."""
+    n = int(lib().etc_staging_bound(old.h, new.h, flags))
+    if n < 0:
+        raise EtcError(n)
+    return n
+
+
+def _model_struct(model: dict) -> "_ModelDesc":
+    return _ModelDesc(style=model["style"], n_layers=model["n_layers"], hidden=model["hidden"],
+                      n_q_heads=model["n_q_heads"], n_kv_heads=model["n_kv_heads"], head_dim=model["head_dim"],
+                      ffn_hidden=model["ffn_hidden"], vocab=model["vocab"], max_pos=model["max_pos"],
+                      tied_embeddings=model["tied"], param_dtype=model["param_bytes"], kinds=model["kinds"],
+                      qkv_order=model.get("qkv_order", 0))
+
+
+def _cfg_struct(cfg: dict) -> "_ParallelCfg":
+    return _ParallelCfg(tp=cfg["tp"], pp=cfg["pp"], dp=cfg["dp"], dist_opt=cfg.get("dist_opt", 0),
+                        pp_first=cfg.get("pp_first", 0), pp_last=cfg.get("pp_last", 0),
+                        dist_opt_align=cfg.get("dist_opt_align", 0), vocab_divisor=cfg.get("vocab_divisor", 0))
+
+
+class MigrateState:
+    """Pre-marshalled arguments of etc_migrate_state for one (model, old cfg, new cfg, buffers): calling it is ONE
+    C-ABI call that enqueues the whole path (a1)-(a6) without a host synchronisation."""
+
+    def __init__(self, model: dict, old_cfg: dict, new_cfg: dict, src_bufs, dst_bufs, staging, flags: int = ETC_LOCAL_DIRECT,
+                 avail=None):
+        _ensure_init()
+        self.m, self.oc, self.nc = _model_struct(model), _cfg_struct(old_cfg), _cfg_struct(new_cfg)
+        n_old = old_cfg["tp"] * old_cfg["pp"] * old_cfg["dp"]
+        n_new = new_cfg["tp"] * new_cfg["pp"] * new_cfg["dp"]
+        self.n_old, self.n_new = n_old, n_new
+        self.src = _ptr_table(src_bufs, n_old) if isinstance(src_bufs, dict) else src_bufs
+        self.dst = _ptr_table(dst_bufs, n_new) if isinstance(dst_bufs, dict) else dst_bufs
+        self.keep = (src_bufs, dst_bufs, staging, avail)
+        self.stg = staging.data_ptr() if staging is not None and staging.numel() else 0
+        self.stg_bytes = staging.numel() * staging.element_size() if staging is not None else 0
+        self.avail = avail.data_ptr() if avail is not None else 0
+        self.flags = flags
+
+    def __call__(self, stream=None, want_plan: bool = False):
+        h = C.c_void_p()
+        _check(lib().etc_migrate_state(C.byref(self.m), C.byref(self.oc), C.byref(self.nc), self.src, self.dst, self.stg,
+                                       self.stg_bytes, self.avail, self.flags, C.byref(h) if want_plan else None,
+                                       _stream(stream)))
+        if want_plan:
+            p = Plan(h, lazy=True)
+            p.n_old, p.n_new = self.n_old, self.n_new
+            return p
+        return None
+
+
+def etc_migrate_state(model: dict, old_cfg: dict, new_cfg: dict, src_bufs, dst_bufs, staging, flags: int = ETC_LOCAL_DIRECT,
+                      avail=None, stream=None, want_plan: bool = True):
+    """include/etc.h etc_migrate_state: the whole path in one call.  Returns the plan (lazy statistics) or None."""
+    return MigrateState(model, old_cfg, new_cfg, src_bufs, dst_bufs, staging, flags, avail)(stream, want_plan)
 
 
 def _ptr_table(bufs, n_dev):
@@ -353,14 +429,17 @@ def _ptr_table(bufs, n_dev):
 def etc_migrate(plan: Plan, src_bufs: dict, dst_bufs: dict, staging, phases: int = ETC_PHASE_ALL, stream=None):
     """(a5,a6) src_bufs {(old_dev, kind): CUDA tensor}, dst_bufs {(new_rank, kind): CUDA tensor}, staging: CUDA tensor
     of at least plan.stats.staging_bytes bytes (or None).  Asynchronous; no allocation."""
-    st = plan.stats
+    n_old, n_new = getattr(plan, "n_old", None), getattr(plan, "n_new", None)
+    if n_old is None:
+        n_old, n_new = plan.stats.n_old, plan.stats.n_new
     if isinstance(src_bufs, dict):
-        src_bufs = _ptr_table(src_bufs, st.n_old)
+        src_bufs = _ptr_table(src_bufs, n_old)
     if isinstance(dst_bufs, dict):
-        dst_bufs = _ptr_table(dst_bufs, st.n_new)
+        dst_bufs = _ptr_table(dst_bufs, n_new)
     sp = 0
     if staging is not None and staging.numel() > 0:
-        assert staging.numel() * staging.element_size() >= st.staging_bytes
+        if plan._stats is not None:                   # a lazy (ETC_NO_SYNC) plan: the caller sized it by etc_staging_bound
+            assert staging.numel() * staging.element_size() >= plan._stats.staging_bytes
         sp = staging.data_ptr()
     _check(lib().etc_migrate_phase(plan.h, src_bufs, dst_bufs, sp, phases, _stream(stream)))
 

@@ -178,10 +178,11 @@ __device__ __forceinline__ void realign_copy_chunk(char* tile, const char* __res
 }
 
 // One chunk through the path its shape and alignment select.  All threads of the CTA call this.
+template <int MIN_ROW = TMA_MIN_ROW>
 __device__ __forceinline__ void copy_one_chunk(char* tile, uint64_t* bar, const char* src, char* dst, int nrows,
                                                uint32_t row_bytes, uint32_t sp, uint32_t dp, int vec) {
   if (vec == 16) {
-    if (nrows == 1 || row_bytes >= TMA_MIN_ROW) {
+    if (nrows == 1 || row_bytes >= (uint32_t)MIN_ROW) {
       if (threadIdx.x < 32) tma_copy_chunk(tile, bar, src, dst, nrows, row_bytes, sp, dp);
     } else {
       short_rows_copy_chunk(tile, bar, src, dst, nrows, row_bytes, sp, dp);

@@ -110,6 +110,8 @@ extern "C" etc_status etc_cost_matrix(const etc_layout* old_l, const etc_layout*
   if (!old_l || !new_l || !d_overlap || !d_need || !d_hold) return ETC_ERR_INVALID_ARG;
   if (!same_model(old_l, new_l)) return ETC_ERR_MISMATCH;
   const int P = old_l->t.n_dev > new_l->t.n_dev ? old_l->t.n_dev : new_l->t.n_dev;
+  ETC_CUDA_TRY(layout_use(old_l, (cudaStream_t)stream));
+  ETC_CUDA_TRY(layout_use(new_l, (cudaStream_t)stream));
   const long long jobs = (long long)new_l->t.n_dev * P + new_l->t.n_dev + P;
   if (jobs <= 8192)
     cost_matrix_kernel<COST_WARPS><<<(unsigned)jobs, COST_WARPS * 32, 0, (cudaStream_t)stream>>>(
@@ -119,7 +121,6 @@ extern "C" etc_status etc_cost_matrix(const etc_layout* old_l, const etc_layout*
         old_l->t, new_l->t, P, d_overlap, d_need, d_hold);
   ETC_CUDA_TRY(cudaGetLastError());
   count_launch();
-  old_l->streams.note((cudaStream_t)stream); new_l->streams.note((cudaStream_t)stream);
   return ETC_OK;
 }
 

@@ -89,7 +89,11 @@ struct etc_layout {
   int32_t vocab_rows = 0;                 // rows of the embedding tensors in this layout (padded vocabulary, reading A31)
   int32_t lm_head_id = -1;                // logical tensor id of lm_head (-1: tied); word_embeddings is tensor 0
   int32_t n_emb_pieces = 0;               // pieces of the embedding tensors (upper bound of the zero-fill list)
+  std::vector<int32_t> grp_pieces;        // [n_grp] pieces of each (kind, tensor) group over all devices (plan size bounds)
+  bool aligned16 = true;                  // every piece offset, pitch, column range and held flat range is a multiple of 16 B
+  int64_t total_bytes = 0;                // sum of all buffer sizes
   void* d_blob = nullptr;                 // one allocation holding all device tables
+  cudaEvent_t ready = nullptr;            // recorded behind the upload of d_blob (layout_use waits for it)
   mutable etc::StreamSet streams;         // streams that kernels reading the tables were enqueued on
 };
 
@@ -108,6 +112,7 @@ struct DeviceGuard {
   }
   ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
 };
+cudaError_t layout_use(const etc_layout* L, cudaStream_t st);   // `st` waits for the tables' upload; noted as a reader
 // xfer.cu: metadata transfers as kernels on the caller's stream, so that they never queue behind bulk DMA transfers
 cudaError_t write_small(void* d_dst, const void* h_src, size_t bytes, cudaStream_t st);      // host -> device via kernel parameters
 cudaError_t copy_by_kernel(void* dst, const void* src, size_t bytes, cudaStream_t st);       // device / pinned host, either way

@@ -33,7 +33,7 @@ inline bool region_same(const Region& a, const Region& b) {
 // contiguous 1-D regions of one buffer merged.
 static etc_status source_regions(const etc_plan* pl) {
   if (pl->h_regions_ready) return ETC_OK;
-  const PlanTotals& t = pl->totals;
+  const PlanTotals& t = plan_totals(pl);
   std::vector<etc_slice> sl((size_t)(t.n_slices_staged + t.n_slices_local));
   ETC_CUDA_TRY(cudaStreamSynchronize(pl->stream_created_on));
   if (t.n_slices_staged)

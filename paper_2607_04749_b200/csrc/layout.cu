@@ -120,22 +120,45 @@ extern "C" etc_status etc_init(int32_t cuda_device) {
   return ETC_OK;
 }
 
-// grow-only pinned staging buffer + private upload stream (layout tables are built straight into pinned memory and
-// uploaded with one async copy; the only wait is on that private stream)
+// Pinned slabs + private upload stream: the layout tables are built straight into a pinned slab and uploaded with one
+// async copy on the upload stream.  etc_layout_create does not wait for the copy: it records the layout's `ready` event
+// behind it, and every call that reads the tables on a stream makes that stream wait for the event (layout_use).  A slab
+// is reused only after the upload that last read it has finished (its `done` event; with N_SLABS uploads in flight this
+// wait is never taken in practice).
 namespace etc {
 static std::mutex g_up_mu;
-static void* g_pinned = nullptr; static size_t g_pinned_cap = 0;
 static cudaStream_t g_up_stream = nullptr;
-static cudaError_t upload_prepare(size_t bytes) {
+constexpr int N_SLABS = 8;
+struct Slab { void* p = nullptr; size_t cap = 0; cudaEvent_t done = nullptr; bool in_flight = false; };
+static Slab g_slabs[N_SLABS];
+static unsigned g_slab_next = 0;
+static cudaError_t slab_acquire(size_t bytes, Slab** out) {
   if (!g_up_stream) { cudaError_t e = cudaStreamCreateWithFlags(&g_up_stream, cudaStreamNonBlocking); if (e) return e; }
-  if (bytes > g_pinned_cap) {
-    if (g_pinned) cudaFreeHost(g_pinned);
-    g_pinned = nullptr; g_pinned_cap = 0;
+  Slab& s = g_slabs[g_slab_next++ % N_SLABS];
+  if (!s.done) { cudaError_t e = cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming); if (e) return e; }
+  if (s.in_flight) { cudaError_t e = cudaEventSynchronize(s.done); if (e) return e; s.in_flight = false; }
+  if (bytes > s.cap) {
+    if (s.p) cudaFreeHost(s.p);
+    s.p = nullptr; s.cap = 0;
     const size_t cap = std::max<size_t>(bytes + bytes / 2, 1 << 20);
-    cudaError_t e = cudaMallocHost(&g_pinned, cap); if (e) return e;
-    g_pinned_cap = cap;
+    cudaError_t e = cudaMallocHost(&s.p, cap); if (e) return e;
+    s.cap = cap;
   }
+  *out = &s;
   return cudaSuccess;
+}
+
+// Call before enqueueing anything that reads the layout's device tables on `st`.
+cudaError_t layout_use(const etc_layout* L, cudaStream_t st) {
+  cudaError_t e = cudaSuccess;
+  if (L->ready) {
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    e = cudaStreamIsCapturing(st, &cap);
+    if (e == cudaSuccess)
+      e = cudaStreamWaitEvent(st, L->ready, cap == cudaStreamCaptureStatusActive ? cudaEventWaitExternal : cudaEventWaitDefault);
+  }
+  L->streams.note(st);
+  return e;
 }
 // TP shard of one tensor instance: up to 3 row blocks (first logical row rb, rows nr, first local row ls) stored one
 // after the other, times a column range.  rep / rbase per block: the TP ranks [rbase, rbase + rep) hold its elements.
@@ -200,9 +223,10 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   std::lock_guard<std::mutex> lock(g_up_mu);
   DeviceGuard guard;                                       // the caller's current device is restored on return
   cudaError_t e = guard.err;
-  if (e == cudaSuccess) e = upload_prepare(max_total);
+  Slab* slab = nullptr;
+  if (e == cudaSuccess) e = slab_acquire(max_total, &slab);
   if (e != cudaSuccess) { set_error_detail("etc_layout_create staging", e); return ETC_ERR_CUDA; }
-  char* host = static_cast<char*>(g_pinned);
+  char* host = static_cast<char*>(slab->p);
   int32_t* dev_start = reinterpret_cast<int32_t*>(host + o_start);
   int32_t* first = reinterpret_cast<int32_t*>(host + o_first);
   uint32_t* ltmask = reinterpret_cast<uint32_t*>(host + o_mask);
@@ -213,6 +237,8 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   int64_t* bufbytes = new int64_t[(size_t)n_dev * ETC_NUM_KINDS]();
   size_t np = 0;
   int32_t n_emb_pieces = 0;
+  std::vector<int32_t> grp_pieces((size_t)nG, 0);
+  int64_t align_or = 0, total_bytes = 0;
 
   std::vector<std::vector<Sh>> shr(tp);     // shards of (stage, tp-rank r), in GROUP order: tied replica first
   for (int s = 0; s < pp; ++s) {
@@ -274,6 +300,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
             lo = std::min<int64_t>(Lloc, (int64_t)d * chunk); hi = std::min<int64_t>(Lloc, (int64_t)(d + 1) * chunk);
           }
           bufbytes[(size_t)dev * ETC_NUM_KINDS + kind] = (hi - lo) * es;
+          total_bytes += (hi - lo) * es;
           for (const Sh& q : sh) {
             const int64_t a = std::max(lo, q.start) - q.start, b = std::min(hi, q.start + q.n) - q.start;
             if (b <= a) continue;
@@ -315,7 +342,9 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
               p.rep = q.rep[blk]; p.rbase = q.rbase[blk];
               p.boff = (q.start + i0 * q.W + j0 - lo) * es;
               p.f0 = a; p.f1 = b;
+              align_or |= p.boff | ((int64_t)p.W * es) | ((int64_t)p.c0 * es) | ((int64_t)p.nc * es) | (a * es) | (b * es);
             }
+            grp_pieces[(size_t)grp] += (int32_t)(np - np_before);
             if (q.lt == 0 || (!m.tied_embeddings && q.lt == nT - 1)) n_emb_pieces += (int32_t)(np - np_before);
           }
         }
@@ -330,14 +359,19 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   etc_layout* L = new etc_layout();
   L->model = m; L->cfg = *cfg; L->h_buffer_bytes = bufbytes; L->max_dev_pieces = max_dev_pieces;
   L->vocab_rows = (int32_t)vocab_rows(m, *cfg); L->lm_head_id = m.tied_embeddings ? -1 : nT - 1; L->n_emb_pieces = n_emb_pieces;
+  L->grp_pieces = std::move(grp_pieces); L->aligned16 = (align_or & 15) == 0; L->total_bytes = total_bytes;
   e = cudaMallocAsync(&L->d_blob, total, g_up_stream);
   // a DMA copy on the private upload stream: it runs beside the copy kernels of a migration in flight (a copy kernel
-  // here was measured to wait for them: 0.16 -> 1.7 ms per layout pair on c2)
+  // here was measured to wait for them: 0.16 -> 1.7 ms per layout pair on c2).  No host wait: readers wait for `ready`.
   if (e == cudaSuccess) e = cudaMemcpyAsync(L->d_blob, host, total, cudaMemcpyHostToDevice, g_up_stream);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(g_up_stream);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&L->ready, cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaEventRecord(L->ready, g_up_stream);
+  if (e == cudaSuccess) { e = cudaEventRecord(slab->done, g_up_stream); slab->in_flight = e == cudaSuccess; }
   if (e != cudaSuccess) {
     set_error_detail("etc_layout_create upload", e);
+    cudaStreamSynchronize(g_up_stream);                    // the slab may still be being read
     if (L->d_blob) cudaFreeAsync(L->d_blob, g_up_stream);
+    if (L->ready) cudaEventDestroy(L->ready);
     delete[] bufbytes; delete L;
     return ETC_ERR_CUDA;
   }
@@ -359,6 +393,7 @@ extern "C" void etc_layout_destroy(etc_layout* L) {
   if (!L) return;
   // stream-ordered free, ordered after every kernel already enqueued on any stream that read the tables
   if (L->d_blob) cudaFreeAsync(L->d_blob, L->streams.join(g_up_stream));
+  if (L->ready) cudaEventDestroy(L->ready);
   delete[] L->h_buffer_bytes;
   delete L;
 }

@@ -30,10 +30,14 @@ template <bool UNPACK, bool PARAM_PTRS>
 __global__ void __launch_bounds__(CP_THREADS)
 migrate_copy_kernel(const Chunk* __restrict__ chA, long long nA, const Chunk* __restrict__ chB,
                     const void* const* __restrict__ tab, int ns, char* __restrict__ staging,
-                    const __grid_constant__ PtrParams pp) {
-  extern __shared__ __align__(128) char tile[];                 // TILE_BYTES: TMA path and cp.async staged paths
+                    const PlanTotals* __restrict__ lazy, const __grid_constant__ PtrParams pp) {
+  extern __shared__ __align__(128) char tile[];                 // TILE_BYTES: the staging tile of every copy path
   __shared__ uint64_t bar;
   const long long b = blockIdx.x;
+  if (lazy) {                                                   // ETC_NO_SYNC plan: the grid is an upper bound, the counts are here
+    nA = lazy->n_chunks_staged;
+    if (b >= nA + (UNPACK ? 0 : lazy->n_chunks_local)) return;
+  }
   const bool staged = b < nA;
   const Chunk c = staged ? chA[b] : chB[b - nA];
   const char* src; char* dst; uint32_t sp, dp;
@@ -70,7 +74,8 @@ __device__ __forceinline__ void fill_rows(char* dst, int nrows, uint32_t row_byt
 template <bool PARAM_PTRS>
 __global__ void __launch_bounds__(CP_THREADS)
 migrate_fill_kernel(const etc_slice* __restrict__ fills, const void* const* __restrict__ tab, int ns, int only_kind,
-                    const __grid_constant__ PtrParams pp) {
+                    const PlanTotals* __restrict__ lazy, const __grid_constant__ PtrParams pp) {
+  if (lazy && (long long)blockIdx.x >= lazy->n_fills) return;
   const etc_slice f = fills[blockIdx.x];
   if (only_kind >= 0 && f.kind != only_kind) return;
   const int di = ns + f.dst_rank * ETC_NUM_KINDS + f.kind;
@@ -114,7 +119,8 @@ using namespace etc;
 // chunk ranges.  `staging` is addressed relative to stg_base.
 static etc_status launch_migrate(const etc_plan* pl, const void* const* src_bufs, void* const* dst_bufs, void* staging,
                                  int32_t phases, cudaStream_t st, void** d_ptrs, int only_kind, long long ca, long long nA,
-                                 long long la, long long nB, int64_t stg_base, int64_t stg_need, bool with_fills) {
+                                 long long la, long long nB, int64_t stg_base, int64_t stg_need, bool with_fills,
+                                 long long n_fills, const PlanTotals* lazy) {
   if (!pl || !src_bufs || !dst_bufs || phases < 1 || phases > ETC_PHASE_ALL) return ETC_ERR_INVALID_ARG;
   if (stg_need > 0 && !staging) return ETC_ERR_INVALID_ARG;
   if (reinterpret_cast<uintptr_t>(staging) & 15) return ETC_ERR_INVALID_ARG;
@@ -148,24 +154,24 @@ static etc_status launch_migrate(const etc_plan* pl, const void* const* src_bufs
   char* stg = static_cast<char*>(staging) - stg_base;          // chunk records carry offsets of the full staging layout
   if ((phases & ETC_PHASE_PACK) && nA + nB > 0) {
     if (in_params) migrate_copy_kernel<false, true><<<(unsigned)(nA + nB), CP_THREADS, TILE_BYTES, st>>>(
-        pl->d_ch_staged + ca, nA, pl->d_ch_local + la, tab, (int)ns, stg, pp);
+        pl->d_ch_staged + ca, nA, pl->d_ch_local + la, tab, (int)ns, stg, lazy, pp);
     else migrate_copy_kernel<false, false><<<(unsigned)(nA + nB), CP_THREADS, TILE_BYTES, st>>>(
-        pl->d_ch_staged + ca, nA, pl->d_ch_local + la, tab, (int)ns, stg, pp);
+        pl->d_ch_staged + ca, nA, pl->d_ch_local + la, tab, (int)ns, stg, lazy, pp);
     ETC_CUDA_TRY(cudaGetLastError());
     count_launch();
   }
-  if ((phases & ETC_PHASE_PACK) && with_fills && pl->totals.n_fills > 0) {      // reading A31: bytes with no source
-    const dim3 grid((unsigned)pl->totals.n_fills, FILL_SPLIT);
-    if (in_params) migrate_fill_kernel<true><<<grid, CP_THREADS, 0, st>>>(pl->d_fills, tab, (int)ns, only_kind, pp);
-    else migrate_fill_kernel<false><<<grid, CP_THREADS, 0, st>>>(pl->d_fills, tab, (int)ns, only_kind, pp);
+  if ((phases & ETC_PHASE_PACK) && with_fills && n_fills > 0) {                 // reading A31: bytes with no source
+    const dim3 grid((unsigned)n_fills, FILL_SPLIT);
+    if (in_params) migrate_fill_kernel<true><<<grid, CP_THREADS, 0, st>>>(pl->d_fills, tab, (int)ns, only_kind, lazy, pp);
+    else migrate_fill_kernel<false><<<grid, CP_THREADS, 0, st>>>(pl->d_fills, tab, (int)ns, only_kind, lazy, pp);
     ETC_CUDA_TRY(cudaGetLastError());
     count_launch();
   }
   if ((phases & ETC_PHASE_UNPACK) && nA > 0) {
     if (in_params) migrate_copy_kernel<true, true><<<(unsigned)nA, CP_THREADS, TILE_BYTES, st>>>(
-        pl->d_ch_staged + ca, nA, nullptr, tab, (int)ns, stg, pp);
+        pl->d_ch_staged + ca, nA, nullptr, tab, (int)ns, stg, lazy, pp);
     else migrate_copy_kernel<true, false><<<(unsigned)nA, CP_THREADS, TILE_BYTES, st>>>(
-        pl->d_ch_staged + ca, nA, nullptr, tab, (int)ns, stg, pp);
+        pl->d_ch_staged + ca, nA, nullptr, tab, (int)ns, stg, lazy, pp);
     ETC_CUDA_TRY(cudaGetLastError());
     count_launch();
   }
@@ -176,9 +182,25 @@ extern "C" etc_status etc_migrate_phase(const etc_plan* pl, const void* const* s
                                         void* staging, int32_t phases, void* stream) {
   clear_error_detail();
   if (!pl) return ETC_ERR_INVALID_ARG;
-  const PlanTotals& t = pl->totals;
+  if (pl->lazy && !pl->resolved) {
+    // ETC_NO_SYNC plan whose counts are still on the device: grids from the host-side bounds (staged + local chunks
+    // together never exceed bound_chunks), the kernels read the real counts and idle CTAs leave at once
+    const bool direct = (pl->flags & ETC_ALL_DIRECT) != 0;
+    if (!direct && !staging) return ETC_ERR_INVALID_ARG;
+    if (direct) phases &= ~ETC_PHASE_UNPACK;
+    if (phases == 0) return ETC_OK;
+    const long long nb = pl->bound_chunks;
+    if (phases == ETC_PHASE_UNPACK)
+      return launch_migrate(pl, src_bufs, dst_bufs, staging, phases, (cudaStream_t)stream, pl->d_ptrs, -1, 0, nb, 0, 0, 0, 0,
+                            false, 0, pl->d_totals);
+    return launch_migrate(pl, src_bufs, dst_bufs, staging, phases, (cudaStream_t)stream, pl->d_ptrs, -1, 0, direct ? 0 : nb, 0,
+                          direct ? nb : 0, 0, 0, true, pl->bound_fills, pl->d_totals);
+  }
+  etc_status rc = ETC_OK;
+  const PlanTotals& t = plan_totals(pl, &rc);
+  if (rc != ETC_OK) return rc;
   return launch_migrate(pl, src_bufs, dst_bufs, staging, phases, (cudaStream_t)stream, pl->d_ptrs, -1, 0,
-                        t.n_chunks_staged, 0, t.n_chunks_local, 0, t.staging_bytes, true);
+                        t.n_chunks_staged, 0, t.n_chunks_local, 0, t.staging_bytes, true, t.n_fills, nullptr);
 }
 
 extern "C" etc_status etc_migrate(const etc_plan* pl, const void* const* src_bufs, void* const* dst_bufs, void* staging,
@@ -195,5 +217,5 @@ extern "C" etc_status etc_migrate_round(const etc_plan* pl, int32_t round, const
   const size_t n_ptrs = ((size_t)(pl->n_old + pl->n_new) * ETC_NUM_KINDS * sizeof(void*) + 255) / 256 * 256 / sizeof(void*);
   return launch_migrate(pl, src_bufs, dst_bufs, staging, phases, (cudaStream_t)stream,
                         pl->d_round_ptrs + n_ptrs * (size_t)round, r.kind, r.ca, r.cb - r.ca, r.la, r.lb - r.la,
-                        r.stg_base, r.stg_span, r.sub == 0);
+                        r.stg_base, r.stg_span, r.sub == 0, plan_totals(pl).n_fills, nullptr);
 }

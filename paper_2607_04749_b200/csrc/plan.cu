@@ -204,7 +204,7 @@ constexpr int SCAN_THREADS = 1024;
 __global__ void __launch_bounds__(SCAN_THREADS)
 plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int K, int n_old, int n_new, int P, int flags,
                  const int32_t* __restrict__ device_map, UnitBase* __restrict__ bases, int64_t* __restrict__ traffic,
-                 PlanTotals* __restrict__ totals) {
+                 PlanTotals* __restrict__ totals, int64_t bound_slices, int64_t bound_chunks, int64_t bound_staging) {
   __shared__ int64_t s_w[5][32];
   __shared__ int64_t s_carry[5];
   __shared__ int64_t s_loc[32], s_rem[32];
@@ -284,6 +284,14 @@ plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int K, int n_
       t.n_slices_local = s_carry[3]; t.n_chunks_local = s_carry[4];
       t.local_bytes = loc; t.remote_bytes = rem; t.bad_map = bad ? 1 : 0;
       t.fill_bytes = 0; t.n_fills = 0;                          // plan_fills_kernel adds to these
+      // ETC_NO_SYNC: the tables were sized from host-side upper bounds before these counts existed.  Should a bound
+      // ever fall short, or the map be bad, the counts are zeroed so that no later kernel writes or copies anything.
+      t.overflow = (bound_slices > 0 && (t.n_slices_staged > bound_slices || t.n_slices_local > bound_slices ||
+                                         t.n_chunks_staged > bound_chunks || t.n_chunks_local > bound_chunks ||
+                                         t.staging_bytes > bound_staging)) ? 1 : 0;
+      if (bound_slices > 0 && (t.overflow || t.bad_map)) {
+        t.n_slices_staged = t.n_chunks_staged = t.n_slices_local = t.n_chunks_local = 0; t.staging_bytes = 0;
+      }
       for (int k = 0; k < ETC_NUM_KINDS; ++k) for (int j = 0; j < 3; ++j) t.kind_base[k][j] = s_kind[k][j];
       t.kind_base[ETC_NUM_KINDS][0] = s_carry[1]; t.kind_base[ETC_NUM_KINDS][1] = s_carry[2];
       t.kind_base[ETC_NUM_KINDS][2] = s_carry[4];
@@ -299,7 +307,8 @@ plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict
                  const uint8_t* __restrict__ failed, int flags, int K, int B,
                  const BlockCount* __restrict__ blocks, const UnitBase* __restrict__ bases,
                  etc_slice* __restrict__ sl_staged, etc_slice* __restrict__ sl_local,
-                 int64_t* __restrict__ c0_staged, int64_t* __restrict__ c0_local) {
+                 int64_t* __restrict__ c0_staged, int64_t* __restrict__ c0_local, const PlanTotals* __restrict__ lazy) {
+  if (lazy && (lazy->bad_map || lazy->overflow)) return;
   const int lane = threadIdx.x & 31;
   const long long w = (long long)blockIdx.x * PLAN_WARPS + (threadIdx.x >> 5);
   const long long U = (long long)K * oldT.n_dev * newT.n_dev;
@@ -373,7 +382,11 @@ plan_fills_kernel(DeviceTables newT, const int32_t* __restrict__ device_map, int
 // pass 3: one thread per chunk: find its slice by binary search over the slices' first-chunk indices, cut the chunk out
 __global__ void __launch_bounds__(256)
 plan_chunks_kernel(const etc_slice* __restrict__ slices, const int64_t* __restrict__ chunk0, long long n_slices,
-                   long long n_chunks, Chunk* __restrict__ out) {
+                   long long n_chunks, Chunk* __restrict__ out, const PlanTotals* __restrict__ lazy, int which) {
+  if (lazy) {                                                   // ETC_NO_SYNC: the counts never went to the host
+    n_slices = which == 0 ? lazy->n_slices_staged : lazy->n_slices_local;
+    n_chunks = which == 0 ? lazy->n_chunks_staged : lazy->n_chunks_local;
+  }
   const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= n_chunks) return;
   long long lo = 0, hi = n_slices - 1;                          // last slice with chunk0 <= c
@@ -455,22 +468,69 @@ static bool on_device_ptr(const void* p) {
   return attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged;
 }
 
+const PlanTotals& etc::plan_totals(const etc_plan* cpl, etc_status* rc) {
+  etc_plan* pl = const_cast<etc_plan*>(cpl);
+  std::lock_guard<std::mutex> lock(pl->resolve_mu);
+  if (!pl->resolved) {
+    etc_status st = ETC_OK;
+    cudaError_t e = pl->ready ? cudaEventSynchronize(pl->ready) : cudaStreamSynchronize(pl->stream_created_on);
+    if (e == cudaSuccess) e = cudaMemcpy(&pl->totals, pl->d_totals, sizeof(PlanTotals), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) { set_error_detail("plan totals read-back", e); st = ETC_ERR_CUDA; }
+    else if (pl->totals.bad_map) st = ETC_ERR_BAD_MAP;
+    else if (pl->totals.overflow) st = ETC_ERR_WORKSPACE;
+    else if (pl->totals.local_bytes + pl->totals.remote_bytes + pl->totals.fill_bytes != pl->need_bytes) st = ETC_ERR_UNRECOVERABLE;
+    pl->resolve_status = st;
+    pl->resolved = true;
+  }
+  if (rc) *rc = pl->resolve_status;
+  return pl->totals;
+}
+
 extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
                                       int32_t flags, etc_plan** out, void* stream) {
   return etc_plan_create_failed(old_l, new_l, device_map, nullptr, flags, out, stream);
+}
+
+// Upper bounds of a plan's tables from what the host knows about the two layouts (ETC_NO_SYNC):
+//   slices: a slice comes from one (new piece, old piece) pair of the same (kind, tensor) group — at most 4 of them when
+//           the old kind is DP-sharded (the destination's own flat range is cut out of the rectangle), else 1;
+//   chunks (per list): every slice ends in at most one short chunk, and every other chunk carries more than
+//           ETC_CHUNK_BYTES / 2 bytes — or, on the re-aligning path, more than 4 KB (rows_per_chunk);
+//   staging: payload + 16 bytes of padding per slice + 512 per (kind, source, destination) segment.
+static void plan_bounds(const etc_layout* old_l, const etc_layout* new_l, int K, etc_plan* pl) {
+  const int nT = old_l->t.n_tensors;
+  const bool old_sharded = old_l->cfg.dist_opt && old_l->cfg.dp > 1;
+  int64_t sl = 0;
+  for (size_t g = 0; g < old_l->grp_pieces.size() && g < new_l->grp_pieces.size(); ++g)
+    sl += (int64_t)old_l->grp_pieces[g] * new_l->grp_pieces[g] * ((old_sharded && (int)(g / nT) >= 1) ? 4 : 1);
+  const int64_t need = new_l->total_bytes;
+  const int64_t min_pay = (old_l->aligned16 && new_l->aligned16) ? ETC_CHUNK_BYTES / 2 : 4096;
+  pl->bound_slices = sl + 1;
+  pl->bound_chunks = sl + need / min_pay + 2;
+  pl->bound_staging = need + 16 * sl + 512ll * K * old_l->t.n_dev * new_l->t.n_dev + 512;
+  pl->need_bytes = need;
+}
+
+extern "C" int64_t etc_staging_bound(const etc_layout* old_l, const etc_layout* new_l, int32_t flags) {
+  if (!old_l || !new_l || !etc_same_model(old_l, new_l)) return ETC_ERR_INVALID_ARG;
+  if (flags & ETC_ALL_DIRECT) return 0;
+  etc_plan tmp;
+  plan_bounds(old_l, new_l, (flags & ETC_KIND_MAJOR) ? ETC_NUM_KINDS : 1, &tmp);
+  return tmp.bound_staging;
 }
 
 extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
                                              const uint8_t* failed, int32_t flags, etc_plan** out, void* stream) {
   clear_error_detail();
   if (!old_l || !new_l || !device_map || !out) return ETC_ERR_INVALID_ARG;
-  if (flags < 0 || flags > (ETC_ALL_STAGED | ETC_KIND_MAJOR | ETC_ALL_DIRECT)) return ETC_ERR_INVALID_ARG;
+  if (flags < 0 || flags > (ETC_ALL_STAGED | ETC_KIND_MAJOR | ETC_ALL_DIRECT | ETC_NO_SYNC)) return ETC_ERR_INVALID_ARG;
   if ((flags & ETC_ALL_STAGED) && (flags & ETC_ALL_DIRECT)) return ETC_ERR_INVALID_ARG;
   if (!etc_same_model(old_l, new_l)) return ETC_ERR_MISMATCH;
   const int n_old = old_l->t.n_dev, n_new = new_l->t.n_dev, P = n_old > n_new ? n_old : n_new;
   if ((long long)P * ETC_NUM_KINDS > 65535) return ETC_ERR_WORKSPACE;
   cudaStream_t st = (cudaStream_t)stream;
-  old_l->streams.note(st); new_l->streams.note(st);
+  ETC_CUDA_TRY(layout_use(old_l, st));
+  ETC_CUDA_TRY(layout_use(new_l, st));
   const int K = (flags & ETC_KIND_MAJOR) ? ETC_NUM_KINDS : 1;
   const long long U = (long long)K * n_old * n_new;
   // sub-blocks per unit: enough warps to fill the machine when there are few units, 1 when there are many
@@ -478,15 +538,21 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
   const int B = (int)std::max<long long>(1, std::min<long long>(want, 65536 / U));
 
   etc_plan* pl = new etc_plan();
-  pl->n_old = n_old; pl->n_new = n_new; pl->P = P; pl->flags = flags; pl->stream_created_on = st;
+  pl->n_old = n_old; pl->n_new = n_new; pl->P = P; pl->flags = flags & ~ETC_NO_SYNC; pl->stream_created_on = st;
   pl->streams.note(st);
   pl->old_bytes.assign(old_l->h_buffer_bytes, old_l->h_buffer_bytes + (size_t)n_old * ETC_NUM_KINDS);
   pl->new_bytes.assign(new_l->h_buffer_bytes, new_l->h_buffer_bytes + (size_t)n_new * ETC_NUM_KINDS);
+  plan_bounds(old_l, new_l, K, pl);
+  // reading A31: the new layout's padded vocabulary has rows the old one lacks -> those are zero-filled
+  const bool grows = new_l->vocab_rows > old_l->vocab_rows && new_l->n_emb_pieces > 0;
+  pl->bound_fills = grows ? new_l->n_emb_pieces : 0;
+  // ETC_NO_SYNC is honoured while the bound-sized tables stay small; a big plan is made the exact way (one host sync
+  // costs nothing next to its copy kernels, and exact grids keep its copy launches free of idle CTAs)
+  const size_t bound_tb = (size_t)pl->bound_slices * 2 * (sizeof(etc_slice) + 8) + (size_t)pl->bound_chunks * 2 * sizeof(Chunk);
+  const bool lazy = (flags & ETC_NO_SYNC) && bound_tb <= ((size_t)64 << 20);
+  pl->lazy = lazy; pl->resolved = !lazy;
   auto fail = [&](etc_status s) { etc_plan_destroy(pl); return s; };
 #define PLAN_TRY(expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) { set_error_detail(#expr, _e); return fail(ETC_ERR_CUDA); } } while (0)
-
-  if (!g_pinned_totals) PLAN_TRY(cudaMallocHost(&g_pinned_totals, sizeof(PlanTotals) * N_PINNED_TOTALS));
-  PlanTotals* h_tot = &g_pinned_totals[__atomic_fetch_add(&g_pinned_next, 1u, __ATOMIC_RELAXED) % N_PINNED_TOTALS];
 
   // device_map may live on the host or on the device
   const bool on_device = on_device_ptr(device_map);
@@ -498,8 +564,6 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
       seen[p] = 1;
     }
   }
-  // reading A31: the new layout's padded vocabulary has rows the old one lacks -> those are zero-filled
-  const bool grows = new_l->vocab_rows > old_l->vocab_rows && new_l->n_emb_pieces > 0;
   // workspace blob 1: units | bases | blocks | traffic | totals | map | pointer tables | failure mask | zero-fill list
   auto al = [](size_t x) { return (x + 255) & ~size_t(255); };
   const size_t o_units = 0, o_bases = o_units + al(sizeof(UnitCount) * (size_t)U),
@@ -531,8 +595,9 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
   plan_count_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, d_failed, K, B, pl->d_units,
                                                       pl->d_blocks);
   PLAN_TRY(cudaGetLastError());
-  plan_scan_kernel<<<1, SCAN_THREADS, 0, st>>>(pl->d_units, U, K, n_old, n_new, P, flags, pl->d_map, pl->d_bases,
-                                               pl->d_traffic, pl->d_totals);
+  plan_scan_kernel<<<1, SCAN_THREADS, 0, st>>>(pl->d_units, U, K, n_old, n_new, P, pl->flags, pl->d_map, pl->d_bases,
+                                               pl->d_traffic, pl->d_totals, lazy ? pl->bound_slices : 0,
+                                               pl->bound_chunks, pl->bound_staging);
   PLAN_TRY(cudaGetLastError());
   count_launch(2);
   if (grows) {
@@ -542,23 +607,28 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
     PLAN_TRY(cudaGetLastError());
     count_launch();
   }
-  PLAN_TRY(copy_by_kernel(h_tot, pl->d_totals, sizeof(PlanTotals), st));      // h_tot is pinned: the kernel writes it
-  PLAN_TRY(cudaStreamSynchronize(st));                          // the one host sync: sizes must come back
-  pl->totals = *h_tot;
-  if (pl->totals.bad_map) return fail(ETC_ERR_BAD_MAP);
-  {                                                             // every needed byte must have found its one source
-    int64_t need = 0;
-    for (int64_t b : pl->new_bytes) need += b;
-    if (pl->totals.local_bytes + pl->totals.remote_bytes + pl->totals.fill_bytes != need) return fail(ETC_ERR_UNRECOVERABLE);
+  int64_t n_sl_s, n_sl_l, n_ch_s, n_ch_l;                       // table capacities
+  if (!lazy) {
+    if (!g_pinned_totals) PLAN_TRY(cudaMallocHost(&g_pinned_totals, sizeof(PlanTotals) * N_PINNED_TOTALS));
+    PlanTotals* h_tot = &g_pinned_totals[__atomic_fetch_add(&g_pinned_next, 1u, __ATOMIC_RELAXED) % N_PINNED_TOTALS];
+    PLAN_TRY(copy_by_kernel(h_tot, pl->d_totals, sizeof(PlanTotals), st));    // h_tot is pinned: the kernel writes it
+    PLAN_TRY(cudaStreamSynchronize(st));                        // the one host sync: sizes must come back
+    pl->totals = *h_tot;
+    if (pl->totals.bad_map) return fail(ETC_ERR_BAD_MAP);
+    // every needed byte must have found its one source
+    if (pl->totals.local_bytes + pl->totals.remote_bytes + pl->totals.fill_bytes != pl->need_bytes) return fail(ETC_ERR_UNRECOVERABLE);
+    n_sl_s = pl->totals.n_slices_staged; n_sl_l = pl->totals.n_slices_local;
+    n_ch_s = pl->totals.n_chunks_staged; n_ch_l = pl->totals.n_chunks_local;
+  } else {
+    n_sl_s = n_sl_l = pl->bound_slices; n_ch_s = n_ch_l = pl->bound_chunks;
   }
 
   // blob 2: slice records | first-chunk indices | chunk descriptors
-  const PlanTotals& t = pl->totals;
-  const size_t o_sls = 0, o_sll = o_sls + al(sizeof(etc_slice) * (size_t)t.n_slices_staged),
-               o_c0s = o_sll + al(sizeof(etc_slice) * (size_t)t.n_slices_local),
-               o_c0l = o_c0s + al(8 * (size_t)t.n_slices_staged), o_chs = o_c0l + al(8 * (size_t)t.n_slices_local),
-               o_chl = o_chs + al(sizeof(Chunk) * (size_t)t.n_chunks_staged),
-               tb_bytes = o_chl + al(sizeof(Chunk) * (size_t)t.n_chunks_local);
+  const size_t o_sls = 0, o_sll = o_sls + al(sizeof(etc_slice) * (size_t)n_sl_s),
+               o_c0s = o_sll + al(sizeof(etc_slice) * (size_t)n_sl_l),
+               o_c0l = o_c0s + al(8 * (size_t)n_sl_s), o_chs = o_c0l + al(8 * (size_t)n_sl_l),
+               o_chl = o_chs + al(sizeof(Chunk) * (size_t)n_ch_s),
+               tb_bytes = o_chl + al(sizeof(Chunk) * (size_t)n_ch_l);
   if (tb_bytes) {
     PLAN_TRY(cudaMallocAsync(&pl->d_tb, tb_bytes, st));
     char* tb = static_cast<char*>(pl->d_tb);
@@ -566,21 +636,23 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
     pl->d_c0_staged = reinterpret_cast<int64_t*>(tb + o_c0s); pl->d_c0_local = reinterpret_cast<int64_t*>(tb + o_c0l);
     pl->d_ch_staged = reinterpret_cast<Chunk*>(tb + o_chs); pl->d_ch_local = reinterpret_cast<Chunk*>(tb + o_chl);
   }
-  if (t.n_slices_staged + t.n_slices_local) {
-    plan_fill_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, d_failed, flags, K, B, pl->d_blocks, pl->d_bases,
-                                                       pl->d_sl_staged, pl->d_sl_local, pl->d_c0_staged, pl->d_c0_local);
+  const PlanTotals* d_lazy = lazy ? pl->d_totals : nullptr;
+  if (n_sl_s + n_sl_l) {
+    plan_fill_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, d_failed, pl->flags, K, B, pl->d_blocks, pl->d_bases,
+                                                       pl->d_sl_staged, pl->d_sl_local, pl->d_c0_staged, pl->d_c0_local, d_lazy);
     PLAN_TRY(cudaGetLastError());
     count_launch();
   }
-  if (t.n_chunks_staged) {
-    plan_chunks_kernel<<<(unsigned)((t.n_chunks_staged + 255) / 256), 256, 0, st>>>(
-        pl->d_sl_staged, pl->d_c0_staged, t.n_slices_staged, t.n_chunks_staged, pl->d_ch_staged);
+  // an ETC_NO_SYNC plan that cannot stage anything (ETC_ALL_DIRECT) has no staged list to expand
+  if (n_ch_s && !(lazy && (pl->flags & ETC_ALL_DIRECT))) {
+    plan_chunks_kernel<<<(unsigned)((n_ch_s + 255) / 256), 256, 0, st>>>(
+        pl->d_sl_staged, pl->d_c0_staged, n_sl_s, n_ch_s, pl->d_ch_staged, d_lazy, 0);
     PLAN_TRY(cudaGetLastError());
     count_launch();
   }
-  if (t.n_chunks_local) {
-    plan_chunks_kernel<<<(unsigned)((t.n_chunks_local + 255) / 256), 256, 0, st>>>(
-        pl->d_sl_local, pl->d_c0_local, t.n_slices_local, t.n_chunks_local, pl->d_ch_local);
+  if (n_ch_l) {
+    plan_chunks_kernel<<<(unsigned)((n_ch_l + 255) / 256), 256, 0, st>>>(
+        pl->d_sl_local, pl->d_c0_local, n_sl_l, n_ch_l, pl->d_ch_local, d_lazy, 1);
     PLAN_TRY(cudaGetLastError());
     count_launch();
   }
@@ -604,7 +676,9 @@ extern "C" void etc_plan_destroy(etc_plan* pl) {
 
 extern "C" etc_status etc_plan_get_stats(const etc_plan* pl, etc_plan_stats* out) {
   if (!pl || !out) return ETC_ERR_INVALID_ARG;
-  const PlanTotals& t = pl->totals;
+  etc_status rc = ETC_OK;
+  const PlanTotals& t = plan_totals(pl, &rc);                   // an ETC_NO_SYNC plan is waited for here
+  if (rc != ETC_OK) return rc;
   out->staging_bytes = t.staging_bytes; out->local_bytes = t.local_bytes; out->remote_bytes = t.remote_bytes;
   out->staged_bytes = (pl->flags & ETC_ALL_STAGED) ? t.local_bytes + t.remote_bytes : ((pl->flags & ETC_ALL_DIRECT) ? 0 : t.remote_bytes);
   out->n_slices_local = t.n_slices_local; out->n_slices_staged = t.n_slices_staged;
@@ -622,10 +696,18 @@ extern "C" etc_status etc_plan_get_traffic(const etc_plan* pl, int64_t* h_traffi
   return ETC_OK;
 }
 
+extern "C" etc_status etc_plan_get_map(const etc_plan* pl, int32_t* h_device_map) {
+  clear_error_detail();
+  if (!pl || !h_device_map) return ETC_ERR_INVALID_ARG;
+  ETC_CUDA_TRY(cudaStreamSynchronize(pl->stream_created_on));
+  ETC_CUDA_TRY(cudaMemcpy(h_device_map, pl->d_map, sizeof(int32_t) * (size_t)pl->n_new, cudaMemcpyDeviceToHost));
+  return ETC_OK;
+}
+
 extern "C" etc_status etc_plan_get_slices(const etc_plan* pl, int32_t which, etc_slice* h_out) {
   clear_error_detail();
   if (!pl || !h_out || (which != 0 && which != 1)) return ETC_ERR_INVALID_ARG;
-  const int64_t n = which == 0 ? pl->totals.n_slices_staged : pl->totals.n_slices_local;
+  const int64_t n = which == 0 ? plan_totals(pl).n_slices_staged : plan_totals(pl).n_slices_local;
   const etc_slice* src = which == 0 ? pl->d_sl_staged : pl->d_sl_local;
   ETC_CUDA_TRY(cudaStreamSynchronize(pl->stream_created_on));
   if (n) ETC_CUDA_TRY(cudaMemcpy(h_out, src, sizeof(etc_slice) * (size_t)n, cudaMemcpyDeviceToHost));
@@ -636,7 +718,8 @@ extern "C" etc_status etc_plan_get_fills(const etc_plan* pl, etc_slice* h_out) {
   clear_error_detail();
   if (!pl || !h_out) return ETC_ERR_INVALID_ARG;
   ETC_CUDA_TRY(cudaStreamSynchronize(pl->stream_created_on));
-  if (pl->totals.n_fills) ETC_CUDA_TRY(cudaMemcpy(h_out, pl->d_fills, sizeof(etc_slice) * (size_t)pl->totals.n_fills, cudaMemcpyDeviceToHost));
+  const int64_t nf = plan_totals(pl).n_fills;
+  if (nf) ETC_CUDA_TRY(cudaMemcpy(h_out, pl->d_fills, sizeof(etc_slice) * (size_t)nf, cudaMemcpyDeviceToHost));
   return ETC_OK;
 }
 
@@ -654,7 +737,7 @@ extern "C" etc_status etc_plan_validate(const etc_plan* pl, int64_t* n_bad, void
   VAL_TRY(cudaMemcpyAsync(d_sizes + ns, pl->new_bytes.data(), sizeof(int64_t) * nd, cudaMemcpyHostToDevice, st));
   unsigned long long* d_bad = reinterpret_cast<unsigned long long*>(d_sizes + ns + nd);
   VAL_TRY(cudaMemsetAsync(d_bad, 0, sizeof(unsigned long long), st));
-  const PlanTotals& t = pl->totals;
+  const PlanTotals& t = plan_totals(pl);
   if (t.n_chunks_staged) {
     plan_validate_kernel<<<(unsigned)((t.n_chunks_staged + 255) / 256), 256, 0, st>>>(pl->d_ch_staged, t.n_chunks_staged, 1, d_sizes,
                                                                                      d_sizes + ns, t.staging_bytes, d_bad);

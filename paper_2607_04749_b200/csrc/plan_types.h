@@ -12,6 +12,7 @@ struct PlanTotals {
   int64_t n_slices_staged, n_chunks_staged, staging_bytes, n_slices_local, n_chunks_local;
   int64_t local_bytes, remote_bytes, bad_map;
   int64_t fill_bytes, n_fills;           // zero-filled destination bytes / descriptors (reading A31); added after the scan
+  int64_t overflow;                      // ETC_NO_SYNC plans: the tables sized from host-side bounds would not have sufficed
   // kind-major plans: [kind][0] first staged chunk, [1] first staging byte, [2] first local chunk of the kind;
   // entry [ETC_NUM_KINDS] = the totals
   int64_t kind_base[ETC_NUM_KINDS + 1][3];
@@ -61,6 +62,9 @@ namespace etc {
 // Call before enqueueing anything that reads the plan's tables on `st`: a stream other than the one the plan was created
 // on is made to wait for the plan's last table-writing kernel, and `st` is noted as a reader (frees are ordered after it).
 cudaError_t plan_use(const etc_plan* pl, cudaStream_t st);
+// The plan's totals on the host.  For an ETC_NO_SYNC plan the first call waits for the plan's kernels and reads them
+// back; *rc receives ETC_ERR_BAD_MAP / ETC_ERR_UNRECOVERABLE / ETC_ERR_WORKSPACE if the device found the plan unusable.
+const PlanTotals& plan_totals(const etc_plan* pl, etc_status* rc = nullptr);
 }
 
 struct etc_plan {
@@ -68,7 +72,13 @@ struct etc_plan {
   cudaStream_t stream_created_on = nullptr;
   cudaEvent_t ready = nullptr;                     // recorded on stream_created_on after the last table-writing kernel
   mutable etc::StreamSet streams;                  // streams the plan's tables were written / read on (frees are ordered after them)
-  etc::PlanTotals totals{};
+  etc::PlanTotals totals{};                        // valid once `resolved` (always, unless created with ETC_NO_SYNC)
+  // ETC_NO_SYNC: tables sized from upper bounds, counts live on the device until someone asks (plan_totals)
+  bool lazy = false;
+  bool resolved = true;
+  etc_status resolve_status = ETC_OK;
+  int64_t bound_slices = 0, bound_chunks = 0, bound_staging = 0, bound_fills = 0, need_bytes = 0;
+  std::mutex resolve_mu;
   void* d_ws = nullptr;                            // blob 1: the tables below up to d_ptrs
   void* d_tb = nullptr;                            // blob 2: slices, first-chunk indices, chunks
   int32_t* d_map = nullptr;

@@ -66,7 +66,7 @@ extern "C" etc_status etc_plan_set_rounds(etc_plan* pl, int64_t max_staging_byte
   if (max_staging_bytes < 2 * (int64_t)ETC_CHUNK_BYTES) return ETC_ERR_INVALID_ARG;
   const int64_t window = (max_staging_bytes - ETC_CHUNK_BYTES) & ~(int64_t)511;
   cudaStream_t st = (cudaStream_t)stream;
-  const PlanTotals& t = pl->totals;
+  const PlanTotals& t = plan_totals(pl);
 
   std::vector<RoundSpec> specs;
   std::vector<RoundRec> recs;
