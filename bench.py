@@ -718,10 +718,12 @@ def e2e(E, torch, args, w, dev, world, barrier):
     flags = E.ETC_ALL_STAGED if args.all_staged else E.ETC_LOCAL_DIRECT
 
     def leg(**kw):
+        if not kw.get("zero_copy"):                  # the DMA legs need a device copy of every shard: allocate it once
+            kw = dict(kw, d_src=E.alloc_buffers(lo, dev), d_dst=E.alloc_buffers(ln, dev))
         mk = lambda: HostMigration(model, wi["old"], wi["new"], h_src, h_dst, dev, args.e2e_staging, flags, **kw)
         warm = mk(); warm.run(); barrier()
-        hm = mk()
         del warm
+        hm = mk()
         barrier()
         for _ in range(n):
             plan = hm.run()
@@ -800,8 +802,8 @@ def main():
     ap.add_argument("--config-steps", type=int, default=8, help="timed steps of each per_config workload")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--e2e-config", default="", help="force the e2e workload (default: the headline one if it can be pinned)")
-    ap.add_argument("--e2e-max-bytes", type=int, default=48 << 30,
-                    help="largest old+new state the e2e leg will pin in host memory (pinning costs ~0.3 s/GB)")
+    ap.add_argument("--e2e-max-bytes", type=int, default=120 << 30,
+                    help="largest old+new state the e2e leg will pin in host memory (c4: 100 GB, ~40 s to pin)")
     ap.add_argument("--e2e-staging", type=int, default=1 << 30, help="staging bound (bytes) of the e2e / chunked legs")
     ap.add_argument("--chunked-config", default="c2", help="workload of the chunked eager-release context leg")
     ap.add_argument("--ref-elems", type=int, default=48_000_000, help="--impl reference: oracle sample (elements) per step")

@@ -56,6 +56,21 @@ WORKLOADS = {
     "c5b": dict(name="c5b", data=False, seed=0xE7C00006,
                 model=_model(STYLE_LLAMA, 80, 8192, 64, 8, 128, 28672, 128256, 0, 0, 2, _ALL4),
                 old=_cfg(8, 16, 4), new=_cfg(8, 16, 3)),
+    # ---- not BASELINE.json configs: short-row and misaligned stress workloads for the copy kernels.
+    # A TP change splits the row-parallel weights (proj, fc2) into column blocks; at high TP degrees the rows of such a
+    # slice get short.  c2's model from TP2 PP2 DP2 to TP16: proj slices have rows of 128 B (bf16) / 256 B (fp32).
+    "x128": dict(name="x128", data=True, seed=0xE7C00012,
+                 model=_model(STYLE_GPT, 24, 1024, 16, 16, 64, 4096, 50304, 2048, 1, 2, _ALL4),
+                 old=_cfg(2, 2, 2), new=_cfg(16, 1, 1)),
+    # head_dim 32, hidden 512, to TP16: proj rows of 64 B (bf16) / 128 B (fp32), fc2 rows of 256 / 512 B
+    "x64": dict(name="x64", data=True, seed=0xE7C00013,
+                model=_model(STYLE_GPT, 48, 512, 16, 16, 32, 2048, 50304, 2048, 1, 2, _ALL4),
+                old=_cfg(2, 2, 2), new=_cfg(16, 1, 1)),
+    # odd hidden size: every bf16 row is only 2-byte aligned, every fp32 row 4-byte aligned (the re-aligning copy path),
+    # c2's reconfiguration
+    "xodd": dict(name="xodd", data=True, seed=0xE7C00014,
+                 model=_model(STYLE_GPT, 24, 1025, 16, 16, 64, 4096, 50304, 2048, 1, 2, _ALL4),
+                 old=_cfg(2, 2, 2), new=_cfg(4, 2, 1)),
 }
 
 # Scaled-down twins: same parallel reconfiguration, same style/kinds/tied-ness, dims shrunk so the
@@ -77,11 +92,18 @@ _SCALED = {
                          vocab=3000, max_pos=96)),
     "s5b": ("c5b", dict(n_layers=16, hidden=64, n_q_heads=16, n_kv_heads=8, head_dim=4, ffn_hidden=128,
                         vocab=256, max_pos=0)),
+    # twins of the stress workloads: 16-byte aligned rows of 32 ... 256 B (short-row path), and an odd hidden size
+    # (2-byte aligned bf16 rows: the byte-phase re-aligning path)
+    "sx64": ("x64", dict(n_layers=4, hidden=256, n_q_heads=16, n_kv_heads=16, head_dim=16, ffn_hidden=1024,
+                         vocab=3008, max_pos=64)),
+    "sxodd": ("xodd", dict(n_layers=4, hidden=193, n_q_heads=12, n_kv_heads=12, head_dim=16, ffn_hidden=768,
+                           vocab=3000, max_pos=96)),
 }
 
 
 def workload(name: str) -> dict:
-    """Return a deep copy of the named workload ("c1".."c5", "c5b", "s2".."s5", "s2odd", "s4odd", "s5b")."""
+    """Return a deep copy of the named workload ("c1".."c5", "c5b", "s2".."s5", "s2odd", "s4odd", "s5b", and the copy-kernel
+    stress workloads "x128", "x64", "xodd" with their scaled twins "sx64", "sxodd")."""
     if name in WORKLOADS:
         return copy.deepcopy(WORKLOADS[name])
     base, over = _SCALED[name]

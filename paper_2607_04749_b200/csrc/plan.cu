@@ -5,10 +5,12 @@
 //                                                        (source, destination) pair — message coalescing
 // Source of every needed element (reading A6): local first, else the designated holder.
 //
-// One warp owns one (source device od, new rank n) unit, i.e. one cell of the traffic matrix and one pair segment.
-// Pass 1 counts slices / chunks / bytes per unit; a single-CTA scan turns the counts into slice indices, chunk indices
-// and segment offsets (warp-shuffle prefix sums); pass 2 recomputes the slices and writes them at their final
-// positions.  Order inside a segment is canonical (piece order), so the staging layout is deterministic.
+// A (source device od, new rank n) unit is one cell of the traffic matrix and one pair segment; it is cut into sub-blocks
+// of pieces, one warp each.  Three launches: pass 1 counts slices / chunks / bytes per sub-block (no atomics); a
+// single-CTA scan sums the sub-blocks of each unit and turns the unit counts into slice indices, chunk indices and segment
+// offsets (warp-shuffle prefix sums); pass 2 recomputes the slices, writes them at their final positions and expands them
+// into copy work items ("chunks") warp-cooperatively.  Order inside a segment is canonical (piece order), so the staging
+// layout is deterministic.
 #include <algorithm>
 #include <cstring>
 #include <vector>
@@ -160,11 +162,10 @@ __device__ __forceinline__ void sub_range(const DeviceTables& newT, int n, int k
   i0 = min(qe, qb + b * span); i1 = min(qe, i0 + span);
 }
 
-// pass 1: per-(unit, sub-block) counts; unit totals accumulated with integer atomics (order-independent sums).
+// pass 1: per-(unit, sub-block) counts.
 __global__ void __launch_bounds__(PLAN_WARPS * 32)
 plan_count_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict__ device_map,
-                  const uint8_t* __restrict__ failed, int K, int B,
-                  UnitCount* __restrict__ units, BlockCount* __restrict__ blocks) {
+                  const uint8_t* __restrict__ failed, int K, int B, BlockCount* __restrict__ blocks) {
   const int lane = threadIdx.x & 31;
   const long long w = (long long)blockIdx.x * PLAN_WARPS + (threadIdx.x >> 5);
   const long long U = (long long)K * oldT.n_dev * newT.n_dev;
@@ -188,23 +189,16 @@ plan_count_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restric
     }
   }
   n_sl = warp_sum64(n_sl); n_ch = warp_sum64(n_ch); bytes = warp_sum64(bytes); padded = warp_sum64(padded);
-  if (lane == 0) {
-    blocks[w] = BlockCount{n_sl, n_ch, padded};
-    if (n_sl) {
-      atomicAdd(reinterpret_cast<unsigned long long*>(&units[u].slices), (unsigned long long)n_sl);
-      atomicAdd(reinterpret_cast<unsigned long long*>(&units[u].chunks), (unsigned long long)n_ch);
-      atomicAdd(reinterpret_cast<unsigned long long*>(&units[u].bytes), (unsigned long long)bytes);
-      atomicAdd(reinterpret_cast<unsigned long long*>(&units[u].padded), (unsigned long long)padded);
-    }
-  }
+  if (lane == 0) blocks[w] = BlockCount{n_sl, n_ch, padded, bytes};
 }
 
 // single-CTA exclusive scan over units (+ map validation, traffic matrix, totals)
 constexpr int SCAN_THREADS = 1024;
 __global__ void __launch_bounds__(SCAN_THREADS)
-plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int K, int n_old, int n_new, int P, int flags,
-                 const int32_t* __restrict__ device_map, UnitBase* __restrict__ bases, int64_t* __restrict__ traffic,
-                 PlanTotals* __restrict__ totals, int64_t bound_slices, int64_t bound_chunks, int64_t bound_staging) {
+plan_scan_kernel(const BlockCount* __restrict__ blocks, int B, long long U, int K, int n_old, int n_new, int P, int flags,
+                 const int32_t* __restrict__ device_map, int32_t* __restrict__ map_copy, UnitBase* __restrict__ bases,
+                 int64_t* __restrict__ traffic, PlanTotals* __restrict__ totals, PlanTotals* __restrict__ totals_host,
+                 int64_t bound_slices, int64_t bound_chunks, int64_t bound_staging) {
   __shared__ int64_t s_w[5][32];
   __shared__ int64_t s_carry[5];
   __shared__ int64_t s_loc[32], s_rem[32];
@@ -218,8 +212,9 @@ plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int K, int n_
   if (tid == 0) s_bad = 0;
   for (int i = tid; i < 1024; i += SCAN_THREADS) s_seen[i] = 0;
   __syncthreads();
-  for (int n = tid; n < n_new; n += SCAN_THREADS) {            // injective into [0,P)?
+  for (int n = tid; n < n_new; n += SCAN_THREADS) {            // injective into [0,P)?  (and the plan keeps its own copy)
     const int p = device_map[n];
+    if (map_copy != device_map) map_copy[n] = p;
     if (p < 0 || p >= P) s_bad = 1;
     else if (atomicOr(&s_seen[p >> 5], 1u << (p & 31)) & (1u << (p & 31))) s_bad = 1;
   }
@@ -229,10 +224,13 @@ plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int K, int n_
   int64_t loc = 0, rem = 0;
   for (long long base = 0; base < U; base += SCAN_THREADS) {
     const long long u = base + tid;
-    UnitCount c{0, 0, 0, 0};
+    BlockCount c{0, 0, 0, 0};
     bool staged = false; int od = 0, p = 0;
     if (u < U) {
-      c = units[u];
+      for (int k = 0; k < B; ++k) {                             // the unit's sub-blocks
+        const BlockCount x = blocks[u * B + k];
+        c.slices += x.slices; c.chunks += x.chunks; c.padded += x.padded; c.bytes += x.bytes;
+      }
       od = (int)((u / n_new) % n_old); p = device_map[(int)(u % n_new)];
       staged = !(flags & ETC_ALL_DIRECT) && ((od != p) || (flags & ETC_ALL_STAGED));
       c.padded = (c.padded + 511) & ~(int64_t)511;             // pair segments start 512-byte aligned
@@ -296,18 +294,45 @@ plan_scan_kernel(const UnitCount* __restrict__ units, long long U, int K, int n_
       t.kind_base[ETC_NUM_KINDS][0] = s_carry[1]; t.kind_base[ETC_NUM_KINDS][1] = s_carry[2];
       t.kind_base[ETC_NUM_KINDS][2] = s_carry[4];
       *totals = t;
+      if (totals_host) *totals_host = t;                        // pinned host slot: the sizes the host is waiting for
     }
   }
 }
 
-// pass 2: recompute the slices of each (unit, sub-block) and write slice records (+ first chunk index) at their final
-// positions: unit base (scan) + earlier sub-blocks of the unit + warp-level prefix inside the sub-block.
+// One copy work item of a slice: chunk k of slice s (see slice_chunks for the count).
+__device__ __forceinline__ Chunk cut_chunk(const etc_slice& s, int vec, long long k) {
+  Chunk ch;
+  ch.src_buf = (uint16_t)(s.src_dev * ETC_NUM_KINDS + s.kind); ch.dst_buf = (uint16_t)(s.dst_rank * ETC_NUM_KINDS + s.kind);
+  ch.src_stride = s.src_stride; ch.dst_stride = s.dst_stride; ch.pad = 0;
+  ch.vec = (int16_t)vec;
+  const int64_t stg = s.stg_off >= 0 ? s.stg_off : 0;
+  if (s.nrows == 1 || s.row_bytes >= ETC_CHUNK_BYTES) {
+    const long long cpr = (s.row_bytes + ETC_CHUNK_BYTES - 1) / ETC_CHUNK_BYTES;
+    const long long row = k / cpr; const int64_t b = (k % cpr) * ETC_CHUNK_BYTES;
+    ch.src_off = s.src_off + row * s.src_stride + b;
+    ch.dst_off = s.dst_off + row * s.dst_stride + b;
+    ch.stg_off = stg + row * s.row_bytes + b;
+    ch.nrows = 1; ch.row_bytes = (int32_t)min((int64_t)ETC_CHUNK_BYTES, s.row_bytes - b);
+  } else {
+    const int rpc = rows_per_chunk(s.row_bytes, vec == 16);
+    const long long row = k * rpc;
+    ch.src_off = s.src_off + row * s.src_stride;
+    ch.dst_off = s.dst_off + row * s.dst_stride;
+    ch.stg_off = stg + row * s.row_bytes;
+    ch.nrows = (int32_t)min((long long)rpc, s.nrows - row); ch.row_bytes = (int32_t)s.row_bytes;
+  }
+  return ch;
+}
+
+// pass 2: recompute the slices of each (unit, sub-block), write the slice records at their final positions — unit base
+// (scan) + earlier sub-blocks of the unit + warp-level prefix inside the sub-block — and expand them into chunks: the
+// warp walks over the slices its lanes have just written and the 32 lanes cut chunk k, k + 32, ... of each.
 __global__ void __launch_bounds__(PLAN_WARPS * 32)
 plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict__ device_map,
                  const uint8_t* __restrict__ failed, int flags, int K, int B,
                  const BlockCount* __restrict__ blocks, const UnitBase* __restrict__ bases,
                  etc_slice* __restrict__ sl_staged, etc_slice* __restrict__ sl_local,
-                 int64_t* __restrict__ c0_staged, int64_t* __restrict__ c0_local, const PlanTotals* __restrict__ lazy) {
+                 Chunk* __restrict__ ch_staged, Chunk* __restrict__ ch_local, const PlanTotals* __restrict__ lazy) {
   if (lazy && (lazy->bad_map || lazy->overflow)) return;
   const int lane = threadIdx.x & 31;
   const long long w = (long long)blockIdx.x * PLAN_WARPS + (threadIdx.x >> 5);
@@ -320,7 +345,7 @@ plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict
   const int p = device_map[n];
   const bool local_unit = (od == p), staged = !(flags & ETC_ALL_DIRECT) && (!local_unit || (flags & ETC_ALL_STAGED));
   etc_slice* sl_out = staged ? sl_staged : sl_local;
-  int64_t* c0_out = staged ? c0_staged : c0_local;
+  Chunk* ch_out = staged ? ch_staged : ch_local;
   int64_t pre_sl = 0, pre_ch = 0, pre_pad = 0;                 // totals of the unit's earlier sub-blocks
   for (int k = lane; k < b; k += 32) { const BlockCount c = blocks[u * B + k]; pre_sl += c.slices; pre_ch += c.chunks; pre_pad += c.padded; }
   int64_t run_sl = ub.slice0 + warp_sum64(pre_sl), run_ch = ub.chunk0 + warp_sum64(pre_ch);
@@ -340,17 +365,30 @@ plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict
     int64_t o_sl = run_sl + warp_excl_scan64(my_sl, lane, tot_sl);       // warp-level prefix sums for slice offsets
     int64_t o_ch = run_ch + warp_excl_scan64(my_ch, lane, tot_ch);
     int64_t o_stg = run_stg + warp_excl_scan64(my_pad, lane, tot_pad);
-    run_sl += tot_sl; run_ch += tot_ch; run_stg += tot_pad;
     if (i < i1 && my_sl) {
       for_each_slice(oldT, q, od, p, local_unit, es, kind, failed, [&](const SliceGeom& s) {
         etc_slice r;
         r.src_off = s.src_off; r.dst_off = s.dst_off; r.stg_off = staged ? o_stg : -1; r.row_bytes = s.row_bytes;
         r.src_stride = s.src_stride; r.dst_stride = s.dst_stride; r.nrows = s.nrows;
         r.src_dev = od; r.dst_rank = n; r.dst_phys = p; r.kind = kind; r.pad = 0;
-        sl_out[o_sl] = r; c0_out[o_sl] = o_ch;
-        o_sl += 1; o_ch += slice_chunks(s); o_stg += slice_padded(s);
+        sl_out[o_sl] = r;
+        o_sl += 1; o_stg += slice_padded(s);
       });
     }
+    // chunk expansion of the slices [run_sl, run_sl + tot_sl) this iteration wrote, whose chunks are
+    // [run_ch, run_ch + tot_ch) in the same order
+    __syncwarp();
+    int64_t c0 = run_ch;
+    for (int64_t j = 0; j < tot_sl; ++j) {
+      const etc_slice s = sl_out[run_sl + j];                   // written by a lane of this warp just above
+      const int vec = slice_vec(s.src_off, s.dst_off, s.row_bytes, s.src_stride, s.dst_stride, s.nrows);
+      SliceGeom g; g.src_off = s.src_off; g.dst_off = s.dst_off; g.row_bytes = s.row_bytes; g.src_stride = s.src_stride;
+      g.dst_stride = s.dst_stride; g.nrows = s.nrows; g.kind = s.kind;
+      const int64_t nch = slice_chunks(g);
+      for (int64_t k = lane; k < nch; k += 32) ch_out[c0 + k] = cut_chunk(s, vec, k);
+      c0 += nch;
+    }
+    run_sl += tot_sl; run_ch += tot_ch; run_stg += tot_pad;
   }
 }
 
@@ -377,43 +415,6 @@ plan_fills_kernel(DeviceTables newT, const int32_t* __restrict__ device_map, int
   const unsigned long long slot = atomicAdd(reinterpret_cast<unsigned long long*>(&totals->n_fills), 1ull);
   fills[slot] = f;
   atomicAdd(reinterpret_cast<unsigned long long*>(&totals->fill_bytes), (unsigned long long)((int64_t)(r1 - r0) * q.nc * es));
-}
-
-// pass 3: one thread per chunk: find its slice by binary search over the slices' first-chunk indices, cut the chunk out
-__global__ void __launch_bounds__(256)
-plan_chunks_kernel(const etc_slice* __restrict__ slices, const int64_t* __restrict__ chunk0, long long n_slices,
-                   long long n_chunks, Chunk* __restrict__ out, const PlanTotals* __restrict__ lazy, int which) {
-  if (lazy) {                                                   // ETC_NO_SYNC: the counts never went to the host
-    n_slices = which == 0 ? lazy->n_slices_staged : lazy->n_slices_local;
-    n_chunks = which == 0 ? lazy->n_chunks_staged : lazy->n_chunks_local;
-  }
-  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= n_chunks) return;
-  long long lo = 0, hi = n_slices - 1;                          // last slice with chunk0 <= c
-  while (lo < hi) { const long long mid = (lo + hi + 1) >> 1; if (chunk0[mid] <= c) lo = mid; else hi = mid - 1; }
-  const etc_slice s = slices[lo];
-  const long long k = c - chunk0[lo];
-  Chunk ch;
-  ch.src_buf = (uint16_t)(s.src_dev * ETC_NUM_KINDS + s.kind); ch.dst_buf = (uint16_t)(s.dst_rank * ETC_NUM_KINDS + s.kind);
-  ch.src_stride = s.src_stride; ch.dst_stride = s.dst_stride; ch.pad = 0;
-  const int64_t stg = s.stg_off >= 0 ? s.stg_off : 0;
-  ch.vec = (int16_t)slice_vec(s.src_off, s.dst_off, s.row_bytes, s.src_stride, s.dst_stride, s.nrows);
-  if (s.nrows == 1 || s.row_bytes >= ETC_CHUNK_BYTES) {
-    const long long cpr = (s.row_bytes + ETC_CHUNK_BYTES - 1) / ETC_CHUNK_BYTES;
-    const long long row = k / cpr; const int64_t b = (k % cpr) * ETC_CHUNK_BYTES;
-    ch.src_off = s.src_off + row * s.src_stride + b;
-    ch.dst_off = s.dst_off + row * s.dst_stride + b;
-    ch.stg_off = stg + row * s.row_bytes + b;
-    ch.nrows = 1; ch.row_bytes = (int32_t)min((int64_t)ETC_CHUNK_BYTES, s.row_bytes - b);
-  } else {
-    const int rpc = rows_per_chunk(s.row_bytes, ch.vec == 16);
-    const long long row = k * rpc;
-    ch.src_off = s.src_off + row * s.src_stride;
-    ch.dst_off = s.dst_off + row * s.dst_stride;
-    ch.stg_off = stg + row * s.row_bytes;
-    ch.nrows = (int32_t)min((long long)rpc, s.nrows - row); ch.row_bytes = (int32_t)s.row_bytes;
-  }
-  out[c] = ch;
 }
 
 // Bounds check of the finished plan (a safety net of our own: compute-sanitizer is not available everywhere): every
@@ -548,7 +549,7 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
   pl->bound_fills = grows ? new_l->n_emb_pieces : 0;
   // ETC_NO_SYNC is honoured while the bound-sized tables stay small; a big plan is made the exact way (one host sync
   // costs nothing next to its copy kernels, and exact grids keep its copy launches free of idle CTAs)
-  const size_t bound_tb = (size_t)pl->bound_slices * 2 * (sizeof(etc_slice) + 8) + (size_t)pl->bound_chunks * 2 * sizeof(Chunk);
+  const size_t bound_tb = (size_t)pl->bound_slices * 2 * sizeof(etc_slice) + (size_t)pl->bound_chunks * 2 * sizeof(Chunk);
   const bool lazy = (flags & ETC_NO_SYNC) && bound_tb <= ((size_t)64 << 20);
   pl->lazy = lazy; pl->resolved = !lazy;
   auto fail = [&](etc_status s) { etc_plan_destroy(pl); return s; };
@@ -564,10 +565,9 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
       seen[p] = 1;
     }
   }
-  // workspace blob 1: units | bases | blocks | traffic | totals | map | pointer tables | failure mask | zero-fill list
+  // workspace blob 1: bases | blocks | traffic | totals | map | pointer tables | failure mask | zero-fill list
   auto al = [](size_t x) { return (x + 255) & ~size_t(255); };
-  const size_t o_units = 0, o_bases = o_units + al(sizeof(UnitCount) * (size_t)U),
-               o_blocks = o_bases + al(sizeof(UnitBase) * (size_t)U),
+  const size_t o_bases = 0, o_blocks = o_bases + al(sizeof(UnitBase) * (size_t)U),
                o_traffic = o_blocks + al(sizeof(BlockCount) * (size_t)U * B),
                o_totals = o_traffic + al(sizeof(int64_t) * (size_t)P * P), o_map = o_totals + al(sizeof(PlanTotals)),
                o_ptrs = o_map + al(sizeof(int32_t) * (size_t)n_new),
@@ -576,14 +576,14 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
                ws_bytes = o_fills + (grows ? al(sizeof(etc_slice) * (size_t)new_l->n_emb_pieces) : 0);
   PLAN_TRY(cudaMallocAsync(&pl->d_ws, ws_bytes, st));
   char* ws = static_cast<char*>(pl->d_ws);
-  pl->d_units = reinterpret_cast<UnitCount*>(ws + o_units); pl->d_bases = reinterpret_cast<UnitBase*>(ws + o_bases);
+  pl->d_bases = reinterpret_cast<UnitBase*>(ws + o_bases);
   pl->d_blocks = reinterpret_cast<BlockCount*>(ws + o_blocks); pl->d_traffic = reinterpret_cast<int64_t*>(ws + o_traffic);
   pl->d_totals = reinterpret_cast<PlanTotals*>(ws + o_totals); pl->d_map = reinterpret_cast<int32_t*>(ws + o_map);
   pl->d_ptrs = reinterpret_cast<void**>(ws + o_ptrs);
-  // metadata moves as kernels on `st`, never through the copy engines (xfer.cu)
-  if (on_device) PLAN_TRY(copy_by_kernel(pl->d_map, device_map, sizeof(int32_t) * (size_t)n_new, st));
-  else PLAN_TRY(write_small(pl->d_map, device_map, sizeof(int32_t) * (size_t)n_new, st));
-  PLAN_TRY(cudaMemsetAsync(pl->d_units, 0, sizeof(UnitCount) * (size_t)U, st));
+  // metadata moves as kernels on `st`, never through the copy engines (xfer.cu).  A device map is read in place by the
+  // count and scan kernels; the scan kernel keeps a copy in the plan, which everything later uses.
+  const int32_t* map_in = device_map;
+  if (!on_device) { PLAN_TRY(write_small(pl->d_map, device_map, sizeof(int32_t) * (size_t)n_new, st)); map_in = pl->d_map; }
   const uint8_t* d_failed = nullptr;
   if (failed) {                                                 // reading A26: host or device mask [n_old]
     if (on_device_ptr(failed)) PLAN_TRY(copy_by_kernel(ws + o_failed, failed, (size_t)n_old, st));
@@ -592,12 +592,16 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
   }
 
   const unsigned grid = (unsigned)((U * B + PLAN_WARPS - 1) / PLAN_WARPS);
-  plan_count_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, d_failed, K, B, pl->d_units,
-                                                      pl->d_blocks);
+  plan_count_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, map_in, d_failed, K, B, pl->d_blocks);
   PLAN_TRY(cudaGetLastError());
-  plan_scan_kernel<<<1, SCAN_THREADS, 0, st>>>(pl->d_units, U, K, n_old, n_new, P, pl->flags, pl->d_map, pl->d_bases,
-                                               pl->d_traffic, pl->d_totals, lazy ? pl->bound_slices : 0,
-                                               pl->bound_chunks, pl->bound_staging);
+  PlanTotals* h_tot = nullptr;                                  // pinned slot for the totals read-back (not for no-sync plans)
+  if (!lazy) {
+    if (!g_pinned_totals) PLAN_TRY(cudaMallocHost(&g_pinned_totals, sizeof(PlanTotals) * N_PINNED_TOTALS));
+    h_tot = &g_pinned_totals[__atomic_fetch_add(&g_pinned_next, 1u, __ATOMIC_RELAXED) % N_PINNED_TOTALS];
+  }
+  plan_scan_kernel<<<1, SCAN_THREADS, 0, st>>>(pl->d_blocks, B, U, K, n_old, n_new, P, pl->flags, map_in, pl->d_map,
+                                               pl->d_bases, pl->d_traffic, pl->d_totals, grows ? nullptr : h_tot,
+                                               lazy ? pl->bound_slices : 0, pl->bound_chunks, pl->bound_staging);
   PLAN_TRY(cudaGetLastError());
   count_launch(2);
   if (grows) {
@@ -609,9 +613,8 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
   }
   int64_t n_sl_s, n_sl_l, n_ch_s, n_ch_l;                       // table capacities
   if (!lazy) {
-    if (!g_pinned_totals) PLAN_TRY(cudaMallocHost(&g_pinned_totals, sizeof(PlanTotals) * N_PINNED_TOTALS));
-    PlanTotals* h_tot = &g_pinned_totals[__atomic_fetch_add(&g_pinned_next, 1u, __ATOMIC_RELAXED) % N_PINNED_TOTALS];
-    PLAN_TRY(copy_by_kernel(h_tot, pl->d_totals, sizeof(PlanTotals), st));    // h_tot is pinned: the kernel writes it
+    // the scan kernel wrote the totals straight into the pinned slot, unless the zero-fill kernel still had to add to them
+    if (grows) PLAN_TRY(copy_by_kernel(h_tot, pl->d_totals, sizeof(PlanTotals), st));
     PLAN_TRY(cudaStreamSynchronize(st));                        // the one host sync: sizes must come back
     pl->totals = *h_tot;
     if (pl->totals.bad_map) return fail(ETC_ERR_BAD_MAP);
@@ -623,36 +626,20 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
     n_sl_s = n_sl_l = pl->bound_slices; n_ch_s = n_ch_l = pl->bound_chunks;
   }
 
-  // blob 2: slice records | first-chunk indices | chunk descriptors
+  // blob 2: slice records | chunk descriptors
   const size_t o_sls = 0, o_sll = o_sls + al(sizeof(etc_slice) * (size_t)n_sl_s),
-               o_c0s = o_sll + al(sizeof(etc_slice) * (size_t)n_sl_l),
-               o_c0l = o_c0s + al(8 * (size_t)n_sl_s), o_chs = o_c0l + al(8 * (size_t)n_sl_l),
-               o_chl = o_chs + al(sizeof(Chunk) * (size_t)n_ch_s),
+               o_chs = o_sll + al(sizeof(etc_slice) * (size_t)n_sl_l), o_chl = o_chs + al(sizeof(Chunk) * (size_t)n_ch_s),
                tb_bytes = o_chl + al(sizeof(Chunk) * (size_t)n_ch_l);
   if (tb_bytes) {
     PLAN_TRY(cudaMallocAsync(&pl->d_tb, tb_bytes, st));
     char* tb = static_cast<char*>(pl->d_tb);
     pl->d_sl_staged = reinterpret_cast<etc_slice*>(tb + o_sls); pl->d_sl_local = reinterpret_cast<etc_slice*>(tb + o_sll);
-    pl->d_c0_staged = reinterpret_cast<int64_t*>(tb + o_c0s); pl->d_c0_local = reinterpret_cast<int64_t*>(tb + o_c0l);
     pl->d_ch_staged = reinterpret_cast<Chunk*>(tb + o_chs); pl->d_ch_local = reinterpret_cast<Chunk*>(tb + o_chl);
   }
-  const PlanTotals* d_lazy = lazy ? pl->d_totals : nullptr;
   if (n_sl_s + n_sl_l) {
-    plan_fill_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, d_failed, pl->flags, K, B, pl->d_blocks, pl->d_bases,
-                                                       pl->d_sl_staged, pl->d_sl_local, pl->d_c0_staged, pl->d_c0_local, d_lazy);
-    PLAN_TRY(cudaGetLastError());
-    count_launch();
-  }
-  // an ETC_NO_SYNC plan that cannot stage anything (ETC_ALL_DIRECT) has no staged list to expand
-  if (n_ch_s && !(lazy && (pl->flags & ETC_ALL_DIRECT))) {
-    plan_chunks_kernel<<<(unsigned)((n_ch_s + 255) / 256), 256, 0, st>>>(
-        pl->d_sl_staged, pl->d_c0_staged, n_sl_s, n_ch_s, pl->d_ch_staged, d_lazy, 0);
-    PLAN_TRY(cudaGetLastError());
-    count_launch();
-  }
-  if (n_ch_l) {
-    plan_chunks_kernel<<<(unsigned)((n_ch_l + 255) / 256), 256, 0, st>>>(
-        pl->d_sl_local, pl->d_c0_local, n_sl_l, n_ch_l, pl->d_ch_local, d_lazy, 1);
+    plan_fill_kernel<<<grid, PLAN_WARPS * 32, 0, st>>>(old_l->t, new_l->t, pl->d_map, d_failed, pl->flags, K, B, pl->d_blocks,
+                                                       pl->d_bases, pl->d_sl_staged, pl->d_sl_local, pl->d_ch_staged,
+                                                       pl->d_ch_local, lazy ? pl->d_totals : nullptr);
     PLAN_TRY(cudaGetLastError());
     count_launch();
   }

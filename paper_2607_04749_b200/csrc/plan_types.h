@@ -5,8 +5,7 @@
 
 namespace etc {
 
-struct UnitCount { int64_t slices, chunks, bytes, padded; };   // per (source device, new rank) unit
-struct BlockCount { int64_t slices, chunks, padded; };          // per (unit, sub-block of pieces)
+struct BlockCount { int64_t slices, chunks, padded, bytes; };   // per (unit, sub-block of pieces); unit = (source device, new rank)
 struct UnitBase { int64_t slice0, chunk0, stg0; };
 struct PlanTotals {
   int64_t n_slices_staged, n_chunks_staged, staging_bytes, n_slices_local, n_chunks_local;
@@ -82,14 +81,12 @@ struct etc_plan {
   void* d_ws = nullptr;                            // blob 1: the tables below up to d_ptrs
   void* d_tb = nullptr;                            // blob 2: slices, first-chunk indices, chunks
   int32_t* d_map = nullptr;
-  etc::UnitCount* d_units = nullptr;
   etc::UnitBase* d_bases = nullptr;
   etc::BlockCount* d_blocks = nullptr;
   int64_t* d_traffic = nullptr;
   etc::PlanTotals* d_totals = nullptr;
   etc_slice* d_sl_staged = nullptr; etc_slice* d_sl_local = nullptr;
   etc::Chunk* d_ch_staged = nullptr; etc::Chunk* d_ch_local = nullptr;
-  int64_t* d_c0_staged = nullptr; int64_t* d_c0_local = nullptr;
   etc_slice* d_fills = nullptr;                    // zero-fill descriptors (in d_ws; totals.n_fills of them), reading A31
   std::vector<int64_t> old_bytes, new_bytes;       // buffer sizes [dev*4+kind], for argument checks in migrate
   void** d_ptrs = nullptr;                         // [n_old*4] source pointers then [n_new*4] destination pointers

@@ -219,7 +219,7 @@ def test_migrate_config1(E, flags):
     _check_migration(E, w["model"], w["old"], w["new"], w["seed"], flags=flags, payload="stamp")
 
 
-@pytest.mark.parametrize("name", ["s2", "s2odd", "s3", "s4", "s4odd", "s5"])
+@pytest.mark.parametrize("name", ["s2", "s2odd", "s3", "s4", "s4odd", "s5", "sx64", "sxodd"])
 @pytest.mark.parametrize("flags", [0, 1, 2, 3, 4, 6])        # 2, 3: + ETC_KIND_MAJOR; 4, 6: ETC_ALL_DIRECT (nothing staged)
 def test_migrate_scaled_configs(E, name, flags):
     w = workload(name)
