@@ -262,7 +262,11 @@ def migrate(old: Layout, new: Layout, device_map, src_bufs: dict | None, want_ov
     """Element-wise migration.  src_bufs: {(old_dev, kind): 1-D uint16/uint32 array} or None (traffic only).
     Returns (dst_bufs {(n, kind): array} or None, T[P][P], overrides).  fill_out: optional int64 array [n_new] that
     receives the bytes of each new rank that have no source and are zero-filled (reading A31).  The destination buffers
-    start out poisoned, so a zero in them was written."""
+    start out poisoned, so a zero in them was written.
+
+    Orchestration only: small problems are one call of orc_migrate_fill (OpenMP over new ranks); larger ones hand
+    element ranges of the new buffers to host threads, each range through orc_migrate_range_fill with its own traffic
+    matrix, summed afterwards — the per-element code is the same."""
     P = P_of(old, new)
     dm = np.ascontiguousarray(device_map, np.int32)
     T = np.zeros((P, P), np.int64); ovr = C.c_int64(0)
@@ -277,11 +281,51 @@ def migrate(old: Layout, new: Layout, device_map, src_bufs: dict | None, want_ov
         dt = _ptr_table(dst, new.n_dev)
     if fill_out is not None:
         assert fill_out.dtype == np.int64 and fill_out.shape == (new.n_dev,) and fill_out.flags.c_contiguous
-    rc = lib().orc_migrate_fill(old.h, new.h, _ptr(dm), st, dt, _ptr(T), C.byref(ovr) if want_overrides else None,
-                                _ptr(fill_out))
-    if rc:
-        raise OracleError(rc)
+    total = sum(new.buffer_elems(n, k) for n in range(new.n_dev) for k in new.kinds())
+    if total < _PARALLEL_MIN_ELEMS:
+        rc = lib().orc_migrate_fill(old.h, new.h, _ptr(dm), st, dt, _ptr(T), C.byref(ovr) if want_overrides else None,
+                                    _ptr(fill_out))
+        if rc:
+            raise OracleError(rc)
+        return dst, T, int(ovr.value)
+    # ---- large problem: element ranges over a thread pool (the C code runs outside the GIL)
+    from concurrent.futures import ThreadPoolExecutor
+    if orc_check_map(dm, new.n_dev, P):
+        raise OracleError(-1)
+    L = lib()
+    L.orc_migrate_range_fill.restype = C.c_int32
+    L.orc_migrate_range_fill.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_int64,
+                                         C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    tasks = [(n, k, l0, min(new.buffer_elems(n, k), l0 + _PARALLEL_CHUNK))
+             for n in range(new.n_dev) for k in new.kinds() for l0 in range(0, new.buffer_elems(n, k), _PARALLEL_CHUNK)]
+
+    def one(t):
+        n, k, l0, l1 = t
+        Tt = np.zeros((P, P), np.int64); o = C.c_int64(0); f = C.c_int64(0)
+        rc = L.orc_migrate_range_fill(old.h, new.h, _ptr(dm), n, k, l0, l1, st, _ptr(dst[(n, k)]) if dst is not None else None,
+                                      _ptr(Tt), C.byref(o) if want_overrides else None, None, C.byref(f))
+        return rc, Tt, int(o.value), n, int(f.value)
+
+    if fill_out is not None:
+        fill_out[:] = 0
+    with ThreadPoolExecutor(os.cpu_count() or 1) as ex:
+        for rc, Tt, o, n, f in ex.map(one, tasks):
+            if rc:
+                raise OracleError(rc)
+            T += Tt
+            ovr.value += o
+            if fill_out is not None:
+                fill_out[n] += f
     return dst, T, int(ovr.value)
+
+
+_PARALLEL_MIN_ELEMS = 4_000_000
+_PARALLEL_CHUNK = 1 << 19
+
+
+def orc_check_map(dm, n_new, P) -> bool:
+    """True if dm is not an injective map [0, n_new) -> [0, P) (what orc_migrate_fill rejects up front)."""
+    return bool(((dm < 0) | (dm >= P)).any() or len(set(dm.tolist())) != n_new)
 
 
 def migrate_range(old: Layout, new: Layout, device_map, n, kind, l0, l1, src_bufs: dict | None, dst=None,

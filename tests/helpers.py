@@ -84,6 +84,13 @@ def sharded_payload(layout: O.Layout, seed: int, payload: str = "stamp", padded_
     return _memo(key, make)
 
 
+def oracle_overlap(old: O.Layout, new: O.Layout, method: str = "elementwise"):
+    """O.overlap(old, new, method=...) -> (overlap, need, hold), memoised (no failure masks)."""
+    if getattr(old, "failed", None) is not None:
+        return O.overlap(old, new, method=method)
+    return _memo(("overlap", _lkey(old), _lkey(new), method), lambda: O.overlap(old, new, method=method))
+
+
 def oracle_migrate(old: O.Layout, new: O.Layout, device_map, src_bufs):
     """O.migrate(old, new, device_map, src_bufs) -> (dst, T, overrides); memoised when src_bufs came from
     sharded_payload (its key names the payload)."""

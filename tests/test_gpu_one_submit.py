@@ -14,7 +14,7 @@ pytestmark = pytest.mark.gpu
 
 from etc_inputs import workload
 from oracle import oracle as O
-from helpers import sharded_payload, oracle_migrate, random_variant_case, make_logical, shard_all
+from helpers import sharded_payload, oracle_migrate, oracle_overlap, random_variant_case, make_logical, shard_all
 from gpu_helpers import upload, download
 
 
@@ -132,7 +132,7 @@ def test_migrate_state_is_one_call(E, name, flags):
     plan = call(want_plan=True)
     torch.cuda.synchronize()
     dmap = plan.device_map()
-    o_ov, _, _ = O.overlap(oo, on)
+    o_ov, _, _ = oracle_overlap(oo, on)
     assert plan.stats.local_bytes == (O.sketch_bruteforce(o_ov)[1] if o_ov.shape[1] <= 8 else O.sketch_hungarian(o_ov)[1])
     exp, T, _ = oracle_migrate(oo, on, dmap, src_np)
     _compare(on, dst, exp, name)
@@ -165,7 +165,7 @@ def test_migrate_state_with_availability_mask(E):
     torch.cuda.synchronize()
     dmap = plan.device_map()
     assert set(dmap.tolist()).isdisjoint({12, 13, 14, 15})
-    o_ov, _, _ = O.overlap(oo, on)
+    o_ov, _, _ = oracle_overlap(oo, on)
     assert plan.stats.local_bytes == O.sketch_hungarian(o_ov, avail)[1]
     exp, _, _ = oracle_migrate(oo, on, dmap, src_np)
     _compare(on, dst, exp, "avail")

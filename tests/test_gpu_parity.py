@@ -13,7 +13,7 @@ pytestmark = pytest.mark.gpu
 
 from etc_inputs import workload, tiny_models, tiny_parallel_cfgs, position_stamp
 from oracle import oracle as O
-from helpers import make_logical, shard_all, stamp_all, sharded_payload, oracle_migrate
+from helpers import make_logical, shard_all, stamp_all, sharded_payload, oracle_migrate, oracle_overlap
 
 
 @pytest.fixture(scope="module")
@@ -171,7 +171,7 @@ def _check_migration(E, model, old_cfg, new_cfg, seed, device_map=None, flags=0,
     oo, on = O.Layout(model, old_cfg), O.Layout(model, new_cfg)
     src = sharded_payload(oo, seed, payload)
     g = run_gpu_migration(model, old_cfg, new_cfg, src, device_map=device_map, flags=flags)
-    ov, need, hold = O.overlap(oo, on)
+    ov, need, hold = oracle_overlap(oo, on)
     assert np.array_equal(g["overlap"], ov) and np.array_equal(g["need"], need) and np.array_equal(g["hold"], hold)
     dm = g["device_map"]
     if device_map is None:
