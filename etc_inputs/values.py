@@ -72,11 +72,12 @@ def logical_values(seed: int, kind: int, tensor_id: int, n: int, elem_bytes: int
     raise ValueError(elem_bytes)
 
 
-def index_stamp(kind: int, tensor_id: int, n: int, elem_bytes: int) -> np.ndarray:
-    """P8: a hash of (kind, tensor, flat index) per logical element: any misplaced element differs."""
+def index_stamp(kind: int, tensor_id: int, n: int, elem_bytes: int, salt: int = 0) -> np.ndarray:
+    """P8: a hash of (kind, tensor, flat index) per logical element: any misplaced element differs.  `salt` gives a
+    different (equally cheap) payload of the same kind, for tests that push several payloads through one plan."""
     with np.errstate(over="ignore"):
         h = _splitmix64(np.arange(n, dtype=np.uint64) + (np.uint64(kind) << np.uint64(56))
-                        + (np.uint64(tensor_id) << np.uint64(36)))
+                        + (np.uint64(tensor_id) << np.uint64(36)) + np.uint64(salt & 0xFFFFFFFF) * np.uint64(0x9E3779B97F4A7C15))
     if elem_bytes == 2:
         return (h & np.uint64(0xFFFF)).astype(np.uint16)
     return (h & np.uint64(0xFFFFFFFF)).astype(np.uint32)

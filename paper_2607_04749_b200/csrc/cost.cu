@@ -107,6 +107,8 @@ bool etc_same_model(const etc_layout* a, const etc_layout* b) { return same_mode
 extern "C" etc_status etc_cost_matrix(const etc_layout* old_l, const etc_layout* new_l, int64_t* d_overlap,
                                       int64_t* d_need, int64_t* d_hold, void* stream) {
   clear_error_detail();
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!old_l || !new_l || !d_overlap || !d_need || !d_hold) return ETC_ERR_INVALID_ARG;
   if (!same_model(old_l, new_l)) return ETC_ERR_MISMATCH;
   const int P = old_l->t.n_dev > new_l->t.n_dev ? old_l->t.n_dev : new_l->t.n_dev;
@@ -140,6 +142,8 @@ __global__ void mask_failed_kernel(int64_t* __restrict__ overlap, int64_t* __res
 extern "C" etc_status etc_mask_failed(int64_t* d_overlap, int64_t* d_hold, int32_t n_new, int32_t n_old, int32_t P,
                                       const uint8_t* d_failed, void* stream) {
   etc::clear_error_detail();
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!d_overlap || !d_failed || n_new < 1 || n_old < 1 || P < n_old || P < n_new) return ETC_ERR_INVALID_ARG;
   const long long total = (long long)(n_new + 1) * n_old;
   etc::mask_failed_kernel<<<(unsigned)((total + 255) / 256), 256, 0, (cudaStream_t)stream>>>(d_overlap, d_hold, n_new,
@@ -163,6 +167,8 @@ __global__ void mask_cross_dp_kernel(int64_t* __restrict__ overlap, int n_new, i
 
 extern "C" etc_status etc_mask_cross_dp(const etc_layout* old_l, const etc_layout* new_l, int64_t* d_overlap, void* stream) {
   etc::clear_error_detail();
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!old_l || !new_l || !d_overlap) return ETC_ERR_INVALID_ARG;
   if (!same_model(old_l, new_l)) return ETC_ERR_MISMATCH;
   const int n_old = old_l->t.n_dev, n_new = new_l->t.n_dev, P = n_old > n_new ? n_old : n_new;

@@ -131,6 +131,8 @@ using namespace etc;
 extern "C" etc_status etc_defrag(const int32_t* d_device_map, int32_t pw, int32_t cw, int32_t devices_per_node,
                                  int32_t mode, int32_t* d_out_map, int32_t* d_ops, int32_t* d_n_ops, void* stream) {
   clear_error_detail();
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!d_device_map || !d_out_map || !d_n_ops) return ETC_ERR_INVALID_ARG;
   if (pw < 1 || cw < 1 || devices_per_node < 1) return ETC_ERR_INVALID_ARG;
   if (mode < ETC_DEFRAG_OCCUPANCY || mode > ETC_DEFRAG_BOTH) return ETC_ERR_INVALID_ARG;

@@ -67,6 +67,8 @@ static etc_status source_regions(const etc_plan* pl) {
 extern "C" etc_status etc_upload_sources(const etc_plan* pl, const void* const* h_src_bufs, void* const* d_src_bufs,
                                          int32_t only_kind, int64_t* bytes_out, void* stream) {
   clear_error_detail();
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!pl || !h_src_bufs || !d_src_bufs || only_kind < -1 || only_kind >= ETC_NUM_KINDS) return ETC_ERR_INVALID_ARG;
   etc_status rc = source_regions(pl);
   if (rc != ETC_OK) return rc;

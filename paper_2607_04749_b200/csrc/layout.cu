@@ -391,6 +391,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
 
 extern "C" void etc_layout_destroy(etc_layout* L) {
   if (!L) return;
+  DeviceGuard device_guard;
   // stream-ordered free, ordered after every kernel already enqueued on any stream that read the tables
   if (L->d_blob) cudaFreeAsync(L->d_blob, L->streams.join(g_up_stream));
   if (L->ready) cudaEventDestroy(L->ready);

@@ -181,6 +181,8 @@ static etc_status launch_migrate(const etc_plan* pl, const void* const* src_bufs
 extern "C" etc_status etc_migrate_phase(const etc_plan* pl, const void* const* src_bufs, void* const* dst_bufs,
                                         void* staging, int32_t phases, void* stream) {
   clear_error_detail();
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!pl) return ETC_ERR_INVALID_ARG;
   if (pl->lazy && !pl->resolved) {
     // ETC_NO_SYNC plan whose counts are still on the device: grids from the host-side bounds (staged + local chunks
@@ -212,6 +214,8 @@ extern "C" etc_status etc_migrate(const etc_plan* pl, const void* const* src_buf
 extern "C" etc_status etc_migrate_round(const etc_plan* pl, int32_t round, const void* const* src_bufs,
                                         void* const* dst_bufs, void* staging, int32_t phases, void* stream) {
   clear_error_detail();
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!pl || round < 0 || (size_t)round >= pl->rounds.size()) return ETC_ERR_INVALID_ARG;
   const RoundRec& r = pl->rounds[round];
   const size_t n_ptrs = ((size_t)(pl->n_old + pl->n_new) * ETC_NUM_KINDS * sizeof(void*) + 255) / 256 * 256 / sizeof(void*);

@@ -523,6 +523,8 @@ extern "C" int64_t etc_staging_bound(const etc_layout* old_l, const etc_layout* 
 extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
                                              const uint8_t* failed, int32_t flags, etc_plan** out, void* stream) {
   clear_error_detail();
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!old_l || !new_l || !device_map || !out) return ETC_ERR_INVALID_ARG;
   if (flags < 0 || flags > (ETC_ALL_STAGED | ETC_KIND_MAJOR | ETC_ALL_DIRECT | ETC_NO_SYNC)) return ETC_ERR_INVALID_ARG;
   if ((flags & ETC_ALL_STAGED) && (flags & ETC_ALL_DIRECT)) return ETC_ERR_INVALID_ARG;
@@ -653,6 +655,7 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
 
 extern "C" void etc_plan_destroy(etc_plan* pl) {
   if (!pl) return;
+  etc::DeviceGuard device_guard;
   cudaStream_t st = pl->streams.join(pl->stream_created_on);
   if (pl->d_ws) cudaFreeAsync(pl->d_ws, st);
   if (pl->d_tb) cudaFreeAsync(pl->d_tb, st);
@@ -677,6 +680,8 @@ extern "C" etc_status etc_plan_get_stats(const etc_plan* pl, etc_plan_stats* out
 
 extern "C" etc_status etc_plan_get_traffic(const etc_plan* pl, int64_t* h_traffic) {
   clear_error_detail();
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!pl || !h_traffic) return ETC_ERR_INVALID_ARG;
   ETC_CUDA_TRY(cudaStreamSynchronize(pl->stream_created_on));
   ETC_CUDA_TRY(cudaMemcpy(h_traffic, pl->d_traffic, sizeof(int64_t) * (size_t)pl->P * pl->P, cudaMemcpyDeviceToHost));
@@ -685,6 +690,8 @@ extern "C" etc_status etc_plan_get_traffic(const etc_plan* pl, int64_t* h_traffi
 
 extern "C" etc_status etc_plan_get_map(const etc_plan* pl, int32_t* h_device_map) {
   clear_error_detail();
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!pl || !h_device_map) return ETC_ERR_INVALID_ARG;
   ETC_CUDA_TRY(cudaStreamSynchronize(pl->stream_created_on));
   ETC_CUDA_TRY(cudaMemcpy(h_device_map, pl->d_map, sizeof(int32_t) * (size_t)pl->n_new, cudaMemcpyDeviceToHost));
@@ -693,6 +700,8 @@ extern "C" etc_status etc_plan_get_map(const etc_plan* pl, int32_t* h_device_map
 
 extern "C" etc_status etc_plan_get_slices(const etc_plan* pl, int32_t which, etc_slice* h_out) {
   clear_error_detail();
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!pl || !h_out || (which != 0 && which != 1)) return ETC_ERR_INVALID_ARG;
   const int64_t n = which == 0 ? plan_totals(pl).n_slices_staged : plan_totals(pl).n_slices_local;
   const etc_slice* src = which == 0 ? pl->d_sl_staged : pl->d_sl_local;
@@ -703,6 +712,8 @@ extern "C" etc_status etc_plan_get_slices(const etc_plan* pl, int32_t which, etc
 
 extern "C" etc_status etc_plan_get_fills(const etc_plan* pl, etc_slice* h_out) {
   clear_error_detail();
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!pl || !h_out) return ETC_ERR_INVALID_ARG;
   ETC_CUDA_TRY(cudaStreamSynchronize(pl->stream_created_on));
   const int64_t nf = plan_totals(pl).n_fills;
@@ -712,6 +723,8 @@ extern "C" etc_status etc_plan_get_fills(const etc_plan* pl, etc_slice* h_out) {
 
 extern "C" etc_status etc_plan_validate(const etc_plan* pl, int64_t* n_bad, void* stream) {
   clear_error_detail();
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!pl || !n_bad) return ETC_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   ETC_CUDA_TRY(plan_use(pl, st));

@@ -61,6 +61,8 @@ using namespace etc;
 
 extern "C" etc_status etc_plan_set_rounds(etc_plan* pl, int64_t max_staging_bytes, int32_t* n_rounds, void* stream) {
   clear_error_detail();
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!pl || !n_rounds) return ETC_ERR_INVALID_ARG;
   if (!(pl->flags & ETC_KIND_MAJOR)) return ETC_ERR_INVALID_ARG;
   if (max_staging_bytes < 2 * (int64_t)ETC_CHUNK_BYTES) return ETC_ERR_INVALID_ARG;

@@ -281,6 +281,8 @@ using namespace etc;
 extern "C" etc_status etc_sketch(const int64_t* d_overlap, int32_t n_new, int32_t P, const uint8_t* d_avail,
                                  int32_t method, int32_t* d_device_map, int64_t* d_local_bytes, void* stream) {
   clear_error_detail();
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!d_overlap || !d_device_map || !d_local_bytes || n_new < 1 || P < n_new) return ETC_ERR_INVALID_ARG;
   if (method == ETC_SKETCH_AUTO) method = ETC_SKETCH_HUNGARIAN;   // measured: faster than enumeration even at P = 8
   cudaStream_t st = (cudaStream_t)stream;

@@ -30,7 +30,12 @@ def make_logical(model: dict, seed: int, payload: str = "values", lts=None):
         arrs = []
         for t, (rows, cols, *_r) in enumerate(lts):
             n = rows * cols
-            v = logical_values(seed, k, t, n, es) if payload == "values" else index_stamp(k, t, n, es)
+            if payload == "values":
+                v = logical_values(seed, k, t, n, es)
+            elif payload == "salted":                      # index stamp that also depends on the seed (cheap to make)
+                v = index_stamp(k, t, n, es, salt=seed)
+            else:
+                v = index_stamp(k, t, n, es)
             arrs.append(v.reshape(rows, cols))
         out[k] = arrs
     return out

@@ -39,7 +39,7 @@ def test_host_migration_vs_oracle(E, name, cap):
     w = workload(name)
     model = w["model"]
     oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
-    payloads = [sharded_payload(oo, w["seed"] + i, "stamp" if i == 0 else "values") for i in range(2)]
+    payloads = [sharded_payload(oo, w["seed"] + i, "stamp" if i == 0 else "salted") for i in range(2)]
     h_src = _pinned(payloads[0])
     h_dst = {(n, k): torch.full((on.buffer_elems(n, k) * on.elem_bytes(k),), 0x77, dtype=torch.uint8).pin_memory()
              for n in range(on.n_dev) for k in on.kinds() if on.buffer_elems(n, k)}
@@ -105,7 +105,7 @@ def test_host_migration_uploads_only_what_the_plan_reads(E, name):
     w = workload(name)
     model = w["model"]
     oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
-    payloads = [sharded_payload(oo, w["seed"] + i, "stamp" if i == 0 else "values") for i in range(2)]
+    payloads = [sharded_payload(oo, w["seed"] + i, "stamp" if i == 0 else "salted") for i in range(2)]
     h_src = _pinned(payloads[0])
     h_dst = {(n, k): torch.full((on.buffer_elems(n, k) * on.elem_bytes(k),), 0x77, dtype=torch.uint8).pin_memory()
              for n in range(on.n_dev) for k in on.kinds() if on.buffer_elems(n, k)}
@@ -152,7 +152,7 @@ def test_host_migration_zero_copy(E, name, flags):
     w = workload(name)
     model = w["model"]
     oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
-    payloads = [sharded_payload(oo, w["seed"] + i, "stamp" if i == 0 else "values") for i in range(2)]
+    payloads = [sharded_payload(oo, w["seed"] + i, "stamp" if i == 0 else "salted") for i in range(2)]
     h_src = _pinned(payloads[0])
     h_dst = {(n, k): torch.full((on.buffer_elems(n, k) * on.elem_bytes(k),), 0x77, dtype=torch.uint8).pin_memory()
              for n in range(on.n_dev) for k in on.kinds() if on.buffer_elems(n, k)}

@@ -189,7 +189,7 @@ def test_whole_path_in_one_cuda_graph(E, name, flags):
     w = workload(name)
     model = w["model"]
     oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
-    payloads = [sharded_payload(oo, w["seed"] + i, "stamp" if i == 0 else "values") for i in range(3)]
+    payloads = [sharded_payload(oo, w["seed"] + i, "stamp" if i == 0 else "salted") for i in range(3)]
     old, new = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])
     src = upload(payloads[0])
     dst = E.alloc_buffers(new, fill=0x3C)

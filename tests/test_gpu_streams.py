@@ -75,7 +75,7 @@ def test_migrate_is_cuda_graph_capturable(E, name, flags):
     w = workload(name)
     model = w["model"]
     oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
-    payloads = [sharded_payload(oo, w["seed"] + i, "stamp" if i == 0 else "values") for i in range(3)]
+    payloads = [sharded_payload(oo, w["seed"] + i, "stamp" if i == 0 else "salted") for i in range(3)]
     old, new = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])
     dm, _ = E.etc_sketch(E.etc_cost_matrix(old, new)[0])
     plan = E.etc_plan_create(old, new, dm, flags)
