@@ -383,7 +383,7 @@ class Resident:
             torch.cuda.synchronize()
             if i >= 3:
                 walls.append((time.perf_counter() - t0) * 1e3)
-        n = 50 if self.stats.hbm_bytes < (1 << 32) else 6
+        n = 300 if self.stats.hbm_bytes < (1 << 30) else (50 if self.stats.hbm_bytes < (1 << 34) else 6)
         a, b = self.ev(), self.ev()
         torch.cuda.synchronize()
         a.record(self.stream)

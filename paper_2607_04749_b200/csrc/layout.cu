@@ -281,19 +281,44 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
         q.flags = (inst[i].second ? PF_POST_COPY : 0) | ((two_inst && inst[i].first == 0) ? 0 : PF_SOLE_INST);
       }
     }
+    // The pieces of an UNSHARDED buffer (every kind without the distributed optimizer; PARAM with it) depend on (s, r)
+    // only, up to the device id, the kind's group offset and the element size: they are built once per (s, r) and
+    // copied with those fields patched for the other DP ranks and kinds (4 ns instead of 15 ns per piece).
+    struct Tmpl { size_t begin = 0, count = 0; int64_t es = 0; int kind = -1; int32_t emb = 0; };
+    std::vector<Tmpl> tmpl((size_t)tp);
     for (int d = 0; d < dp; ++d)
       for (int r = 0; r < tp; ++r) {
         const int dev = r + tp * (d + dp * s);
         const std::vector<Sh>& sh = shr[r];
         int64_t Lloc = 0; for (const Sh& q : sh) Lloc += q.n;
         dev_start[dev] = (int32_t)np;
-        for (const Sh& q : sh) ltmask[(size_t)dev * mask_words + q.lt / 32] |= 1u << (q.lt % 32);
+        if (d == 0) { for (const Sh& q : sh) ltmask[(size_t)dev * mask_words + q.lt / 32] |= 1u << (q.lt % 32); }
+        else memcpy(&ltmask[(size_t)dev * mask_words], &ltmask[(size_t)(r + tp * (dp * s)) * mask_words], (size_t)mask_words * 4);
         for (int kind = 0; kind < ETC_NUM_KINDS; ++kind) {
           kind_start[(size_t)dev * (ETC_NUM_KINDS + 1) + kind] = (int32_t)np;
           if (!((m.kinds >> kind) & 1)) continue;
           const int64_t es = kind == 0 ? m.param_dtype : 4;
           const bool dp_sharded = cfg->dist_opt && dp > 1 && kind >= 1;
           int64_t lo = 0, hi = Lloc;
+          Tmpl& tm = tmpl[(size_t)r];
+          if (!dp_sharded && tm.kind >= 0) {                 // copy the template of (s, r), patching what differs
+            bufbytes[(size_t)dev * ETC_NUM_KINDS + kind] = Lloc * es;
+            total_bytes += Lloc * es;
+            const int32_t dgrp = (kind - tm.kind) * nT;
+            int32_t prev_grp = -1;
+            for (size_t i = 0; i < tm.count; ++i) {
+              Piece& p = pieces[np];
+              p = pieces[tm.begin + i];
+              p.dev = dev; p.grp += dgrp; p.d = (int16_t)d; p.boff = p.boff / tm.es * es;
+              if (p.grp != prev_grp) { first[(size_t)dev * nG + p.grp] = (int32_t)np; prev_grp = p.grp; }
+              grp_pieces[(size_t)p.grp] += 1;
+              align_or |= p.boff | ((int64_t)p.W * es) | ((int64_t)p.c0 * es) | ((int64_t)p.nc * es) | (p.f1 * es);
+              ++np;
+            }
+            n_emb_pieces += tm.emb;
+            continue;
+          }
+          const size_t tm_begin = np; const int32_t tm_emb0 = n_emb_pieces;
           if (dp_sharded) {                                  // readings A14 / A28: contiguous flat range of `chunk` elements
             const int64_t unit = (int64_t)dp * std::max(1, cfg->dist_opt_align);
             const int64_t chunk = (Lloc + unit - 1) / unit * std::max(1, cfg->dist_opt_align);
@@ -347,6 +372,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
             grp_pieces[(size_t)grp] += (int32_t)(np - np_before);
             if (q.lt == 0 || (!m.tied_embeddings && q.lt == nT - 1)) n_emb_pieces += (int32_t)(np - np_before);
           }
+          if (!dp_sharded) { tm.begin = tm_begin; tm.count = np - tm_begin; tm.es = es; tm.kind = kind; tm.emb = n_emb_pieces - tm_emb0; }
         }
         kind_start[(size_t)dev * (ETC_NUM_KINDS + 1) + ETC_NUM_KINDS] = (int32_t)np;
       }

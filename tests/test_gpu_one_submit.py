@@ -223,3 +223,36 @@ def test_whole_path_in_one_cuda_graph(E, name, flags):
         dm_h = out_sk[0].cpu().numpy()
         exp, _, _ = oracle_migrate(oo, on, dm_h, payloads[i])
         _compare(on, dst, exp, (name, i))
+
+
+def test_many_interleaved_one_call_migrations(E):
+    """Back-to-back etc_migrate_state calls of reconfigurations of different sizes on two streams, with no host
+    synchronisation in between: the layout upload slabs are reused while earlier uploads may still be in flight, plans and
+    layouts are released in stream order while their kernels are queued.  Every result must still equal the oracle."""
+    cases = []
+    for name, flags in (("c1", 0), ("s4", 0), ("s2odd", 1), ("s3", 4), ("sx64", 0)):
+        w = workload(name)
+        model = w["model"]
+        oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
+        src_np = sharded_payload(oo, w["seed"], "stamp")
+        old, new = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])
+        src, dst = upload(src_np), E.alloc_buffers(new, fill=0x3C)
+        staging = torch.empty(max(E.etc_staging_bound(old, new, flags), 16), dtype=torch.uint8, device="cuda")
+        cases.append(dict(name=name, oo=oo, on=on, src_np=src_np, dst=dst,
+                          call=E.MigrateState(model, w["old"], w["new"], src, dst, staging, flags)))
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    torch.cuda.synchronize()
+    plans = {}
+    for it in range(40):
+        for j, c in enumerate(cases):
+            st = streams[j % 2]                          # a case always runs on the same stream (its buffers are reused)
+            last = it == 39
+            p = c["call"](stream=st, want_plan=last)
+            if last:
+                plans[c["name"]] = p
+    torch.cuda.synchronize()
+    for c in cases:
+        dmap = plans[c["name"]].device_map()
+        exp, T, _ = oracle_migrate(c["oo"], c["on"], dmap, c["src_np"])
+        _compare(c["on"], c["dst"], exp, c["name"])
+        assert np.array_equal(plans[c["name"]].traffic(), T)
