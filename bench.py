@@ -678,7 +678,7 @@ def e2e(E, torch, args, w, dev, world, barrier):
         wi = workload(name)
         lo, ln = E.etc_layout_create(wi["model"], wi["old"]), E.etc_layout_create(wi["model"], wi["new"])
         total = lo.total_bytes() + ln.total_bytes()
-        ok = 1.0 if (total <= args.e2e_max_bytes and host_memory_ok(total)) else 0.0
+        ok = 1.0 if (total <= args.e2e_max_bytes // max(1, world) and host_memory_ok(total * max(1, world))) else 0.0   # every rank pins its own copy
         h_src, h_dst = {}, {}
         if ok:
             try:
