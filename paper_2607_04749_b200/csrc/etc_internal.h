@@ -112,6 +112,7 @@ struct DeviceGuard {
   }
   ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
 };
+etc_status validate_config(const etc_model_desc* m, const etc_parallel_cfg* c);   // host-only checks of etc_layout_create
 cudaError_t layout_use(const etc_layout* L, cudaStream_t st);   // `st` waits for the tables' upload; noted as a reader
 // xfer.cu: metadata transfers as kernels on the caller's stream, so that they never queue behind bulk DMA transfers
 cudaError_t write_small(void* d_dst, const void* h_src, size_t bytes, cudaStream_t st);      // host -> device via kernel parameters

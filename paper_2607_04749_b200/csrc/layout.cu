@@ -78,7 +78,7 @@ static int stage_begin(int n_layers, const etc_parallel_cfg& c, int s) {
   return c.pp_first ? c.pp_first + (s - 1) * per : s * per;
 }
 
-static etc_status validate(const etc_model_desc* m, const etc_parallel_cfg* c) {
+etc_status validate_config(const etc_model_desc* m, const etc_parallel_cfg* c) {
   if (!m || !c) return ETC_ERR_INVALID_ARG;
   if (c->tp < 1 || c->pp < 1 || c->dp < 1 || (c->dist_opt != 0 && c->dist_opt != 1) || c->dist_opt_align < 0 ||
       c->vocab_divisor < 0) return ETC_ERR_INVALID_ARG;
@@ -198,7 +198,7 @@ static void qkv_blocks(const etc_model_desc& m, int tp, int r, Sh& s) {
 extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_parallel_cfg* cfg, etc_layout** out) {
   clear_error_detail();
   if (!out) return ETC_ERR_INVALID_ARG;
-  etc_status st = validate(model, cfg);
+  etc_status st = validate_config(model, cfg);
   if (st != ETC_OK) return st;
   const etc_model_desc& m = *model;
   const int tp = cfg->tp, pp = cfg->pp, dp = cfg->dp;

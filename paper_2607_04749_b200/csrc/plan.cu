@@ -523,9 +523,9 @@ extern "C" int64_t etc_staging_bound(const etc_layout* old_l, const etc_layout* 
 extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
                                              const uint8_t* failed, int32_t flags, etc_plan** out, void* stream) {
   clear_error_detail();
+  if (!old_l || !new_l || !device_map || !out) return ETC_ERR_INVALID_ARG;
   etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
   if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
-  if (!old_l || !new_l || !device_map || !out) return ETC_ERR_INVALID_ARG;
   if (flags < 0 || flags > (ETC_ALL_STAGED | ETC_KIND_MAJOR | ETC_ALL_DIRECT | ETC_NO_SYNC)) return ETC_ERR_INVALID_ARG;
   if ((flags & ETC_ALL_STAGED) && (flags & ETC_ALL_DIRECT)) return ETC_ERR_INVALID_ARG;
   if (!etc_same_model(old_l, new_l)) return ETC_ERR_MISMATCH;

@@ -15,16 +15,19 @@ extern "C" etc_status etc_migrate_state(const etc_model_desc* model, const etc_p
                                         void* const* dst_bufs, void* staging, int64_t staging_bytes,
                                         const uint8_t* d_avail, int32_t flags, etc_plan** plan_out, void* stream) {
   clear_error_detail();
-  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
-  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!model || !old_cfg || !new_cfg || !src_bufs || !dst_bufs || staging_bytes < 0) return ETC_ERR_INVALID_ARG;
   if (flags & (ETC_KIND_MAJOR | ETC_NO_SYNC)) return ETC_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   etc_layout *lo = nullptr, *ln = nullptr;
   etc_plan* pl = nullptr;
   char* tmp = nullptr;
-  etc_status rc = etc_layout_create(model, old_cfg, &lo);                                          // (a1)
+  etc_status rc = validate_config(model, old_cfg);      // bad arguments and bad configurations fail before any CUDA call
+  if (rc == ETC_OK) rc = validate_config(model, new_cfg);
+  if (rc != ETC_OK) return rc;
+  rc = etc_layout_create(model, old_cfg, &lo);                                                     // (a1)
   if (rc == ETC_OK) rc = etc_layout_create(model, new_cfg, &ln);
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); if (lo) etc_layout_destroy(lo); if (ln) etc_layout_destroy(ln); return ETC_ERR_CUDA; }
   auto done = [&](etc_status r) {
     if (tmp) cudaFreeAsync(tmp, st);
     if (r != ETC_OK && pl) { etc_plan_destroy(pl); pl = nullptr; }

@@ -59,6 +59,27 @@ def test_layout_validation_without_gpu(lib):
     assert h.value is None
 
 
+def test_one_call_primitive_validates_before_any_cuda_call(lib):
+    """etc_migrate_state / etc_staging_bound / etc_plan_create reject bad arguments on the host."""
+    from paper_2607_04749_b200.binding import _ModelDesc, _ParallelCfg
+    m = _ModelDesc(style=0, n_layers=4, hidden=12, n_q_heads=2, n_kv_heads=2, head_dim=6, ffn_hidden=28, vocab=20,
+                   max_pos=0, tied_embeddings=1, param_dtype=2, kinds=15)
+    c = _ParallelCfg(1, 1, 1, 0)
+    tab = (C.c_void_p * 4)()
+    h = C.c_void_p()
+    args = lambda **kw: [kw.get("m", C.byref(m)), kw.get("oc", C.byref(c)), kw.get("nc", C.byref(c)), kw.get("src", tab),
+                         kw.get("dst", tab), None, kw.get("stg_bytes", 0), None, kw.get("flags", 0), C.byref(h), None]
+    assert lib.etc_migrate_state(*args(m=None)) == -1
+    assert lib.etc_migrate_state(*args(src=None)) == -1
+    assert lib.etc_migrate_state(*args(stg_bytes=-1)) == -1
+    assert lib.etc_migrate_state(*args(flags=2)) == -1            # ETC_KIND_MAJOR is for rounds, not for the one-call path
+    assert lib.etc_migrate_state(*args(flags=8)) == -1            # ETC_NO_SYNC is implied, not a caller's flag here
+    assert lib.etc_migrate_state(*args(nc=C.byref(_ParallelCfg(1, 3, 1, 0)))) == -2      # layers % pp (PAPER.md:277)
+    assert h.value is None
+    assert lib.etc_staging_bound(None, None, 0) == -1
+    assert lib.etc_plan_create(None, None, None, 0, C.byref(h), None) == -1
+
+
 def test_product_path_has_no_oracle_or_cpu_fallback():
     """The package must not import the oracle, and must fail loudly without a CUDA device."""
     import torch
@@ -66,7 +87,7 @@ def test_product_path_has_no_oracle_or_cpu_fallback():
     pkg = os.path.join(ROOT, "paper_2607_04749_b200")
     for dirpath, _, files in os.walk(pkg):
         for f in files:
-            if f.endswith((".py", ".cu", ".h", ".cpp")):
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
                 txt = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in txt and "from oracle" not in txt and "liboracle" not in txt, f
     if not torch.cuda.is_available():
