@@ -487,7 +487,9 @@ def run_cuda(args, w):
 
     peak, peak_src = measured_peak()
     flags = E.ETC_ALL_STAGED if args.all_staged else E.ETC_LOCAL_DIRECT
-    mode = "ALL_STAGED" if args.all_staged else "LOCAL_DIRECT"
+    if args.no_reorder:
+        flags |= E.ETC_NO_REORDER
+    mode = ("ALL_STAGED" if args.all_staged else "LOCAL_DIRECT") + ("|NO_REORDER" if args.no_reorder else "")
 
     # ---- the timed line: whole path on the headline workload, inputs resident in HBM
     R = Resident(E, torch, w, dev, flags)
@@ -795,6 +797,8 @@ def main():
     ap.add_argument("--config", default="c4", help="workload: c1..c5 (BASELINE.json configs[0..4]); default configs[3], "
                                                     "the largest that fits one GPU")
     ap.add_argument("--all-staged", action="store_true", help="ETC_ALL_STAGED: every slice goes through pack/unpack")
+    ap.add_argument("--no-reorder", action="store_true", help="ETC_NO_REORDER: copy launches walk the chunk lists unit by "
+                    "unit instead of in address order (A/B measurement)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip per_config, all-staged rates and the context legs")

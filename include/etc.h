@@ -162,7 +162,7 @@ etc_status etc_defrag(const int32_t* d_device_map, int32_t pw, int32_t cw, int32
  * etc_plan_set_rounds, etc_plan_validate) makes that stream wait for those kernels itself (an event recorded at the end
  * of this call), so no caller-side ordering is needed.  Fails with ETC_ERR_BAD_MAP if the map is not injective into
  * [0,P). */
-enum { ETC_LOCAL_DIRECT = 0, ETC_ALL_STAGED = 1, ETC_KIND_MAJOR = 2, ETC_ALL_DIRECT = 4, ETC_NO_SYNC = 8 };
+enum { ETC_LOCAL_DIRECT = 0, ETC_ALL_STAGED = 1, ETC_KIND_MAJOR = 2, ETC_ALL_DIRECT = 4, ETC_NO_SYNC = 8, ETC_NO_REORDER = 16 };
 /* ETC_NO_SYNC (OR-ed into flags): etc_plan_create does NOT synchronise.  The slice / chunk tables are sized from upper
  * bounds the host derives from the two layouts (pieces per tensor, bytes needed), the real counts stay on the device, and
  * etc_migrate / etc_migrate_phase launch bound-sized grids whose surplus CTAs leave at once: a whole reconfiguration is
@@ -171,7 +171,14 @@ enum { ETC_LOCAL_DIRECT = 0, ETC_ALL_STAGED = 1, ETC_KIND_MAJOR = 2, ETC_ALL_DIR
  * bound that falls short is detected ON THE DEVICE: the plan then copies nothing, and the error is reported by the
  * first call that needs the counts on the host — etc_plan_get_stats (which waits for the plan's kernels), and likewise
  * etc_plan_get_traffic / _slices / _fills / etc_plan_set_rounds / etc_plan_validate.  A hint: plans whose bound-sized
- * tables would exceed 64 MB are made the synchronising way (their copy kernels dwarf one host sync). */
+ * tables would exceed 64 MB are made the synchronising way (their copy kernels dwarf one host sync).
+ * Launch order.  A plan whose counts the host knows (every plan but a bound-sized ETC_NO_SYNC one) also keeps its copy
+ * work items in ADDRESS order — launch 1 (pack + local) by source address, launch 2 (unpack) by destination address —
+ * and etc_migrate / etc_migrate_phase walk those lists: work items that read interleaved column blocks of the same
+ * rows (a TP change of a row-parallel weight), or the same source range for several new ranks (replicated state fanning
+ * out to more DP groups), then run side by side and share DRAM pages and L2 lines.  The result is the same bytes either
+ * way.  ETC_NO_REORDER (OR-ed into flags) keeps the launches in list order (unit by unit): a measurement mode.
+ * etc_migrate_round always walks its chunk range in list order. */
 int64_t etc_staging_bound(const etc_layout* old_l, const etc_layout* new_l, int32_t flags);   /* bytes; < 0 on bad arguments */
 etc_status etc_plan_create(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
                            int32_t flags, etc_plan** out, void* stream);
@@ -229,10 +236,29 @@ typedef struct {
   int32_t pad;
 } etc_slice;
 etc_status etc_plan_get_slices(const etc_plan* plan, int32_t which, etc_slice* h_out);
+/* The copy work items ("chunks": at most ETC_CHUNK_BYTES of payload each, nrows x row_bytes with a row pitch per side;
+ * what one CTA of the copy kernels moves).  which = 0: the staged chunks in plan order (unit by unit), 1: the local
+ * chunks in plan order, 2: the launch-1 list in address order (every chunk of pack + local sorted by source address;
+ * `staged` tells the two apart), 3: the launch-2 list (the staged chunks sorted by destination address).  h_out must
+ * hold n_chunks_staged (0, 3), n_chunks_local (1) or their sum (2) entries; copied to HOST memory.  2 and 3 return
+ * ETC_ERR_INVALID_ARG for a plan that keeps no ordered lists (ETC_NO_REORDER, or a bound-sized ETC_NO_SYNC plan).
+ * Address order means: non-decreasing buffer index, and inside a buffer non-decreasing 64 KB block of the offset (for
+ * layouts beyond 256 GB in all, a coarser block); the order inside a block is unspecified. */
+typedef struct {
+  int64_t src_off, dst_off, stg_off;  /* byte offsets in the source buffer, destination buffer, staging buffer */
+  int32_t src_stride, dst_stride;     /* row pitch in bytes (the staging pitch is row_bytes) */
+  int32_t row_bytes, nrows;
+  uint16_t src_buf, dst_buf;          /* old_dev*4+kind, new_rank*4+kind */
+  int16_t vec;                        /* widest power-of-two access (<= 16 B) every address of the chunk is aligned to */
+  int16_t staged;                     /* lists 2: 1 = packed into staging, 0 = copied old -> new buffer; else 0 */
+} etc_chunk;
+etc_status etc_plan_get_chunks(const etc_plan* plan, int32_t which, etc_chunk* h_out);
 /* Bounds check of a finished plan, on the device: counts the copy work items whose source, destination or staging
  * extent does not lie inside the buffer it addresses (sizes from the layouts the plan was made from), or whose declared
- * access width does not divide its addresses.  *n_bad (HOST) = 0 for every plan this library makes; a debugging and
- * test aid (one thread per work item, synchronises `stream`). */
+ * access width does not divide its addresses; the address-ordered launch lists (whole-plan and per-round) are checked
+ * the same way and must be permutations of the plan's lists (order-independent checksums), else one more is counted.
+ * *n_bad (HOST) = 0 for every plan this library makes; a debugging and test aid (one thread per work item,
+ * synchronises `stream`). */
 etc_status etc_plan_validate(const etc_plan* plan, int64_t* n_bad, void* stream);
 /* The zero-fill descriptors (reading A31) as etc_slice records with no source: src_dev = -1, src_off = stg_off = -1,
  * src_stride = 0; h_out must hold etc_plan_stats.n_fills entries (order unspecified).  Copied to HOST memory. */

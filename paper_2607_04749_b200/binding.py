@@ -12,7 +12,7 @@ _LIB_PATH = os.path.join(_HERE, "libetc.so")
 _lib = None
 _inited = False
 
-ETC_LOCAL_DIRECT, ETC_ALL_STAGED, ETC_KIND_MAJOR, ETC_ALL_DIRECT, ETC_NO_SYNC = 0, 1, 2, 4, 8
+ETC_LOCAL_DIRECT, ETC_ALL_STAGED, ETC_KIND_MAJOR, ETC_ALL_DIRECT, ETC_NO_SYNC, ETC_NO_REORDER = 0, 1, 2, 4, 8, 16
 ETC_SKETCH_AUTO, ETC_SKETCH_EXHAUSTIVE, ETC_SKETCH_HUNGARIAN = 0, 1, 2
 ETC_PHASE_PACK, ETC_PHASE_UNPACK, ETC_PHASE_ALL = 1, 2, 3
 ETC_DEFRAG_OCCUPANCY, ETC_DEFRAG_EFFICIENCY, ETC_DEFRAG_BOTH = 1, 2, 3
@@ -25,6 +25,7 @@ EXPORTED_SYMBOLS = (
     "etc_status_string", "etc_last_error_detail", "etc_kernel_launches", "etc_defrag",
     "etc_plan_set_rounds", "etc_plan_get_round", "etc_migrate_round", "etc_plan_create_failed", "etc_mask_failed",
     "etc_upload_sources", "etc_plan_validate", "etc_mask_cross_dp", "etc_staging_bound", "etc_migrate_state", "etc_plan_get_map",
+    "etc_plan_get_chunks",
 )
 
 
@@ -95,6 +96,7 @@ def lib():
         L.etc_plan_get_traffic.restype = i32; L.etc_plan_get_traffic.argtypes = [vp, vp]
         L.etc_plan_get_slices.restype = i32; L.etc_plan_get_slices.argtypes = [vp, i32, vp]
         L.etc_plan_get_map.restype = i32; L.etc_plan_get_map.argtypes = [vp, vp]
+        L.etc_plan_get_chunks.restype = i32; L.etc_plan_get_chunks.argtypes = [vp, i32, vp]
         L.etc_plan_get_fills.restype = i32; L.etc_plan_get_fills.argtypes = [vp, vp]
         L.etc_plan_validate.restype = i32; L.etc_plan_validate.argtypes = [vp, C.POINTER(i64), vp]
         L.etc_migrate.restype = i32; L.etc_migrate.argtypes = [vp, vp, vp, vp, vp]
@@ -288,6 +290,19 @@ class Plan:
         assert dt.itemsize == C.sizeof(_Slice)
         arr = np.zeros(max(n, 1), dt)
         _check(lib().etc_plan_get_slices(self.h, which, arr.ctypes.data))
+        return arr[:n]
+
+    def chunks(self, which: int):
+        """etc_plan_get_chunks: 0 staged / 1 local chunks in plan order, 2 / 3 the address-ordered launch lists."""
+        import numpy as np
+        st = self.stats
+        n = st.n_chunks_local if which == 1 else (st.n_chunks_staged + st.n_chunks_local if which == 2 else st.n_chunks_staged)
+        dt = np.dtype([("src_off", np.int64), ("dst_off", np.int64), ("stg_off", np.int64), ("src_stride", np.int32),
+                       ("dst_stride", np.int32), ("row_bytes", np.int32), ("nrows", np.int32), ("src_buf", np.uint16),
+                       ("dst_buf", np.uint16), ("vec", np.int16), ("staged", np.int16)])
+        assert dt.itemsize == 48
+        arr = np.zeros(max(n, 1), dt)
+        _check(lib().etc_plan_get_chunks(self.h, which, arr.ctypes.data))
         return arr[:n]
 
     def validate(self, stream=None) -> int:

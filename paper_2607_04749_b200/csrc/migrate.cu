@@ -26,11 +26,14 @@ struct PtrParams { const void* p[PTR_PARAM_MAX]; };
 
 // UNPACK = false: blocks [0,nA) pack staged chunks (src -> staging), blocks [nA,nA+nB) copy local chunks (src -> dst)
 // UNPACK = true : blocks [0,nA) unpack staged chunks (staging -> dst)
+// `ordered` (or null): the same chunks as ONE list in the order the launch should walk them (plan_order.cu: by source
+// address for launch 1, staged chunks flagged; by destination address for launch 2); block b then takes ordered[b].
 template <bool UNPACK, bool PARAM_PTRS>
 __global__ void __launch_bounds__(CP_THREADS)
 migrate_copy_kernel(const Chunk* __restrict__ chA, long long nA, const Chunk* __restrict__ chB,
                     const void* const* __restrict__ tab, int ns, char* __restrict__ staging,
-                    const PlanTotals* __restrict__ lazy, const __grid_constant__ PtrParams pp) {
+                    const PlanTotals* __restrict__ lazy, const Chunk* __restrict__ ordered,
+                    const __grid_constant__ PtrParams pp) {
   extern __shared__ __align__(128) char tile[];                 // TILE_BYTES: the staging tile of every copy path
   __shared__ uint64_t bar;
   const long long b = blockIdx.x;
@@ -38,8 +41,8 @@ migrate_copy_kernel(const Chunk* __restrict__ chA, long long nA, const Chunk* __
     nA = lazy->n_chunks_staged;
     if (b >= nA + (UNPACK ? 0 : lazy->n_chunks_local)) return;
   }
-  const bool staged = b < nA;
-  const Chunk c = staged ? chA[b] : chB[b - nA];
+  const Chunk c = ordered ? ordered[b] : (b < nA ? chA[b] : chB[b - nA]);
+  const bool staged = UNPACK || (ordered ? (c.pad & CHUNK_STAGED) != 0 : b < nA);
   const char* src; char* dst; uint32_t sp, dp;
   auto src_ptr = [&]() { return static_cast<const char*>(PARAM_PTRS ? pp.p[c.src_buf] : tab[c.src_buf]); };
   auto dst_ptr = [&]() { return static_cast<char*>(const_cast<void*>(PARAM_PTRS ? pp.p[ns + c.dst_buf] : tab[ns + c.dst_buf])); };
@@ -120,7 +123,8 @@ using namespace etc;
 static etc_status launch_migrate(const etc_plan* pl, const void* const* src_bufs, void* const* dst_bufs, void* staging,
                                  int32_t phases, cudaStream_t st, void** d_ptrs, int only_kind, long long ca, long long nA,
                                  long long la, long long nB, int64_t stg_base, int64_t stg_need, bool with_fills,
-                                 long long n_fills, const PlanTotals* lazy) {
+                                 long long n_fills, const PlanTotals* lazy, const Chunk* order1 = nullptr,
+                                 const Chunk* order2 = nullptr) {
   if (!pl || !src_bufs || !dst_bufs || phases < 1 || phases > ETC_PHASE_ALL) return ETC_ERR_INVALID_ARG;
   if (stg_need > 0 && !staging) return ETC_ERR_INVALID_ARG;
   if (reinterpret_cast<uintptr_t>(staging) & 15) return ETC_ERR_INVALID_ARG;
@@ -154,9 +158,9 @@ static etc_status launch_migrate(const etc_plan* pl, const void* const* src_bufs
   char* stg = static_cast<char*>(staging) - stg_base;          // chunk records carry offsets of the full staging layout
   if ((phases & ETC_PHASE_PACK) && nA + nB > 0) {
     if (in_params) migrate_copy_kernel<false, true><<<(unsigned)(nA + nB), CP_THREADS, TILE_BYTES, st>>>(
-        pl->d_ch_staged + ca, nA, pl->d_ch_local + la, tab, (int)ns, stg, lazy, pp);
+        pl->d_ch_staged + ca, nA, pl->d_ch_local + la, tab, (int)ns, stg, lazy, order1, pp);
     else migrate_copy_kernel<false, false><<<(unsigned)(nA + nB), CP_THREADS, TILE_BYTES, st>>>(
-        pl->d_ch_staged + ca, nA, pl->d_ch_local + la, tab, (int)ns, stg, lazy, pp);
+        pl->d_ch_staged + ca, nA, pl->d_ch_local + la, tab, (int)ns, stg, lazy, order1, pp);
     ETC_CUDA_TRY(cudaGetLastError());
     count_launch();
   }
@@ -169,9 +173,9 @@ static etc_status launch_migrate(const etc_plan* pl, const void* const* src_bufs
   }
   if ((phases & ETC_PHASE_UNPACK) && nA > 0) {
     if (in_params) migrate_copy_kernel<true, true><<<(unsigned)nA, CP_THREADS, TILE_BYTES, st>>>(
-        pl->d_ch_staged + ca, nA, nullptr, tab, (int)ns, stg, lazy, pp);
+        pl->d_ch_staged + ca, nA, nullptr, tab, (int)ns, stg, lazy, order2, pp);
     else migrate_copy_kernel<true, false><<<(unsigned)nA, CP_THREADS, TILE_BYTES, st>>>(
-        pl->d_ch_staged + ca, nA, nullptr, tab, (int)ns, stg, lazy, pp);
+        pl->d_ch_staged + ca, nA, nullptr, tab, (int)ns, stg, lazy, order2, pp);
     ETC_CUDA_TRY(cudaGetLastError());
     count_launch();
   }
@@ -202,7 +206,8 @@ extern "C" etc_status etc_migrate_phase(const etc_plan* pl, const void* const* s
   const PlanTotals& t = plan_totals(pl, &rc);
   if (rc != ETC_OK) return rc;
   return launch_migrate(pl, src_bufs, dst_bufs, staging, phases, (cudaStream_t)stream, pl->d_ptrs, -1, 0,
-                        t.n_chunks_staged, 0, t.n_chunks_local, 0, t.staging_bytes, true, t.n_fills, nullptr);
+                        t.n_chunks_staged, 0, t.n_chunks_local, 0, t.staging_bytes, true, t.n_fills, nullptr,
+                        pl->d_ch1, pl->d_ch2);
 }
 
 extern "C" etc_status etc_migrate(const etc_plan* pl, const void* const* src_bufs, void* const* dst_bufs, void* staging,
@@ -221,5 +226,6 @@ extern "C" etc_status etc_migrate_round(const etc_plan* pl, int32_t round, const
   const size_t n_ptrs = ((size_t)(pl->n_old + pl->n_new) * ETC_NUM_KINDS * sizeof(void*) + 255) / 256 * 256 / sizeof(void*);
   return launch_migrate(pl, src_bufs, dst_bufs, staging, phases, (cudaStream_t)stream,
                         pl->d_round_ptrs + n_ptrs * (size_t)round, r.kind, r.ca, r.cb - r.ca, r.la, r.lb - r.la,
-                        r.stg_base, r.stg_span, r.sub == 0, plan_totals(pl).n_fills, nullptr);
+                        r.stg_base, r.stg_span, r.sub == 0, plan_totals(pl).n_fills, nullptr,
+                        pl->d_rch1 ? pl->d_rch1 + r.ca + r.la : nullptr, pl->d_rch2 ? pl->d_rch2 + r.ca : nullptr);
 }

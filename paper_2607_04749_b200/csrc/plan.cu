@@ -419,12 +419,20 @@ plan_fills_kernel(DeviceTables newT, const int32_t* __restrict__ device_map, int
 
 // Bounds check of the finished plan (a safety net of our own: compute-sanitizer is not available everywhere): every
 // chunk's source, destination and staging extent must lie inside the buffer it addresses.  One thread per chunk.
+// staged: 1 / 0 for the plan's two lists, -1 for an address-ordered list (each record says which it is).  `sum` receives
+// an order-independent checksum of the records, so that the ordered lists can be checked to be permutations of the
+// plan's lists.
+__device__ __forceinline__ unsigned long long mix64(unsigned long long x) {
+  x ^= x >> 33; x *= 0xff51afd7ed558ccdull; x ^= x >> 33; x *= 0xc4ceb9fe1a85ec53ull; x ^= x >> 33; return x;
+}
 __global__ void __launch_bounds__(256)
-plan_validate_kernel(const Chunk* __restrict__ ch, long long n, int staged, const int64_t* __restrict__ old_bytes,
-                     const int64_t* __restrict__ new_bytes, int64_t staging_bytes, unsigned long long* __restrict__ bad) {
+plan_validate_kernel(const Chunk* __restrict__ ch, long long n, int staged_list, const int64_t* __restrict__ old_bytes,
+                     const int64_t* __restrict__ new_bytes, int64_t staging_bytes, unsigned long long* __restrict__ bad,
+                     unsigned long long* __restrict__ sum) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const Chunk c = ch[i];
+  const bool live = i < n;                                       // every lane stays for the warp reduction below
+  const Chunk c = ch[live ? i : 0];
+  const bool staged = staged_list < 0 ? (c.pad & CHUNK_STAGED) != 0 : staged_list != 0;
   const int64_t span_src = (int64_t)(c.nrows - 1) * c.src_stride + c.row_bytes;
   const int64_t span_dst = (int64_t)(c.nrows - 1) * c.dst_stride + c.row_bytes;
   bool ok = c.nrows >= 1 && c.row_bytes >= 1 && (int64_t)c.nrows * c.row_bytes <= ETC_CHUNK_BYTES;
@@ -437,7 +445,15 @@ plan_validate_kernel(const Chunk* __restrict__ ch, long long n, int staged, cons
     if (c.nrows > 1) al |= (int64_t)c.src_stride | (int64_t)c.dst_stride;
     ok = ok && (al & (c.vec - 1)) == 0;
   }
-  if (!ok) atomicAdd(bad, 1ull);
+  if (live && !ok) atomicAdd(bad, 1ull);
+  unsigned long long h = mix64((unsigned long long)c.src_off ^ mix64((unsigned long long)c.dst_off ^ mix64((unsigned long long)c.stg_off)));
+  h = mix64(h ^ ((unsigned long long)(uint32_t)c.src_stride << 32 | (uint32_t)c.dst_stride));
+  h = mix64(h ^ ((unsigned long long)(uint32_t)c.row_bytes << 32 | (uint32_t)c.nrows));
+  h = mix64(h ^ ((unsigned long long)c.src_buf << 32 | (unsigned long long)c.dst_buf << 16 | (unsigned long long)(uint16_t)c.vec) ^ (staged ? 0x9e3779b97f4a7c15ull : 0));
+  if (!live) h = 0;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) h += __shfl_xor_sync(0xffffffffu, h, o);
+  if ((threadIdx.x & 31) == 0 && h) atomicAdd(sum, h);
 }
 
 }  // namespace etc
@@ -526,7 +542,7 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
   if (!old_l || !new_l || !device_map || !out) return ETC_ERR_INVALID_ARG;
   etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
   if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
-  if (flags < 0 || flags > (ETC_ALL_STAGED | ETC_KIND_MAJOR | ETC_ALL_DIRECT | ETC_NO_SYNC)) return ETC_ERR_INVALID_ARG;
+  if (flags < 0 || flags > (ETC_ALL_STAGED | ETC_KIND_MAJOR | ETC_ALL_DIRECT | ETC_NO_SYNC | ETC_NO_REORDER)) return ETC_ERR_INVALID_ARG;
   if ((flags & ETC_ALL_STAGED) && (flags & ETC_ALL_DIRECT)) return ETC_ERR_INVALID_ARG;
   if (!etc_same_model(old_l, new_l)) return ETC_ERR_MISMATCH;
   const int n_old = old_l->t.n_dev, n_new = new_l->t.n_dev, P = n_old > n_new ? n_old : n_new;
@@ -541,7 +557,7 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
   const int B = (int)std::max<long long>(1, std::min<long long>(want, 65536 / U));
 
   etc_plan* pl = new etc_plan();
-  pl->n_old = n_old; pl->n_new = n_new; pl->P = P; pl->flags = flags & ~ETC_NO_SYNC; pl->stream_created_on = st;
+  pl->n_old = n_old; pl->n_new = n_new; pl->P = P; pl->flags = flags & ~(ETC_NO_SYNC | ETC_NO_REORDER); pl->stream_created_on = st;
   pl->streams.note(st);
   pl->old_bytes.assign(old_l->h_buffer_bytes, old_l->h_buffer_bytes + (size_t)n_old * ETC_NUM_KINDS);
   pl->new_bytes.assign(new_l->h_buffer_bytes, new_l->h_buffer_bytes + (size_t)n_new * ETC_NUM_KINDS);
@@ -645,6 +661,8 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
     PLAN_TRY(cudaGetLastError());
     count_launch();
   }
+  // the launch lists in address order (plan_order.cu); bound-sized ETC_NO_SYNC plans launch in list order
+  if (!lazy && !(flags & ETC_NO_REORDER)) PLAN_TRY(plan_build_order(pl, n_ch_s, n_ch_l, st));
   // the tables are complete once `st` reaches this point: readers on other streams wait for it (plan_use)
   PLAN_TRY(cudaEventCreateWithFlags(&pl->ready, cudaEventDisableTiming));
   PLAN_TRY(cudaEventRecord(pl->ready, st));
@@ -660,6 +678,8 @@ extern "C" void etc_plan_destroy(etc_plan* pl) {
   if (pl->d_ws) cudaFreeAsync(pl->d_ws, st);
   if (pl->d_tb) cudaFreeAsync(pl->d_tb, st);
   if (pl->d_rounds_ws) cudaFreeAsync(pl->d_rounds_ws, st);
+  if (pl->d_order_ws) cudaFreeAsync(pl->d_order_ws, st);
+  if (pl->d_round_order_ws) cudaFreeAsync(pl->d_round_order_ws, st);
   if (pl->ready) cudaEventDestroy(pl->ready);
   delete pl;
 }
@@ -710,6 +730,23 @@ extern "C" etc_status etc_plan_get_slices(const etc_plan* pl, int32_t which, etc
   return ETC_OK;
 }
 
+static_assert(sizeof(etc_chunk) == sizeof(etc::Chunk), "etc_chunk mirrors Chunk");
+extern "C" etc_status etc_plan_get_chunks(const etc_plan* pl, int32_t which, etc_chunk* h_out) {
+  clear_error_detail();
+  etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
+  if (!pl || !h_out || which < 0 || which > 3) return ETC_ERR_INVALID_ARG;
+  etc_status rc = ETC_OK;
+  const PlanTotals& t = plan_totals(pl, &rc);
+  if (rc != ETC_OK) return rc;
+  const Chunk* src = which == 0 ? pl->d_ch_staged : which == 1 ? pl->d_ch_local : which == 2 ? pl->d_ch1 : pl->d_ch2;
+  const int64_t n = which == 1 ? t.n_chunks_local : which == 2 ? t.n_chunks_staged + t.n_chunks_local : t.n_chunks_staged;
+  if (which >= 2 && !pl->d_ch1) return ETC_ERR_INVALID_ARG;
+  ETC_CUDA_TRY(cudaStreamSynchronize(pl->stream_created_on));
+  if (n) ETC_CUDA_TRY(cudaMemcpy(h_out, src, sizeof(Chunk) * (size_t)n, cudaMemcpyDeviceToHost));
+  return ETC_OK;
+}
+
 extern "C" etc_status etc_plan_get_fills(const etc_plan* pl, etc_slice* h_out) {
   clear_error_detail();
   etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
@@ -730,27 +767,38 @@ extern "C" etc_status etc_plan_validate(const etc_plan* pl, int64_t* n_bad, void
   ETC_CUDA_TRY(plan_use(pl, st));
   const size_t ns = pl->old_bytes.size(), nd = pl->new_bytes.size();
   int64_t* d_sizes = nullptr;
-  ETC_CUDA_TRY(cudaMallocAsync(&d_sizes, sizeof(int64_t) * (ns + nd + 1), st));
+  ETC_CUDA_TRY(cudaMallocAsync(&d_sizes, sizeof(int64_t) * (ns + nd + 7), st));
   auto done = [&](etc_status rc) { cudaFreeAsync(d_sizes, st); return rc; };
 #define VAL_TRY(expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) { set_error_detail(#expr, _e); return done(ETC_ERR_CUDA); } } while (0)
   VAL_TRY(cudaMemcpyAsync(d_sizes, pl->old_bytes.data(), sizeof(int64_t) * ns, cudaMemcpyHostToDevice, st));
   VAL_TRY(cudaMemcpyAsync(d_sizes + ns, pl->new_bytes.data(), sizeof(int64_t) * nd, cudaMemcpyHostToDevice, st));
+  // d_bad[0] = bad chunks; [1], [2] checksums of the staged / local list; [3], [4] of the ordered launch lists; [5], [6]
+  // of the per-round ordered lists
   unsigned long long* d_bad = reinterpret_cast<unsigned long long*>(d_sizes + ns + nd);
-  VAL_TRY(cudaMemsetAsync(d_bad, 0, sizeof(unsigned long long), st));
+  VAL_TRY(cudaMemsetAsync(d_bad, 0, 7 * sizeof(unsigned long long), st));
   const PlanTotals& t = plan_totals(pl);
-  if (t.n_chunks_staged) {
-    plan_validate_kernel<<<(unsigned)((t.n_chunks_staged + 255) / 256), 256, 0, st>>>(pl->d_ch_staged, t.n_chunks_staged, 1, d_sizes,
-                                                                                     d_sizes + ns, t.staging_bytes, d_bad);
-    VAL_TRY(cudaGetLastError()); count_launch();
-  }
-  if (t.n_chunks_local) {
-    plan_validate_kernel<<<(unsigned)((t.n_chunks_local + 255) / 256), 256, 0, st>>>(pl->d_ch_local, t.n_chunks_local, 0, d_sizes,
-                                                                                    d_sizes + ns, t.staging_bytes, d_bad);
-    VAL_TRY(cudaGetLastError()); count_launch();
-  }
-  unsigned long long h_bad = 0;
-  VAL_TRY(cudaMemcpyAsync(&h_bad, d_bad, sizeof(h_bad), cudaMemcpyDeviceToHost, st));
+  auto check = [&](const Chunk* list, long long n, int staged, int slot) -> cudaError_t {
+    if (!n || !list) return cudaSuccess;
+    plan_validate_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(list, n, staged, d_sizes, d_sizes + ns, t.staging_bytes, d_bad,
+                                                                       d_bad + slot);
+    count_launch();
+    return cudaGetLastError();
+  };
+  VAL_TRY(check(pl->d_ch_staged, t.n_chunks_staged, 1, 1));
+  VAL_TRY(check(pl->d_ch_local, t.n_chunks_local, 0, 2));
+  VAL_TRY(check(pl->d_ch1, t.n_chunks_staged + t.n_chunks_local, -1, 3));
+  VAL_TRY(check(pl->d_ch2, t.n_chunks_staged, 1, 4));
+  VAL_TRY(check(pl->d_rch1, t.n_chunks_staged + t.n_chunks_local, -1, 5));
+  VAL_TRY(check(pl->d_rch2, t.n_chunks_staged, 1, 6));
+  unsigned long long h[7] = {0, 0, 0, 0, 0, 0, 0};
+  VAL_TRY(cudaMemcpyAsync(h, d_bad, sizeof(h), cudaMemcpyDeviceToHost, st));
   VAL_TRY(cudaStreamSynchronize(st));
+  // the ordered lists must hold exactly the plan's chunks (order-independent checksums)
+  if (pl->d_ch1 && h[3] != h[1] + h[2]) h[0] += 1;
+  if (pl->d_ch2 && t.n_chunks_staged && h[4] != h[1]) h[0] += 1;
+  if (pl->d_rch1 && h[5] != h[1] + h[2]) h[0] += 1;
+  if (pl->d_rch2 && t.n_chunks_staged && h[6] != h[1]) h[0] += 1;
+  const unsigned long long h_bad = h[0];
 #undef VAL_TRY
   *n_bad = (int64_t)h_bad;
   return done(ETC_OK);

@@ -40,8 +40,9 @@ struct Chunk {
   int32_t row_bytes, nrows;
   uint16_t src_buf, dst_buf;           // pointer-table indices: device*4 + kind
   int16_t vec;                         // widest power-of-two access (<= 16 B) every address of the chunk is aligned to
-  int16_t pad;
+  int16_t pad;                         // 0 in the plan's lists; CHUNK_STAGED marks staged chunks in the ordered launch-1 list
 };
+constexpr int16_t CHUNK_STAGED = 1;
 static_assert(sizeof(Chunk) == 48, "Chunk layout");
 
 // One round of state chunking: a contiguous range of staged chunks whose staging footprint fits the
@@ -64,6 +65,9 @@ cudaError_t plan_use(const etc_plan* pl, cudaStream_t st);
 // The plan's totals on the host.  For an ETC_NO_SYNC plan the first call waits for the plan's kernels and reads them
 // back; *rc receives ETC_ERR_BAD_MAP / ETC_ERR_UNRECOVERABLE / ETC_ERR_WORKSPACE if the device found the plan unusable.
 const PlanTotals& plan_totals(const etc_plan* pl, etc_status* rc = nullptr);
+// plan_order.cu: the address-ordered launch lists of a plan whose chunk counts (nA staged, nB local) the host knows
+cudaError_t plan_build_order(etc_plan* pl, long long nA, long long nB, cudaStream_t st);
+cudaError_t plan_build_round_order(etc_plan* pl, cudaStream_t st);     // after etc_plan_set_rounds filled pl->rounds
 }
 
 struct etc_plan {
@@ -87,6 +91,14 @@ struct etc_plan {
   etc::PlanTotals* d_totals = nullptr;
   etc_slice* d_sl_staged = nullptr; etc_slice* d_sl_local = nullptr;
   etc::Chunk* d_ch_staged = nullptr; etc::Chunk* d_ch_local = nullptr;
+  // address-ordered launch lists (plan_order.cu), or null (launch in list order): d_ch1 = every chunk of launch 1 (staged
+  // ones flagged CHUNK_STAGED in `pad`, then packed; the others copied old -> new buffer) sorted by source address,
+  // d_ch2 = the staged chunks sorted by destination address for launch 2
+  etc::Chunk* d_ch1 = nullptr; etc::Chunk* d_ch2 = nullptr;
+  void* d_order_ws = nullptr;
+  // the same per round (etc_plan_set_rounds): round i walks d_rch1[ca + la, cb + lb) and d_rch2[ca, cb)
+  etc::Chunk* d_rch1 = nullptr; etc::Chunk* d_rch2 = nullptr;
+  void* d_round_order_ws = nullptr;
   etc_slice* d_fills = nullptr;                    // zero-fill descriptors (in d_ws; totals.n_fills of them), reading A31
   std::vector<int64_t> old_bytes, new_bytes;       // buffer sizes [dev*4+kind], for argument checks in migrate
   void** d_ptrs = nullptr;                         // [n_old*4] source pointers then [n_new*4] destination pointers

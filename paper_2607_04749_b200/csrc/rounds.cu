@@ -92,6 +92,7 @@ extern "C" etc_status etc_plan_set_rounds(etc_plan* pl, int64_t max_staging_byte
   }
   const size_t R = specs.size();
   if (pl->d_rounds_ws) { cudaFreeAsync(pl->d_rounds_ws, pl->streams.join(st)); pl->d_rounds_ws = nullptr; pl->d_round_ptrs = nullptr; }
+  if (pl->d_round_order_ws) { cudaFreeAsync(pl->d_round_order_ws, pl->streams.join(st)); pl->d_round_order_ws = nullptr; pl->d_rch1 = pl->d_rch2 = nullptr; }
   ETC_CUDA_TRY(plan_use(pl, st));
   pl->rounds.clear(); pl->round_staging_cap = max_staging_bytes;
   *n_rounds = (int32_t)R;
@@ -124,6 +125,7 @@ extern "C" etc_status etc_plan_set_rounds(etc_plan* pl, int64_t max_staging_byte
   }
   for (size_t i = 0; i < R; ++i) { got[i].kind = recs[i].kind; got[i].sub = recs[i].sub; got[i].n_sub = recs[i].n_sub; }
   pl->rounds = std::move(got);
+  ETC_CUDA_TRY(plan_build_round_order(pl, st));                // each round's launch lists in address order (plan_order.cu)
   return ETC_OK;
 }
 
