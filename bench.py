@@ -451,6 +451,27 @@ def all_staged_rates(E, torch, R, peak):
     return out
 
 
+def list_order_rates(E, torch, R, peak, flags):
+    """The two copy launches of the resident workload with ETC_NO_REORDER (chunk lists walked unit by unit instead of in
+    address order): the A/B figure for csrc/plan_order.cu, same buffers, same map, CUDA events on the launching stream."""
+    ev, stream = R.ev, R.stream
+    ov, _, _ = E.etc_cost_matrix(R.lay_old, R.lay_new, out=R.out_cost)
+    dm, _ = E.etc_sketch(ov, out=R.out_sk)
+    plan = E.etc_plan_create(R.lay_old, R.lay_new, dm, flags | E.ETC_NO_REORDER)
+    t1, t2 = [], []
+    for i in range(6):
+        a, b, c = ev(), ev(), ev()
+        a.record(stream); E.etc_migrate(plan, R.src_tab, R.dst_tab, R.staging, E.ETC_PHASE_PACK, stream=stream)
+        b.record(stream); E.etc_migrate(plan, R.src_tab, R.dst_tab, R.staging, E.ETC_PHASE_UNPACK, stream=stream)
+        c.record(stream)
+        torch.cuda.synchronize()
+        if i >= 2:
+            t1.append(a.elapsed_time(b)); t2.append(b.elapsed_time(c))
+    b1, b2 = copy_launch_bytes(plan.stats)
+    return {"pack_local_list_order": kernel_entry(b1, statistics.mean(t1), peak),
+            "unpack_list_order": kernel_entry(b2, statistics.mean(t2), peak)}
+
+
 def config_entry(res, peak, one_shot_ms=None):
     st, bd = res["stats"], res["breakdown"]
     b1, b2 = copy_launch_bytes(st)
@@ -516,6 +537,13 @@ def run_cuda(args, w):
                 "per_kernel": per_kernel}
     for key, kn in (("pack_local", "migrate_copy_kernel<false>"), ("unpack", "migrate_copy_kernel<true>")):
         per_kernel[key]["traffic"] = ncu_traffic(w["name"], mode, kn)
+        if per_kernel[key]["traffic"] and per_kernel[key]["ms"]:
+            # physical DRAM rate: below the algorithmic rate where source ranges that several new ranks need are read
+            # from DRAM once and shared in L2 (address-ordered launch, csrc/plan_order.cu)
+            per_kernel[key]["dram_GBs"] = per_kernel[key]["traffic"] / per_kernel[key]["ms"] / 1e6
+            per_kernel[key]["dram_frac"] = per_kernel[key]["dram_GBs"] / peak
+    roofline["launch_order"] = "list order (ETC_NO_REORDER)" if args.no_reorder else \
+        "address order: launch 1 by source address, launch 2 by destination address (csrc/plan_order.cu)"
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -537,6 +565,11 @@ def run_cuda(args, w):
             line["one_shot_error"] = repr(ex)[:160]
     per_config = {w["name"]: config_entry(res, peak, one)}
     if extras_on:
+        if not args.no_reorder:
+            try:
+                per_kernel.update(list_order_rates(E, torch, R, peak, flags))
+            except Exception as ex:
+                per_kernel["list_order_error"] = repr(ex)[:160]
         if not args.all_staged:
             try:
                 per_kernel.update(all_staged_rates(E, torch, R, peak))
