@@ -186,9 +186,10 @@ class Layout:
         lt, _, row, col = self.global_of(dev, kind)
         dt = np.uint16 if self.elem_bytes(kind) == 2 else np.uint32
         out = np.zeros(lt.shape[0], dt)
-        for t in np.unique(lt):
-            sel = lt == t
-            out[sel] = logical[t][row[sel], col[sel]]
+        # the buffer is a concatenation of tensor shards: one gather per run of equal tensor id
+        cuts = np.concatenate(([0], np.flatnonzero(np.diff(lt)) + 1, [lt.shape[0]])) if lt.shape[0] else np.zeros(1, np.int64)
+        for a, b in zip(cuts[:-1], cuts[1:]):
+            out[a:b] = logical[int(lt[a])][row[a:b], col[a:b]]
         return out
 
 

@@ -55,7 +55,7 @@ import json
 _MEMO: "collections.OrderedDict" = collections.OrderedDict()
 
 
-def _memo(key, fn, keep=10):
+def _memo(key, fn, keep=16):
     if key in _MEMO:
         _MEMO.move_to_end(key)
         return _MEMO[key]
