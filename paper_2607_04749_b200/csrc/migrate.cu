@@ -198,9 +198,9 @@ extern "C" etc_status etc_migrate_phase(const etc_plan* pl, const void* const* s
     const long long nb = pl->bound_chunks;
     if (phases == ETC_PHASE_UNPACK)
       return launch_migrate(pl, src_bufs, dst_bufs, staging, phases, (cudaStream_t)stream, pl->d_ptrs, -1, 0, nb, 0, 0, 0, 0,
-                            false, 0, pl->d_totals);
+                            false, 0, pl->d_totals, pl->d_ch1, pl->d_ch2);
     return launch_migrate(pl, src_bufs, dst_bufs, staging, phases, (cudaStream_t)stream, pl->d_ptrs, -1, 0, direct ? 0 : nb, 0,
-                          direct ? nb : 0, 0, 0, true, pl->bound_fills, pl->d_totals);
+                          direct ? nb : 0, 0, 0, true, pl->bound_fills, pl->d_totals, pl->d_ch1, pl->d_ch2);
   }
   etc_status rc = ETC_OK;
   const PlanTotals& t = plan_totals(pl, &rc);

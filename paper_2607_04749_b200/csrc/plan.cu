@@ -514,6 +514,7 @@ extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout*
 //   chunks (per list): every slice ends in at most one short chunk, and every other chunk carries more than
 //           ETC_CHUNK_BYTES / 2 bytes — or, on the re-aligning path, more than 4 KB (rows_per_chunk);
 //   staging: payload + 16 bytes of padding per slice + 512 per (kind, source, destination) segment.
+constexpr int64_t ORDER_MIN_LAZY_BYTES = 128ll << 20;      // about the size of the L2: below it DRAM locality is moot
 static void plan_bounds(const etc_layout* old_l, const etc_layout* new_l, int K, etc_plan* pl) {
   const int nT = old_l->t.n_tensors;
   const bool old_sharded = old_l->cfg.dist_opt && old_l->cfg.dp > 1;
@@ -661,8 +662,11 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
     PLAN_TRY(cudaGetLastError());
     count_launch();
   }
-  // the launch lists in address order (plan_order.cu); bound-sized ETC_NO_SYNC plans launch in list order
-  if (!lazy && !(flags & ETC_NO_REORDER)) PLAN_TRY(plan_build_order(pl, n_ch_s, n_ch_l, st));
+  // the launch lists in address order (plan_order.cu).  A bound-sized ETC_NO_SYNC plan gets them only if it moves enough
+  // for the order to matter (a state that fits the L2 gains nothing; its four extra launches would be a tenth of
+  // the whole migration)
+  if (!(flags & ETC_NO_REORDER) && (!lazy || pl->need_bytes >= ORDER_MIN_LAZY_BYTES))
+    PLAN_TRY(plan_build_order(pl, n_ch_s, n_ch_l, st, lazy ? pl->d_totals : nullptr));
   // the tables are complete once `st` reaches this point: readers on other streams wait for it (plan_use)
   PLAN_TRY(cudaEventCreateWithFlags(&pl->ready, cudaEventDisableTiming));
   PLAN_TRY(cudaEventRecord(pl->ready, st));

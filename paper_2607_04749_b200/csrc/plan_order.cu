@@ -35,8 +35,9 @@ __global__ void __launch_bounds__(ORD_THREADS)
 order_hist_kernel(const Chunk* __restrict__ chA, long long nA, const Chunk* __restrict__ chB, long long nB,
                   const int64_t* __restrict__ obase, const int64_t* __restrict__ nbase, int shift1, int shift2,
                   uint32_t* __restrict__ bins1, uint32_t* __restrict__ bins2, uint32_t* __restrict__ rank1,
-                  uint32_t* __restrict__ rank2) {
+                  uint32_t* __restrict__ rank2, const PlanTotals* __restrict__ lazy) {
   const long long i = (long long)blockIdx.x * ORD_THREADS + threadIdx.x;
+  if (lazy) { nA = lazy->n_chunks_staged; nB = lazy->n_chunks_local; }   // ETC_NO_SYNC: the grid is an upper bound
   if (i >= nA + nB) return;
   const Chunk* c = i < nA ? chA + i : chB + (i - nA);
   const int sb = c->src_buf; const int64_t so = c->src_off;
@@ -98,8 +99,9 @@ order_scatter_kernel(const Chunk* __restrict__ chA, long long nA, const Chunk* _
                      const int64_t* __restrict__ obase, const int64_t* __restrict__ nbase, int shift1, int shift2,
                      const uint32_t* __restrict__ bins1, const uint32_t* __restrict__ bins2,
                      const uint32_t* __restrict__ rank1, const uint32_t* __restrict__ rank2, Chunk* __restrict__ out1,
-                     Chunk* __restrict__ out2) {
+                     Chunk* __restrict__ out2, const PlanTotals* __restrict__ lazy) {
   const long long i = (long long)blockIdx.x * ORD_THREADS + threadIdx.x;
+  if (lazy) { nA = lazy->n_chunks_staged; nB = lazy->n_chunks_local; }
   if (i >= nA + nB) return;
   Chunk c = i < nA ? chA[i] : chB[i - nA];
   if (i < nA) out2[bins2[bin_of(nbase, c.dst_buf, c.dst_off, shift2)] - (uint32_t)(nA + nB) + rank2[i]] = c;
@@ -133,7 +135,7 @@ static cudaError_t scratch_make(const etc_plan* pl, long long max_a, long long m
   s.shift1 = pick_shift(pl->old_bytes, ob, s.n1); s.shift2 = pick_shift(pl->new_bytes, nb, s.n2);
   const long long n_bins = s.n1 + s.n2, n_tiles = (n_bins + SCAN_TILE - 1) / SCAN_TILE;
   auto al = [](size_t x) { return (x + 255) & ~size_t(255); };
-  const size_t o_ob = 0, o_nb = o_ob + al(sizeof(int64_t) * ob.size()), o_bins = o_nb + al(sizeof(int64_t) * nb.size()),
+  const size_t o_ob = 0, o_nb = o_ob + sizeof(int64_t) * ob.size(), o_bins = al(o_nb + sizeof(int64_t) * nb.size()),
                o_sums = o_bins + al(sizeof(uint32_t) * (size_t)n_bins), o_r1 = o_sums + al(sizeof(uint32_t) * (size_t)n_tiles),
                o_r2 = o_r1 + al(sizeof(uint32_t) * (size_t)max_ab), bytes = o_r2 + al(sizeof(uint32_t) * (size_t)max_a);
   cudaError_t e = cudaMallocAsync(&s.tmp, bytes, st);
@@ -141,41 +143,46 @@ static cudaError_t scratch_make(const etc_plan* pl, long long max_a, long long m
   s.d_ob = reinterpret_cast<int64_t*>(s.tmp + o_ob); s.d_nb = reinterpret_cast<int64_t*>(s.tmp + o_nb);
   s.bins = reinterpret_cast<uint32_t*>(s.tmp + o_bins); s.sums = reinterpret_cast<uint32_t*>(s.tmp + o_sums);
   s.r1 = reinterpret_cast<uint32_t*>(s.tmp + o_r1); s.r2 = reinterpret_cast<uint32_t*>(s.tmp + o_r2);
-  if ((e = write_small(s.d_ob, ob.data(), sizeof(int64_t) * ob.size(), st)) != cudaSuccess) return e;
-  return write_small(s.d_nb, nb.data(), sizeof(int64_t) * nb.size(), st);
+  ob.insert(ob.end(), nb.begin(), nb.end());                     // both base tables in one upload
+  return write_small(s.d_ob, ob.data(), sizeof(int64_t) * ob.size(), st);
 }
 
 // Sort one range: staged chunks chA[0,nA), local chunks chB[0,nB) -> out1[0,nA+nB) by source address, out2[0,nA) by
 // destination address.
 static cudaError_t order_range(const OrderScratch& s, const Chunk* chA, long long nA, const Chunk* chB, long long nB,
-                               Chunk* out1, Chunk* out2, cudaStream_t st) {
-  if (nA + nB == 0) return cudaSuccess;
+                               Chunk* out1, Chunk* out2, cudaStream_t st, const PlanTotals* lazy = nullptr,
+                               long long bound = 0) {
+  if (!lazy && nA + nB == 0) return cudaSuccess;
   const long long n_bins = s.n1 + s.n2, n_tiles = (n_bins + SCAN_TILE - 1) / SCAN_TILE;
   cudaError_t e = cudaMemsetAsync(s.bins, 0, sizeof(uint32_t) * (size_t)n_bins, st);
   if (e != cudaSuccess) return e;
-  const unsigned grid = (unsigned)((nA + nB + ORD_THREADS - 1) / ORD_THREADS);
+  const unsigned grid = (unsigned)(((lazy ? bound : nA + nB) + ORD_THREADS - 1) / ORD_THREADS);
   order_hist_kernel<<<grid, ORD_THREADS, 0, st>>>(chA, nA, chB, nB, s.d_ob, s.d_nb, s.shift1, s.shift2, s.bins, s.bins + s.n1,
-                                                   s.r1, s.r2);
+                                                   s.r1, s.r2, lazy);
   order_tile_sums_kernel<<<(unsigned)n_tiles, 1024, 0, st>>>(s.bins, n_bins, s.sums);
   order_scan_kernel<<<(unsigned)n_tiles, 1024, 0, st>>>(s.bins, n_bins, s.sums);
   order_scatter_kernel<<<grid, ORD_THREADS, 0, st>>>(chA, nA, chB, nB, s.d_ob, s.d_nb, s.shift1, s.shift2, s.bins, s.bins + s.n1,
-                                                      s.r1, s.r2, out1, out2);
+                                                      s.r1, s.r2, out1, out2, lazy);
   count_launch(4);
   return cudaGetLastError();
 }
 
 static size_t list_bytes(long long n) { return ((sizeof(Chunk) * (size_t)n) + 255) & ~size_t(255); }
 
-// Build pl->d_ch1 / pl->d_ch2 from the finished chunk lists on `st` (counts known on the host: not for ETC_NO_SYNC plans).
-cudaError_t plan_build_order(etc_plan* pl, long long nA, long long nB, cudaStream_t st) {
+// Build pl->d_ch1 / pl->d_ch2 from the finished chunk lists on `st`.  nA, nB: the chunk counts — or, for an ETC_NO_SYNC
+// plan (`lazy` = its device-side totals), the bound both lists together stay below: grids and lists are then sized by
+// the bound and the kernels read the counts from `lazy`.
+cudaError_t plan_build_order(etc_plan* pl, long long nA, long long nB, cudaStream_t st, const PlanTotals* lazy) {
+  if (lazy) nA = nB = std::max(nA, nB);
   if (nA + nB == 0 || nA + nB >= (1ll << 32)) return cudaSuccess;
-  cudaError_t e = cudaMallocAsync(&pl->d_order_ws, list_bytes(nA + nB) + list_bytes(nA), st);
+  const long long n1 = lazy ? nA : nA + nB;                      // capacity of list 1
+  cudaError_t e = cudaMallocAsync(&pl->d_order_ws, list_bytes(n1) + list_bytes(nA), st);
   if (e != cudaSuccess) return e;
   Chunk* out1 = static_cast<Chunk*>(pl->d_order_ws);
-  Chunk* out2 = reinterpret_cast<Chunk*>(static_cast<char*>(pl->d_order_ws) + list_bytes(nA + nB));
+  Chunk* out2 = reinterpret_cast<Chunk*>(static_cast<char*>(pl->d_order_ws) + list_bytes(n1));
   OrderScratch s;
-  e = scratch_make(pl, nA, nA + nB, st, s);
-  if (e == cudaSuccess) e = order_range(s, pl->d_ch_staged, nA, pl->d_ch_local, nB, out1, out2, st);
+  e = scratch_make(pl, nA, n1, st, s);
+  if (e == cudaSuccess) e = order_range(s, pl->d_ch_staged, nA, pl->d_ch_local, nB, out1, out2, st, lazy, n1);
   if (s.tmp) cudaFreeAsync(s.tmp, st);
   if (e == cudaSuccess) { pl->d_ch1 = out1; pl->d_ch2 = out2; }
   return e;

@@ -65,8 +65,9 @@ cudaError_t plan_use(const etc_plan* pl, cudaStream_t st);
 // The plan's totals on the host.  For an ETC_NO_SYNC plan the first call waits for the plan's kernels and reads them
 // back; *rc receives ETC_ERR_BAD_MAP / ETC_ERR_UNRECOVERABLE / ETC_ERR_WORKSPACE if the device found the plan unusable.
 const PlanTotals& plan_totals(const etc_plan* pl, etc_status* rc = nullptr);
-// plan_order.cu: the address-ordered launch lists of a plan whose chunk counts (nA staged, nB local) the host knows
-cudaError_t plan_build_order(etc_plan* pl, long long nA, long long nB, cudaStream_t st);
+// plan_order.cu: the address-ordered launch lists of a plan (nA staged, nB local chunks; for an ETC_NO_SYNC plan their
+// common bound and the device-side totals)
+cudaError_t plan_build_order(etc_plan* pl, long long nA, long long nB, cudaStream_t st, const etc::PlanTotals* lazy = nullptr);
 cudaError_t plan_build_round_order(etc_plan* pl, cudaStream_t st);     // after etc_plan_set_rounds filled pl->rounds
 }
 

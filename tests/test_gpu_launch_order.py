@@ -62,6 +62,32 @@ def _plan(E, w, flags, device_map=None):
 def test_ordered_lists_are_sorted_permutations(E, name, flags):
     w = workload(name)
     old, new, plan = _plan(E, w, flags)
+    _check_lists(plan, new)
+
+
+@pytest.mark.parametrize("name", ["s3", "s5"])
+@pytest.mark.parametrize("flags", [0, 1])
+def test_no_sync_plans_keep_ordered_lists_when_the_state_exceeds_l2(E, name, flags):
+    """A bound-sized ETC_NO_SYNC plan sorts with bound-sized grids and device-side counts (states of 128 MB and more)."""
+    w = workload(name)
+    old, new, plan = _plan(E, w, flags | E.ETC_NO_SYNC)
+    assert new.total_bytes() >= 128 << 20
+    _check_lists(plan, new)
+    # and the migration through them == oracle
+    oo, on = O.Layout(w["model"], w["old"]), O.Layout(w["model"], w["new"])
+    src_np = sharded_payload(oo, w["seed"], "stamp")
+    src, dst = upload(src_np), E.alloc_buffers(new, fill=0x4D)
+    staging = torch.full((max(E.etc_staging_bound(old, new, flags), 16),), 0x4D, dtype=torch.uint8, device="cuda")
+    E.etc_migrate(plan, src, dst, staging)
+    torch.cuda.synchronize()
+    exp, T, _ = oracle_migrate(oo, on, plan.device_map(), src_np)
+    assert np.array_equal(plan.traffic(), T)
+    for (n, k), e in exp.items():
+        if e.shape[0]:
+            assert np.array_equal(download(dst[(n, k)], e.itemsize), e), (n, k)
+
+
+def _check_lists(plan, new):
     st = plan.stats
     a, b = plan.chunks(0), plan.chunks(1)
     l1, l2 = plan.chunks(2), plan.chunks(3)

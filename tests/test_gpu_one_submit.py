@@ -53,7 +53,9 @@ def test_no_sync_plan_vs_oracle_and_vs_synchronising_plan(E, name, flags):
     E.etc_migrate(plan, src, dst, staging)                    # enqueued before any count has reached the host
     assert plan._stats is None
     torch.cuda.synchronize()
-    assert E.kernel_launches() - launches0 <= 9
+    # count, scan, fill, two copy launches, table uploads; + base-table upload and 4 sort launches when the state is big
+    # enough for the plan to keep address-ordered launch lists (csrc/plan_order.cu)
+    assert E.kernel_launches() - launches0 <= (14 if new.total_bytes() >= 128 << 20 else 9)
     exp, T, _ = oracle_migrate(oo, on, dm.cpu().numpy(), src_np)
     _compare(on, dst, exp, name)
     a, b = plan.stats, ref.stats
