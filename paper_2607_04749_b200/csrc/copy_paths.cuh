@@ -14,8 +14,9 @@
 //     * the byte-phase re-aligning path: every source row is loaded as the 16-byte ALIGNED slots that cover it (cp.async
 //       16 B; up to 15 bytes before and after the row are read and dropped — inside the 16-byte granule of the buffer,
 //       whose base is 16-byte aligned), row r of the tile starts at the row's phase (address mod 16), and every aligned
-//       16-byte slot of the DESTINATION row is assembled from five aligned 32-bit shared-memory words with funnel shifts
-//       and written with one 16-byte store; only the ragged ends of a row use narrow stores.
+//       16-byte slot of the DESTINATION row is assembled from the two aligned 16-byte tile slots that cover it (two
+//       LDS.128, word selects, funnel shifts) and written with one 16-byte store; only the ragged ends of a row use
+//       narrow stores.
 #pragma once
 #include <cstdint>
 #include "plan_types.h"
@@ -159,15 +160,27 @@ __device__ __forceinline__ void realign_copy_chunk(char* tile, const char* __res
     const int32_t lo = max((int32_t)(k << 4) - (int32_t)dphase, 0);                       // row bytes [lo, hi) of this slot
     const int32_t hi = min((int32_t)(k << 4) - (int32_t)dphase + 16, (int32_t)row_bytes);
     if (hi <= lo) continue;
-    const char* t = tile + (size_t)row * RP + sphase + lo;
+    const uint32_t toff = row * RP + sphase + (uint32_t)lo;     // tile offset of the first byte this slot needs
+    const char* t = tile + toff;
     char* d = reinterpret_cast<char*>(da) + lo;
     if (hi - lo == 16) {
-      const uint32_t sh = ((uint32_t)(uintptr_t)t & 3u) << 3;
-      const uint32_t* w = reinterpret_cast<const uint32_t*>(reinterpret_cast<uintptr_t>(t) & ~(uintptr_t)3);
-      const uint32_t w0 = w[0], w1 = w[1], w2 = w[2], w3 = w[3], w4 = w[4];
-      uint4 q;
-      q.x = __funnelshift_r(w0, w1, sh); q.y = __funnelshift_r(w1, w2, sh);
-      q.z = __funnelshift_r(w2, w3, sh); q.w = __funnelshift_r(w3, w4, sh);
+      // the 16 bytes [t, t+16) out of the two ALIGNED 16-byte tile slots that cover them: two conflict-free LDS.128
+      // (five LDS.32 at a 16-byte lane stride would be 4-way bank conflicts each), then words W[wi .. wi+4], wi = o / 4,
+      // picked by two rounds of selects (no divergence) and funnel-shifted by the byte remainder
+      const uint4* a = reinterpret_cast<const uint4*>(tile + (toff & ~15u));
+      const uint4 q0 = a[0];
+      const uint32_t o = toff & 15u;
+      uint4 q = q0;
+      if (o != 0) {
+        const uint4 q1 = a[1];
+        const uint32_t sh = (o & 3u) << 3;
+        const bool b1 = (o & 8u) != 0, b0 = (o & 4u) != 0;
+        const uint32_t v0 = b1 ? q0.z : q0.x, v1 = b1 ? q0.w : q0.y, v2 = b1 ? q1.x : q0.z, v3 = b1 ? q1.y : q0.w,
+                       v4 = b1 ? q1.z : q1.x, v5 = b1 ? q1.w : q1.y;
+        const uint32_t u0 = b0 ? v1 : v0, u1 = b0 ? v2 : v1, u2 = b0 ? v3 : v2, u3 = b0 ? v4 : v3, u4 = b0 ? v5 : v4;
+        q.x = __funnelshift_r(u0, u1, sh); q.y = __funnelshift_r(u1, u2, sh);
+        q.z = __funnelshift_r(u2, u3, sh); q.w = __funnelshift_r(u3, u4, sh);
+      }
       st_stream(reinterpret_cast<uint4*>(d), q);
     } else {                                            // ragged end of the row: the chunk's own alignment
       const int32_t n = hi - lo;
