@@ -299,30 +299,45 @@ plan_scan_kernel(const BlockCount* __restrict__ blocks, int B, long long U, int 
   }
 }
 
-// One copy work item of a slice: chunk k of slice s (see slice_chunks for the count).
-__device__ __forceinline__ Chunk cut_chunk(const etc_slice& s, int vec, long long k) {
-  Chunk ch;
-  ch.src_buf = (uint16_t)(s.src_dev * ETC_NUM_KINDS + s.kind); ch.dst_buf = (uint16_t)(s.dst_rank * ETC_NUM_KINDS + s.kind);
-  ch.src_stride = s.src_stride; ch.dst_stride = s.dst_stride; ch.pad = 0;
-  ch.vec = (int16_t)vec;
-  const int64_t stg = s.stg_off >= 0 ? s.stg_off : 0;
-  if (s.nrows == 1 || s.row_bytes >= ETC_CHUNK_BYTES) {
-    const long long cpr = (s.row_bytes + ETC_CHUNK_BYTES - 1) / ETC_CHUNK_BYTES;
-    const long long row = k / cpr; const int64_t b = (k % cpr) * ETC_CHUNK_BYTES;
-    ch.src_off = s.src_off + row * s.src_stride + b;
-    ch.dst_off = s.dst_off + row * s.dst_stride + b;
-    ch.stg_off = stg + row * s.row_bytes + b;
-    ch.nrows = 1; ch.row_bytes = (int32_t)min((int64_t)ETC_CHUNK_BYTES, s.row_bytes - b);
-  } else {
-    const int rpc = rows_per_chunk(s.row_bytes, vec == 16);
-    const long long row = k * rpc;
-    ch.src_off = s.src_off + row * s.src_stride;
-    ch.dst_off = s.dst_off + row * s.dst_stride;
-    ch.stg_off = stg + row * s.row_bytes;
-    ch.nrows = (int32_t)min((long long)rpc, s.nrows - row); ch.row_bytes = (int32_t)s.row_bytes;
+// The copy work items of one slice (see slice_chunks for the count).  Built once per slice — the divisions that depend on
+// the slice alone (rows per chunk, chunks per row) are done here, not once per chunk: a unit that keeps a whole
+// embedding shard local is a single slice of thousands of chunks, expanded by one warp.
+struct ChunkCutter {
+  Chunk proto;                 // fields every chunk of the slice shares
+  int64_t src_off, dst_off, stg_off, row_bytes;
+  int32_t src_stride, dst_stride, nrows;
+  uint32_t cpr;                // chunks per row (rows >= ETC_CHUNK_BYTES, or one contiguous run)
+  int rpc;                     // rows per chunk (shorter rows)
+  bool long_rows;
+  __device__ __forceinline__ ChunkCutter(const etc_slice& s, int vec) {
+    proto.src_buf = (uint16_t)(s.src_dev * ETC_NUM_KINDS + s.kind); proto.dst_buf = (uint16_t)(s.dst_rank * ETC_NUM_KINDS + s.kind);
+    proto.src_stride = s.src_stride; proto.dst_stride = s.dst_stride; proto.pad = 0; proto.vec = (int16_t)vec;
+    src_off = s.src_off; dst_off = s.dst_off; stg_off = s.stg_off >= 0 ? s.stg_off : 0; row_bytes = s.row_bytes;
+    src_stride = s.src_stride; dst_stride = s.dst_stride; nrows = s.nrows;
+    long_rows = s.nrows == 1 || s.row_bytes >= ETC_CHUNK_BYTES;
+    cpr = (uint32_t)((s.row_bytes + ETC_CHUNK_BYTES - 1) / ETC_CHUNK_BYTES);
+    rpc = long_rows ? 1 : rows_per_chunk(s.row_bytes, vec == 16);
   }
-  return ch;
-}
+  __device__ __forceinline__ Chunk cut(long long k) const {
+    Chunk ch = proto;
+    if (long_rows) {
+      long long row = 0; uint32_t part = (uint32_t)k;            // a single row: chunk k is its k-th part
+      if (nrows != 1) { row = k / cpr; part = (uint32_t)(k - row * cpr); }
+      const int64_t b = (int64_t)part * ETC_CHUNK_BYTES;
+      ch.src_off = src_off + row * src_stride + b;
+      ch.dst_off = dst_off + row * dst_stride + b;
+      ch.stg_off = stg_off + row * row_bytes + b;
+      ch.nrows = 1; ch.row_bytes = (int32_t)min((int64_t)ETC_CHUNK_BYTES, row_bytes - b);
+    } else {
+      const long long row = k * rpc;
+      ch.src_off = src_off + row * src_stride;
+      ch.dst_off = dst_off + row * dst_stride;
+      ch.stg_off = stg_off + row * row_bytes;
+      ch.nrows = (int32_t)min((long long)rpc, nrows - row); ch.row_bytes = (int32_t)row_bytes;
+    }
+    return ch;
+  }
+};
 
 // pass 2: recompute the slices of each (unit, sub-block), write the slice records at their final positions — unit base
 // (scan) + earlier sub-blocks of the unit + warp-level prefix inside the sub-block — and expand them into chunks: the
@@ -385,7 +400,8 @@ plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict
       SliceGeom g; g.src_off = s.src_off; g.dst_off = s.dst_off; g.row_bytes = s.row_bytes; g.src_stride = s.src_stride;
       g.dst_stride = s.dst_stride; g.nrows = s.nrows; g.kind = s.kind;
       const int64_t nch = slice_chunks(g);
-      for (int64_t k = lane; k < nch; k += 32) ch_out[c0 + k] = cut_chunk(s, vec, k);
+      const ChunkCutter cutter(s, vec);
+      for (int64_t k = lane; k < nch; k += 32) ch_out[c0 + k] = cutter.cut(k);
       c0 += nch;
     }
     run_sl += tot_sl; run_ch += tot_ch; run_stg += tot_pad;
