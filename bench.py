@@ -542,6 +542,13 @@ def run_cuda(args, w):
             # from DRAM once and shared in L2 (address-ordered launch, csrc/plan_order.cu)
             per_kernel[key]["dram_GBs"] = per_kernel[key]["traffic"] / per_kernel[key]["ms"] / 1e6
             per_kernel[key]["dram_frac"] = per_kernel[key]["dram_GBs"] / peak
+    if dom.get("traffic") and dom["traffic"] < 0.97 * dom["bytes"]:
+        roofline["note"] = ("achieved = ALGORITHMIC bytes / launch time; the launch's DRAM traffic (ncu, `traffic`) is %.3f of the "
+                            "algorithmic bytes because source ranges that several new ranks need (replicated state fanning out to "
+                            "more DP groups) are read from DRAM once and shared in L2 when the chunks are walked in source-address "
+                            "order; DRAM rate = %.0f GB/s = %.3f of peak (per_kernel.*.dram_GBs); the same launch in list order is "
+                            "per_kernel.pack_local_list_order" % (dom["traffic"] / dom["bytes"], dom["traffic"] / dom["ms"] / 1e6,
+                                                                    dom["traffic"] / dom["ms"] / 1e6 / peak))
     roofline["launch_order"] = "list order (ETC_NO_REORDER)" if args.no_reorder else \
         "address order: launch 1 by source address, launch 2 by destination address (csrc/plan_order.cu)"
 

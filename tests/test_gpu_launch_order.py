@@ -196,3 +196,23 @@ def test_rounds_walk_ordered_lists(E, name, cap):
     for (n, k), e in exp.items():
         if e.shape[0]:
             assert np.array_equal(d1[(n, k)].view(e.dtype), e), (n, k)
+
+
+def test_ordered_lists_of_the_512_to_384_device_layout(E):
+    """c5b (3.95 TB of virtual state, metadata only): 45 M chunks, more than 4 M 64 KB blocks, so the sort uses coarser
+    address bins (1 MB here) — the lists must still be bounds-checked permutations in (coarser) address order."""
+    w = workload("c5b")
+    old, new, plan = _plan(E, w, E.ETC_ALL_STAGED)
+    st = plan.stats
+    assert st.n_chunks_staged > 40_000_000 and st.remote_bytes == 0 and st.local_bytes == new.total_bytes()
+    assert plan.validate() == 0                       # bounds + permutation checksums of both ordered lists
+    assert old.total_bytes() >> 16 > 1 << 22           # more 64 KB blocks than the sort has bins: coarser bins
+    shift = 23                                        # 16 MB blocks: coarser than any bin size the sort may pick here
+    l1 = plan.chunks(2)
+    assert l1.shape[0] == st.n_chunks_staged and bool(l1["staged"].all())
+    key = l1["src_buf"].astype(np.int64) * (1 << 44) + (l1["src_off"].astype(np.int64) >> (shift + 1))
+    assert np.all(np.diff(key) >= 0)
+    del l1, key
+    l2 = plan.chunks(3)
+    key = l2["dst_buf"].astype(np.int64) * (1 << 44) + (l2["dst_off"].astype(np.int64) >> (shift + 1))
+    assert np.all(np.diff(key) >= 0)
