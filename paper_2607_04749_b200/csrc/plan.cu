@@ -309,6 +309,21 @@ struct ChunkCutter {
   uint32_t cpr;                // chunks per row (rows >= ETC_CHUNK_BYTES, or one contiguous run)
   int rpc;                     // rows per chunk (shorter rows)
   bool long_rows;
+  __device__ __forceinline__ ChunkCutter() {}
+  // the cutter that lane `from` holds, in every lane of the warp
+  __device__ __forceinline__ ChunkCutter bcast(int from) const {
+    const unsigned m = 0xffffffffu;
+    ChunkCutter c;
+    c.proto.src_buf = (uint16_t)__shfl_sync(m, (int)proto.src_buf, from); c.proto.dst_buf = (uint16_t)__shfl_sync(m, (int)proto.dst_buf, from);
+    c.proto.vec = (int16_t)__shfl_sync(m, (int)proto.vec, from); c.proto.pad = 0;
+    c.src_off = __shfl_sync(m, (long long)src_off, from); c.dst_off = __shfl_sync(m, (long long)dst_off, from);
+    c.stg_off = __shfl_sync(m, (long long)stg_off, from); c.row_bytes = __shfl_sync(m, (long long)row_bytes, from);
+    c.src_stride = __shfl_sync(m, src_stride, from); c.dst_stride = __shfl_sync(m, dst_stride, from);
+    c.proto.src_stride = c.src_stride; c.proto.dst_stride = c.dst_stride;
+    c.nrows = __shfl_sync(m, nrows, from); c.cpr = __shfl_sync(m, cpr, from); c.rpc = __shfl_sync(m, rpc, from);
+    c.long_rows = __shfl_sync(m, (int)long_rows, from) != 0;
+    return c;
+  }
   __device__ __forceinline__ ChunkCutter(const etc_slice& s, int vec) {
     proto.src_buf = (uint16_t)(s.src_dev * ETC_NUM_KINDS + s.kind); proto.dst_buf = (uint16_t)(s.dst_rank * ETC_NUM_KINDS + s.kind);
     proto.src_stride = s.src_stride; proto.dst_stride = s.dst_stride; proto.pad = 0; proto.vec = (int16_t)vec;
@@ -392,17 +407,30 @@ plan_fill_kernel(DeviceTables oldT, DeviceTables newT, const int32_t* __restrict
     }
     // chunk expansion of the slices [run_sl, run_sl + tot_sl) this iteration wrote, whose chunks are
     // [run_ch, run_ch + tot_ch) in the same order
+    // 32 slices at a time: every lane reads ONE of the records (written by a lane of this warp just above) and works out
+    // its chunk count and cutter — the divisions of 32 slices side by side — then the warp takes the slices in turn,
+    // the cutter handed round by shuffles, and the 32 lanes cut chunk k, k + 32, ... of it
     __syncwarp();
     int64_t c0 = run_ch;
-    for (int64_t j = 0; j < tot_sl; ++j) {
-      const etc_slice s = sl_out[run_sl + j];                   // written by a lane of this warp just above
-      const int vec = slice_vec(s.src_off, s.dst_off, s.row_bytes, s.src_stride, s.dst_stride, s.nrows);
-      SliceGeom g; g.src_off = s.src_off; g.dst_off = s.dst_off; g.row_bytes = s.row_bytes; g.src_stride = s.src_stride;
-      g.dst_stride = s.dst_stride; g.nrows = s.nrows; g.kind = s.kind;
-      const int64_t nch = slice_chunks(g);
-      const ChunkCutter cutter(s, vec);
-      for (int64_t k = lane; k < nch; k += 32) ch_out[c0 + k] = cutter.cut(k);
-      c0 += nch;
+    for (int64_t jb = 0; jb < tot_sl; jb += 32) {
+      const int nb = (int)min((int64_t)32, tot_sl - jb);
+      ChunkCutter mine; long long my_n = 0;
+      if (lane < nb) {
+        const etc_slice s = sl_out[run_sl + jb + lane];
+        const int vec = slice_vec(s.src_off, s.dst_off, s.row_bytes, s.src_stride, s.dst_stride, s.nrows);
+        SliceGeom g; g.src_off = s.src_off; g.dst_off = s.dst_off; g.row_bytes = s.row_bytes; g.src_stride = s.src_stride;
+        g.dst_stride = s.dst_stride; g.nrows = s.nrows; g.kind = s.kind;
+        my_n = slice_chunks(g);
+        mine = ChunkCutter(s, vec);
+      } else {
+        mine = ChunkCutter(etc_slice{0, 0, 0, 16, 16, 16, 1, 0, 0, 0, 0, 0}, 16);   // unused filler with defined fields
+      }
+      for (int j = 0; j < nb; ++j) {
+        const long long nch = __shfl_sync(0xffffffffu, my_n, j);
+        const ChunkCutter cutter = mine.bcast(j);
+        for (long long k = lane; k < nch; k += 32) ch_out[c0 + k] = cutter.cut(k);
+        c0 += nch;
+      }
     }
     run_sl += tot_sl; run_ch += tot_ch; run_stg += tot_pad;
   }
