@@ -170,8 +170,9 @@ enum { ETC_LOCAL_DIRECT = 0, ETC_ALL_STAGED = 1, ETC_KIND_MAJOR = 2, ETC_ALL_DIR
  * (the exact size is not known to the host).  A bad device map, an unrecoverable failure mask or (never observed) a
  * bound that falls short is detected ON THE DEVICE: the plan then copies nothing, and the error is reported by the
  * first call that needs the counts on the host — etc_plan_get_stats (which waits for the plan's kernels), and likewise
- * etc_plan_get_traffic / _slices / _fills / etc_plan_set_rounds / etc_plan_validate.  A hint: plans whose bound-sized
- * tables would exceed 64 MB are made the synchronising way (their copy kernels dwarf one host sync).
+ * etc_plan_get_traffic / _slices / _fills / etc_plan_set_rounds / etc_plan_validate.  A hint: plans whose bound exceeds
+ * 32 768 copy work items (states beyond ~1 GB) are made the synchronising way — their copy kernels dwarf one host sync,
+ * and the surplus CTAs of a bound-sized grid would cost more than it.
  * Launch order.  A plan whose counts the host knows (every plan but a bound-sized ETC_NO_SYNC one) also keeps its copy
  * work items in ADDRESS order — launch 1 (pack + local) by source address, launch 2 (unpack) by destination address —
  * and etc_migrate / etc_migrate_phase walk those lists: work items that read interleaved column blocks of the same

@@ -312,7 +312,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
               p.dev = dev; p.grp += dgrp; p.d = (int16_t)d; p.boff = p.boff / tm.es * es;
               if (p.grp != prev_grp) { first[(size_t)dev * nG + p.grp] = (int32_t)np; prev_grp = p.grp; }
               grp_pieces[(size_t)p.grp] += 1;
-              align_or |= p.boff | ((int64_t)p.W * es) | ((int64_t)p.c0 * es) | ((int64_t)p.nc * es) | (p.f1 * es);
+              if (p.W > 1) align_or |= p.boff | ((int64_t)p.W * es) | ((int64_t)p.c0 * es) | ((int64_t)p.nc * es) | (p.f1 * es);
               ++np;
             }
             n_emb_pieces += tm.emb;
@@ -367,7 +367,9 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
               p.rep = q.rep[blk]; p.rbase = q.rbase[blk];
               p.boff = (q.start + i0 * q.W + j0 - lo) * es;
               p.f0 = a; p.f1 = b;
-              align_or |= p.boff | ((int64_t)p.W * es) | ((int64_t)p.c0 * es) | ((int64_t)p.nc * es) | (a * es) | (b * es);
+              // a one-column tensor (a bias stored n x 1) cannot be cut by columns: its slices are contiguous runs whatever
+              // their alignment, so it does not count (see etc_layout::aligned16)
+              if (p.W > 1) align_or |= p.boff | ((int64_t)p.W * es) | ((int64_t)p.c0 * es) | ((int64_t)p.nc * es) | (a * es) | (b * es);
             }
             grp_pieces[(size_t)grp] += (int32_t)(np - np_before);
             if (q.lt == 0 || (!m.tied_embeddings && q.lt == nT - 1)) n_emb_pieces += (int32_t)(np - np_before);

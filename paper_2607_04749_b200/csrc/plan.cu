@@ -558,6 +558,7 @@ extern "C" etc_status etc_plan_create(const etc_layout* old_l, const etc_layout*
 //   chunks (per list): every slice ends in at most one short chunk, and every other chunk carries more than
 //           ETC_CHUNK_BYTES / 2 bytes — or, on the re-aligning path, more than 4 KB (rows_per_chunk);
 //   staging: payload + 16 bytes of padding per slice + 512 per (kind, source, destination) segment.
+constexpr int64_t NO_SYNC_MAX_CHUNKS = 32768;
 constexpr int64_t ORDER_MIN_LAZY_BYTES = 128ll << 20;      // about the size of the L2: below it DRAM locality is moot
 static void plan_bounds(const etc_layout* old_l, const etc_layout* new_l, int K, etc_plan* pl) {
   const int nT = old_l->t.n_tensors;
@@ -610,10 +611,11 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
   // reading A31: the new layout's padded vocabulary has rows the old one lacks -> those are zero-filled
   const bool grows = new_l->vocab_rows > old_l->vocab_rows && new_l->n_emb_pieces > 0;
   pl->bound_fills = grows ? new_l->n_emb_pieces : 0;
-  // ETC_NO_SYNC is honoured while the bound-sized tables stay small; a big plan is made the exact way (one host sync
-  // costs nothing next to its copy kernels, and exact grids keep its copy launches free of idle CTAs)
-  const size_t bound_tb = (size_t)pl->bound_slices * 2 * sizeof(etc_slice) + (size_t)pl->bound_chunks * 2 * sizeof(Chunk);
-  const bool lazy = (flags & ETC_NO_SYNC) && bound_tb <= ((size_t)64 << 20);
+  // ETC_NO_SYNC is honoured while the bound-sized grids stay small: every CTA of a copy launch beyond the real chunk
+  // count costs ~0.7 us of an SM's three CTA slots (it reads the count and leaves), and the bound is about twice the
+  // real count — measured on c2 (196 K bound, 91 K real) the surplus cost 0.17 ms per call where the one host sync of an
+  // exact plan costs 0.02 ms.  Up to NO_SYNC_MAX_CHUNKS the surplus is worth less than a sync (states up to ~1 GB).
+  const bool lazy = (flags & ETC_NO_SYNC) && pl->bound_chunks <= NO_SYNC_MAX_CHUNKS;
   pl->lazy = lazy; pl->resolved = !lazy;
   auto fail = [&](etc_status s) { etc_plan_destroy(pl); return s; };
 #define PLAN_TRY(expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) { set_error_detail(#expr, _e); return fail(ETC_ERR_CUDA); } } while (0)
