@@ -398,11 +398,11 @@ class Resident:
         """(a2)-(a6) — cost matrix, sketch, ETC_NO_SYNC plan, both copy launches, the plan's stream-ordered release —
         captured into ONE CUDA graph over the resident buffers (the two layouts, a1, are made before the capture) and
         replayed back to back: device time per replay.  What a framework that reconfigures between the same two
-        layouts repeatedly pays per migration once the submission cost is gone.  None where the plan is
-        too large for a bound-sized no-sync plan."""
+        layouts repeatedly pays per migration once the submission cost is gone.  Small states only
+        (None otherwise): a larger plan synchronises once to size its tables and cannot be captured."""
         E, torch = self.E, self.torch
         lo, ln = self.lay_old, self.lay_new
-        if ln.total_bytes() > (8 << 30):             # larger plans synchronise once to size their tables: not capturable
+        if ln.total_bytes() > (256 << 20):           # larger plans synchronise once to size their tables: not capturable
             return None
         bound = E.etc_staging_bound(lo, ln, self.flags)   # a no-sync plan needs the bound, not the exact size
         if bound > (self.staging.numel() if self.staging is not None else 0):
