@@ -513,7 +513,7 @@ def list_order_rates(E, torch, R, peak, flags):
             "unpack_list_order": kernel_entry(b2, statistics.mean(t2), peak)}
 
 
-def config_entry(res, peak, one_shot_ms=None):
+def config_entry(res, peak, one_shot_ms=None, name=None, mode="LOCAL_DIRECT"):
     st, bd = res["stats"], res["breakdown"]
     b1, b2 = copy_launch_bytes(st)
     k1, k2 = kernel_entry(b1, bd["pack_local_ms"], peak), kernel_entry(b2, bd["unpack_ms"], peak)
@@ -522,6 +522,12 @@ def config_entry(res, peak, one_shot_ms=None):
            "pack_local_ms": k1["ms"], "pack_local_GBs": k1["GBs"], "pack_local_frac": k1["frac"],
            "unpack_ms": k2["ms"], "unpack_GBs": k2["GBs"], "unpack_frac": k2["frac"],
            "cost_sketch_ms": bd["cost_matrix_ms"] + bd["sketch_ms"], "plan_ms": bd["plan_ms"], "layout_ms": bd["layout_ms"]}
+    if name:                                          # ncu DRAM bytes per launch from the committed captures, where one exists
+        t1, t2 = ncu_traffic(name, mode, "migrate_copy_kernel<false>"), ncu_traffic(name, mode, "migrate_copy_kernel<true>")
+        if t1:
+            out["pack_local_traffic"] = t1
+        if t2:
+            out["unpack_traffic"] = t2
     if one_shot_ms is not None and len(one_shot_ms) > 2 and one_shot_ms[2] is not None:
         out["graph_replay_ms"] = one_shot_ms[2]          # a2-a6 as one CUDA graph, device time per replay
         out["graph_replay_GBs"] = st.hbm_bytes / one_shot_ms[2] / 1e6
@@ -618,7 +624,7 @@ def run_cuda(args, w):
         except Exception as ex:
             one = None
             line["one_shot_error"] = repr(ex)[:160]
-    per_config = {w["name"]: config_entry(res, peak, one)}
+    per_config = {w["name"]: config_entry(res, peak, one, w["name"], mode)}
     if extras_on:
         if not args.no_reorder:
             try:
@@ -648,7 +654,7 @@ def run_cuda(args, w):
                     one_i = one_i + (Ri.graph_replay(),)
                 except Exception:
                     pass
-                per_config[name] = config_entry(ri, peak, one_i)
+                per_config[name] = config_entry(ri, peak, one_i, name, mode)
                 Ri.close()
                 del Ri
             except Exception as ex:
