@@ -173,13 +173,14 @@ enum { ETC_LOCAL_DIRECT = 0, ETC_ALL_STAGED = 1, ETC_KIND_MAJOR = 2, ETC_ALL_DIR
  * etc_plan_get_traffic / _slices / _fills / etc_plan_set_rounds / etc_plan_validate.  A hint: plans whose bound exceeds
  * 32 768 copy work items (states beyond ~1 GB) are made the synchronising way — their copy kernels dwarf one host sync,
  * and the surplus CTAs of a bound-sized grid would cost more than it.
- * Launch order.  A plan whose counts the host knows (every plan but a bound-sized ETC_NO_SYNC one) also keeps its copy
+ * Launch order.  A plan also keeps its copy
  * work items in ADDRESS order — launch 1 (pack + local) by source address, launch 2 (unpack) by destination address —
  * and etc_migrate / etc_migrate_phase walk those lists: work items that read interleaved column blocks of the same
  * rows (a TP change of a row-parallel weight), or the same source range for several new ranks (replicated state fanning
  * out to more DP groups), then run side by side and share DRAM pages and L2 lines.  The result is the same bytes either
- * way.  ETC_NO_REORDER (OR-ed into flags) keeps the launches in list order (unit by unit): a measurement mode.
- * etc_migrate_round always walks its chunk range in list order. */
+ * way.  etc_plan_set_rounds builds the same lists per round, so etc_migrate_round walks each round in address order too.
+ * A bound-sized ETC_NO_SYNC plan keeps the lists if its state exceeds 128 MB (about the L2: below that the order is
+ * moot).  ETC_NO_REORDER (OR-ed into flags) keeps every launch in list order (unit by unit): a measurement mode. */
 int64_t etc_staging_bound(const etc_layout* old_l, const etc_layout* new_l, int32_t flags);   /* bytes; < 0 on bad arguments */
 etc_status etc_plan_create(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
                            int32_t flags, etc_plan** out, void* stream);
@@ -242,7 +243,8 @@ etc_status etc_plan_get_slices(const etc_plan* plan, int32_t which, etc_slice* h
  * chunks in plan order, 2: the launch-1 list in address order (every chunk of pack + local sorted by source address;
  * `staged` tells the two apart), 3: the launch-2 list (the staged chunks sorted by destination address).  h_out must
  * hold n_chunks_staged (0, 3), n_chunks_local (1) or their sum (2) entries; copied to HOST memory.  2 and 3 return
- * ETC_ERR_INVALID_ARG for a plan that keeps no ordered lists (ETC_NO_REORDER, or a bound-sized ETC_NO_SYNC plan).
+ * ETC_ERR_INVALID_ARG for a plan that keeps no ordered lists (ETC_NO_REORDER, or a bound-sized ETC_NO_SYNC plan of a
+ * state below 128 MB).
  * Address order means: non-decreasing buffer index, and inside a buffer non-decreasing 64 KB block of the offset (for
  * layouts beyond 256 GB in all, a coarser block); the order inside a block is unspecified. */
 typedef struct {
