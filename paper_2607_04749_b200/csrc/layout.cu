@@ -129,12 +129,16 @@ namespace etc {
 static std::mutex g_up_mu;
 static cudaStream_t g_up_stream = nullptr;
 constexpr int N_SLABS = 8;
-struct Slab { void* p = nullptr; size_t cap = 0; cudaEvent_t done = nullptr; bool in_flight = false; };
+struct Slab { void* p = nullptr; size_t cap = 0; cudaEvent_t done = nullptr; bool in_flight = false; bool busy = false; };
 static Slab g_slabs[N_SLABS];
 static unsigned g_slab_next = 0;
 static cudaError_t slab_acquire(size_t bytes, Slab** out) {
   if (!g_up_stream) { cudaError_t e = cudaStreamCreateWithFlags(&g_up_stream, cudaStreamNonBlocking); if (e) return e; }
-  Slab& s = g_slabs[g_slab_next++ % N_SLABS];
+  // the next slab that no other host thread is building a layout in (two builders at most in this library: primitive.cu)
+  Slab* pick = nullptr;
+  for (int t = 0; t < N_SLABS && !pick; ++t) { Slab& c = g_slabs[g_slab_next++ % N_SLABS]; if (!c.busy) pick = &c; }
+  if (!pick) return cudaErrorNotReady;
+  Slab& s = *pick;
   if (!s.done) { cudaError_t e = cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming); if (e) return e; }
   if (s.in_flight) { cudaError_t e = cudaEventSynchronize(s.done); if (e) return e; s.in_flight = false; }
   if (bytes > s.cap) {
@@ -144,6 +148,7 @@ static cudaError_t slab_acquire(size_t bytes, Slab** out) {
     cudaError_t e = cudaMallocHost(&s.p, cap); if (e) return e;
     s.cap = cap;
   }
+  s.busy = true;                                         // until the upload has been enqueued (etc_layout_create)
   *out = &s;
   return cudaSuccess;
 }
@@ -220,11 +225,12 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
                o_pieces = o_kstart + al((size_t)n_dev * (ETC_NUM_KINDS + 1) * 4);
   const size_t max_total = o_pieces + (size_t)n_dev * n_kinds * max_inst * 5 * sizeof(Piece);   // <= 5 rectangles / instance
 
-  std::lock_guard<std::mutex> lock(g_up_mu);
+  // The lock covers the slab hand-out and, further down, the upload; the build in between runs unlocked, so two host
+  // threads can build two layouts side by side (etc_migrate_state does).
   DeviceGuard guard;                                       // the caller's current device is restored on return
   cudaError_t e = guard.err;
   Slab* slab = nullptr;
-  if (e == cudaSuccess) e = slab_acquire(max_total, &slab);
+  if (e == cudaSuccess) { std::lock_guard<std::mutex> lock(g_up_mu); e = slab_acquire(max_total, &slab); }
   if (e != cudaSuccess) { set_error_detail("etc_layout_create staging", e); return ETC_ERR_CUDA; }
   char* host = static_cast<char*>(slab->p);
   int32_t* dev_start = reinterpret_cast<int32_t*>(host + o_start);
@@ -388,6 +394,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   L->model = m; L->cfg = *cfg; L->h_buffer_bytes = bufbytes; L->max_dev_pieces = max_dev_pieces;
   L->vocab_rows = (int32_t)vocab_rows(m, *cfg); L->lm_head_id = m.tied_embeddings ? -1 : nT - 1; L->n_emb_pieces = n_emb_pieces;
   L->grp_pieces = std::move(grp_pieces); L->aligned16 = (align_or & 15) == 0; L->total_bytes = total_bytes;
+  std::lock_guard<std::mutex> lock(g_up_mu);               // the upload stream and the slab's state
   e = cudaMallocAsync(&L->d_blob, total, g_up_stream);
   // a DMA copy on the private upload stream: it runs beside the copy kernels of a migration in flight (a copy kernel
   // here was measured to wait for them: 0.16 -> 1.7 ms per layout pair on c2).  No host wait: readers wait for `ready`.
@@ -395,6 +402,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   if (e == cudaSuccess) e = cudaEventCreateWithFlags(&L->ready, cudaEventDisableTiming);
   if (e == cudaSuccess) e = cudaEventRecord(L->ready, g_up_stream);
   if (e == cudaSuccess) { e = cudaEventRecord(slab->done, g_up_stream); slab->in_flight = e == cudaSuccess; }
+  slab->busy = false;
   if (e != cudaSuccess) {
     set_error_detail("etc_layout_create upload", e);
     cudaStreamSynchronize(g_up_stream);                    // the slab may still be being read
