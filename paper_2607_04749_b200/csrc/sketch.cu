@@ -12,6 +12,7 @@ namespace etc {
 
 constexpr int SK_THREADS = 1024;
 constexpr int64_t SK_INF = (int64_t)1 << 62;
+constexpr int64_t SK_UNSOLVED = -2;                 // sketch_tight_kernel -> sketch_hungarian_kernel: "no certificate, go on"
 
 // ---------------------------------------------------------------------------------------------- exhaustive
 __global__ void __launch_bounds__(SK_THREADS)
@@ -76,6 +77,145 @@ sketch_exhaustive_kernel(const int64_t* __restrict__ overlap, int N, int P, cons
   }
 }
 
+// ---------------------------------------------------------------------------------------------- row-maximum certificate
+// sum_n max_o overlap[n][o] bounds every sketch from above.  In the overlap matrices of real reconfigurations most rows
+// have their maximum on a column no other row wants (or on one of several equal replicas, DP groups of the old layout), so
+// a matching that gives EVERY row one of its maximal columns often exists — and any such matching is optimal.  This
+// kernel looks for one greedily and, if it finds it, is done in a few microseconds where the O(k^3) search takes hundreds
+// (512 -> 384 devices: 0.29 ms).  If it does not, it says so and sketch_hungarian_kernel runs as before: the fast path
+// can only ever return an optimum.
+//   1. (sketch_rowmax_kernel, one warp per row over the whole machine) the row maximum over the usable columns and its
+//      first TK columns ("tight" columns); then one CTA (sketch_tight_kernel):
+//   2. rows with a positive maximum claim a tight column (lowest row wins a contested one), rows with the fewest tight
+//      columns first;
+//   3. rows whose maximum is 0 overlap nothing anywhere: they take the columns left over, in order;
+//   4. everyone placed -> device_map, local_bytes = the bound; else local_bytes = SK_UNSOLVED.
+constexpr int TK = 4;                               // tight columns remembered per row
+constexpr int TIGHT_MAX = 1024;                     // rows / columns the fast path handles (shared memory)
+constexpr int RM_WARPS = 8;
+
+// step 1, over the whole machine: one warp per row.  cnt[n] = tight columns found (capped at TK), -1 if the row's maximum is
+// 0, -2 if the row has no usable column.
+__global__ void __launch_bounds__(RM_WARPS * 32)
+sketch_rowmax_kernel(const int64_t* __restrict__ overlap, int N, int P, const uint8_t* __restrict__ avail,
+                     int64_t* __restrict__ rowmax, int32_t* __restrict__ cnt, int32_t* __restrict__ tight) {
+  const int lane = threadIdx.x & 31, n = blockIdx.x * RM_WARPS + (threadIdx.x >> 5);
+  if (n >= N) return;
+  const int64_t* row = overlap + (size_t)n * P;
+  int64_t m = -1;
+#pragma unroll 8
+  for (int j = lane; j < P; j += 32) { const int64_t x = row[j]; if (!avail || avail[j]) m = max(m, x); }   // loads first
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+  int c = m < 0 ? -2 : (m == 0 ? -1 : 0);
+  if (m > 0) {
+    for (int j0 = 0; j0 < P && c < TK; j0 += 32) {
+      const int j = j0 + lane;
+      const bool t = j < P && (!avail || avail[j]) && row[j] == m;
+      const unsigned mask = __ballot_sync(0xffffffffu, t);
+      const int r = c + __popc(mask & ((1u << lane) - 1u));
+      if (t && r < TK) tight[n * TK + r] = j;
+      c += __popc(mask);
+    }
+    c = min(c, TK);
+  }
+  if (lane == 0) { cnt[n] = c; rowmax[n] = m; }
+}
+
+__global__ void __launch_bounds__(SK_THREADS)
+sketch_tight_kernel(int N, int P, const uint8_t* __restrict__ avail, const int64_t* __restrict__ rowmax,
+                    const int32_t* __restrict__ cnt_g, const int32_t* __restrict__ tight_g,
+                    int32_t* __restrict__ device_map, int64_t* __restrict__ local_bytes) {
+  __shared__ int32_t tight[TIGHT_MAX * TK];         // later reused: [0,P) free columns, [P, P+N) zero rows
+  __shared__ int32_t cnt[TIGHT_MAX];                // tight columns of row n (capped at TK); -1: the row's maximum is 0
+  __shared__ int32_t match[TIGHT_MAX];              // row -> column or -1
+  __shared__ int32_t owner[TIGHT_MAX];              // column -> row, -1 free, -2 unusable
+  __shared__ int32_t prop[TIGHT_MAX];               // column -> lowest row proposing to it
+  __shared__ int64_t s_sum[32];
+  __shared__ int32_t s_scan[33];
+  __shared__ int s_bad;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  if (tid == 0) s_bad = 0;
+  __syncthreads();
+  for (int j = tid; j < P; j += SK_THREADS) { owner[j] = (!avail || avail[j]) ? -1 : -2; prop[j] = 0x7fffffff; }
+  int64_t bound = 0;
+  for (int n = tid; n < N; n += SK_THREADS) {
+    match[n] = -1;
+    const int c = cnt_g[n];
+    cnt[n] = c;
+    if (c == -2) s_bad = 1;                                      // a row with no usable column: infeasible, the search says so
+    if (c > 0) bound += rowmax[n];
+  }
+  for (int i = tid; i < N * TK; i += SK_THREADS) tight[i] = tight_g[i];   // entries beyond cnt[n] are never read
+  __syncthreads();
+  // 2. claim tight columns, the most constrained rows first.  Deterministic: in every step the unmatched rows propose to
+  // their next candidate and the LOWEST row wins a contested column (atomicMin), so the map does not depend on timing.
+  for (int pass = 1; pass <= TK; ++pass) {
+    for (int k = 0; k < pass; ++k) {
+      for (int n = tid; n < N; n += SK_THREADS) {
+        if (cnt[n] != pass || match[n] >= 0) continue;
+        const int j = tight[n * TK + (k + n) % pass];            // spread rows that tie on the same columns
+        if (owner[j] == -1) atomicMin(&prop[j], n);
+      }
+      __syncthreads();
+      for (int n = tid; n < N; n += SK_THREADS) {
+        if (cnt[n] != pass || match[n] >= 0) continue;
+        const int j = tight[n * TK + (k + n) % pass];
+        if (owner[j] == -1 && prop[j] == n) { owner[j] = n; match[n] = j; }
+      }
+      __syncthreads();
+    }
+    for (int n = tid; n < N; n += SK_THREADS) if (cnt[n] == pass && match[n] < 0) s_bad = 1;
+    __syncthreads();
+  }
+  const bool bad = s_bad != 0;
+  __syncthreads();
+  if (!bad) {
+    // 3. zero rows take the leftover columns: i-th zero row <-> i-th free column (compaction by block scans)
+    int32_t* freec = tight; int32_t* zrow = tight + P;
+    int n_free = 0, n_zero = 0;
+    for (int pass = 0; pass < 2; ++pass) {
+      const int L = pass == 0 ? P : N;
+      int base = 0;
+      for (int b0 = 0; b0 < L; b0 += SK_THREADS) {
+        const int i = b0 + tid;
+        const bool f = i < L && (pass == 0 ? owner[i] == -1 : cnt[i] == -1);
+        const unsigned mask = __ballot_sync(0xffffffffu, f);
+        if (lane == 0) s_scan[wid] = __popc(mask);
+        __syncthreads();
+        if (wid == 0) {
+          int x = s_scan[lane], y = x;
+#pragma unroll
+          for (int o = 1; o < 32; o <<= 1) { const int z = __shfl_up_sync(0xffffffffu, y, o); if (lane >= o) y += z; }
+          s_scan[lane] = y - x;
+          if (lane == 31) s_scan[32] = y;
+        }
+        __syncthreads();
+        if (f) (pass == 0 ? freec : zrow)[base + s_scan[wid] + __popc(mask & ((1u << lane) - 1u))] = i;
+        base += s_scan[32];
+        __syncthreads();
+      }
+      if (pass == 0) n_free = base; else n_zero = base;
+    }
+    if (n_zero > n_free) { if (tid == 0) s_bad = 1; }
+    else for (int i = tid; i < n_zero; i += SK_THREADS) match[zrow[i]] = freec[i];
+    __syncthreads();
+  }
+  if (s_bad) { if (tid == 0) *local_bytes = SK_UNSOLVED; return; }
+  // 4. every row sits on one of its maximal columns: optimal
+  for (int n = tid; n < N; n += SK_THREADS) device_map[n] = match[n];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) bound += __shfl_xor_sync(0xffffffffu, bound, o);
+  if (lane == 0) s_sum[wid] = bound;
+  __syncthreads();
+  if (wid == 0) {
+    int64_t t = s_sum[lane];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if (lane == 0) *local_bytes = t;
+  }
+}
+
 // ---------------------------------------------------------------------------------------------- Hungarian
 // Shortest augmenting path with potentials (the O(k^3) method Algorithm 1 calls through SciPy, ref [39]).
 // cost(i,j) = -overlap[i][j]; columns masked by `avail` are never entered.  Per-column state lives in registers
@@ -111,8 +251,9 @@ __device__ __forceinline__ ArgMin warp_argmin(const ArgMin& a) {
 template <int SK_T, int SK_CPT>
 __global__ void __launch_bounds__(SK_T)
 sketch_hungarian_kernel(const int64_t* __restrict__ overlap, int N, int P, const uint8_t* __restrict__ avail,
-                        int32_t* __restrict__ device_map, int64_t* __restrict__ local_bytes) {
+                        int32_t* __restrict__ device_map, int64_t* __restrict__ local_bytes, int after_tight) {
   constexpr int SK_THREADS = SK_T, SK_NW = SK_T / 32;
+  if (after_tight && *local_bytes != SK_UNSOLVED) return;      // sketch_tight_kernel found an optimum (uniform: one word)
   extern __shared__ __align__(16) unsigned char smem_raw[];
   int64_t* u = reinterpret_cast<int64_t*>(smem_raw);            // [N] row potentials
   int32_t* rowof = reinterpret_cast<int32_t*>(u + N);           // [P] column -> matched row or -1
@@ -297,8 +438,23 @@ extern "C" etc_status etc_sketch(const int64_t* d_overlap, int32_t n_new, int32_
       count_launch();
       return ETC_OK;
     }
+    // the row-maximum certificate first (a few microseconds); the search below leaves at once if it succeeded
+    const int after_tight = P <= TIGHT_MAX ? 1 : 0;
+    if (after_tight) {
+      char* ws = nullptr;                                       // rowmax [N] | cnt [N] | tight [N][TK]
+      const size_t o_cnt = sizeof(int64_t) * (size_t)n_new, o_tight = o_cnt + sizeof(int32_t) * (size_t)n_new;
+      ETC_CUDA_TRY(cudaMallocAsync(&ws, o_tight + sizeof(int32_t) * (size_t)n_new * TK, st));
+      int64_t* rowmax = reinterpret_cast<int64_t*>(ws);
+      int32_t* cnt = reinterpret_cast<int32_t*>(ws + o_cnt); int32_t* tight = reinterpret_cast<int32_t*>(ws + o_tight);
+      sketch_rowmax_kernel<<<(n_new + RM_WARPS - 1) / RM_WARPS, RM_WARPS * 32, 0, st>>>(d_overlap, n_new, P, d_avail, rowmax, cnt, tight);
+      sketch_tight_kernel<<<1, SK_THREADS, 0, st>>>(n_new, P, d_avail, rowmax, cnt, tight, d_device_map, d_local_bytes);
+      const cudaError_t le = cudaGetLastError();
+      cudaFreeAsync(ws, st);
+      ETC_CUDA_TRY(le);
+      count_launch(2);
+    }
     const size_t smem = (size_t)n_new * 8 + (size_t)P * 8;       // <= 32 KB: below the default dynamic limit
-#define SK_LAUNCH(T, CPT) sketch_hungarian_kernel<T, CPT><<<1, T, smem, st>>>(d_overlap, n_new, P, d_avail, d_device_map, d_local_bytes)
+#define SK_LAUNCH(T, CPT) sketch_hungarian_kernel<T, CPT><<<1, T, smem, st>>>(d_overlap, n_new, P, d_avail, d_device_map, d_local_bytes, after_tight)
     if (P <= 64) SK_LAUNCH(64, 1);
     else if (P <= 128) SK_LAUNCH(128, 1);
     else if (P <= 256) SK_LAUNCH(256, 1);

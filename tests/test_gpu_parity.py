@@ -153,6 +153,65 @@ def test_sketch_large_random_and_structured(E):
         assert sum(int(ov[i, dm[i]]) for i in range(n)) == int(lb.item())
 
 
+def test_sketch_row_maximum_certificate(E):
+    """P > 32: sketch_tight_kernel tries to give every row one of its maximal columns (then the row-maximum bound proves
+    optimality) and otherwise hands over to the Hungarian kernel.  Either way the objective must equal the oracle's /
+    SciPy's: matrices where the certificate holds (replicated maxima as in DP groups, zero rows taking leftover columns,
+    masked columns), where greedy needs the most-constrained-first order, where it cannot hold (contended maxima), and
+    an infeasible mask."""
+    from scipy.optimize import linear_sum_assignment
+    rng = np.random.default_rng(11)
+
+    def check(ov, avail=None):
+        g = torch.from_numpy(np.ascontiguousarray(ov, np.int64)).cuda()
+        av = None if avail is None else torch.from_numpy(avail.astype(np.uint8)).cuda()
+        dm, lb = E.etc_sketch(g, avail=av, method=E.ETC_SKETCH_HUNGARIAN)
+        dm = dm.cpu().numpy(); lb = int(lb.item())
+        m = ov.copy()
+        if avail is not None:
+            m = m[:, avail]
+        if m.shape[1] < m.shape[0]:
+            assert lb == -1 and (dm == -1).all()
+            return
+        r, c = linear_sum_assignment(m, maximize=True)
+        assert lb == int(m[r, c].sum()), (ov.shape, lb, int(m[r, c].sum()))
+        assert len(set(dm.tolist())) == ov.shape[0] and dm.min() >= 0 and dm.max() < ov.shape[1]
+        if avail is not None:
+            assert all(avail[p] for p in dm)
+        assert sum(int(ov[i, dm[i]]) for i in range(ov.shape[0])) == lb
+
+    for n, P, rep in [(48, 64, 4), (96, 128, 4), (384, 512, 4), (200, 1000, 5), (1024, 1024, 1), (33, 40, 8)]:
+        # groups of `rep` equal columns (old DP replicas); every row's maximum sits on one group, <= rep rows per group
+        groups = P // rep
+        ov = np.zeros((n, P), np.int64)
+        for i in range(n):
+            gi = (i // rep) % groups if rep > 1 else i % groups
+            ov[i, gi * rep:(gi + 1) * rep] = 10**9 + 7 * gi
+            ov[i, rng.integers(0, P, size=3)] += rng.integers(0, 1000, size=3)     # noise below / inside the maxima
+        check(ov)
+        # fresh ranks: the last quarter of the rows overlaps nothing (scale-out)
+        ov2 = ov.copy(); ov2[n - n // 4:] = 0
+        check(ov2)
+        # masked columns (pre-emption): the certificate may or may not survive
+        avail = rng.random(P) < 0.9
+        check(ov, avail)
+    # most-constrained-first: row 0 ties on columns {0,1}, row 1 wants column 0 only
+    ov = np.zeros((40, 64), np.int64)
+    ov[0, 0] = ov[0, 1] = 5; ov[1, 0] = 5
+    for i in range(2, 40):
+        ov[i, i + 3] = 9
+    check(ov)
+    # contended maxima: all rows want column 0 -> no certificate, the Hungarian kernel decides
+    ov = rng.integers(0, 100, size=(50, 70)).astype(np.int64); ov[:, 0] = 10**6
+    check(ov)
+    # dense random (fallback) and heavy ties
+    check(rng.integers(0, 10**9, size=(60, 90)).astype(np.int64))
+    check((rng.integers(0, 3, size=(64, 64)) * 10**11).astype(np.int64))
+    # infeasible: fewer usable columns than rows
+    avail = np.zeros(64, bool); avail[:10] = True
+    check(rng.integers(0, 9, size=(40, 64)).astype(np.int64), avail)
+
+
 def test_sketch_infeasible_and_errors(E):
     ov = torch.ones((3, 4), dtype=torch.int64, device="cuda")
     av = torch.tensor([1, 0, 0, 1], dtype=torch.uint8, device="cuda")
