@@ -16,6 +16,7 @@ BASELINE.json, so there is no data-path collective); value = all ranks' bytes / 
 """
 from __future__ import annotations
 import argparse
+import collections
 import gc
 import json
 import os
@@ -133,7 +134,7 @@ def bench_config(w, all_staged: bool, world: int) -> dict:
     """The `config` object of the JSON line: the same for the CUDA arm and for `--impl reference`."""
     return {"workload": w["name"], "old": w["old"], "new": w["new"],
             "mode": "ALL_STAGED" if all_staged else "LOCAL_DIRECT", "l2": "inputs_larger_than_L2",
-            "pipelining": "planning (a1-a4) of step i+1 on its own stream overlaps the copy kernels of step i",
+            "pipelining": "planning (a1-a4) of step i+1 on its own stream overlaps the copy kernels of step i; at most 3 steps in flight",
             "parallelism": "replicas only" if world > 1 else "1 GPU, all virtual devices in one HBM"}
 
 
@@ -265,6 +266,9 @@ def run_reference(args, w):
 
 
 # ------------------------------------------------------------------------------------------------ CUDA arm
+PIPELINE_DEPTH = 3       # steps in flight in the pipelined loop (see Resident.step)
+
+
 class Resident:
     """One workload resident in HBM: old shard buffers (filled with the workload's value distribution), new shard
     buffers, the staging buffer, and the pipelined whole-path step."""
@@ -296,6 +300,7 @@ class Resident:
         self.stream = torch.cuda.current_stream()
         self.plan_stream = torch.cuda.Stream(dev, priority=-1)   # high priority: its small kernels cut in front of copy CTAs
         self.planned = [torch.cuda.Event() for _ in range(4)]
+        self.in_flight = collections.deque()
         self.step_no = 0
 
     def ev(self):
@@ -308,6 +313,14 @@ class Resident:
         E, torch, w = self.E, self.torch, self.w
         ps, stream = self.plan_stream, self.stream
         e = [self.ev() for _ in range(8)] if record is not None else None
+        # At most PIPELINE_DEPTH steps in flight: planning of step i+1 overlaps the copies of step i (and the tail of
+        # step i-1), no further.  Unbounded, the host plans every step ahead of the copy stream (planning ~0.6 ms, a
+        # step's copies ~25 ms on c4), all K plans' tables are alive at once and the stream-ordered pool grows inside the
+        # timed region (seen: a 140 ms host stall in one of eight 20-step runs).  With depth 2 the tables of step i-1 are
+        # freed just as step i+1 is planned and the pool hands them out behind the copy stream's tail (plan_ms 3-40 ms,
+        # overlap lost); with depth 3 the memory a new plan gets was released a whole step earlier (plan_ms 0.6 ms).
+        while len(self.in_flight) >= PIPELINE_DEPTH:
+            self.in_flight.popleft().synchronize()
         with torch.cuda.stream(ps):
             if e: e[0].record(ps)
             lo, ln = E.etc_layout_create(w["model"], w["old"]), E.etc_layout_create(w["model"], w["new"])      # (a1)
@@ -327,13 +340,29 @@ class Resident:
         if e: e[5].record(stream)
         E.etc_migrate(plan, self.src_tab, self.dst_tab, self.staging, E.ETC_PHASE_UNPACK, stream=stream)   # (a6)
         if e: e[6].record(stream)
+        fin = torch.cuda.Event()
+        fin.record(stream)
+        self.in_flight.append(fin)
         if record is not None:
             record.append(e)
-        return plan
+        stats = plan.stats
+        # release the plan NOW (stream-ordered: its tables are freed behind the copy launches just enqueued).  Dropped one
+        # step later, the free would sit behind the NEXT step's copies, and the pool would make the planning stream wait
+        # for them before it hands the memory out again (seen as plan_ms of 3-30 ms and lost overlap)
+        del plan
+        return stats
 
     def timed(self, steps, warmup, barrier, world, sampler=None):
         """W warm-up steps, then exactly K steps between barrier + synchronize; device time, max over ranks."""
         E, torch = self.E, self.torch
+        # prime the stream-ordered pool (untimed, before the warm-up steps): a few plans alive at once, then released, so
+        # that the steps find their tables' memory in the pool instead of growing it (a growth is a host-side stall of
+        # tens of milliseconds)
+        ov, _, _ = E.etc_cost_matrix(self.lay_old, self.lay_new, out=self.out_cost)
+        dm, _ = E.etc_sketch(ov, out=self.out_sk)
+        hold = [E.etc_plan_create(self.lay_old, self.lay_new, dm, self.flags) for _ in range(2 * PIPELINE_DEPTH + 2)]
+        del hold
+        torch.cuda.synchronize()
         for _ in range(max(warmup, 3)):
             self.step()
         barrier()
@@ -345,7 +374,7 @@ class Resident:
         barrier()
         t_begin.record(self.stream)
         for _ in range(steps):
-            plan = self.step(recs)
+            stats = self.step(recs)
         t_end.record(self.stream)
         barrier()
         launches = E.kernel_launches() - launches0
@@ -354,8 +383,8 @@ class Resident:
         phase = lambda a, b: statistics.mean(r[a].elapsed_time(r[b]) for r in recs)
         bd = {"layout_ms": phase(0, 1), "cost_matrix_ms": phase(1, 2), "sketch_ms": phase(2, 3), "plan_ms": phase(3, 4),
               "pack_local_ms": phase(7, 5), "unpack_ms": phase(5, 6)}
-        self.stats = plan.stats
-        return dict(ms_per_step=ms_per_step, breakdown=bd, launches=launches, clocks=clocks, stats=plan.stats)
+        self.stats = stats
+        return dict(ms_per_step=ms_per_step, breakdown=bd, launches=launches, clocks=clocks, stats=stats)
 
     def one_shot(self, reps=10):
         """One migration, cold start to finish, nothing overlapped, through the one-call primitive etc_migrate_state:
