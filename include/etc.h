@@ -184,6 +184,11 @@ enum { ETC_LOCAL_DIRECT = 0, ETC_ALL_STAGED = 1, ETC_KIND_MAJOR = 2, ETC_ALL_DIR
 int64_t etc_staging_bound(const etc_layout* old_l, const etc_layout* new_l, int32_t flags);   /* bytes; < 0 on bad arguments */
 etc_status etc_plan_create(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
                            int32_t flags, etc_plan** out, void* stream);
+/* Releases the plan's tables in stream order, behind everything already enqueued that reads them (on whatever streams):
+ * safe to call right after the last etc_migrate* call on the plan, while its kernels are still queued.  Do call it there
+ * when migrations are pipelined: the tables return to the stream-ordered pool at that point of the copy stream, and a plan
+ * dropped a step later is only reusable a step later (bench.py keeps three steps in flight and releases each plan right
+ * behind its own launches). */
 void etc_plan_destroy(etc_plan* plan);
 
 /* (f4) Failure-aware sourcing ("Fault-tolerance through DP": "the workload on the failed device can be
