@@ -1,5 +1,6 @@
 """-m gpu: BASELINE.json configs c2-c5 at FULL size, in the launch configuration bench.py times (whole path, the GPU's own
-optimal sketch, LOCAL_DIRECT; and every slice staged, ALL_STAGED).  EXHAUSTIVE: the oracle's element-wise migration
+optimal sketch, LOCAL_DIRECT, address-ordered launches; every slice staged, ALL_STAGED; and LOCAL_DIRECT with the launches
+in list order, ETC_NO_REORDER).  EXHAUSTIVE: the oracle's element-wise migration
 (oracle/etc_oracle.c orc_migrate_range: global_of -> holders_of -> source rule A6 -> one element copied) is run over EVERY
 element of EVERY new shard buffer on all host cores, from a host copy of the position-stamped old state, and every new
 shard buffer the CUDA path produced is compared with it byte for byte ("bit-exact fidelity"; north_star:
@@ -122,16 +123,16 @@ def _exhaustive(E, name, modes):
 
 
 def test_fullsize_c2_exhaustive(E):
-    _exhaustive(E, "c2", [(E.ETC_LOCAL_DIRECT, 0x00), (E.ETC_ALL_STAGED, 0xFF)])
+    _exhaustive(E, "c2", [(E.ETC_LOCAL_DIRECT, 0x00), (E.ETC_ALL_STAGED, 0xFF), (E.ETC_LOCAL_DIRECT | E.ETC_NO_REORDER, 0x3C)])
 
 
 def test_fullsize_c3_exhaustive(E):
-    _exhaustive(E, "c3", [(E.ETC_LOCAL_DIRECT, 0x00), (E.ETC_ALL_STAGED, 0xFF)])
+    _exhaustive(E, "c3", [(E.ETC_LOCAL_DIRECT, 0x00), (E.ETC_ALL_STAGED, 0xFF), (E.ETC_LOCAL_DIRECT | E.ETC_NO_REORDER, 0x3C)])
 
 
 def test_fullsize_c4_exhaustive(E):
-    _exhaustive(E, "c4", [(E.ETC_LOCAL_DIRECT, 0xA5), (E.ETC_ALL_STAGED, 0x5A)])
+    _exhaustive(E, "c4", [(E.ETC_LOCAL_DIRECT, 0xA5), (E.ETC_ALL_STAGED, 0x5A), (E.ETC_LOCAL_DIRECT | E.ETC_NO_REORDER, 0x3C)])
 
 
 def test_fullsize_c5_exhaustive(E):
-    _exhaustive(E, "c5", [(E.ETC_LOCAL_DIRECT, 0xA5), (E.ETC_ALL_STAGED, 0x5A)])
+    _exhaustive(E, "c5", [(E.ETC_LOCAL_DIRECT, 0xA5), (E.ETC_ALL_STAGED, 0x5A), (E.ETC_LOCAL_DIRECT | E.ETC_NO_REORDER, 0x3C)])
