@@ -4,6 +4,8 @@
 // One warp (or one CTA, when there are few cells) owns one matrix cell (new rank n, old device o): lanes walk n's pieces, look the matching (kind, tensor)
 // group of o up in o's dense first-piece table, intersect rectangles and warp-reduce.  No atomics, so every cell is
 // written exactly once and the result is order-independent.  Extra warps past the matrix compute need[] and hold[].
+#include <algorithm>
+#include <vector>
 #include "etc_internal.h"
 
 namespace etc {
@@ -25,21 +27,37 @@ constexpr int COST_WARPS = 8;
 // WPC = warps per job.  WPC = 1: eight jobs per CTA (many cells: 512 x 384 layouts).  WPC = 8: the whole CTA shares one
 // job and reduces through shared memory (few cells: the piece lists are long compared with the cell count, so one
 // warp per cell would leave most of the machine idle and serialise ~20 dependent loads per lane).
+// A block of cells that can be non-zero: the devices of one new pipeline stage x the devices of one old stage that shares
+// layers (or embeddings) with it.  base = cells of the blocks before this one.
+struct StageBlock { int32_t n0, nn, o0, on; long long base; };
+
 template <int WPC>
 __global__ void __launch_bounds__(COST_WARPS * 32)
 cost_matrix_kernel(DeviceTables oldT, DeviceTables newT, int P,
-                   int64_t* __restrict__ overlap, int64_t* __restrict__ need, int64_t* __restrict__ hold) {
+                   int64_t* __restrict__ overlap, int64_t* __restrict__ need, int64_t* __restrict__ hold,
+                   const StageBlock* __restrict__ blocks, int n_blocks, long long block_cells) {
   __shared__ int64_t s_part[COST_WARPS];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int sub = wid % WPC;                                  // this warp's share of the job
   const long long job = ((long long)blockIdx.x * COST_WARPS + wid) / WPC;
-  const long long cells = (long long)newT.n_dev * P;
+  // with a block list (many devices: most cells pair different pipeline stages and are zero — the matrix was cleared, and
+  // only the listed blocks get a warp), a job is a cell of one block; otherwise a cell of the whole matrix
+  const long long cells = blocks ? block_cells : (long long)newT.n_dev * P;
   const int stride = 32 * WPC;
   int64_t acc = 0;
   int64_t* out = nullptr;
   if (job < cells) {
-    const int n = (int)(job / P), o = (int)(job % P);
-    out = overlap + job;
+    int n, o;
+    if (blocks) {
+      int lo = 0, hi = n_blocks - 1;                            // the block whose cell range holds `job`
+      while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (blocks[mid].base <= job) lo = mid; else hi = mid - 1; }
+      const StageBlock b = blocks[lo];
+      const long long local = job - b.base;
+      n = b.n0 + (int)(local / b.on); o = b.o0 + (int)(local % b.on);
+    } else {
+      n = (int)(job / P); o = (int)(job % P);
+    }
+    out = overlap + (size_t)n * P + o;
     if (o < oldT.n_dev) {
       // early out: no logical tensor in common (different pipeline stages)
       bool common = false;
@@ -115,12 +133,45 @@ extern "C" etc_status etc_cost_matrix(const etc_layout* old_l, const etc_layout*
   ETC_CUDA_TRY(layout_use(old_l, (cudaStream_t)stream));
   ETC_CUDA_TRY(layout_use(new_l, (cudaStream_t)stream));
   const long long jobs = (long long)new_l->t.n_dev * P + new_l->t.n_dev + P;
-  if (jobs <= 8192)
-    cost_matrix_kernel<COST_WARPS><<<(unsigned)jobs, COST_WARPS * 32, 0, (cudaStream_t)stream>>>(
-        old_l->t, new_l->t, P, d_overlap, d_need, d_hold);
-  else
-    cost_matrix_kernel<1><<<(unsigned)((jobs + COST_WARPS - 1) / COST_WARPS), COST_WARPS * 32, 0, (cudaStream_t)stream>>>(
-        old_l->t, new_l->t, P, d_overlap, d_need, d_hold);
+  cudaStream_t st = (cudaStream_t)stream;
+  if (jobs <= 8192) {
+    cost_matrix_kernel<COST_WARPS><<<(unsigned)jobs, COST_WARPS * 32, 0, st>>>(
+        old_l->t, new_l->t, P, d_overlap, d_need, d_hold, nullptr, 0, 0);
+  } else {
+    // Many devices: list the (new stage, old stage) blocks that can overlap — stages whose layer ranges intersect, and the
+    // first / last stages among themselves (embeddings, final norm, output layer, the tied replica) — clear the matrix and
+    // give warps to those blocks only.  Device ids are stage-major (r + tp*(d + dp*s)), so a stage is a contiguous range.
+    const std::vector<int32_t>&fo = old_l->stage_first, &fn = new_l->stage_first;
+    const int ppo = old_l->t.pp, ppn = new_l->t.pp;
+    const int dso = old_l->t.tp * old_l->t.dp, dsn = new_l->t.tp * new_l->t.dp;
+    std::vector<StageBlock> blocks;
+    long long bc = 0;
+    for (int sn = 0; sn < ppn; ++sn)
+      for (int so = 0; so < ppo; ++so) {
+        const bool layers = std::max(fn[sn], fo[so]) < std::min(fn[sn + 1], fo[so + 1]);
+        const bool ends = (sn == 0 || sn == ppn - 1) && (so == 0 || so == ppo - 1);
+        if (!layers && !ends) continue;
+        blocks.push_back(StageBlock{sn * dsn, dsn, so * dso, dso, bc});
+        bc += (long long)dsn * dso;
+      }
+    if (bc * 2 <= (long long)new_l->t.n_dev * P && !blocks.empty()) {
+      StageBlock* d_blocks = nullptr;
+      ETC_CUDA_TRY(cudaMallocAsync(&d_blocks, sizeof(StageBlock) * blocks.size(), st));
+      cudaError_t e = write_small(d_blocks, blocks.data(), sizeof(StageBlock) * blocks.size(), st);
+      if (e == cudaSuccess) e = cudaMemsetAsync(d_overlap, 0, sizeof(int64_t) * (size_t)new_l->t.n_dev * P, st);
+      if (e == cudaSuccess) {
+        const long long bjobs = bc + new_l->t.n_dev + P;
+        cost_matrix_kernel<1><<<(unsigned)((bjobs + COST_WARPS - 1) / COST_WARPS), COST_WARPS * 32, 0, st>>>(
+            old_l->t, new_l->t, P, d_overlap, d_need, d_hold, d_blocks, (int)blocks.size(), bc);
+        e = cudaGetLastError();
+      }
+      cudaFreeAsync(d_blocks, st);
+      ETC_CUDA_TRY(e);
+    } else {
+      cost_matrix_kernel<1><<<(unsigned)((jobs + COST_WARPS - 1) / COST_WARPS), COST_WARPS * 32, 0, st>>>(
+          old_l->t, new_l->t, P, d_overlap, d_need, d_hold, nullptr, 0, 0);
+    }
+  }
   ETC_CUDA_TRY(cudaGetLastError());
   count_launch();
   return ETC_OK;

@@ -90,6 +90,7 @@ struct etc_layout {
   int32_t lm_head_id = -1;                // logical tensor id of lm_head (-1: tied); word_embeddings is tensor 0
   int32_t n_emb_pieces = 0;               // pieces of the embedding tensors (upper bound of the zero-fill list)
   std::vector<int32_t> grp_pieces;        // [n_grp] pieces of each (kind, tensor) group over all devices (plan size bounds)
+  std::vector<int32_t> stage_first;       // [pp + 1] first layer of each pipeline stage (stage s holds [s], [s+1]) 
   bool aligned16 = true;                  // every piece of a tensor with more than one column has its offset, pitch, column
                                           // range and held flat range at multiples of 16 B: every STRIDED slice (rows that
                                           // do not merge into one run) is then 16-byte aligned and chunked by payload alone

@@ -394,6 +394,7 @@ extern "C" etc_status etc_layout_create(const etc_model_desc* model, const etc_p
   L->model = m; L->cfg = *cfg; L->h_buffer_bytes = bufbytes; L->max_dev_pieces = max_dev_pieces;
   L->vocab_rows = (int32_t)vocab_rows(m, *cfg); L->lm_head_id = m.tied_embeddings ? -1 : nT - 1; L->n_emb_pieces = n_emb_pieces;
   L->grp_pieces = std::move(grp_pieces); L->aligned16 = (align_or & 15) == 0; L->total_bytes = total_bytes;
+  for (int s = 0; s <= pp; ++s) L->stage_first.push_back(stage_begin(m.n_layers, *cfg, s));
   std::lock_guard<std::mutex> lock(g_up_mu);               // the upload stream and the slab's state
   e = cudaMallocAsync(&L->d_blob, total, g_up_stream);
   // a DMA copy on the private upload stream: it runs beside the copy kernels of a migration in flight (a copy kernel

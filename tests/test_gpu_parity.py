@@ -92,6 +92,36 @@ def test_cost_matrix_tiny_sweep(E):
     assert ran > 80
 
 
+def test_cost_matrix_many_devices(E):
+    """More than 8192 cells: etc_cost_matrix lists the (new stage, old stage) blocks that can overlap, clears the matrix and
+    computes those blocks only.  Against the oracle's element-wise definition on layouts of 96-192 devices: even and
+    uneven pipeline splits on either side, tied embeddings (the replica on the last stage overlaps stage 0), distributed
+    optimizer, scale-out onto fresh devices and scale-in, PP1 on one side, both styles."""
+    gpt = dict(style=0, n_layers=12, hidden=16, n_q_heads=4, n_kv_heads=4, head_dim=4, ffn_hidden=32, vocab=48,
+               max_pos=6, tied=1, param_bytes=2, kinds=15)
+    llama = dict(style=1, n_layers=12, hidden=16, n_q_heads=4, n_kv_heads=2, head_dim=4, ffn_hidden=24, vocab=32,
+                 max_pos=0, tied=0, param_bytes=2, kinds=15)
+    c = lambda tp, pp, dp, do=0, **kw: dict(dict(tp=tp, pp=pp, dp=dp, dist_opt=do), **kw)
+    cases = [
+        (gpt, c(2, 6, 8), c(2, 4, 12)),                          # 96 -> 96, stages cut differently
+        (gpt, c(2, 12, 4), c(4, 3, 16, 1)),                      # 96 -> 192 (fresh devices), dist-opt
+        (gpt, c(4, 4, 12, 1), c(2, 6, 8)),                       # 192 -> 96 scale-in
+        (gpt, c(2, 4, 12, 0, pp_first=2, pp_last=4), c(1, 12, 8)),          # uneven old split
+        (gpt, c(1, 1, 96), c(2, 6, 8, 0, pp_first=2)),           # PP1 on one side
+        (llama, c(2, 6, 8), c(1, 12, 10)),                       # 96 -> 120, untied, GQA
+        (llama, c(2, 3, 32, 1), c(2, 4, 16, 0, pp_last=3)),      # 192 -> 128
+    ]
+    for model, a, b in cases:
+        oo, on = O.Layout(model, a), O.Layout(model, b)
+        assert on.n_dev * max(oo.n_dev, on.n_dev) > 8192
+        ov, need, hold = O.overlap(oo, on)
+        go, gn = E.etc_layout_create(model, a), E.etc_layout_create(model, b)
+        g = E.etc_cost_matrix(go, gn)
+        assert np.array_equal(g[0].cpu().numpy(), ov), (a, b)
+        assert np.array_equal(g[1].cpu().numpy(), need) and np.array_equal(g[2].cpu().numpy(), hold), (a, b)
+        assert int(ov.sum()) > 0
+
+
 def test_cost_matrix_mismatch_error(E):
     a = E.etc_layout_create(dict(tiny_models())["gpt_t"], dict(tp=1, pp=1, dp=1, dist_opt=0))
     b = E.etc_layout_create(dict(tiny_models())["gpt_u"], dict(tp=1, pp=1, dp=1, dist_opt=0))
