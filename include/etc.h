@@ -122,8 +122,12 @@ etc_status etc_cost_matrix(const etc_layout* old_l, const etc_layout* new_l,
  * (= Eq. 2's minimisation under Eq. 3/4, reading A4).  d_avail: optional device mask [P] (0 = device may not be
  * used, e.g. pre-empted; NULL = all usable).  method: ETC_SKETCH_HUNGARIAN = shortest augmenting paths (any P up to
  * ETC_SKETCH_MAX_P), ETC_SKETCH_EXHAUSTIVE = every injective map enumerated (P <= 8, the cross-check), ETC_SKETCH_AUTO
- * = the faster one (Hungarian).  Outputs (device memory): d_device_map [n_new] int32, d_local_bytes [1] int64 =
- * the achieved objective.  If no feasible map exists both are filled with -1.  Enqueues on `stream`. */
+ * = the faster one (Hungarian).  For 32 < P <= 1024 the Hungarian method first tries the row-maximum certificate: if
+ * every row can be given one of its maximal columns, that map attains the upper bound sum_n max_o overlap[n][o] and is
+ * returned without a search (deterministic; the search runs otherwise, so the result is an optimum either way).
+ * Outputs (device memory): d_device_map [n_new] int32, d_local_bytes [1] int64 = the achieved objective.  If no
+ * feasible map exists both are filled with -1.  Enqueues on `stream`; no host synchronisation (a few KB of
+ * stream-ordered scratch for P > 32). */
 enum { ETC_SKETCH_AUTO = 0, ETC_SKETCH_EXHAUSTIVE = 1, ETC_SKETCH_HUNGARIAN = 2 };
 etc_status etc_sketch(const int64_t* d_overlap, int32_t n_new, int32_t P, const uint8_t* d_avail, int32_t method,
                       int32_t* d_device_map, int64_t* d_local_bytes, void* stream);
