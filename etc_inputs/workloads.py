@@ -66,6 +66,10 @@ WORKLOADS = {
     "x64": dict(name="x64", data=True, seed=0xE7C00013,
                 model=_model(STYLE_GPT, 48, 512, 16, 16, 32, 2048, 50304, 2048, 1, 2, _ALL4),
                 old=_cfg(2, 2, 2), new=_cfg(16, 1, 1)),
+    # x64 reversed (TP shrinks 16 -> 2): the short rows are on the DESTINATION side (unpack and local copies scatter them)
+    "x64r": dict(name="x64r", data=True, seed=0xE7C00015,
+                 model=_model(STYLE_GPT, 48, 512, 16, 16, 32, 2048, 50304, 2048, 1, 2, _ALL4),
+                 old=_cfg(16, 1, 1), new=_cfg(2, 2, 2)),
     # odd hidden size: every bf16 row is only 2-byte aligned, every fp32 row 4-byte aligned (the re-aligning copy path),
     # c2's reconfiguration
     "xodd": dict(name="xodd", data=True, seed=0xE7C00014,
@@ -96,6 +100,8 @@ _SCALED = {
     # (2-byte aligned bf16 rows: the byte-phase re-aligning path)
     "sx64": ("x64", dict(n_layers=4, hidden=256, n_q_heads=16, n_kv_heads=16, head_dim=16, ffn_hidden=1024,
                          vocab=3008, max_pos=64)),
+    "sx64r": ("x64r", dict(n_layers=4, hidden=256, n_q_heads=16, n_kv_heads=16, head_dim=16, ffn_hidden=1024,
+                           vocab=3008, max_pos=64)),
     "sxodd": ("xodd", dict(n_layers=4, hidden=193, n_q_heads=12, n_kv_heads=12, head_dim=16, ffn_hidden=768,
                            vocab=3000, max_pos=96)),
 }
@@ -103,7 +109,7 @@ _SCALED = {
 
 def workload(name: str) -> dict:
     """Return a deep copy of the named workload ("c1".."c5", "c5b", "s2".."s5", "s2odd", "s4odd", "s5b", and the copy-kernel
-    stress workloads "x128", "x64", "xodd" with their scaled twins "sx64", "sxodd")."""
+    stress workloads "x128", "x64", "x64r", "xodd" with their scaled twins "sx64", "sx64r", "sxodd")."""
     if name in WORKLOADS:
         return copy.deepcopy(WORKLOADS[name])
     base, over = _SCALED[name]

@@ -57,7 +57,7 @@ def _plan(E, w, flags, device_map=None):
     return old, new, E.etc_plan_create(old, new, dm, flags)
 
 
-@pytest.mark.parametrize("name", ["c1", "s2", "s3", "s4", "s4odd", "s5", "sx64", "sxodd"])
+@pytest.mark.parametrize("name", ["c1", "s2", "s3", "s4", "s4odd", "s5", "sx64", "sx64r", "sxodd"])
 @pytest.mark.parametrize("flags", [0, 1, 2, 4])
 def test_ordered_lists_are_sorted_permutations(E, name, flags):
     w = workload(name)
@@ -131,7 +131,7 @@ def _migrate(E, w, src_np, flags, device_map, poison):
     return g
 
 
-@pytest.mark.parametrize("name", ["s2", "s3", "s4", "s4odd", "s5", "sx64", "sxodd"])
+@pytest.mark.parametrize("name", ["s2", "s3", "s4", "s4odd", "s5", "sx64", "sx64r", "sxodd"])
 def test_ordered_and_list_order_launches_agree_with_the_oracle(E, name):
     w = workload(name)
     oo, on = O.Layout(w["model"], w["old"]), O.Layout(w["model"], w["new"])
