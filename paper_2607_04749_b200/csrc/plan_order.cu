@@ -14,8 +14,9 @@
 // indexed: an index array would put a dependent load in front of every CTA's first access.
 //
 // The sort is a counting sort over address bins of >= 64 KB of the concatenated buffers (one atomic per chunk for the
-// histogram and the rank inside the bin, a two-level exclusive scan of the bins, one scatter); order inside a bin is
-// the order the atomics arrived in — chunks of one bin touch the same 64 KB, so it does not matter.
+// histogram and the rank inside the bin, a two-level exclusive scan of the bins, one scatter); the order inside a bin —
+// chunks of one bin touch the same 64 KB, so it does not matter for speed — is then fixed by a per-bin insertion sort,
+// so that the lists are deterministic.
 #include <algorithm>
 #include <vector>
 #include "etc_internal.h"
@@ -109,6 +110,57 @@ order_scatter_kernel(const Chunk* __restrict__ chA, long long nA, const Chunk* _
   out1[bins1[bin_of(obase, c.src_buf, c.src_off, shift1)] + rank1[i]] = c;
 }
 
+// The atomics above leave the order INSIDE a bin to chance.  One thread per bin puts its few records (typically 1-8: a bin is
+// 64 KB of one buffer) into a fixed order — list 1 by (source offset, destination buffer, destination offset), list 2 by
+// (destination offset, source buffer, source offset) — so that a plan's launch lists are the same on every run.
+__device__ __forceinline__ bool rec_less(const Chunk& a, const Chunk& b, bool by_src) {
+  if (by_src) {
+    if (a.src_off != b.src_off) return a.src_off < b.src_off;
+    if (a.dst_buf != b.dst_buf) return a.dst_buf < b.dst_buf;
+    if (a.dst_off != b.dst_off) return a.dst_off < b.dst_off;
+    return a.stg_off < b.stg_off;
+  }
+  if (a.dst_off != b.dst_off) return a.dst_off < b.dst_off;
+  if (a.src_buf != b.src_buf) return a.src_buf < b.src_buf;
+  return a.src_off < b.src_off;
+}
+__global__ void __launch_bounds__(ORD_THREADS)
+order_bin_sort_kernel(const uint32_t* __restrict__ bins, long long n1, long long n2, long long nA, long long nB,
+                      Chunk* __restrict__ out1, Chunk* __restrict__ out2, const PlanTotals* __restrict__ lazy) {
+  const long long b = (long long)blockIdx.x * ORD_THREADS + threadIdx.x;
+  if (b >= n1 + n2) return;
+  if (lazy) { nA = lazy->n_chunks_staged; nB = lazy->n_chunks_local; }
+  const bool first = b < n1;
+  const uint32_t total = (uint32_t)(first ? nA + nB : nA + nB + nA);        // the scan runs on through both bin tables
+  const uint32_t lo = bins[b], hi = (b + 1 == n1 + n2) ? total : (b + 1 == n1 ? (uint32_t)(nA + nB) : bins[b + 1]);
+  if (hi <= lo + 1) return;
+  Chunk* r = first ? out1 + lo : out2 + (lo - (uint32_t)(nA + nB));
+  const uint32_t n = hi - lo;
+  if (n <= 32) {                                                           // insertion sort: the runs are short
+    for (uint32_t i = 1; i < n; ++i) {
+      const Chunk x = r[i];
+      uint32_t j = i;
+      while (j > 0 && rec_less(x, r[j - 1], first)) { r[j] = r[j - 1]; --j; }
+      if (j != i) r[j] = x;
+    }
+    return;
+  }
+  // a crowded bin (many tiny tensors in one 64 KB, or the coarser bins of a very large layout): heap sort, O(n log n)
+  auto sift = [&](uint32_t root, uint32_t end) {
+    const Chunk x = r[root];
+    while (true) {
+      uint32_t child = 2 * root + 1;
+      if (child >= end) break;
+      if (child + 1 < end && rec_less(r[child], r[child + 1], first)) ++child;
+      if (!rec_less(x, r[child], first)) break;
+      r[root] = r[child]; root = child;
+    }
+    r[root] = x;
+  };
+  for (uint32_t i = n / 2; i-- > 0;) sift(i, n);
+  for (uint32_t e = n - 1; e > 0; --e) { const Chunk t = r[0]; r[0] = r[e]; r[e] = t; sift(0, e); }
+}
+
 // exclusive prefix sums of the buffer sizes, each buffer starting on a bin boundary; returns the number of bins
 static long long bases_of(const std::vector<int64_t>& bytes, int shift, std::vector<int64_t>& base) {
   base.resize(bytes.size());
@@ -163,7 +215,9 @@ static cudaError_t order_range(const OrderScratch& s, const Chunk* chA, long lon
   order_scan_kernel<<<(unsigned)n_tiles, 1024, 0, st>>>(s.bins, n_bins, s.sums);
   order_scatter_kernel<<<grid, ORD_THREADS, 0, st>>>(chA, nA, chB, nB, s.d_ob, s.d_nb, s.shift1, s.shift2, s.bins, s.bins + s.n1,
                                                       s.r1, s.r2, out1, out2, lazy);
-  count_launch(4);
+  order_bin_sort_kernel<<<(unsigned)((n_bins + ORD_THREADS - 1) / ORD_THREADS), ORD_THREADS, 0, st>>>(s.bins, s.n1, s.n2, nA, nB,
+                                                                                                    out1, out2, lazy);
+  count_launch(5);
   return cudaGetLastError();
 }
 

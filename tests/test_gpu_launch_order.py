@@ -115,6 +115,20 @@ def _check_lists(plan, new):
         assert np.all(c == 1), key
 
 
+@pytest.mark.parametrize("name", ["s3", "s4", "sx64", "c1"])
+def test_ordered_lists_are_deterministic(E, name):
+    """The order inside an address bin is fixed by a per-bin sort: two plans of the same reconfiguration keep identical
+    launch lists, record for record (the histogram's atomics alone would leave it to chance)."""
+    w = workload(name)
+    lists = []
+    for _ in range(3):
+        old, new, plan = _plan(E, w, 0)
+        lists.append((plan.chunks(2).copy(), plan.chunks(3).copy()))
+        assert plan.validate() == 0
+    for l1, l2 in lists[1:]:
+        assert np.array_equal(l1, lists[0][0]) and np.array_equal(l2, lists[0][1])
+
+
 def test_plans_without_ordered_lists_say_so(E):
     w = workload("s2")
     for flags in (E.ETC_NO_REORDER, E.ETC_NO_SYNC):
