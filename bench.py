@@ -655,6 +655,12 @@ def run_cuda(args, w):
             line["one_shot_error"] = repr(ex)[:160]
     per_config = {w["name"]: config_entry(res, peak, one, w["name"], mode)}
     if extras_on:
+        try:
+            per_config[w["name"]]["cost_sketch_wall_ms"], per_config[w["name"]]["cost_sketch_wall_best_ms"] = \
+                cost_sketch_wall_ms(E, torch, R.lay_old, R.lay_new)
+        except Exception as ex:
+            per_config[w["name"]]["cost_sketch_wall_error"] = repr(ex)[:120]
+    if extras_on:
         if not args.no_reorder:
             try:
                 per_kernel.update(list_order_rates(E, torch, R, peak, flags))
@@ -684,6 +690,8 @@ def run_cuda(args, w):
                 except Exception:
                     pass
                 per_config[name] = config_entry(ri, peak, one_i, name, mode)
+                per_config[name]["cost_sketch_wall_ms"], per_config[name]["cost_sketch_wall_best_ms"] = \
+                    cost_sketch_wall_ms(E, torch, Ri.lay_old, Ri.lay_new)
                 Ri.close()
                 del Ri
             except Exception as ex:
@@ -730,6 +738,28 @@ def run_cuda(args, w):
         dist.destroy_process_group()
 
 
+def cost_sketch_wall_ms(E, torch, lo, ln, reps=12):
+    """Host wall clock of etc_cost_matrix + etc_sketch from the call to the device map back on the host (the final D2H
+    included), median; and best.  SURVEY.md 8(d)."""
+    P = max(lo.n_dev, ln.n_dev)
+    dev = torch.device("cuda", torch.cuda.current_device())
+    out_c = (torch.empty((ln.n_dev, P), dtype=torch.int64, device=dev), torch.empty(ln.n_dev, dtype=torch.int64, device=dev),
+             torch.empty(P, dtype=torch.int64, device=dev))
+    out_s = (torch.empty(ln.n_dev, dtype=torch.int32, device=dev), torch.empty(1, dtype=torch.int64, device=dev))
+    host = torch.empty(ln.n_dev, dtype=torch.int32, pin_memory=True)
+    walls = []
+    for i in range(reps):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        E.etc_cost_matrix(lo, ln, out=out_c)
+        E.etc_sketch(out_c[0], out=out_s)
+        host.copy_(out_s[0], non_blocking=True)
+        torch.cuda.synchronize()
+        if i >= 2:
+            walls.append((time.perf_counter() - t0) * 1e3)
+    return statistics.median(walls), min(walls)
+
+
 def metadata_only(E, torch, wb):
     """cost matrix + sketch of the metadata-only 512 -> 384 device layout (BASELINE.json configs[4])."""
     ev = lambda: torch.cuda.Event(enable_timing=True)
@@ -759,8 +789,10 @@ def metadata_only(E, torch, wb):
         E.etc_sketch(out_c[0], out=out_s)
     c.record(stream)
     torch.cuda.synchronize()
+    wall_med, wall_best = cost_sketch_wall_ms(E, torch, lo, ln)
     return {"cost_matrix_ms": statistics.mean(tc), "sketch_ms": statistics.mean(ts),
             "cost_sketch_ms": statistics.mean(tc) + statistics.mean(ts),
+            "cost_sketch_wall_ms": wall_med, "cost_sketch_wall_best_ms": wall_best,
             "cost_matrix_back_to_back_ms": a.elapsed_time(b) / 50, "sketch_back_to_back_ms": b.elapsed_time(c) / 50,
             "local_bytes": int(lb.item()), "devices": [lo.n_dev, ln.n_dev], "pieces": [lo.n_pieces, ln.n_pieces]}
 
