@@ -132,6 +132,37 @@ enum { ETC_SKETCH_AUTO = 0, ETC_SKETCH_EXHAUSTIVE = 1, ETC_SKETCH_HUNGARIAN = 2 
 etc_status etc_sketch(const int64_t* d_overlap, int32_t n_new, int32_t P, const uint8_t* d_avail, int32_t method,
                       int32_t* d_device_map, int64_t* d_local_bytes, void* stream);
 
+/* (a3) The same sketch for callers that cannot allocate device memory.  etc_sketch takes a few KB of work area from
+ * CUDA's stream-ordered pool whenever P > 32.  Three kinds of caller cannot afford that:
+ *   - a trainer whose own caching allocator has already claimed all free HBM (the migration runs exactly when the GPU is
+ *     at its fullest: old state, new state and staging together, 136 of 180 GB on the largest benchmark config), so a
+ *     driver-level allocation made behind its back fails with out-of-memory, or forces it to give memory back;
+ *   - a failure-recovery handler that must not stall: growing a memory pool, like cudaMalloc / cudaFree, may wait for
+ *     every stream of the device, including the ones still running the surviving ranks' work;
+ *   - a process that was given a fixed device-memory budget up front and is not allowed to exceed it later.
+ * etc_sketch_static computes what etc_sketch(..., ETC_SKETCH_HUNGARIAN, ...) computes — same arguments (minus `method`),
+ * same outputs, the same device_map bit for bit (warp search for P <= 32; row-maximum certificate, then the CTA search,
+ * for P > 32) — and calls no cudaMalloc, cudaMallocAsync, cudaFree or any library routine that allocates.  Its work area is
+ * a fixed array of ETC_SKETCH_STATIC_SCRATCH_BYTES (28 KB) inside libetc.so's device image: every GPU that loads the
+ * library holds those 28 KB until the process exits, whether or not this entry point is ever called.
+ * Limit: P <= ETC_SKETCH_STATIC_MAX_P (1024 devices; the paper's Algorithm 1 is quoted for k < 1024).  A
+ * larger P is refused with ETC_ERR_WORKSPACE and a text in etc_last_error_detail(); nothing is launched or written.
+ * Rules that come with a shared, resident work area:
+ *   - The first call on a device looks up where the array lives on that device (cudaGetSymbolAddress, which may also make
+ *     the CUDA runtime load the library's kernels).  Make that first call during start-up, outside any stream capture and
+ *     outside the time-critical path; later calls on the device only launch kernels.
+ *   - All calls share the one array, and it keeps what the previous call wrote.  No part of it needs clearing: each call
+ *     overwrites every entry it later reads.  But two calls whose kernels can run at the same time on one GPU (different
+ *     streams without an ordering between them, or two host threads doing that) overwrite each other's rows and the
+ *     results are undefined: keep calls on one stream, or order them with events.  Calls on different GPUs do not
+ *     interact (each device has its own copy of the array).
+ *   - The caller still owns and passes d_overlap, d_avail, d_device_map and d_local_bytes as for etc_sketch; if no
+ *     feasible map exists both outputs are filled with -1.  Enqueues on `stream`; no host synchronisation. */
+#define ETC_SKETCH_STATIC_MAX_P 1024
+#define ETC_SKETCH_STATIC_SCRATCH_BYTES 28672
+etc_status etc_sketch_static(const int64_t* d_overlap, int32_t n_new, int32_t P, const uint8_t* d_avail,
+                             int32_t* d_device_map, int64_t* d_local_bytes, void* stream);
+
 /* (f1) Virtual rank allocator: Algorithm 2 "Placement-Aware Remapping" (the garbled listing is read
  * from the prose PAPER.md:220-222, reading A23) composed with the sketch into one final device map
  * (communication coalescing): pass d_out_map to etc_plan_create and every element moves in ONE hop.

@@ -14,6 +14,7 @@ _inited = False
 
 ETC_LOCAL_DIRECT, ETC_ALL_STAGED, ETC_KIND_MAJOR, ETC_ALL_DIRECT, ETC_NO_SYNC, ETC_NO_REORDER = 0, 1, 2, 4, 8, 16
 ETC_SKETCH_AUTO, ETC_SKETCH_EXHAUSTIVE, ETC_SKETCH_HUNGARIAN = 0, 1, 2
+ETC_SKETCH_STATIC_MAX_P, ETC_SKETCH_STATIC_SCRATCH_BYTES = 1024, 28672
 ETC_PHASE_PACK, ETC_PHASE_UNPACK, ETC_PHASE_ALL = 1, 2, 3
 ETC_DEFRAG_OCCUPANCY, ETC_DEFRAG_EFFICIENCY, ETC_DEFRAG_BOTH = 1, 2, 3
 
@@ -25,7 +26,7 @@ EXPORTED_SYMBOLS = (
     "etc_status_string", "etc_last_error_detail", "etc_kernel_launches", "etc_defrag",
     "etc_plan_set_rounds", "etc_plan_get_round", "etc_migrate_round", "etc_plan_create_failed", "etc_mask_failed",
     "etc_upload_sources", "etc_plan_validate", "etc_mask_cross_dp", "etc_staging_bound", "etc_migrate_state", "etc_plan_get_map",
-    "etc_plan_get_chunks",
+    "etc_plan_get_chunks", "etc_sketch_static",
 )
 
 
@@ -85,6 +86,7 @@ def lib():
         L.etc_layout_buffer_bytes.restype = i64; L.etc_layout_buffer_bytes.argtypes = [vp, i32, i32]
         L.etc_cost_matrix.restype = i32; L.etc_cost_matrix.argtypes = [vp, vp, vp, vp, vp, vp]
         L.etc_sketch.restype = i32; L.etc_sketch.argtypes = [vp, i32, i32, vp, i32, vp, vp, vp]
+        L.etc_sketch_static.restype = i32; L.etc_sketch_static.argtypes = [vp, i32, i32, vp, vp, vp, vp]
         L.etc_defrag.restype = i32; L.etc_defrag.argtypes = [vp, i32, i32, i32, i32, vp, vp, vp, vp]
         L.etc_plan_create.restype = i32; L.etc_plan_create.argtypes = [vp, vp, vp, i32, C.POINTER(vp), vp]
         L.etc_plan_create_failed.restype = i32
@@ -208,6 +210,28 @@ def etc_sketch(overlap, avail=None, method: int = ETC_SKETCH_AUTO, stream=None, 
         assert avail.is_cuda and avail.dtype == torch.uint8 and avail.numel() == P
         av = avail.data_ptr()
     _check(lib().etc_sketch(overlap.data_ptr(), n_new, P, av, method, dm.data_ptr(), lb.data_ptr(), _stream(stream)))
+    return dm, lb
+
+
+def etc_sketch_static(overlap, out, avail=None, stream=None):
+    """(a3) etc_sketch for callers that must not allocate device memory (a trainer whose caching allocator already owns all
+    free HBM, a recovery handler that must not stall on the allocator, a process with a fixed memory budget): the work area
+    is a 28 KB array resident in libetc.so's device image, so this wrapper allocates nothing either — `out` =
+    (device_map [n_new] int32, local_bytes [1] int64) must be passed in.  P <= ETC_SKETCH_STATIC_MAX_P (1024), else
+    EtcError(ETC_ERR_WORKSPACE).  Same result as etc_sketch(method=ETC_SKETCH_HUNGARIAN).  All calls share the one work area:
+    keep them on one stream (or order them); the first call on a device does a one-time address look-up, so make it at
+    start-up.  Asynchronous; returns `out`."""
+    import torch
+    _ensure_init()
+    n_new, P = overlap.shape
+    assert overlap.is_cuda and overlap.dtype == torch.int64 and overlap.is_contiguous()
+    dm, lb = out
+    assert dm.is_cuda and dm.dtype == torch.int32 and dm.numel() >= n_new and lb.is_cuda and lb.dtype == torch.int64
+    av = 0
+    if avail is not None:
+        assert avail.is_cuda and avail.dtype == torch.uint8 and avail.numel() == P
+        av = avail.data_ptr()
+    _check(lib().etc_sketch_static(overlap.data_ptr(), n_new, P, av, dm.data_ptr(), lb.data_ptr(), _stream(stream)))
     return dm, lb
 
 

@@ -103,6 +103,7 @@ struct etc_layout {
 // ---- error plumbing
 namespace etc {
 void set_error_detail(const char* what, cudaError_t e);
+void set_error_text(const char* text);                 // a detail that is not a CUDA error (read by etc_last_error_detail)
 void clear_error_detail();
 void count_launch(int n = 1);
 int current_device();

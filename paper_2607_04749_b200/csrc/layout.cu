@@ -19,6 +19,7 @@ void set_error_detail(const char* what, cudaError_t e) {
   g_detail = std::string(what) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")";
   (void)cudaGetLastError();
 }
+void set_error_text(const char* text) { g_detail = text; }
 void clear_error_detail() { g_detail.clear(); }
 void count_launch(int n) { __atomic_add_fetch(&g_launches, (long long)n, __ATOMIC_RELAXED); }
 int current_device() { return g_device; }

@@ -6,6 +6,7 @@
 //   * Hungarian:  shortest augmenting paths with dual potentials on the rectangular matrix (rows <= columns, so no
 //     zero padding is needed: padded rows of Algorithm 1 line 3 would cost 0 on every column and are dropped again by
 //     lines 6-8).  One thread per column, block-wide arg-min per Dijkstra step.
+#include <cstdio>
 #include "etc_internal.h"
 
 namespace etc {
@@ -467,5 +468,87 @@ extern "C" etc_status etc_sketch(const int64_t* d_overlap, int32_t n_new, int32_
   }
   ETC_CUDA_TRY(cudaGetLastError());
   count_launch();
+  return ETC_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- etc_sketch_static
+// The sketch for callers that must not allocate (include/etc.h has the user-facing text).  etc_sketch above takes the
+// work area of the row-maximum certificate (rowmax [N] int64 | cnt [N] int32 | tight [N][TK] int32) from the
+// stream-ordered pool on every call with P > 32; here the same three arrays live in ONE array that is part of the
+// library's device image, sized for the largest matrix the certificate handles (TIGHT_MAX rows: 28 KB).  Every GPU that
+// loads libetc.so carries those 28 KB from the moment the module is loaded until the process exits.
+namespace etc {
+
+constexpr size_t STATIC_SCRATCH_BYTES = (size_t)TIGHT_MAX * (sizeof(int64_t) + sizeof(int32_t) + sizeof(int32_t) * TK);
+static_assert(STATIC_SCRATCH_BYTES == ETC_SKETCH_STATIC_SCRATCH_BYTES, "etc.h states the size of the resident work area");
+static_assert(TIGHT_MAX == ETC_SKETCH_STATIC_MAX_P, "etc.h states the largest P of etc_sketch_static");
+static __device__ __align__(256) unsigned char g_sketch_static_scratch[STATIC_SCRATCH_BYTES];
+
+// In host code `g_sketch_static_scratch` is only a handle for the runtime: it is NOT the array's address on the GPU, and a
+// kernel handed it would read and write somewhere else.  The address on a given GPU comes from cudaGetSymbolAddress, asked
+// once per device while that device is current, and is remembered here.
+constexpr int STATIC_MAX_DEVICES = 64;
+static std::mutex g_static_mu;
+static unsigned char* g_static_addr[STATIC_MAX_DEVICES] = {};
+
+static cudaError_t sketch_static_scratch(unsigned char** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_addr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_sketch_static_scratch);      // no allocation: the array came with the module
+    if (e != cudaSuccess) return e;
+    g_static_addr[dev] = static_cast<unsigned char*>(p);
+  }
+  *out = g_static_addr[dev];
+  return cudaSuccess;
+}
+
+}  // namespace etc
+
+extern "C" etc_status etc_sketch_static(const int64_t* d_overlap, int32_t n_new, int32_t P, const uint8_t* d_avail,
+                                        int32_t* d_device_map, int64_t* d_local_bytes, void* stream) {
+  clear_error_detail();
+  if (!d_overlap || !d_device_map || !d_local_bytes || n_new < 1 || P < n_new) return ETC_ERR_INVALID_ARG;
+  if (P > ETC_SKETCH_STATIC_MAX_P) {
+    char msg[160];
+    snprintf(msg, sizeof msg, "etc_sketch_static: P = %d exceeds ETC_SKETCH_STATIC_MAX_P = %d (the resident work area holds "
+             "%d rows); use etc_sketch", (int)P, (int)ETC_SKETCH_STATIC_MAX_P, (int)ETC_SKETCH_STATIC_MAX_P);
+    etc::set_error_text(msg);
+    return ETC_ERR_WORKSPACE;
+  }
+  etc::DeviceGuard device_guard;                 // the library's device is current from here on (the address is per device)
+  if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
+  cudaStream_t st = (cudaStream_t)stream;
+  if (P <= 32) {                                 // one warp, everything on chip: never needed a work area
+    sketch_hungarian_warp_kernel<<<1, 32, 0, st>>>(d_overlap, n_new, P, d_avail, d_device_map, d_local_bytes);
+    ETC_CUDA_TRY(cudaGetLastError());
+    count_launch();
+    return ETC_OK;
+  }
+  unsigned char* ws = nullptr;
+  ETC_CUDA_TRY(sketch_static_scratch(&ws));
+  // Same carving as etc_sketch.  Nothing in the work area has to start at zero: sketch_rowmax_kernel writes rowmax[n] and
+  // cnt[n] for every row before sketch_tight_kernel reads them, and of tight[n][*] only the first cnt[n] entries — written
+  // in this call — are ever used; what an earlier call left behind the valid entries is loaded and ignored.
+  const size_t o_cnt = sizeof(int64_t) * (size_t)n_new, o_tight = o_cnt + sizeof(int32_t) * (size_t)n_new;
+  int64_t* rowmax = reinterpret_cast<int64_t*>(ws);
+  int32_t* cnt = reinterpret_cast<int32_t*>(ws + o_cnt); int32_t* tight = reinterpret_cast<int32_t*>(ws + o_tight);
+  sketch_rowmax_kernel<<<(n_new + RM_WARPS - 1) / RM_WARPS, RM_WARPS * 32, 0, st>>>(d_overlap, n_new, P, d_avail, rowmax, cnt, tight);
+  sketch_tight_kernel<<<1, SK_THREADS, 0, st>>>(n_new, P, d_avail, rowmax, cnt, tight, d_device_map, d_local_bytes);
+  ETC_CUDA_TRY(cudaGetLastError());
+  const size_t smem = (size_t)n_new * 8 + (size_t)P * 8;         // <= 16 KB
+#define SK_LAUNCH(T) sketch_hungarian_kernel<T, 1><<<1, T, smem, st>>>(d_overlap, n_new, P, d_avail, d_device_map, d_local_bytes, 1)
+  if (P <= 64) SK_LAUNCH(64);
+  else if (P <= 128) SK_LAUNCH(128);
+  else if (P <= 256) SK_LAUNCH(256);
+  else if (P <= 512) SK_LAUNCH(512);
+  else SK_LAUNCH(1024);
+#undef SK_LAUNCH
+  ETC_CUDA_TRY(cudaGetLastError());
+  count_launch(3);
   return ETC_OK;
 }
