@@ -219,6 +219,12 @@ enum { ETC_LOCAL_DIRECT = 0, ETC_ALL_STAGED = 1, ETC_KIND_MAJOR = 2, ETC_ALL_DIR
 int64_t etc_staging_bound(const etc_layout* old_l, const etc_layout* new_l, int32_t flags);   /* bytes; < 0 on bad arguments */
 etc_status etc_plan_create(const etc_layout* old_l, const etc_layout* new_l, const int32_t* device_map,
                            int32_t flags, etc_plan** out, void* stream);
+/* Whether ETC_NO_SYNC was honoured for this plan: 1 = deferred (tables sized from host-side bounds, counts still on the
+ * device, etc_plan_create did not synchronise — safe inside a stream capture), 0 = made the synchronising way (no
+ * ETC_NO_SYNC flag, or the bound exceeded 32 768 copy work items: etc_plan_create called cudaStreamSynchronize, which is
+ * not allowed while `stream` is being captured — probe with a plan made outside the capture first), < 0 on a NULL plan.
+ * Host-only; never synchronises. */
+int32_t etc_plan_is_deferred(const etc_plan* plan);
 /* Releases the plan's tables in stream order, behind everything already enqueued that reads them (on whatever streams):
  * safe to call right after the last etc_migrate* call on the plan, while its kernels are still queued.  Do call it there
  * when migrations are pipelined: the tables return to the stream-ordered pool at that point of the copy stream, and a plan

@@ -330,19 +330,25 @@ def orc_check_map(dm, n_new, P) -> bool:
 
 
 def migrate_range(old: Layout, new: Layout, device_map, n, kind, l0, l1, src_bufs: dict | None, dst=None,
-                  T=None, written=None, src_windows: dict | None = None):
+                  T=None, written=None, src_windows: dict | None = None, dst_first: int = 0):
     """Element-wise migration of local indices [l0, l1) of new buffer (n, kind) (orc_migrate_range).  src_bufs:
     {(old_dev, kind): whole old buffer}.  src_windows (instead of src_bufs): {(old_dev, kind): (first, array)} where
     `array` holds only the elements [first, first + len(array)) of that old buffer — for callers that know which part of
     the old state a range reads and cannot hold all of it in host memory; the table entry is the address the whole
-    buffer would start at, so elements outside the window must not be read."""
+    buffer would start at, so elements outside the window must not be read.  dst_first: `dst` holds only the elements
+    [dst_first, dst_first + len(dst)) of the new buffer (same address trick on the destination side; [l0, l1) must lie
+    inside it) — orchestration only, the per-element C routine is the same."""
     dm = np.ascontiguousarray(device_map, np.int32)
+    dst_p = _ptr(dst)
+    if dst_first:
+        assert dst is not None and dst_first <= l0 and l1 <= dst_first + dst.shape[0]
+        dst_p = C.c_void_p(dst.ctypes.data - int(dst_first) * dst.itemsize)
     st = _ptr_table(src_bufs, old.n_dev) if src_bufs is not None else None
     if src_windows is not None:
         assert src_bufs is None
         st = (C.c_void_p * (old.n_dev * 4))()
         for (dev, k), (first, a) in src_windows.items():
             st[dev * 4 + k] = a.ctypes.data - int(first) * a.itemsize
-    rc = lib().orc_migrate_range(old.h, new.h, _ptr(dm), n, kind, l0, l1, st, _ptr(dst), _ptr(T), None, _ptr(written))
+    rc = lib().orc_migrate_range(old.h, new.h, _ptr(dm), n, kind, l0, l1, st, dst_p, _ptr(T), None, _ptr(written))
     if rc:
         raise OracleError(rc)

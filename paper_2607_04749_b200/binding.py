@@ -26,7 +26,7 @@ EXPORTED_SYMBOLS = (
     "etc_status_string", "etc_last_error_detail", "etc_kernel_launches", "etc_defrag",
     "etc_plan_set_rounds", "etc_plan_get_round", "etc_migrate_round", "etc_plan_create_failed", "etc_mask_failed",
     "etc_upload_sources", "etc_plan_validate", "etc_mask_cross_dp", "etc_staging_bound", "etc_migrate_state", "etc_plan_get_map",
-    "etc_plan_get_chunks", "etc_sketch_static",
+    "etc_plan_get_chunks", "etc_sketch_static", "etc_plan_is_deferred",
 )
 
 
@@ -95,6 +95,7 @@ def lib():
         L.etc_mask_cross_dp.restype = i32; L.etc_mask_cross_dp.argtypes = [vp, vp, vp, vp]
         L.etc_plan_destroy.restype = None; L.etc_plan_destroy.argtypes = [vp]
         L.etc_plan_get_stats.restype = i32; L.etc_plan_get_stats.argtypes = [vp, C.POINTER(_PlanStats)]
+        L.etc_plan_is_deferred.restype = i32; L.etc_plan_is_deferred.argtypes = [vp]
         L.etc_plan_get_traffic.restype = i32; L.etc_plan_get_traffic.argtypes = [vp, vp]
         L.etc_plan_get_slices.restype = i32; L.etc_plan_get_slices.argtypes = [vp, i32, vp]
         L.etc_plan_get_map.restype = i32; L.etc_plan_get_map.argtypes = [vp, vp]
@@ -328,6 +329,13 @@ class Plan:
         arr = np.zeros(max(n, 1), dt)
         _check(lib().etc_plan_get_chunks(self.h, which, arr.ctypes.data))
         return arr[:n]
+
+    @property
+    def deferred(self) -> bool:
+        """etc_plan_is_deferred: True if ETC_NO_SYNC was honoured (counts still on the device; creation did not synchronise)."""
+        r = lib().etc_plan_is_deferred(self.h)
+        _check(min(r, 0))
+        return r == 1
 
     def validate(self, stream=None) -> int:
         """device-side bounds check of every copy work item; returns the number of bad ones (0 for a sound plan)"""

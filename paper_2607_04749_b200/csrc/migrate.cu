@@ -101,9 +101,11 @@ template <typename K> static cudaError_t big_smem(K kernel) {
 }
 static cudaError_t copy_kernel_attrs() {
   static bool done[64] = {};
+  static std::mutex mu;                                         // etc_migrate* may be called from several host threads
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> lock(mu);
   if (dev >= 0 && dev < 64 && done[dev]) return cudaSuccess;
   e = big_smem(migrate_copy_kernel<false, false>);
   if (e == cudaSuccess) e = big_smem(migrate_copy_kernel<false, true>);

@@ -285,8 +285,8 @@ plan_scan_kernel(const BlockCount* __restrict__ blocks, int B, long long U, int 
       // ETC_NO_SYNC: the tables were sized from host-side upper bounds before these counts existed.  Should a bound
       // ever fall short, or the map be bad, the counts are zeroed so that no later kernel writes or copies anything.
       t.overflow = (bound_slices > 0 && (t.n_slices_staged > bound_slices || t.n_slices_local > bound_slices ||
-                                         t.n_chunks_staged > bound_chunks || t.n_chunks_local > bound_chunks ||
-                                         t.staging_bytes > bound_staging)) ? 1 : 0;
+                                         t.n_chunks_staged + t.n_chunks_local > bound_chunks ||   // grids, the ordered
+                                         t.staging_bytes > bound_staging)) ? 1 : 0;                 // lists and ranks hold the SUM
       if (bound_slices > 0 && (t.overflow || t.bad_map)) {
         t.n_slices_staged = t.n_chunks_staged = t.n_slices_local = t.n_chunks_local = 0; t.staging_bytes = 0;
       }
@@ -444,6 +444,9 @@ plan_fills_kernel(DeviceTables newT, const int32_t* __restrict__ device_map, int
                   etc_slice* __restrict__ fills, PlanTotals* __restrict__ totals) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= newT.n_pieces) return;
+  // plan_scan_kernel ran before this kernel on the same stream: a plan it found unusable (bad map, bound overflow) must
+  // write nothing at all, so it gets no zero-fill descriptors either (n_fills stays 0 and migrate_fill_kernel leaves)
+  if (totals->bad_map || totals->overflow) return;
   const Piece q = newT.pieces[i];
   const int t = q.grp % newT.n_tensors, kind = q.grp / newT.n_tensors;
   if (t != 0 && t != lm_head_id) return;
@@ -661,7 +664,11 @@ extern "C" etc_status etc_plan_create_failed(const etc_layout* old_l, const etc_
   PLAN_TRY(cudaGetLastError());
   PlanTotals* h_tot = nullptr;                                  // pinned slot for the totals read-back (not for no-sync plans)
   if (!lazy) {
-    if (!g_pinned_totals) PLAN_TRY(cudaMallocHost(&g_pinned_totals, sizeof(PlanTotals) * N_PINNED_TOTALS));
+    {
+      static std::mutex mu;                                     // plans may be created from several host threads
+      std::lock_guard<std::mutex> lock(mu);
+      if (!g_pinned_totals) PLAN_TRY(cudaMallocHost(&g_pinned_totals, sizeof(PlanTotals) * N_PINNED_TOTALS));
+    }
     h_tot = &g_pinned_totals[__atomic_fetch_add(&g_pinned_next, 1u, __ATOMIC_RELAXED) % N_PINNED_TOTALS];
   }
   plan_scan_kernel<<<1, SCAN_THREADS, 0, st>>>(pl->d_blocks, B, U, K, n_old, n_new, P, pl->flags, map_in, pl->d_map,
@@ -734,6 +741,11 @@ extern "C" void etc_plan_destroy(etc_plan* pl) {
   delete pl;
 }
 
+extern "C" int32_t etc_plan_is_deferred(const etc_plan* pl) {
+  if (!pl) return ETC_ERR_INVALID_ARG;
+  return pl->lazy ? 1 : 0;
+}
+
 extern "C" etc_status etc_plan_get_stats(const etc_plan* pl, etc_plan_stats* out) {
   if (!pl || !out) return ETC_ERR_INVALID_ARG;
   etc_status rc = ETC_OK;
@@ -753,6 +765,7 @@ extern "C" etc_status etc_plan_get_traffic(const etc_plan* pl, int64_t* h_traffi
   etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
   if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!pl || !h_traffic) return ETC_ERR_INVALID_ARG;
+  { etc_status rc = ETC_OK; plan_totals(pl, &rc); if (rc != ETC_OK) return rc; }   // a device-detected error of an ETC_NO_SYNC plan
   ETC_CUDA_TRY(cudaStreamSynchronize(pl->stream_created_on));
   ETC_CUDA_TRY(cudaMemcpy(h_traffic, pl->d_traffic, sizeof(int64_t) * (size_t)pl->P * pl->P, cudaMemcpyDeviceToHost));
   return ETC_OK;
@@ -773,7 +786,10 @@ extern "C" etc_status etc_plan_get_slices(const etc_plan* pl, int32_t which, etc
   etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
   if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!pl || !h_out || (which != 0 && which != 1)) return ETC_ERR_INVALID_ARG;
-  const int64_t n = which == 0 ? plan_totals(pl).n_slices_staged : plan_totals(pl).n_slices_local;
+  etc_status rc = ETC_OK;
+  const PlanTotals& t = plan_totals(pl, &rc);
+  if (rc != ETC_OK) return rc;
+  const int64_t n = which == 0 ? t.n_slices_staged : t.n_slices_local;
   const etc_slice* src = which == 0 ? pl->d_sl_staged : pl->d_sl_local;
   ETC_CUDA_TRY(cudaStreamSynchronize(pl->stream_created_on));
   if (n) ETC_CUDA_TRY(cudaMemcpy(h_out, src, sizeof(etc_slice) * (size_t)n, cudaMemcpyDeviceToHost));
@@ -802,8 +818,10 @@ extern "C" etc_status etc_plan_get_fills(const etc_plan* pl, etc_slice* h_out) {
   etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
   if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!pl || !h_out) return ETC_ERR_INVALID_ARG;
+  etc_status rc = ETC_OK;
+  const int64_t nf = plan_totals(pl, &rc).n_fills;
+  if (rc != ETC_OK) return rc;
   ETC_CUDA_TRY(cudaStreamSynchronize(pl->stream_created_on));
-  const int64_t nf = plan_totals(pl).n_fills;
   if (nf) ETC_CUDA_TRY(cudaMemcpy(h_out, pl->d_fills, sizeof(etc_slice) * (size_t)nf, cudaMemcpyDeviceToHost));
   return ETC_OK;
 }
@@ -813,6 +831,9 @@ extern "C" etc_status etc_plan_validate(const etc_plan* pl, int64_t* n_bad, void
   etc::DeviceGuard device_guard;                 // the library's device for this call; the caller's is restored on return
   if (device_guard.err != cudaSuccess) { etc::set_error_detail("cudaSetDevice", device_guard.err); return ETC_ERR_CUDA; }
   if (!pl || !n_bad) return ETC_ERR_INVALID_ARG;
+  etc_status plan_rc = ETC_OK;
+  const PlanTotals& t = plan_totals(pl, &plan_rc);
+  if (plan_rc != ETC_OK) return plan_rc;                        // an unusable ETC_NO_SYNC plan has nothing to validate
   cudaStream_t st = (cudaStream_t)stream;
   ETC_CUDA_TRY(plan_use(pl, st));
   const size_t ns = pl->old_bytes.size(), nd = pl->new_bytes.size();
@@ -826,7 +847,6 @@ extern "C" etc_status etc_plan_validate(const etc_plan* pl, int64_t* n_bad, void
   // of the per-round ordered lists
   unsigned long long* d_bad = reinterpret_cast<unsigned long long*>(d_sizes + ns + nd);
   VAL_TRY(cudaMemsetAsync(d_bad, 0, 7 * sizeof(unsigned long long), st));
-  const PlanTotals& t = plan_totals(pl);
   auto check = [&](const Chunk* list, long long n, int staged, int slot) -> cudaError_t {
     if (!n || !list) return cudaSuccess;
     plan_validate_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(list, n, staged, d_sizes, d_sizes + ns, t.staging_bytes, d_bad,

@@ -1,5 +1,6 @@
 // plan_types.h — plan-side tables shared by plan.cu (which writes them) and migrate.cu (which reads them).
 #pragma once
+#include <atomic>
 #include <vector>
 #include "etc_internal.h"
 
@@ -79,7 +80,7 @@ struct etc_plan {
   etc::PlanTotals totals{};                        // valid once `resolved` (always, unless created with ETC_NO_SYNC)
   // ETC_NO_SYNC: tables sized from upper bounds, counts live on the device until someone asks (plan_totals)
   bool lazy = false;
-  bool resolved = true;
+  std::atomic<bool> resolved{true};                // read without resolve_mu by etc_migrate_phase / etc_migrate_state; totals are read under it
   etc_status resolve_status = ETC_OK;
   int64_t bound_slices = 0, bound_chunks = 0, bound_staging = 0, bound_fills = 0, need_bytes = 0;
   std::mutex resolve_mu;

@@ -68,7 +68,9 @@ extern "C" etc_status etc_plan_set_rounds(etc_plan* pl, int64_t max_staging_byte
   if (max_staging_bytes < 2 * (int64_t)ETC_CHUNK_BYTES) return ETC_ERR_INVALID_ARG;
   const int64_t window = (max_staging_bytes - ETC_CHUNK_BYTES) & ~(int64_t)511;
   cudaStream_t st = (cudaStream_t)stream;
-  const PlanTotals& t = plan_totals(pl);
+  etc_status plan_rc = ETC_OK;
+  const PlanTotals& t = plan_totals(pl, &plan_rc);
+  if (plan_rc != ETC_OK) return plan_rc;                       // device-detected error of an ETC_NO_SYNC plan
 
   std::vector<RoundSpec> specs;
   std::vector<RoundRec> recs;

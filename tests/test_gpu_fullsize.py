@@ -136,3 +136,11 @@ def test_fullsize_c4_exhaustive(E):
 
 def test_fullsize_c5_exhaustive(E):
     _exhaustive(E, "c5", [(E.ETC_LOCAL_DIRECT, 0xA5), (E.ETC_ALL_STAGED, 0x5A), (E.ETC_LOCAL_DIRECT | E.ETC_NO_REORDER, 0x3C)])
+
+
+@pytest.mark.parametrize("name", ["x64", "x64r", "x128", "xodd"])
+def test_fullsize_stress_workloads_exhaustive(E, name):
+    """The copy-kernel stress workloads at FULL size: rows of 64-512 B on the source side (x64, x128) or
+    the destination side (x64r), and 2-byte-aligned long rows (xodd: the byte-phase re-aligning path).  DESIGN.md quotes their
+    copy rates, so every byte they write is compared with the oracle too — direct + staged, and every slice staged."""
+    _exhaustive(E, name, [(E.ETC_LOCAL_DIRECT, 0xA5), (E.ETC_ALL_STAGED, 0x5A)])

@@ -91,6 +91,42 @@ def test_no_sync_plan_detects_bad_maps_on_the_device(E):
         assert e.value.code == -4                                         # ETC_ERR_BAD_MAP
 
 
+def test_unusable_no_sync_plan_is_reported_by_every_query_and_writes_nothing(E):
+    """include/etc.h: a device-detected error of an ETC_NO_SYNC plan (here a map that is not injective) comes back from
+    EVERY call that needs the plan's counts on the host — not only etc_plan_get_stats — and such a plan writes nothing,
+    the zero-fill of a grown padded vocabulary (reading A31) included.  Raw C-ABI calls: the Python wrappers read .stats
+    first and would hide which entry point reported the error."""
+    import ctypes as C
+    from test_vocab_padding_pins import _model, _cfg
+    model, a, b = _model(), _cfg(1), _cfg(2)                      # vocab 5 padded to 6 -> 8 rows: the new layout has fill rows
+    old, new = E.etc_layout_create(model, a), E.etc_layout_create(model, b)
+    src = E.alloc_buffers(old, fill=1)
+    staging = torch.empty(max(E.etc_staging_bound(old, new, E.ETC_KIND_MAJOR), 16), dtype=torch.uint8, device="cuda")
+    good = E.etc_plan_create(old, new, torch.arange(new.n_dev, dtype=torch.int32, device="cuda"), E.ETC_NO_SYNC | E.ETC_KIND_MAJOR)
+    assert good.stats.n_fills > 0                                 # the case does have bytes with no source
+    L = E.lib()
+    for order in range(5):
+        dst = E.alloc_buffers(new, fill=0x3C)
+        dm = torch.zeros(new.n_dev, dtype=torch.int32, device="cuda")     # both new ranks on device 0
+        plan = E.etc_plan_create(old, new, dm, E.ETC_NO_SYNC | E.ETC_KIND_MAJOR)
+        E.etc_migrate(plan, src, dst, staging)
+        torch.cuda.synchronize()
+        for t in dst.values():
+            assert bool((t == 0x3C).all())                        # not even the padded vocabulary rows were zeroed
+        n_bad, n_rounds = C.c_int64(-9), C.c_int32(-9)
+        T = np.full((2, 2), -9, np.int64)
+        rec = np.zeros(4096, np.uint8)
+        calls = [lambda: L.etc_plan_validate(plan.h, C.byref(n_bad), 0),
+                 lambda: L.etc_plan_set_rounds(plan.h, 1 << 20, C.byref(n_rounds), 0),
+                 lambda: L.etc_plan_get_traffic(plan.h, T.ctypes.data),
+                 lambda: L.etc_plan_get_slices(plan.h, 0, rec.ctypes.data),
+                 lambda: L.etc_plan_get_fills(plan.h, rec.ctypes.data)]
+        calls = calls[order:] + calls[:order]                     # each of them is once the FIRST query of a fresh plan
+        for call in calls:
+            assert call() == -4                                   # ETC_ERR_BAD_MAP
+        assert n_bad.value == -9 and n_rounds.value == -9 and (T == -9).all() and not rec.any()   # outputs untouched
+
+
 def test_no_sync_plan_with_variants_failures_and_fills(E):
     """Random reconfigurations drawing on every layout variant (incl. grown padded vocabularies -> zero-fill list with a
     device-side count) and failure masks through ETC_NO_SYNC plans."""

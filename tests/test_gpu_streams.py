@@ -160,3 +160,55 @@ def test_plan_used_on_another_stream_without_a_manual_wait(E, name, flags):
             if e.shape[0]:
                 assert np.array_equal(download(dst[key], on.elem_bytes(key[1])), e), (mode, key)
         del plan
+
+
+@pytest.mark.parametrize("name,flags", [("s3", 0), ("s5", 1), ("s4odd", 0)])
+def test_one_plan_two_host_threads(E, name, flags):
+    """include/etc.h "Concurrency": a plan is immutable and may be used by several etc_migrate* calls at once, from different
+    host threads, on different streams with different buffer sets.  Two threads start together (a
+    barrier) on a FRESH plan — so the first-use set-up inside the library (kernel attributes, the plan's ready event) is hit
+    from both — and each migrates its own payload 8 times; an ETC_NO_SYNC plan is used the same way, so that both threads
+    also race to resolve its device-side counts.  Every result must equal the oracle's element-wise migration."""
+    import threading
+    w = workload(name)
+    model = w["model"]
+    oo, on = O.Layout(model, w["old"]), O.Layout(model, w["new"])
+    payloads = [sharded_payload(oo, w["seed"] + 10 + i, "stamp" if i == 0 else "salted") for i in range(2)]
+    old, new = E.etc_layout_create(model, w["old"]), E.etc_layout_create(model, w["new"])
+    dm, _ = E.etc_sketch(E.etc_cost_matrix(old, new)[0])
+    dm_h = dm.cpu().numpy()
+    exp = [oracle_migrate(oo, on, dm_h, p)[0] for p in payloads]
+    srcs = [upload(p) for p in payloads]
+    bound = max(E.etc_staging_bound(old, new, flags), 16)
+    for plan_flags in (flags, flags | E.ETC_NO_SYNC):
+        plan = E.etc_plan_create(old, new, dm, plan_flags)
+        dsts = [E.alloc_buffers(new, fill=0x3C) for _ in range(2)]
+        stagings = [torch.full((bound,), 0x3C, dtype=torch.uint8, device="cuda") for _ in range(2)]
+        streams = [torch.cuda.Stream() for _ in range(2)]
+        torch.cuda.synchronize()
+        gate = threading.Barrier(2)
+        errors = []
+
+        def worker(i):
+            try:
+                torch.cuda.set_device(dsts[i][next(iter(dsts[i]))].device)
+                gate.wait()
+                for rep in range(8):
+                    E.etc_migrate(plan, srcs[i], dsts[i], stagings[i], stream=streams[i])
+                    if rep == 3:
+                        assert plan.stats.n_old == old.n_dev       # resolves a deferred plan from both threads
+                streams[i].synchronize()
+            except Exception as ex:                                # surfaced below: an assert in a thread is otherwise lost
+                errors.append((i, repr(ex)))
+
+        threads = [threading.Thread(target=worker, args=(i,)) for i in range(2)]
+        for t in threads:
+            t.start()
+        for t in threads:
+            t.join()
+        torch.cuda.synchronize()
+        assert not errors, errors
+        for i in range(2):
+            for key, e in exp[i].items():
+                if e.shape[0]:
+                    assert np.array_equal(download(dsts[i][key], on.elem_bytes(key[1])), e), (plan_flags, i, key)
