@@ -80,6 +80,28 @@ def test_one_call_primitive_validates_before_any_cuda_call(lib):
     assert lib.etc_plan_create(None, None, None, 0, C.byref(h), None) == -1
 
 
+def test_static_sketch_and_deferred_query_validate_on_the_host(lib):
+    """etc_sketch_static refuses bad arguments and sizes beyond its resident work area before any CUDA call (so this runs
+    without a GPU), with a readable text in etc_last_error_detail; the header's constants match the library's array
+    (a static_assert in sketch.cu ties them to the kernel's row format); etc_plan_is_deferred(NULL) is an error."""
+    src = open(os.path.join(ROOT, "include", "etc.h")).read()
+    max_p = int(re.search(r"#define ETC_SKETCH_STATIC_MAX_P (\d+)", src).group(1))
+    nbytes = int(re.search(r"#define ETC_SKETCH_STATIC_SCRATCH_BYTES (\d+)", src).group(1))
+    from paper_2607_04749_b200 import ETC_SKETCH_STATIC_MAX_P, ETC_SKETCH_STATIC_SCRATCH_BYTES
+    assert (max_p, nbytes) == (ETC_SKETCH_STATIC_MAX_P, ETC_SKETCH_STATIC_SCRATCH_BYTES) == (1024, 1024 * 28)
+    buf = (C.c_int64 * 4)()
+    p = C.addressof(buf)                                          # never dereferenced: every call below fails first
+    assert lib.etc_sketch_static(None, 2, 4, None, p, p, None) == -1
+    assert lib.etc_sketch_static(p, 2, 4, None, None, p, None) == -1
+    assert lib.etc_sketch_static(p, 0, 4, None, p, p, None) == -1
+    assert lib.etc_sketch_static(p, 5, 4, None, p, p, None) == -1            # more rows than columns
+    assert lib.etc_sketch_static(p, 2, max_p + 1, None, p, p, None) == -5    # ETC_ERR_WORKSPACE
+    detail = lib.etc_last_error_detail().decode()
+    assert "ETC_SKETCH_STATIC_MAX_P" in detail and str(max_p + 1) in detail and "etc_sketch" in detail
+    assert lib.etc_sketch_static(None, 2, 4, None, p, p, None) == -1 and lib.etc_last_error_detail() == b""   # cleared per call
+    assert lib.etc_plan_is_deferred(None) == -1
+
+
 def test_product_path_has_no_oracle_or_cpu_fallback():
     """The package must not import the oracle, and must fail loudly without a CUDA device."""
     import torch
