@@ -1010,6 +1010,21 @@ def e2e(E, torch, args, w, dev, world, barrier):
     out["config"] = wi["name"]
     out["note"] = f"{best} on {wi['name']}; " + legs[best].get("note", "")
     out["legs"] = {k: {kk: vv for kk, vv in v.items() if kk != "note"} for k, v in legs.items()}
+    # The rule behind the choice, from plan statistics alone: the zero-copy leg reads every destination
+    # byte's source over PCIe separately, the DMA leg uploads each DISTINCT source byte once.  Their ratio says how much
+    # replicated state fans out; well below 1 the DMA leg should win wherever the copy engines are at least as fast as
+    # SM-issued PCIe reads.  Reported beside the measured choice, which stays the headline.
+    try:
+        zc, dm = legs["zero_copy"], legs.get("dma_needed_only", {})
+        if zc.get("h2d_bytes_per_step") and dm.get("h2d_bytes_per_step"):
+            ratio = dm["h2d_bytes_per_step"] / zc["h2d_bytes_per_step"]
+            out["distinct_source_fraction"] = ratio
+            out["rule_predicts"] = "dma_needed_only" if ratio < 0.9 else "zero_copy"
+            out["rule_agrees"] = out["rule_predicts"] == best
+            out["note"] += (f"; rule: distinct source bytes / bytes read = {ratio:.3f} -> {out['rule_predicts']} "
+                            f"({'agrees with' if out['rule_agrees'] else 'differs from'} the measured choice)")
+    except Exception:
+        pass
     return out
 
 
